@@ -1,0 +1,192 @@
+/*
+ * piper.h — C-ABI boundary of the B200 (sm_100a) MoE-chunk library.
+ *
+ * What it is: the per-device expert-parallel MoE chunk that Piper's DualPipeV schedule overlaps
+ * (§6.3; Fig. 3b): router top-k, histogram + scan + stable permutation
+ * into the per-expert buffers an EP all-to-all would carry (the payload of the `Shard` directive,
+ * PAPER.md:185), grouped SwiGLU expert FFN forward / dgrad / wgrad, gate-weighted combine, and the
+ * forward chunk of one microbatch co-scheduled with the backward chunk of another on two logical
+ * streams (list scheduling PAPER.md:267-271; event rule PAPER.md:279-286) under an
+ * explicit SM split (beyond the paper).  The paper states none of the MoE arithmetic;
+ * it is fixed by BASELINE.json:north_star / configs and restated in SURVEY.md §8(c) "Definition" and
+ * DESIGN.md.  Every entry point below cites the step of SURVEY.md §8(a) it implements.
+ *
+ * Conventions (all entry points):
+ *  - return value: PIPER_OK or a negative PIPER_ERR_* code; never throws, never aborts;
+ *  - every tensor pointer is a DEVICE pointer owned by the caller, 16-byte aligned, row-major,
+ *    contiguous; the library never allocates or frees device memory after piper_create() and never
+ *    frees caller memory; `workspace` (device, caller-owned) must outlive the context;
+ *  - `stream` is a cudaStream_t passed as void*; calls only enqueue work: no host synchronisation,
+ *    no host read-back of device data (the packed row count A lives on the device in
+ *    offsets[E_loc]);
+ *  - activation / weight element type is `desc.dtype` (0 = fp32, 1 = bf16 with fp32 accumulation);
+ *    logits, gates, gate_rows, dgates, dz_sel are always fp32; indices are int32;
+ *  - row buffers (xp, o, d_o, dxp, g_save, u_save, h_save, src_of, gate_rows) hold
+ *    A_cap = T*min(k,E_loc) + E_loc*(row_align-1) rows; rows >= offsets[E_loc] are never written and
+ *    their contents are unspecified;
+ *  - preconditions checked on the host: shapes > 0, k <= E, k <= 8, E <= 512, d % 8 == 0, I % 8 == 0,
+ *    I_shared % 8 == 0, pointers non-null and 16-byte aligned.  Logits must be finite (or -inf with
+ *    at least k finite entries per row, reading c-7); the device does not validate data;
+ *  - a piper_ctx is not thread-safe.
+ */
+#ifndef PIPER_H_
+#define PIPER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIPER_OK 0
+#define PIPER_ERR_INVALID (-1)     /* bad shape, null or misaligned pointer                         */
+#define PIPER_ERR_UNSUPPORTED (-2) /* valid request this build does not implement                   */
+#define PIPER_ERR_WORKSPACE (-3)   /* workspace too small                                           */
+#define PIPER_ERR_CUDA (-4)        /* a CUDA call failed: see piper_last_cuda_error()               */
+
+#define PIPER_DTYPE_F32 0
+#define PIPER_DTYPE_BF16 1
+
+#define PIPER_GATE_SOFTMAX_RENORM 0 /* g_j = exp(z_j - z_0) / sum_{j'<k} exp(z_j' - z_0)            */
+#define PIPER_GATE_SIGMOID_RENORM 1 /* s_j = 1/(1+exp(-z_j)); g_j = s_j / sum_{j'<k} s_j'           */
+#define PIPER_GATE_SOFTMAX_FULL 2   /* g_j = exp(z_j - m) / sum_{e<E} exp(z_e - m)                  */
+
+#define PIPER_GEMM_AUTO 0 /* bf16: tcgen05/TMEM/TMA kernels; fp32: FP32-ALU kernels (1e-5 bar)     */
+#define PIPER_GEMM_SIMT 1 /* force the FP32-ALU grouped GEMM (debug cross-check of the tcgen05 path) */
+
+typedef struct piper_ctx piper_ctx;
+
+/* Layer description (SURVEY.md §8 notation).  Local experts are [e_lo, e_lo + E_loc). */
+typedef struct {
+    int32_t T, d, E, k, e_lo, E_loc, I, I_shared; /* I_shared = 0: no shared expert                 */
+    int32_t dtype;     /* PIPER_DTYPE_*                                                             */
+    int32_t gate_mode; /* PIPER_GATE_*                                                              */
+    int32_t row_align; /* >= 1: each expert's row segment is padded to a multiple; pad rows are 0   */
+    int32_t dw_dtype;  /* element type of dW outputs; must equal dtype in this build                */
+    int32_t gemm_impl; /* PIPER_GEMM_*                                                              */
+} piper_moe_desc;
+
+/* Device workspace the context needs (scan scratch, tile counters).  Host call. */
+int piper_workspace_bytes(const piper_moe_desc* desc, size_t* bytes);
+/* Creates a context on CUDA device `device`.  `workspace` is a device pointer of at least
+ * piper_workspace_bytes() bytes, 256-byte aligned, owned by the caller. */
+int piper_create(const piper_moe_desc* desc, int device, void* workspace, size_t workspace_bytes, piper_ctx** out);
+int piper_destroy(piper_ctx* ctx);
+/* Text of the last CUDA error seen by this context (host string owned by the context). */
+const char* piper_last_cuda_error(const piper_ctx* ctx);
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t piper_kernel_launches(const piper_ctx* ctx);
+/* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */
+int64_t piper_a_cap(const piper_moe_desc* desc);
+
+/* F1 route_topk (SURVEY.md §8a F1, §8c Definition 1; BASELINE.json:north_star part 1).
+ * logits [T,E] fp32 -> topk_idx [T,k] (k largest, ties to the lowest expert index, listed by
+ * descending logit), gates [T,k] fp32 (desc.gate_mode), counts_global [E] (selections per expert =
+ * the split sizes an all-to-all would announce). */
+int piper_route_topk(piper_ctx* ctx, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global,
+                     void* stream);
+
+/* F2 + F3 dispatch_pack (SURVEY.md §8a F2/F3, §8c Definition 2; north_star part 2).
+ * counts [E_loc]; offsets [E_loc+1] = exclusive scan of counts rounded up to row_align;
+ * row_of [T,k] = destination row of each assignment (stable by token), -1 if its expert is not local;
+ * src_of [A_cap] = flat assignment id t*k+j of each row, -1 for pad rows and for every row >=
+ * offsets[E_loc]; gate_rows [A_cap] fp32; xp [A_cap,d] = x rows gathered per expert (bit-exact copies;
+ * pad rows zero).  x [T,d]. */
+int piper_dispatch_pack(piper_ctx* ctx, const void* x, const int32_t* topk_idx, const float* gates, int32_t* counts,
+                        int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* xp, void* stream);
+
+/* F4 expert_ffn_fwd (SURVEY.md §8a F4, §8c Definition 3; north_star part 3).  Per row r of local
+ * expert e: g = xp[r] W_gate[e], u = xp[r] W_up[e], h = silu(g)*u, o[r] = h W_down[e].
+ * w_gate, w_up [E_loc,d,I]; w_down [E_loc,I,d].  g_save, u_save, h_save [A_cap,I] are opaque scratch
+ * handed to piper_expert_ffn_bwd; o [A_cap,d] is the unscaled expert output. */
+int piper_expert_ffn_fwd(piper_ctx* ctx, const void* xp, const int32_t* offsets, const void* w_gate, const void* w_up,
+                         const void* w_down, void* g_save, void* u_save, void* h_save, void* o, void* stream);
+/* Shared expert (reading c-11): the same FFN as one group over all T rows of x, intermediate
+ * I_shared.  ws_gate, ws_up [d,I_shared]; ws_down [I_shared,d]; saves [T,I_shared]; s [T,d]. */
+int piper_shared_ffn_fwd(piper_ctx* ctx, const void* x, const void* ws_gate, const void* ws_up, const void* ws_down,
+                         void* g_save, void* u_save, void* h_save, void* s, void* stream);
+
+/* F5 combine (SURVEY.md §8a F5, §8c Definition 4; north_star part 4).
+ * y[t] = sum_{j: row_of[t,j] >= 0} gates[t,j] * o[row_of[t,j]]  (+ s[t] if s != NULL). */
+int piper_combine(piper_ctx* ctx, const void* o, const int32_t* row_of, const float* gates, const void* s, void* y,
+                  void* stream);
+
+/* B1 combine_bwd (SURVEY.md §8a B1, §8c Definition 5).  d_o[r] = gates[src_of[r]] * dy[token(r)] for
+ * every non-pad row below offsets[E_loc] (pad rows zero); dgates[t,j] = <dy[t], o[row_of[t,j]]>, 0 for
+ * non-local slots.  d_o is opaque scratch handed to piper_expert_ffn_bwd. */
+int piper_combine_bwd(piper_ctx* ctx, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
+                      const float* gates, const int32_t* offsets, void* d_o, float* dgates, void* stream);
+
+/* B2-B4 expert_ffn_bwd (SURVEY.md §8a B2/B3/B4, §8c Definition 5; north_star part 3 "dgrad and
+ * wgrad").  dh = d_o W_down^T; dg = dh*u*silu'(g); du = dh*silu(g); dxp = dg W_gate^T + du W_up^T;
+ * dw_down[e] = h^T d_o, dw_gate[e] = xp^T dg, dw_up[e] = xp^T du summed over the expert's rows
+ * (exact zeros for empty experts).  dg, du [A_cap,I] are opaque scratch.  accumulate must be 0 in
+ * this build. */
+int piper_expert_ffn_bwd(piper_ctx* ctx, const void* d_o, const void* xp, const void* g_save, const void* u_save,
+                         const void* h_save, const int32_t* offsets, const void* w_gate, const void* w_up,
+                         const void* w_down, void* dg, void* du, void* dxp, void* dw_gate, void* dw_up, void* dw_down,
+                         int accumulate, void* stream);
+/* Shared expert backward: one group of T rows, d_o = dy, xp = x; dgs, dus [T,I_shared] scratch;
+ * dxs [T,d]. */
+int piper_shared_ffn_bwd(piper_ctx* ctx, const void* dy, const void* x, const void* g_save, const void* u_save,
+                         const void* h_save, const void* ws_gate, const void* ws_up, const void* ws_down, void* dgs,
+                         void* dus, void* dxs, void* dws_gate, void* dws_up, void* dws_down, int accumulate,
+                         void* stream);
+
+/* B5 dispatch_unpack.  dx[t] = sum_{j local} dxp[row_of[t,j]] (+ dx_shared[t]). */
+int piper_dispatch_unpack(piper_ctx* ctx, const void* dxp, const int32_t* row_of, const void* dx_shared, void* dx,
+                          void* stream);
+
+/* B6 route_bwd (gate-normalisation backward of Definition 5).
+ * gate modes 0/1: dz_sel [T,k] (gradient w.r.t. the k selected logits); mode 2: dz_sel is [T,E]. */
+int piper_route_bwd(piper_ctx* ctx, const float* logits, const int32_t* topk_idx, const float* gates,
+                    const float* dgates, float* dz_sel, void* stream);
+
+/* Every pointer of one microbatch (inputs, outputs and the scratch between forward and backward). */
+typedef struct {
+    const float* logits;                         /* [T,E]                                           */
+    const void *x, *dy;                          /* [T,d]                                           */
+    const void *w_gate, *w_up, *w_down;          /* routed experts                                  */
+    const void *ws_gate, *ws_up, *ws_down;       /* shared expert (NULL when I_shared = 0)          */
+    int32_t *topk_idx, *counts_global, *counts, *offsets, *row_of, *src_of;
+    float *gates, *gate_rows, *dgates, *dz_sel;
+    void *xp, *g_save, *u_save, *h_save, *o;     /* routed activations [A_cap, d or I]              */
+    void *gs_save, *us_save, *hs_save, *s;       /* shared-expert activations [T, I_shared or d]    */
+    void* y;                                     /* [T,d]                                           */
+    void *d_o, *dg, *du, *dxp, *dgs, *dus, *dxs, *dx; /* backward activations                      */
+    void *dw_gate, *dw_up, *dw_down, *dws_gate, *dws_up, *dws_down;
+} piper_chunk_args;
+
+/* Whole forward chunk F1..F5 (+ shared expert) / backward chunk B1..B6 on one stream, all SMs:
+ * the serial baseline of step P. */
+int piper_run_chunk_fwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
+int piper_run_chunk_bwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
+
+/* P run_chunk_pair (SURVEY.md §8a P, §8c c-sched; north_star part 5).  Enqueues the forward chunk of
+ * `fwd_mb` and the backward chunk of `bwd_mb` as the 14-task DAG of SURVEY.md §8c on two logical
+ * streams: GEMM tasks on a partition of `sm_gemm` SMs, pack/combine-side tasks on a partition of
+ * `sm_comm` SMs.  Task order = Piper's list scheduling (reading c-21); a task waits
+ * on an event only for a dependency that ran on the other stream and records one only when a
+ * consumer runs on the other stream.  Both partitions fork from and join
+ * into `stream`.  sm_gemm + sm_comm must not exceed the device's SM count; each must be a positive
+ * multiple of 8 except that sm_gemm may take the remainder.  Results are bit-identical to
+ * piper_run_chunk_fwd + piper_run_chunk_bwd. */
+int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const piper_chunk_args* bwd_mb, int sm_gemm,
+                         int sm_comm, void* stream);
+/* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
+ * grids on two plain streams (green contexts unavailable), 0 = never called. */
+int piper_pair_partition_mode(const piper_ctx* ctx);
+
+/* Host-only list scheduler used by piper_run_chunk_pair (reading c-21),
+ * exposed so it can be tested without a GPU.  n tasks, edges [n_edges][2] (src,dst), stream_of[n],
+ * prio[n] (lower first on ties) -> order[n] (pick sequence), waits [<= n_edges][2] (producer,
+ * consumer) for every direct cross-stream edge, *n_waits, records[n] (1 iff the task records an
+ * event).  Returns PIPER_ERR_INVALID on a cycle or a bad edge. */
+int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const int32_t* prio,
+                        int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIPER_H_ */

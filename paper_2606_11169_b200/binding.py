@@ -1,0 +1,261 @@
+"""Thin ctypes binding over libpiper.so (include/piper.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory and
+streams.  There is no CPU fallback: loading fails loudly when the library is missing, and every
+entry point raises on a non-zero status.  Function names equal the C-ABI names.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+_i32, _vp = ctypes.c_int32, ctypes.c_void_p
+
+PIPER_OK = 0
+DT_F32, DT_BF16 = 0, 1
+GEMM_AUTO, GEMM_SIMT = 0, 1
+
+
+class PiperError(RuntimeError):
+    pass
+
+
+class MoeDesc(ctypes.Structure):
+    """piper_moe_desc"""
+    _fields_ = [(n, _i32) for n in ("T", "d", "E", "k", "e_lo", "E_loc", "I", "I_shared", "dtype", "gate_mode",
+                                    "row_align", "dw_dtype", "gemm_impl")]
+
+
+_CHUNK_FIELDS = ("logits", "x", "dy", "w_gate", "w_up", "w_down", "ws_gate", "ws_up", "ws_down",
+                 "topk_idx", "counts_global", "counts", "offsets", "row_of", "src_of",
+                 "gates", "gate_rows", "dgates", "dz_sel",
+                 "xp", "g_save", "u_save", "h_save", "o",
+                 "gs_save", "us_save", "hs_save", "s", "y",
+                 "d_o", "dg", "du", "dxp", "dgs", "dus", "dxs", "dx",
+                 "dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down")
+
+
+class ChunkArgs(ctypes.Structure):
+    """piper_chunk_args (field order of include/piper.h)"""
+    _fields_ = [(n, _vp) for n in _CHUNK_FIELDS]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libpiper.so (building it in-tree if the sources are newer).  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        if not os.path.exists(path):
+            raise PiperError(f"CUDA library missing: {path}")
+        L = ctypes.CDLL(path)
+        L.piper_a_cap.restype = ctypes.c_int64
+        L.piper_kernel_launches.restype = ctypes.c_int64
+        L.piper_last_cuda_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    if t is None:
+        return _vp(0)
+    if not t.is_cuda or not t.is_contiguous():
+        raise PiperError("tensor arguments must be contiguous CUDA tensors")
+    return _vp(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return _vp(s.cuda_stream)
+
+
+def make_desc(T, d, E, k, I, e_lo=0, E_loc=-1, I_shared=0, dtype=DT_BF16, gate_mode=0, row_align=1,
+              gemm_impl=GEMM_AUTO) -> MoeDesc:
+    return MoeDesc(T, d, E, k, e_lo, E if E_loc < 0 else E_loc, I, I_shared, dtype, gate_mode, row_align, dtype,
+                   gemm_impl)
+
+
+class Context:
+    """piper_ctx + the workspace tensor it lives on."""
+
+    def __init__(self, desc: MoeDesc, device: int = 0):
+        L = lib()
+        if not torch.cuda.is_available():
+            raise PiperError("no CUDA device: the piper library has no CPU path")
+        self.desc = desc
+        self.device = torch.device("cuda", device)
+        nbytes = ctypes.c_size_t(0)
+        rc = L.piper_workspace_bytes(ctypes.byref(desc), ctypes.byref(nbytes))
+        if rc != PIPER_OK:
+            raise PiperError(f"piper_workspace_bytes: status {rc} (invalid layer description)")
+        self.workspace = torch.zeros(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self._h = _vp(0)
+        rc = L.piper_create(ctypes.byref(desc), device, _vp(base), ctypes.c_size_t(nbytes.value), ctypes.byref(self._h))
+        if rc != PIPER_OK:
+            raise PiperError(f"piper_create: status {rc}")
+
+    def close(self):
+        if self._h:
+            lib().piper_destroy(self._h)
+            self._h = _vp(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def a_cap(self) -> int:
+        return int(lib().piper_a_cap(ctypes.byref(self.desc)))
+
+    @property
+    def torch_dtype(self):
+        return torch.bfloat16 if self.desc.dtype == DT_BF16 else torch.float32
+
+    def check(self, rc: int, what: str):
+        if rc != PIPER_OK:
+            msg = lib().piper_last_cuda_error(self._h).decode() if rc == -4 else ""
+            raise PiperError(f"{what}: status {rc} {msg}")
+
+
+def piper_kernel_launches(ctx: Context) -> int:
+    return int(lib().piper_kernel_launches(ctx._h))
+
+
+def piper_pair_partition_mode(ctx: Context) -> int:
+    return int(lib().piper_pair_partition_mode(ctx._h))
+
+
+def piper_route_topk(ctx, logits, topk_idx, gates, counts_global, stream=None):
+    ctx.check(lib().piper_route_topk(ctx._h, _ptr(logits), _ptr(topk_idx), _ptr(gates), _ptr(counts_global),
+                                     _stream(stream)), "piper_route_topk")
+
+
+def piper_dispatch_pack(ctx, x, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows, xp, stream=None):
+    ctx.check(lib().piper_dispatch_pack(ctx._h, _ptr(x), _ptr(topk_idx), _ptr(gates), _ptr(counts), _ptr(offsets),
+                                        _ptr(row_of), _ptr(src_of), _ptr(gate_rows), _ptr(xp), _stream(stream)),
+              "piper_dispatch_pack")
+
+
+def piper_expert_ffn_fwd(ctx, xp, offsets, w_gate, w_up, w_down, g_save, u_save, h_save, o, stream=None):
+    ctx.check(lib().piper_expert_ffn_fwd(ctx._h, _ptr(xp), _ptr(offsets), _ptr(w_gate), _ptr(w_up), _ptr(w_down),
+                                         _ptr(g_save), _ptr(u_save), _ptr(h_save), _ptr(o), _stream(stream)),
+              "piper_expert_ffn_fwd")
+
+
+def piper_shared_ffn_fwd(ctx, x, ws_gate, ws_up, ws_down, g_save, u_save, h_save, s, stream=None):
+    ctx.check(lib().piper_shared_ffn_fwd(ctx._h, _ptr(x), _ptr(ws_gate), _ptr(ws_up), _ptr(ws_down), _ptr(g_save),
+                                         _ptr(u_save), _ptr(h_save), _ptr(s), _stream(stream)), "piper_shared_ffn_fwd")
+
+
+def piper_combine(ctx, o, row_of, gates, s, y, stream=None):
+    ctx.check(lib().piper_combine(ctx._h, _ptr(o), _ptr(row_of), _ptr(gates), _ptr(s), _ptr(y), _stream(stream)),
+              "piper_combine")
+
+
+def piper_combine_bwd(ctx, dy, o, src_of, row_of, gates, offsets, d_o, dgates, stream=None):
+    ctx.check(lib().piper_combine_bwd(ctx._h, _ptr(dy), _ptr(o), _ptr(src_of), _ptr(row_of), _ptr(gates),
+                                      _ptr(offsets), _ptr(d_o), _ptr(dgates), _stream(stream)), "piper_combine_bwd")
+
+
+def piper_expert_ffn_bwd(ctx, d_o, xp, g_save, u_save, h_save, offsets, w_gate, w_up, w_down, dg, du, dxp, dw_gate,
+                         dw_up, dw_down, accumulate=0, stream=None):
+    ctx.check(lib().piper_expert_ffn_bwd(ctx._h, _ptr(d_o), _ptr(xp), _ptr(g_save), _ptr(u_save), _ptr(h_save),
+                                         _ptr(offsets), _ptr(w_gate), _ptr(w_up), _ptr(w_down), _ptr(dg), _ptr(du),
+                                         _ptr(dxp), _ptr(dw_gate), _ptr(dw_up), _ptr(dw_down), int(accumulate),
+                                         _stream(stream)), "piper_expert_ffn_bwd")
+
+
+def piper_shared_ffn_bwd(ctx, dy, x, g_save, u_save, h_save, ws_gate, ws_up, ws_down, dgs, dus, dxs, dws_gate, dws_up,
+                         dws_down, accumulate=0, stream=None):
+    ctx.check(lib().piper_shared_ffn_bwd(ctx._h, _ptr(dy), _ptr(x), _ptr(g_save), _ptr(u_save), _ptr(h_save),
+                                         _ptr(ws_gate), _ptr(ws_up), _ptr(ws_down), _ptr(dgs), _ptr(dus), _ptr(dxs),
+                                         _ptr(dws_gate), _ptr(dws_up), _ptr(dws_down), int(accumulate),
+                                         _stream(stream)), "piper_shared_ffn_bwd")
+
+
+def piper_dispatch_unpack(ctx, dxp, row_of, dx_shared, dx, stream=None):
+    ctx.check(lib().piper_dispatch_unpack(ctx._h, _ptr(dxp), _ptr(row_of), _ptr(dx_shared), _ptr(dx), _stream(stream)),
+              "piper_dispatch_unpack")
+
+
+def piper_route_bwd(ctx, logits, topk_idx, gates, dgates, dz_sel, stream=None):
+    ctx.check(lib().piper_route_bwd(ctx._h, _ptr(logits), _ptr(topk_idx), _ptr(gates), _ptr(dgates), _ptr(dz_sel),
+                                    _stream(stream)), "piper_route_bwd")
+
+
+def chunk_args(bufs: dict) -> ChunkArgs:
+    """piper_chunk_args from a dict of tensors (missing / None entries become NULL)."""
+    a = ChunkArgs()
+    for n in _CHUNK_FIELDS:
+        setattr(a, n, _ptr(bufs.get(n)))
+    return a
+
+
+def piper_run_chunk_fwd(ctx, args: ChunkArgs, stream=None):
+    ctx.check(lib().piper_run_chunk_fwd(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_fwd")
+
+
+def piper_run_chunk_bwd(ctx, args: ChunkArgs, stream=None):
+    ctx.check(lib().piper_run_chunk_bwd(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_bwd")
+
+
+def piper_run_chunk_pair(ctx, fwd_args: ChunkArgs, bwd_args: ChunkArgs, sm_gemm: int, sm_comm: int, stream=None):
+    ctx.check(lib().piper_run_chunk_pair(ctx._h, ctypes.byref(fwd_args), ctypes.byref(bwd_args), int(sm_gemm),
+                                         int(sm_comm), _stream(stream)), "piper_run_chunk_pair")
+
+
+def piper_list_schedule(n, edges, stream_of, prio):
+    """Host-only: returns (order, waits[(producer, consumer)], records)."""
+    import numpy as np
+    edges = np.ascontiguousarray(edges, np.int32).reshape(-1, 2)
+    stream_of = np.ascontiguousarray(stream_of, np.int32)
+    prio = np.ascontiguousarray(prio, np.int32)
+    order = np.empty(n, np.int32)
+    waits = np.empty((max(1, len(edges)), 2), np.int32)
+    records = np.empty(n, np.int32)
+    nw = _i32(0)
+    rc = lib().piper_list_schedule(_i32(n), _i32(len(edges)), _vp(edges.ctypes.data), _vp(stream_of.ctypes.data),
+                                   _vp(prio.ctypes.data), _vp(order.ctypes.data), _vp(waits.ctypes.data),
+                                   ctypes.byref(nw), _vp(records.ctypes.data))
+    if rc != PIPER_OK:
+        raise PiperError(f"piper_list_schedule: status {rc}")
+    return order, waits[: nw.value].copy(), records
+
+
+# ---------------------------------------------------------------------------------- memory plumbing
+def alloc_buffers(ctx: Context, backward: bool = True) -> dict:
+    """Every output / scratch tensor of one microbatch, as torch CUDA tensors (no arithmetic here)."""
+    D, dev, dt = ctx.desc, ctx.device, ctx.torch_dtype
+    A = ctx.a_cap
+    i32, f32 = torch.int32, torch.float32
+
+    def e(shape, dtype):
+        return torch.empty(shape, dtype=dtype, device=dev)
+
+    b = dict(topk_idx=e((D.T, D.k), i32), counts_global=e((D.E,), i32), counts=e((D.E_loc,), i32),
+             offsets=e((D.E_loc + 4,), i32), row_of=e((D.T, D.k), i32), src_of=e((A,), i32),
+             gates=e((D.T, D.k), f32), gate_rows=e((A,), f32),
+             xp=e((A, D.d), dt), g_save=e((A, D.I), dt), u_save=e((A, D.I), dt), h_save=e((A, D.I), dt),
+             o=e((A, D.d), dt), y=e((D.T, D.d), dt))
+    if D.I_shared:
+        b.update(gs_save=e((D.T, D.I_shared), dt), us_save=e((D.T, D.I_shared), dt), hs_save=e((D.T, D.I_shared), dt),
+                 s=e((D.T, D.d), dt))
+    if backward:
+        b.update(dgates=e((D.T, D.k), f32), dz_sel=e((D.T, D.E if D.gate_mode == 2 else D.k), f32),
+                 d_o=e((A, D.d), dt), dg=e((A, D.I), dt), du=e((A, D.I), dt), dxp=e((A, D.d), dt),
+                 dx=e((D.T, D.d), dt), dw_gate=e((D.E_loc, D.d, D.I), dt), dw_up=e((D.E_loc, D.d, D.I), dt),
+                 dw_down=e((D.E_loc, D.I, D.d), dt))
+        if D.I_shared:
+            b.update(dgs=e((D.T, D.I_shared), dt), dus=e((D.T, D.I_shared), dt), dxs=e((D.T, D.d), dt),
+                     dws_gate=e((D.d, D.I_shared), dt), dws_up=e((D.d, D.I_shared), dt),
+                     dws_down=e((D.I_shared, D.d), dt))
+    return b

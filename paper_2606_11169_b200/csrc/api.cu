@@ -1,0 +1,218 @@
+// api.cu — context management and the per-step C-ABI entry points of include/piper.h.
+// Argument checks happen here on the host; the kernels live in route.cu / permute.cu / gemm_*.cu.
+#include "piper_internal.cuh"
+
+using namespace piper;
+
+namespace {
+
+bool desc_ok(const piper_moe_desc* D) {
+    if (!D) return false;
+    if (D->T < 1 || D->d < 8 || D->E < 1 || D->k < 1 || D->E_loc < 1 || D->I < 8 || D->I_shared < 0) return false;
+    if (D->k > D->E || D->k > kMaxK || D->E > kMaxE) return false;
+    if (D->e_lo < 0 || D->e_lo + D->E_loc > D->E) return false;
+    if (D->d % 8 || D->I % 8 || D->I_shared % 8) return false;
+    if (D->dtype != PIPER_DTYPE_F32 && D->dtype != PIPER_DTYPE_BF16) return false;
+    if (D->gate_mode < 0 || D->gate_mode > 2) return false;
+    if (D->row_align < 1 || D->row_align > 1024) return false;
+    if (D->dw_dtype != D->dtype) return false;
+    if (D->gemm_impl != PIPER_GEMM_AUTO && D->gemm_impl != PIPER_GEMM_SIMT) return false;
+    if ((int64_t)D->T * D->k > (1ll << 30)) return false;
+    return true;
+}
+
+inline int n_chunks_of(const piper_moe_desc* D) { return cdiv(D->T * D->k, kScanChunk); }
+inline size_t round256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+struct WsLayout {
+    size_t chunk_counts, chunk_base, shared_offsets, tc_scratch, total;
+};
+WsLayout ws_layout(const piper_moe_desc* D) {
+    WsLayout L{};
+    const size_t per = round256(sizeof(int32_t) * (size_t)n_chunks_of(D) * D->E_loc);
+    size_t at = 0;
+    L.chunk_counts = at, at += per;
+    L.chunk_base = at, at += per;
+    L.shared_offsets = at, at += 256;
+    L.tc_scratch = at, at += tc_scratch_bytes(D);
+    L.total = at;
+    return L;
+}
+
+template <typename... P>
+bool all_aligned(P... ptrs) {
+    return (aligned16(ptrs) && ...);
+}
+
+inline Lane full_lane(piper_ctx* c, void* stream) { return Lane{static_cast<cudaStream_t>(stream), c->num_sms}; }
+
+}  // namespace
+
+extern "C" {
+
+int64_t piper_a_cap(const piper_moe_desc* D) {
+    if (!D) return 0;
+    const int64_t kk = D->k < D->E_loc ? D->k : D->E_loc;
+    return (int64_t)D->T * kk + (int64_t)D->E_loc * (D->row_align - 1);
+}
+
+int piper_workspace_bytes(const piper_moe_desc* D, size_t* bytes) {
+    if (!desc_ok(D) || !bytes) return PIPER_ERR_INVALID;
+    *bytes = ws_layout(D).total;
+    return PIPER_OK;
+}
+
+int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t workspace_bytes, piper_ctx** out) {
+    if (!desc_ok(D) || !out || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return PIPER_ERR_INVALID;
+    const WsLayout L = ws_layout(D);
+    if (workspace_bytes < L.total) return PIPER_ERR_WORKSPACE;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) return PIPER_ERR_CUDA;
+    piper_ctx* c = new (std::nothrow) piper_ctx();
+    if (!c) return PIPER_ERR_INVALID;
+    memset(c, 0, sizeof(*c));
+    c->D = *D;
+    c->device = device;
+    c->ws = static_cast<char*>(workspace);
+    c->ws_bytes = workspace_bytes;
+    c->n_chunks = n_chunks_of(D);
+    c->chunk_counts = reinterpret_cast<int32_t*>(c->ws + L.chunk_counts);
+    c->chunk_base = reinterpret_cast<int32_t*>(c->ws + L.chunk_base);
+    c->shared_offsets = reinterpret_cast<int32_t*>(c->ws + L.shared_offsets);
+    c->tc_scratch = c->ws + L.tc_scratch;
+    bool ok = cudaSetDevice(device) == cudaSuccess &&
+              cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess;
+    const int32_t so[2] = {0, D->T};
+    ok = ok && cudaMemcpy(c->shared_offsets, so, sizeof(so), cudaMemcpyHostToDevice) == cudaSuccess;
+    for (int i = 0; ok && i < kMaxEvents; ++i)
+        ok = cudaEventCreateWithFlags(&c->events[i], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && tc_init(c) == PIPER_OK;
+    if (!ok) {
+        piper_destroy(c);
+        return PIPER_ERR_CUDA;
+    }
+    *out = c;
+    return PIPER_OK;
+}
+
+int piper_destroy(piper_ctx* c) {
+    if (!c) return PIPER_ERR_INVALID;
+    pair_release(c);
+    for (int i = 0; i < kMaxEvents; ++i)
+        if (c->events[i]) cudaEventDestroy(c->events[i]);
+    delete c;
+    return PIPER_OK;
+}
+
+const char* piper_last_cuda_error(const piper_ctx* c) { return c ? c->err : "null context"; }
+int64_t piper_kernel_launches(const piper_ctx* c) { return c ? c->launches : 0; }
+int piper_pair_partition_mode(const piper_ctx* c) { return c ? c->pair_mode : 0; }
+
+int piper_route_topk(piper_ctx* c, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global,
+                     void* stream) {
+    if (!c || !all_aligned(logits, topk_idx, gates, counts_global)) return PIPER_ERR_INVALID;
+    return launch_route_topk(c, full_lane(c, stream), logits, topk_idx, gates, counts_global);
+}
+
+int piper_dispatch_pack(piper_ctx* c, const void* x, const int32_t* topk_idx, const float* gates, int32_t* counts,
+                        int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* xp, void* stream) {
+    if (!c || !all_aligned(x, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows, xp)) return PIPER_ERR_INVALID;
+    const Lane ln = full_lane(c, stream);
+    const int rc = launch_scan_rank(c, ln, topk_idx, counts, offsets, row_of, src_of);
+    if (rc != PIPER_OK) return rc;
+    return launch_pack(c, ln, x, gates, offsets, row_of, src_of, gate_rows, xp);
+}
+
+int piper_expert_ffn_fwd(piper_ctx* c, const void* xp, const int32_t* offsets, const void* w_gate, const void* w_up,
+                         const void* w_down, void* g_save, void* u_save, void* h_save, void* o, void* stream) {
+    if (!c || !all_aligned(xp, offsets, w_gate, w_up, w_down, g_save, u_save, h_save, o)) return PIPER_ERR_INVALID;
+    piper_chunk_args a{};
+    a.xp = const_cast<void*>(xp), a.offsets = const_cast<int32_t*>(offsets);
+    a.w_gate = w_gate, a.w_up = w_up, a.w_down = w_down;
+    a.g_save = g_save, a.u_save = u_save, a.h_save = h_save, a.o = o;
+    const FfnProblem p = routed_problem(c, &a);
+    const Lane ln = full_lane(c, stream);
+    const int rc = ffn_gemm1(c, ln, p);
+    return rc != PIPER_OK ? rc : ffn_gemm2(c, ln, p);
+}
+
+int piper_shared_ffn_fwd(piper_ctx* c, const void* x, const void* ws_gate, const void* ws_up, const void* ws_down,
+                         void* g_save, void* u_save, void* h_save, void* s, void* stream) {
+    if (!c || c->D.I_shared == 0 || !all_aligned(x, ws_gate, ws_up, ws_down, g_save, u_save, h_save, s))
+        return PIPER_ERR_INVALID;
+    piper_chunk_args a{};
+    a.x = x, a.ws_gate = ws_gate, a.ws_up = ws_up, a.ws_down = ws_down;
+    a.gs_save = g_save, a.us_save = u_save, a.hs_save = h_save, a.s = s;
+    const FfnProblem p = shared_problem(c, &a);
+    const Lane ln = full_lane(c, stream);
+    const int rc = ffn_gemm1(c, ln, p);
+    return rc != PIPER_OK ? rc : ffn_gemm2(c, ln, p);
+}
+
+int piper_combine(piper_ctx* c, const void* o, const int32_t* row_of, const float* gates, const void* s, void* y,
+                  void* stream) {
+    if (!c || !all_aligned(o, row_of, gates, y) || (s && !aligned16(s))) return PIPER_ERR_INVALID;
+    return launch_combine(c, full_lane(c, stream), o, row_of, gates, s, y, true);
+}
+
+int piper_combine_bwd(piper_ctx* c, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
+                      const float* gates, const int32_t* offsets, void* d_o, float* dgates, void* stream) {
+    if (!c || !all_aligned(dy, o, src_of, row_of, gates, offsets, d_o, dgates)) return PIPER_ERR_INVALID;
+    return launch_combine_bwd(c, full_lane(c, stream), dy, o, src_of, row_of, gates, offsets, d_o, dgates);
+}
+
+int piper_expert_ffn_bwd(piper_ctx* c, const void* d_o, const void* xp, const void* g_save, const void* u_save,
+                         const void* h_save, const int32_t* offsets, const void* w_gate, const void* w_up,
+                         const void* w_down, void* dg, void* du, void* dxp, void* dw_gate, void* dw_up, void* dw_down,
+                         int accumulate, void* stream) {
+    if (!c || !all_aligned(d_o, xp, g_save, u_save, h_save, offsets, w_gate, w_up, w_down, dg, du, dxp, dw_gate, dw_up,
+                           dw_down))
+        return PIPER_ERR_INVALID;
+    if (accumulate) return PIPER_ERR_UNSUPPORTED;
+    piper_chunk_args a{};
+    a.d_o = const_cast<void*>(d_o), a.xp = const_cast<void*>(xp), a.offsets = const_cast<int32_t*>(offsets);
+    a.g_save = const_cast<void*>(g_save), a.u_save = const_cast<void*>(u_save), a.h_save = const_cast<void*>(h_save);
+    a.w_gate = w_gate, a.w_up = w_up, a.w_down = w_down;
+    a.dg = dg, a.du = du, a.dxp = dxp, a.dw_gate = dw_gate, a.dw_up = dw_up, a.dw_down = dw_down;
+    const FfnProblem p = routed_problem(c, &a);
+    const Lane ln = full_lane(c, stream);
+    int rc = ffn_dgrad1(c, ln, p);
+    if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
+    if (rc == PIPER_OK) rc = ffn_wgrad(c, ln, p);
+    return rc;
+}
+
+int piper_shared_ffn_bwd(piper_ctx* c, const void* dy, const void* x, const void* g_save, const void* u_save,
+                         const void* h_save, const void* ws_gate, const void* ws_up, const void* ws_down, void* dgs,
+                         void* dus, void* dxs, void* dws_gate, void* dws_up, void* dws_down, int accumulate,
+                         void* stream) {
+    if (!c || c->D.I_shared == 0 ||
+        !all_aligned(dy, x, g_save, u_save, h_save, ws_gate, ws_up, ws_down, dgs, dus, dxs, dws_gate, dws_up, dws_down))
+        return PIPER_ERR_INVALID;
+    if (accumulate) return PIPER_ERR_UNSUPPORTED;
+    piper_chunk_args a{};
+    a.dy = dy, a.x = x;
+    a.gs_save = const_cast<void*>(g_save), a.us_save = const_cast<void*>(u_save), a.hs_save = const_cast<void*>(h_save);
+    a.ws_gate = ws_gate, a.ws_up = ws_up, a.ws_down = ws_down;
+    a.dgs = dgs, a.dus = dus, a.dxs = dxs, a.dws_gate = dws_gate, a.dws_up = dws_up, a.dws_down = dws_down;
+    const FfnProblem p = shared_problem(c, &a);
+    const Lane ln = full_lane(c, stream);
+    int rc = ffn_dgrad1(c, ln, p);
+    if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
+    if (rc == PIPER_OK) rc = ffn_wgrad(c, ln, p);
+    return rc;
+}
+
+int piper_dispatch_unpack(piper_ctx* c, const void* dxp, const int32_t* row_of, const void* dx_shared, void* dx,
+                          void* stream) {
+    if (!c || !all_aligned(dxp, row_of, dx) || (dx_shared && !aligned16(dx_shared))) return PIPER_ERR_INVALID;
+    return launch_combine(c, full_lane(c, stream), dxp, row_of, nullptr, dx_shared, dx, false);
+}
+
+int piper_route_bwd(piper_ctx* c, const float* logits, const int32_t* topk_idx, const float* gates, const float* dgates,
+                    float* dz_sel, void* stream) {
+    if (!c || !all_aligned(logits, topk_idx, gates, dgates, dz_sel)) return PIPER_ERR_INVALID;
+    return launch_route_bwd(c, full_lane(c, stream), logits, topk_idx, gates, dgates, dz_sel);
+}
+
+}  // extern "C"

@@ -1,0 +1,272 @@
+// chunk.cu — whole-chunk entry points: piper_run_chunk_fwd / _bwd (serial baseline, one stream, all SMs)
+// and P piper_run_chunk_pair (SURVEY.md §8a P, §8c c-sched; BASELINE.json:north_star part 5).
+//
+// The pair is the task DAG of SURVEY.md §8c on two logical streams:
+//   "comm"  (pack/combine side): F.route, F.scan, F.pack, F.combine, B.cgrad, B.unpack, B.route_bwd
+//   "gemm"  (compute side)     : F.gemm1, F.gemm2, F.shared, B.dgrad1, B.dgrad2, B.wgrad, B.shared_bwd
+// ordered by piper_list_schedule and synchronised by the event rule of PAPER.md:279-286:
+// a task waits only on dependencies that ran on the other stream, and records an event only if a
+// consumer runs on the other stream.  The SM split is enforced with green contexts (driver API reached
+// through cudaGetDriverEntryPoint, so the library has no link-time dependency on libcuda); if they are
+// unavailable the two streams are plain streams and every kernel bounds its own grid to its lane's SM
+// count.  The paper itself leaves SM allocation to the GPU.
+#include "piper_internal.cuh"
+
+using namespace piper;
+
+namespace piper {
+
+struct GreenPartition {
+    int sm_gemm = 0, sm_comm = 0;
+    CUgreenCtx gctx[2] = {nullptr, nullptr};  // 0 = comm, 1 = gemm
+    cudaStream_t stream[2] = {nullptr, nullptr};
+    bool green = false;
+};
+
+namespace {
+
+struct DriverApi {
+    CUresult (*DeviceGet)(CUdevice*, int) = nullptr;
+    CUresult (*DeviceGetDevResource)(CUdevice, CUdevResource*, CUdevResourceType) = nullptr;
+    CUresult (*DevSmResourceSplitByCount)(CUdevResource*, unsigned int*, const CUdevResource*, CUdevResource*,
+                                          unsigned int, unsigned int) = nullptr;
+    CUresult (*DevResourceGenerateDesc)(CUdevResourceDesc*, CUdevResource*, unsigned int) = nullptr;
+    CUresult (*GreenCtxCreate)(CUgreenCtx*, CUdevResourceDesc, CUdevice, unsigned int) = nullptr;
+    CUresult (*GreenCtxDestroy)(CUgreenCtx) = nullptr;
+    CUresult (*GreenCtxStreamCreate)(CUstream*, CUgreenCtx, unsigned int, int) = nullptr;
+    bool ok = false;
+};
+
+template <typename F>
+bool resolve(const char* name, F& fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint(name, &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !p)
+        return false;
+    fn = reinterpret_cast<F>(p);
+    return true;
+}
+
+DriverApi& driver() {
+    static DriverApi d = [] {
+        DriverApi a;
+        a.ok = resolve("cuDeviceGet", a.DeviceGet) && resolve("cuDeviceGetDevResource", a.DeviceGetDevResource) &&
+               resolve("cuDevSmResourceSplitByCount", a.DevSmResourceSplitByCount) &&
+               resolve("cuDevResourceGenerateDesc", a.DevResourceGenerateDesc) &&
+               resolve("cuGreenCtxCreate", a.GreenCtxCreate) && resolve("cuGreenCtxDestroy", a.GreenCtxDestroy) &&
+               resolve("cuGreenCtxStreamCreate", a.GreenCtxStreamCreate);
+        return a;
+    }();
+    return d;
+}
+
+void destroy_partition(GreenPartition* g) {
+    if (!g) return;
+    for (int i = 0; i < 2; ++i) {
+        if (g->stream[i]) cudaStreamDestroy(g->stream[i]);
+        if (g->gctx[i] && driver().ok) driver().GreenCtxDestroy(g->gctx[i]);
+    }
+    delete g;
+}
+
+// Split the device's SMs into {sm_comm, rest}; the gemm side keeps the first sm_gemm of the rest.
+GreenPartition* make_partition(piper_ctx* c, int sm_gemm, int sm_comm) {
+    GreenPartition* g = new GreenPartition();
+    g->sm_gemm = sm_gemm, g->sm_comm = sm_comm;
+    DriverApi& api = driver();
+    bool ok = api.ok;
+    CUdevice dev = 0;
+    CUdevResource all{}, part{}, rest{};
+    unsigned int n_groups = 1;
+    ok = ok && api.DeviceGet(&dev, c->device) == CUDA_SUCCESS;
+    ok = ok && api.DeviceGetDevResource(dev, &all, CU_DEV_RESOURCE_TYPE_SM) == CUDA_SUCCESS;
+    ok = ok && api.DevSmResourceSplitByCount(&part, &n_groups, &all, &rest, 0, (unsigned)sm_comm) == CUDA_SUCCESS &&
+         n_groups == 1 && (int)part.sm.smCount == sm_comm && (int)rest.sm.smCount >= sm_gemm;
+    if (ok && (int)rest.sm.smCount > sm_gemm) {  // trim the compute side to sm_gemm (multiples of the granularity)
+        CUdevResource keep{}, drop{};
+        unsigned int one = 1;
+        ok = api.DevSmResourceSplitByCount(&keep, &one, &rest, &drop, 0, (unsigned)sm_gemm) == CUDA_SUCCESS &&
+             one == 1 && (int)keep.sm.smCount == sm_gemm;
+        rest = keep;
+    }
+    CUdevResource res[2] = {part, rest};
+    for (int i = 0; ok && i < 2; ++i) {
+        CUdevResourceDesc desc{};
+        ok = api.DevResourceGenerateDesc(&desc, &res[i], 1) == CUDA_SUCCESS &&
+             api.GreenCtxCreate(&g->gctx[i], desc, dev, CU_GREEN_CTX_DEFAULT_STREAM) == CUDA_SUCCESS;
+        CUstream s = nullptr;
+        ok = ok && api.GreenCtxStreamCreate(&s, g->gctx[i], CU_STREAM_NON_BLOCKING, 0) == CUDA_SUCCESS;
+        g->stream[i] = reinterpret_cast<cudaStream_t>(s);
+    }
+    if (ok) {
+        g->green = true;
+        return g;
+    }
+    // fallback: plain streams, grids bounded by Lane::sms
+    for (int i = 0; i < 2; ++i) {
+        if (g->stream[i]) cudaStreamDestroy(g->stream[i]), g->stream[i] = nullptr;
+        if (g->gctx[i] && api.ok) api.GreenCtxDestroy(g->gctx[i]), g->gctx[i] = nullptr;
+    }
+    cudaGetLastError();
+    for (int i = 0; i < 2; ++i)
+        if (cudaStreamCreateWithFlags(&g->stream[i], cudaStreamNonBlocking) != cudaSuccess) {
+            destroy_partition(g);
+            return nullptr;
+        }
+    g->green = false;
+    return g;
+}
+
+// ---- the tasks ------------------------------------------------------------------------------------
+enum Task {
+    F_ROUTE, F_SCAN, F_PACK, F_GEMM1, F_GEMM2, F_SHARED, F_COMBINE,
+    B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD, N_TASKS
+};
+constexpr int COMM = 0, GEMM = 1;
+const int kStreamOf[N_TASKS] = {COMM, COMM, COMM, GEMM, GEMM, GEMM, COMM, COMM, GEMM, GEMM, GEMM, GEMM, COMM, COMM};
+const int kEdges[][2] = {{F_ROUTE, F_SCAN},   {F_SCAN, F_PACK},    {F_PACK, F_GEMM1},     {F_GEMM1, F_GEMM2},
+                         {F_GEMM2, F_COMBINE}, {F_SCAN, F_GEMM1},   {F_SCAN, F_COMBINE},   {F_SHARED, F_COMBINE},
+                         {B_CGRAD, B_DGRAD1},  {B_DGRAD1, B_DGRAD2}, {B_DGRAD2, B_UNPACK},  {B_CGRAD, B_WGRAD},
+                         {B_DGRAD1, B_WGRAD},  {B_SHARED, B_UNPACK}, {B_CGRAD, B_ROUTE_BWD}};
+
+int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b) {
+    switch (task) {
+        case F_ROUTE: return launch_route_topk(c, ln, f->logits, f->topk_idx, f->gates, f->counts_global);
+        case F_SCAN: return launch_scan_rank(c, ln, f->topk_idx, f->counts, f->offsets, f->row_of, f->src_of);
+        case F_PACK: return launch_pack(c, ln, f->x, f->gates, f->offsets, f->row_of, f->src_of, f->gate_rows, f->xp);
+        case F_GEMM1: return ffn_gemm1(c, ln, routed_problem(c, f));
+        case F_GEMM2: return ffn_gemm2(c, ln, routed_problem(c, f));
+        case F_SHARED: {
+            const FfnProblem p = shared_problem(c, f);
+            const int rc = ffn_gemm1(c, ln, p);
+            return rc != PIPER_OK ? rc : ffn_gemm2(c, ln, p);
+        }
+        case F_COMBINE:
+            return launch_combine(c, ln, f->o, f->row_of, f->gates, c->D.I_shared ? f->s : nullptr, f->y, true);
+        case B_CGRAD:
+            return launch_combine_bwd(c, ln, b->dy, b->o, b->src_of, b->row_of, b->gates, b->offsets, b->d_o, b->dgates);
+        case B_DGRAD1: return ffn_dgrad1(c, ln, routed_problem(c, b));
+        case B_DGRAD2: return ffn_dgrad2(c, ln, routed_problem(c, b));
+        case B_WGRAD: return ffn_wgrad(c, ln, routed_problem(c, b));
+        case B_SHARED: {
+            const FfnProblem p = shared_problem(c, b);
+            int rc = ffn_dgrad1(c, ln, p);
+            if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
+            if (rc == PIPER_OK) rc = ffn_wgrad(c, ln, p);
+            return rc;
+        }
+        case B_UNPACK:
+            return launch_combine(c, ln, b->dxp, b->row_of, nullptr, c->D.I_shared ? b->dxs : nullptr, b->dx, false);
+        case B_ROUTE_BWD: return launch_route_bwd(c, ln, b->logits, b->topk_idx, b->gates, b->dgates, b->dz_sel);
+    }
+    return PIPER_ERR_INVALID;
+}
+
+bool fwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
+    bool ok = a && aligned16(a->logits) && aligned16(a->x) && aligned16(a->w_gate) && aligned16(a->w_up) &&
+              aligned16(a->w_down) && aligned16(a->topk_idx) && aligned16(a->counts_global) && aligned16(a->counts) &&
+              aligned16(a->offsets) && aligned16(a->row_of) && aligned16(a->src_of) && aligned16(a->gates) &&
+              aligned16(a->gate_rows) && aligned16(a->xp) && aligned16(a->g_save) && aligned16(a->u_save) &&
+              aligned16(a->h_save) && aligned16(a->o) && aligned16(a->y);
+    if (ok && c->D.I_shared)
+        ok = aligned16(a->ws_gate) && aligned16(a->ws_up) && aligned16(a->ws_down) && aligned16(a->gs_save) &&
+             aligned16(a->us_save) && aligned16(a->hs_save) && aligned16(a->s);
+    return ok;
+}
+bool bwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
+    bool ok = fwd_args_ok(c, a) && aligned16(a->dy) && aligned16(a->dgates) && aligned16(a->dz_sel) &&
+              aligned16(a->d_o) && aligned16(a->dg) && aligned16(a->du) && aligned16(a->dxp) && aligned16(a->dx) &&
+              aligned16(a->dw_gate) && aligned16(a->dw_up) && aligned16(a->dw_down);
+    if (ok && c->D.I_shared)
+        ok = aligned16(a->dgs) && aligned16(a->dus) && aligned16(a->dxs) && aligned16(a->dws_gate) &&
+             aligned16(a->dws_up) && aligned16(a->dws_down);
+    return ok;
+}
+
+}  // namespace
+
+void pair_release(piper_ctx* c) {
+    destroy_partition(c->green);
+    c->green = nullptr;
+}
+
+}  // namespace piper
+
+extern "C" {
+
+int piper_run_chunk_fwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
+    if (!c || !fwd_args_ok(c, a)) return PIPER_ERR_INVALID;
+    const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    const int seq[] = {F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE};
+    for (int t : seq) {
+        if (t == F_SHARED && !c->D.I_shared) continue;
+        const int rc = run_task(c, t, ln, a, nullptr);
+        if (rc != PIPER_OK) return rc;
+    }
+    return PIPER_OK;
+}
+
+int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
+    if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
+    const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+    for (int t : seq) {
+        if (t == B_SHARED && !c->D.I_shared) continue;
+        const int rc = run_task(c, t, ln, nullptr, a);
+        if (rc != PIPER_OK) return rc;
+    }
+    return PIPER_OK;
+}
+
+int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_chunk_args* b, int sm_gemm, int sm_comm,
+                         void* stream) {
+    if (!c || !fwd_args_ok(c, f) || !bwd_args_ok(c, b)) return PIPER_ERR_INVALID;
+    if (sm_gemm < 1 || sm_comm < 8 || sm_comm % 8 || sm_gemm + sm_comm > c->num_sms) return PIPER_ERR_INVALID;
+    if (!c->green || c->green->sm_gemm != sm_gemm || c->green->sm_comm != sm_comm) {
+        pair_release(c);
+        c->green = make_partition(c, sm_gemm, sm_comm);
+        if (!c->green) return cuda_fail(c, cudaErrorUnknown, "make_partition");
+    }
+    GreenPartition* g = c->green;
+    c->pair_mode = g->green ? 1 : 2;
+
+    // task list of this layer (no shared expert -> its two tasks and their edges drop out)
+    const bool shared = c->D.I_shared != 0;
+    int32_t id_of[N_TASKS], task_of[N_TASKS], n = 0;
+    for (int t = 0; t < N_TASKS; ++t) {
+        id_of[t] = -1;
+        if (!shared && (t == F_SHARED || t == B_SHARED)) continue;
+        id_of[t] = n, task_of[n] = t, ++n;
+    }
+    int32_t edges[32][2], n_edges = 0, stream_of[N_TASKS], prio[N_TASKS];
+    for (const auto& e : kEdges)
+        if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
+    for (int i = 0; i < n; ++i) stream_of[i] = kStreamOf[task_of[i]], prio[i] = task_of[i] >= B_CGRAD ? 1 : 0;
+    int32_t order[N_TASKS], waits[32][2], n_waits = 0, records[N_TASKS];
+    int rc = piper_list_schedule(n, n_edges, &edges[0][0], stream_of, prio, order, &waits[0][0], &n_waits, records);
+    if (rc != PIPER_OK) return rc;
+
+    cudaStream_t user = static_cast<cudaStream_t>(stream);
+    const Lane lanes[2] = {{g->stream[COMM], sm_comm}, {g->stream[GEMM], sm_gemm}};
+    // fork: both partitions start after the work already queued on the caller's stream
+    cudaEvent_t fork = c->events[kMaxEvents - 1], join0 = c->events[kMaxEvents - 2], join1 = c->events[kMaxEvents - 3];
+    PIPER_CUDA(c, cudaEventRecord(fork, user));
+    PIPER_CUDA(c, cudaStreamWaitEvent(lanes[0].stream, fork, 0));
+    PIPER_CUDA(c, cudaStreamWaitEvent(lanes[1].stream, fork, 0));
+    for (int step = 0; step < n; ++step) {
+        const int v = order[step];
+        const Lane ln = lanes[stream_of[v]];
+        for (int w = 0; w < n_waits; ++w)  // wait for dependencies that ran on another stream
+            if (waits[w][1] == v) PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, c->events[waits[w][0]], 0));
+        rc = run_task(c, task_of[v], ln, f, b);
+        if (rc != PIPER_OK) return rc;
+        if (records[v]) PIPER_CUDA(c, cudaEventRecord(c->events[v], ln.stream));
+    }
+    PIPER_CUDA(c, cudaEventRecord(join0, lanes[0].stream));
+    PIPER_CUDA(c, cudaEventRecord(join1, lanes[1].stream));
+    PIPER_CUDA(c, cudaStreamWaitEvent(user, join0, 0));
+    PIPER_CUDA(c, cudaStreamWaitEvent(user, join1, 0));
+    return PIPER_OK;
+}
+
+}  // extern "C"

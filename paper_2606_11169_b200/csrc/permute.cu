@@ -1,0 +1,412 @@
+// permute.cu — F2 histogram + scan + rank, F3 dispatch_pack, F5 combine, B1 combine_bwd, B5 unpack
+// (SURVEY.md §8a, §8c Definition 2, 4, 5).  All HBM-bound row movers are TOKEN-major: a warp owns a
+// token, reads its source row once with 128-bit loads and touches each packed row exactly once, so the
+// traffic equals the algorithmic bytes of SURVEY.md §8d.  Ranks are deterministic (no atomics decide an
+// index): per-chunk histograms, a prefix over chunks, then __match_any_sync ranks inside a chunk.
+#include "piper_internal.cuh"
+
+namespace piper {
+namespace {
+
+constexpr int kMoveWarps = 8;  // warps per block of the row movers
+
+// ---- F2 phase 1: per-chunk histogram of local experts ------------------------------------------
+__global__ void __launch_bounds__(kScanChunk)
+chunk_hist_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_loc,
+                  int32_t* __restrict__ chunk_counts) {
+    extern __shared__ int32_t hist[];
+    for (int e = threadIdx.x; e < E_loc; e += blockDim.x) hist[e] = 0;
+    __syncthreads();
+    const int a = blockIdx.x * kScanChunk + threadIdx.x;
+    if (a < n_assign) {
+        const int i = topk_idx[a] - e_lo;
+        if (i >= 0 && i < E_loc) atomicAdd(&hist[i], 1);  // integer count: order-independent
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < E_loc; e += blockDim.x) chunk_counts[(size_t)blockIdx.x * E_loc + e] = hist[e];
+}
+
+// ---- F2 phase 2: prefix over chunks per expert, counts, aligned exclusive scan -> offsets --------
+// One block of 512 threads (E_loc <= kMaxE = 512): thread e walks its column of chunk_counts.
+__global__ void __launch_bounds__(512)
+chunk_scan_kernel(const int32_t* __restrict__ chunk_counts, int n_chunks, int E_loc, int row_align,
+                  int32_t* __restrict__ chunk_base, int32_t* __restrict__ counts, int32_t* __restrict__ offsets) {
+    __shared__ int32_t warp_tot[16];
+    const int e = threadIdx.x, lane = e & 31, w = e >> 5;
+    int run = 0;
+    if (e < E_loc) {
+        for (int c = 0; c < n_chunks; ++c) {
+            const int v = chunk_counts[(size_t)c * E_loc + e];
+            chunk_base[(size_t)c * E_loc + e] = run;
+            run += v;
+        }
+        counts[e] = run;
+    }
+    const int padded = e < E_loc ? (run + row_align - 1) / row_align * row_align : 0;
+    int inc = padded;  // inclusive warp scan by shuffles
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += o;
+    }
+    if (lane == 31) warp_tot[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int t = lane < 16 ? warp_tot[lane] : 0, ti = t;
+#pragma unroll
+        for (int off = 1; off < 16; off <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, ti, off);
+            if (lane >= off) ti += o;
+        }
+        if (lane < 16) warp_tot[lane] = ti - t;  // exclusive
+    }
+    __syncthreads();
+    const int excl = warp_tot[w] + inc - padded;
+    if (e < E_loc) offsets[e] = excl;
+    if (e == E_loc - 1) offsets[E_loc] = excl + padded;
+}
+
+// ---- F2 phase 3: stable rank of every assignment, row_of and src_of ------------------------------
+// Block = one chunk of kScanChunk assignments in flat order a = t*k + j.  Warps take turns (ascending
+// a): inside a warp __match_any_sync groups equal experts and the rank is the number of lower lanes
+// of the group; a shared running count per expert carries the rank across warps.
+__global__ void __launch_bounds__(kScanChunk)
+rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_loc,
+            const int32_t* __restrict__ chunk_base, const int32_t* __restrict__ offsets,
+            int32_t* __restrict__ row_of, int32_t* __restrict__ src_of) {
+    extern __shared__ int32_t run[];
+    for (int e = threadIdx.x; e < E_loc; e += blockDim.x)
+        run[e] = offsets[e] + chunk_base[(size_t)blockIdx.x * E_loc + e];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int a = blockIdx.x * kScanChunk + threadIdx.x;
+    int i = -1;
+    if (a < n_assign) {
+        i = topk_idx[a] - e_lo;
+        if (i < 0 || i >= E_loc) i = -1;
+    }
+    const unsigned peers = __match_any_sync(0xffffffffu, i);
+    const int below = __popc(peers & ((1u << lane) - 1u));
+    const int leader = __ffs(peers) - 1;
+    int row = -1;
+    for (int turn = 0; turn < kScanChunk / 32; ++turn) {
+        if (turn == w && i >= 0) {
+            int base = 0;
+            if (lane == leader) {
+                base = run[i];
+                run[i] = base + __popc(peers);
+            }
+            base = __shfl_sync(peers, base, leader);
+            row = base + below;
+        }
+        __syncthreads();
+    }
+    if (a < n_assign) {
+        row_of[a] = row;
+        if (row >= 0) src_of[row] = a;
+    }
+}
+
+// ---- element helpers for the row movers -----------------------------------------------------------
+// A 16-byte packet holds 8 bf16 or 4 fp32 values; acc[] always has 8 slots.
+template <bool BF16>
+__device__ __forceinline__ void unpack_add(const int4& v, float (&acc)[8], float scale) {
+    if (BF16) {
+        const uint32_t w[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float2 f = bf2_to_f2(w[q]);
+            acc[2 * q] = fmaf(scale, f.x, acc[2 * q]);
+            acc[2 * q + 1] = fmaf(scale, f.y, acc[2 * q + 1]);
+        }
+    } else {
+        acc[0] = fmaf(scale, __int_as_float(v.x), acc[0]);
+        acc[1] = fmaf(scale, __int_as_float(v.y), acc[1]);
+        acc[2] = fmaf(scale, __int_as_float(v.z), acc[2]);
+        acc[3] = fmaf(scale, __int_as_float(v.w), acc[3]);
+    }
+}
+template <bool BF16>
+__device__ __forceinline__ int4 pack_out(const float (&acc)[8]) {
+    int4 r;
+    if (BF16) {
+        r.x = (int)f2_to_bf2(acc[0], acc[1]);
+        r.y = (int)f2_to_bf2(acc[2], acc[3]);
+        r.z = (int)f2_to_bf2(acc[4], acc[5]);
+        r.w = (int)f2_to_bf2(acc[6], acc[7]);
+    } else {
+        r.x = __float_as_int(acc[0]), r.y = __float_as_int(acc[1]);
+        r.z = __float_as_int(acc[2]), r.w = __float_as_int(acc[3]);
+    }
+    return r;
+}
+template <bool BF16>
+__device__ __forceinline__ float dot_packets(const int4& a, const int4& b) {
+    float za[8] = {0, 0, 0, 0, 0, 0, 0, 0}, zb[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    unpack_add<BF16>(a, za, 1.f);
+    unpack_add<BF16>(b, zb, 1.f);
+    float s = 0.f;
+#pragma unroll
+    for (int q = 0; q < (BF16 ? 8 : 4); ++q) s = fmaf(za[q], zb[q], s);
+    return s;
+}
+
+// ---- F3 dispatch_pack ----------------------------------------------------------------------------
+// Work items [0,T): token t -> copy x[t] into each of its local rows, scatter its gates.
+// Work items [T, T+A_cap): row r -> if it is a pad row inside [0, offsets[E_loc]) zero it.
+__global__ void __launch_bounds__(kMoveWarps * 32)
+pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const int32_t* __restrict__ offsets,
+            const int32_t* __restrict__ row_of, const int32_t* __restrict__ src_of, int T, int k, int E_loc, int a_cap,
+            int row_packets, float* __restrict__ gate_rows, int4* __restrict__ xp) {
+    const int lane = threadIdx.x & 31;
+    const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
+    const int nwarps = gridDim.x * kMoveWarps;
+    const int used = offsets[E_loc];
+    for (int item = warp; item < T + a_cap; item += nwarps) {
+        if (item < T) {
+            const int t = item;
+            int rows[kMaxK];
+            int n = 0;
+#pragma unroll
+            for (int j = 0; j < kMaxK; ++j)
+                if (j < k) {
+                    const int r = row_of[(size_t)t * k + j];
+                    if (r >= 0) {
+                        rows[n++] = r;
+                        if (lane == 0) gate_rows[r] = gates[(size_t)t * k + j];
+                    }
+                }
+            if (n == 0) continue;
+            const int4* src = x + (size_t)t * row_packets;
+            for (int p0 = 0; p0 < row_packets; p0 += 128) {
+                int4 v[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int p = p0 + u * 32 + lane;
+                    if (p < row_packets) v[u] = ld_nc16(src + p);
+                }
+                for (int q = 0; q < n; ++q) {
+                    int4* dst = xp + (size_t)rows[q] * row_packets;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int p = p0 + u * 32 + lane;
+                        if (p < row_packets) st16(dst + p, v[u]);
+                    }
+                }
+            }
+        } else {
+            const int r = item - T;
+            if (r >= used || src_of[r] >= 0) continue;
+            if (lane == 0) gate_rows[r] = 0.f;
+            int4* dst = xp + (size_t)r * row_packets;
+            for (int p = lane; p < row_packets; p += 32) st16(dst + p, make_int4(0, 0, 0, 0));
+        }
+    }
+}
+
+// ---- F5 combine / B5 unpack ------------------------------------------------------------------------
+// y[t] = sum_{j local} w_j * o[row_of[t,j]] (+ s[t]);  WEIGHTED: w_j = gates[t,j], else 1 (unpack).
+// fp32 accumulation, one rounding on store.
+template <bool BF16, bool WEIGHTED>
+__global__ void __launch_bounds__(kMoveWarps * 32)
+combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, const float* __restrict__ gates,
+               const int4* __restrict__ s, int T, int k, int row_packets, int4* __restrict__ y) {
+    const int lane = threadIdx.x & 31;
+    const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
+    const int nwarps = gridDim.x * kMoveWarps;
+    for (int t = warp; t < T; t += nwarps) {
+        int rows[kMaxK];
+        float w[kMaxK];
+        int n = 0;
+#pragma unroll
+        for (int j = 0; j < kMaxK; ++j)
+            if (j < k) {
+                const int r = row_of[(size_t)t * k + j];
+                if (r >= 0) {
+                    w[n] = WEIGHTED ? gates[(size_t)t * k + j] : 1.f;
+                    rows[n++] = r;
+                }
+            }
+        for (int p0 = 0; p0 < row_packets; p0 += 64) {
+            float acc[2][8];
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int q = 0; q < 8; ++q) acc[u][q] = 0.f;
+            for (int q = 0; q < n; ++q) {
+                const int4* src = o + (size_t)rows[q] * row_packets;
+                int4 v[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int p = p0 + u * 32 + lane;
+                    if (p < row_packets) v[u] = ld_nc16(src + p);
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (p0 + u * 32 + lane < row_packets) unpack_add<BF16>(v[u], acc[u], w[q]);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int p = p0 + u * 32 + lane;
+                if (p < row_packets) {
+                    if (s != nullptr) unpack_add<BF16>(ld_nc16(s + (size_t)t * row_packets + p), acc[u], 1.f);
+                    st16(y + (size_t)t * row_packets + p, pack_out<BF16>(acc[u]));
+                }
+            }
+        }
+    }
+}
+
+// ---- B1 combine_bwd ---------------------------------------------------------------------------------
+// Token items: d_o[row] = gates[t,j] * dy[t]; dgates[t,j] = <dy[t], o[row]> (0 for non-local slots).
+// Row items: zero the pad rows of d_o inside [0, offsets[E_loc]).
+template <bool BF16>
+__global__ void __launch_bounds__(kMoveWarps * 32)
+combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, const int32_t* __restrict__ src_of,
+                   const int32_t* __restrict__ row_of, const float* __restrict__ gates,
+                   const int32_t* __restrict__ offsets, int T, int k, int E_loc, int a_cap, int row_packets,
+                   int4* __restrict__ d_o, float* __restrict__ dgates) {
+    const int lane = threadIdx.x & 31;
+    const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
+    const int nwarps = gridDim.x * kMoveWarps;
+    const int used = offsets[E_loc];
+    for (int item = warp; item < T + a_cap; item += nwarps) {
+        if (item < T) {
+            const int t = item;
+            int rows[kMaxK], slot[kMaxK];
+            float w[kMaxK], dots[kMaxK];
+            int n = 0;
+#pragma unroll
+            for (int j = 0; j < kMaxK; ++j)
+                if (j < k) {
+                    const int r = row_of[(size_t)t * k + j];
+                    if (r >= 0) {
+                        w[n] = gates[(size_t)t * k + j];
+                        slot[n] = j;
+                        dots[n] = 0.f;
+                        rows[n++] = r;
+                    } else if (lane == 0) {
+                        dgates[(size_t)t * k + j] = 0.f;
+                    }
+                }
+            if (n == 0) continue;
+            const int4* src = dy + (size_t)t * row_packets;
+            for (int p0 = 0; p0 < row_packets; p0 += 64) {
+                int4 v[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int p = p0 + u * 32 + lane;
+                    if (p < row_packets) v[u] = ld_nc16(src + p);
+                }
+                for (int q = 0; q < n; ++q) {
+                    const int4* orow = o + (size_t)rows[q] * row_packets;
+                    int4* drow = d_o + (size_t)rows[q] * row_packets;
+                    int4 ov[2];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int p = p0 + u * 32 + lane;
+                        if (p < row_packets) ov[u] = ld_nc16(orow + p);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int p = p0 + u * 32 + lane;
+                        if (p < row_packets) {
+                            dots[q] += dot_packets<BF16>(v[u], ov[u]);
+                            float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+                            unpack_add<BF16>(v[u], acc, w[q]);
+                            st16(drow + p, pack_out<BF16>(acc));
+                        }
+                    }
+                }
+            }
+            for (int q = 0; q < n; ++q) {
+                float sdot = dots[q];
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) sdot += __shfl_xor_sync(0xffffffffu, sdot, off);
+                if (lane == 0) dgates[(size_t)t * k + slot[q]] = sdot;
+            }
+        } else {
+            const int r = item - T;
+            if (r >= used || src_of[r] >= 0) continue;
+            int4* dst = d_o + (size_t)r * row_packets;
+            for (int p = lane; p < row_packets; p += 32) st16(dst + p, make_int4(0, 0, 0, 0));
+        }
+    }
+}
+
+inline int mover_blocks(Lane ln, int items) {
+    int blocks = cdiv(items, kMoveWarps);
+    const int cap = ln.sms * 8;  // 8 blocks x 8 warps = 64 resident warps per SM
+    return blocks < cap ? (blocks < 1 ? 1 : blocks) : cap;
+}
+
+}  // namespace
+
+int launch_scan_rank(piper_ctx* c, Lane ln, const int32_t* topk_idx, int32_t* counts, int32_t* offsets, int32_t* row_of,
+                     int32_t* src_of) {
+    const piper_moe_desc& D = c->D;
+    const int n_assign = D.T * D.k;
+    const size_t hist_bytes = sizeof(int32_t) * D.E_loc;
+    PIPER_CUDA(c, cudaMemsetAsync(src_of, 0xFF, sizeof(int32_t) * (size_t)piper_a_cap(&D), ln.stream));
+    chunk_hist_kernel<<<c->n_chunks, kScanChunk, hist_bytes, ln.stream>>>(topk_idx, n_assign, D.e_lo, D.E_loc,
+                                                                         c->chunk_counts);
+    PIPER_LAUNCHED(c, "chunk_hist_kernel");
+    chunk_scan_kernel<<<1, 512, 0, ln.stream>>>(c->chunk_counts, c->n_chunks, D.E_loc, D.row_align, c->chunk_base,
+                                                 counts, offsets);
+    PIPER_LAUNCHED(c, "chunk_scan_kernel");
+    rank_kernel<<<c->n_chunks, kScanChunk, hist_bytes, ln.stream>>>(topk_idx, n_assign, D.e_lo, D.E_loc, c->chunk_base,
+                                                                   offsets, row_of, src_of);
+    PIPER_LAUNCHED(c, "rank_kernel");
+    return PIPER_OK;
+}
+
+int launch_pack(piper_ctx* c, Lane ln, const void* x, const float* gates, const int32_t* offsets, const int32_t* row_of,
+                const int32_t* src_of, float* gate_rows, void* xp) {
+    const piper_moe_desc& D = c->D;
+    const int a_cap = (int)piper_a_cap(&D);
+    const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
+    pack_kernel<<<mover_blocks(ln, D.T + a_cap), kMoveWarps * 32, 0, ln.stream>>>(
+        static_cast<const int4*>(x), gates, offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, gate_rows,
+        static_cast<int4*>(xp));
+    PIPER_LAUNCHED(c, "pack_kernel");
+    return PIPER_OK;
+}
+
+int launch_combine(piper_ctx* c, Lane ln, const void* o, const int32_t* row_of, const float* gates, const void* s,
+                   void* y, bool weighted) {
+    const piper_moe_desc& D = c->D;
+    const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
+    const int blocks = mover_blocks(ln, D.T);
+    const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s);
+    int4* y4 = static_cast<int4*>(y);
+#define PIPER_COMBINE(BF, W) \
+    combine_kernel<BF, W><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, D.T, D.k, row_packets, y4)
+    if (D.dtype == PIPER_DTYPE_BF16) {
+        if (weighted) PIPER_COMBINE(true, true); else PIPER_COMBINE(true, false);
+    } else {
+        if (weighted) PIPER_COMBINE(false, true); else PIPER_COMBINE(false, false);
+    }
+#undef PIPER_COMBINE
+    PIPER_LAUNCHED(c, "combine_kernel");
+    return PIPER_OK;
+}
+
+int launch_combine_bwd(piper_ctx* c, Lane ln, const void* dy, const void* o, const int32_t* src_of,
+                       const int32_t* row_of, const float* gates, const int32_t* offsets, void* d_o, float* dgates) {
+    const piper_moe_desc& D = c->D;
+    const int a_cap = (int)piper_a_cap(&D);
+    const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
+    const int blocks = mover_blocks(ln, D.T + a_cap);
+    if (D.dtype == PIPER_DTYPE_BF16)
+        combine_bwd_kernel<true><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(
+            static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
+            D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
+    else
+        combine_bwd_kernel<false><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(
+            static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
+            D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
+    PIPER_LAUNCHED(c, "combine_bwd_kernel");
+    return PIPER_OK;
+}
+
+}  // namespace piper

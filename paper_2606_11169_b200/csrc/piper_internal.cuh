@@ -1,0 +1,152 @@
+// piper_internal.cuh — shared declarations of the CUDA library (not part of the C-ABI).
+// The oracle (oracle/) includes nothing from this directory and this directory nothing from it.
+#pragma once
+#include <cuda.h>  // CUtensorMap type and enums only; the driver is reached through cudaGetDriverEntryPoint
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "piper.h"
+
+namespace piper {
+
+constexpr int kMaxK = 8;          // top-k bound (register arrays in route / combine kernels)
+constexpr int kMaxE = 512;        // expert bound of the router kernel (16 values per lane)
+constexpr int kScanChunk = 1024;  // assignments per block of the histogram / rank kernels
+constexpr int kMaxEvents = 20;    // one per pair task + fork/join
+
+// Where a task's kernels run: stream + the number of SMs its persistent grids may occupy.
+struct Lane {
+    cudaStream_t stream;
+    int sms;
+};
+
+struct GreenPartition;  // chunk_pair.cu
+
+}  // namespace piper
+
+struct piper_ctx {
+    piper_moe_desc D;
+    int device;
+    int num_sms;
+    char* ws;
+    size_t ws_bytes;
+    int n_chunks;            // ceil(T*k / kScanChunk)
+    int32_t* chunk_counts;   // [n_chunks][E_loc]  per-chunk local-expert histogram
+    int32_t* chunk_base;     // [n_chunks][E_loc]  exclusive prefix over chunks
+    int32_t* shared_offsets; // [2] = {0, T}: the shared expert as one group
+    int64_t launches;
+    int pair_mode;
+    char err[256];
+    void* encode_tiled;      // cuTensorMapEncodeTiled, resolved at create time
+    piper::GreenPartition* green;
+    char* tc_scratch;        // tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
+    int tc_next_slot;        // round-robin slot in tc_scratch
+    cudaEvent_t events[piper::kMaxEvents];
+};
+
+namespace piper {
+
+inline int cuda_fail(piper_ctx* c, cudaError_t e, const char* what) {
+    snprintf(c->err, sizeof(c->err), "%s: %s", what, cudaGetErrorString(e));
+    return PIPER_ERR_CUDA;
+}
+#define PIPER_CUDA(ctx, call)                                            \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return piper::cuda_fail(ctx, e__, #call); \
+    } while (0)
+// after a kernel launch
+#define PIPER_LAUNCHED(ctx, name)                                          \
+    do {                                                                   \
+        (ctx)->launches += 1;                                              \
+        cudaError_t e__ = cudaGetLastError();                              \
+        if (e__ != cudaSuccess) return piper::cuda_fail(ctx, e__, name);   \
+    } while (0)
+
+inline bool aligned16(const void* p) { return p != nullptr && (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline size_t esize(int dtype) { return dtype == PIPER_DTYPE_BF16 ? 2 : 4; }
+inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+// ---- launchers implemented per translation unit -------------------------------------------------
+// route.cu
+int launch_route_topk(piper_ctx*, Lane, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global);
+int launch_route_bwd(piper_ctx*, Lane, const float* logits, const int32_t* topk_idx, const float* gates,
+                     const float* dgates, float* dz);
+// permute.cu
+int launch_scan_rank(piper_ctx*, Lane, const int32_t* topk_idx, int32_t* counts, int32_t* offsets, int32_t* row_of,
+                     int32_t* src_of);
+int launch_pack(piper_ctx*, Lane, const void* x, const float* gates, const int32_t* offsets, const int32_t* row_of,
+                const int32_t* src_of, float* gate_rows, void* xp);
+int launch_combine(piper_ctx*, Lane, const void* o, const int32_t* row_of, const float* gates, const void* s, void* y,
+                   bool weighted);
+int launch_combine_bwd(piper_ctx*, Lane, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
+                       const float* gates, const int32_t* offsets, void* d_o, float* dgates);
+
+// One grouped SwiGLU FFN problem: `G` groups; group g owns rows [offsets[g], offsets[g+1]) of the row
+// buffers and weight slice g.  The shared expert is the same problem with G = 1, offsets = {0, T}.
+struct FfnProblem {
+    int G, d, I;
+    int max_rows;            // host-side bound on offsets[G] (sizes the tensor maps and SIMT grids)
+    int max_group_rows;      // host-side bound on the rows of one group
+    const int32_t* offsets;  // device, [G+1]
+    const void *xp, *w_gate, *w_up, *w_down;
+    void *g, *u, *h, *o;                                 // forward outputs
+    const void* d_o;                                     // backward inputs / outputs
+    void *dg, *du, *dxp, *dw_gate, *dw_up, *dw_down;
+};
+// gemm_simt.cu (FP32 ALUs; fp32 or bf16 storage)
+// `which`: bit 0 = first GEMM of the pass (fwd1 / dgrad1), bit 1 = second (fwd2 / dgrad2)
+int simt_ffn_fwd(piper_ctx*, Lane, const FfnProblem&, int which);
+int simt_ffn_dgrad(piper_ctx*, Lane, const FfnProblem&, int which);
+int simt_ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);
+// gemm_tc.cu (tcgen05 / TMEM / TMA; bf16 storage)
+size_t tc_scratch_bytes(const piper_moe_desc*);
+int tc_init(piper_ctx*);  // resolves cuTensorMapEncodeTiled, sets kernel attributes
+bool tc_supported(const piper_ctx*, const FfnProblem&);
+int tc_ffn_fwd1(piper_ctx*, Lane, const FfnProblem&);    // G,U,H = swiglu(xp W_gate, xp W_up)
+int tc_ffn_fwd2(piper_ctx*, Lane, const FfnProblem&);    // O = H W_down
+int tc_ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&);  // dG,dU from dO W_down^T and G,U
+int tc_ffn_dgrad2(piper_ctx*, Lane, const FfnProblem&);  // dXp = dG W_gate^T + dU W_up^T
+int tc_ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);   // dW_gate, dW_up, dW_down
+
+// ffn.cu: dispatch between the two GEMM families, task granularity used by the chunk scheduler
+int ffn_gemm1(piper_ctx*, Lane, const FfnProblem&);
+int ffn_gemm2(piper_ctx*, Lane, const FfnProblem&);
+int ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&);
+int ffn_dgrad2(piper_ctx*, Lane, const FfnProblem&);
+int ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);
+FfnProblem routed_problem(const piper_ctx*, const piper_chunk_args*);
+FfnProblem shared_problem(const piper_ctx*, const piper_chunk_args*);
+// chunk.cu
+void pair_release(piper_ctx*);
+
+// ---- small device helpers -----------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ int4 ld_nc16(const void* p) {
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st16(void* p, const int4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w)
+                 : "memory");
+}
+// bf16x2 <-> float2 (exact widening; RNE narrowing)
+__device__ __forceinline__ float2 bf2_to_f2(uint32_t v) {
+    return make_float2(__uint_as_float(v << 16), __uint_as_float(v & 0xFFFF0000u));
+}
+__device__ __forceinline__ uint32_t f2_to_bf2(float lo, float hi) {
+    __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&b);
+}
+#endif
+
+}  // namespace piper

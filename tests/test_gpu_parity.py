@@ -1,0 +1,196 @@
+"""GPU parity tests: the CUDA path through the C-ABI (paper_2606_11169_b200.binding) against the CPU
+oracle (oracle/) on the same seeded inputs (inputs/).  Integer / index outputs bit-exact; floating
+point within the north_star tolerances (tests/util.py: TOL)."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_11169_b200 as piper
+from inputs import configs
+from oracle import oracle
+from tests import util
+
+pytestmark = pytest.mark.gpu
+
+SMALL = ["C1", "C1s", "C2s", "C3s", "C4s"]
+
+
+def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True):
+    """Runs the whole path; returns (ctx, dict of device tensors)."""
+    ctx = piper.Context(util.desc_of(cfg, gemm_impl))
+    dev = util.upload_inputs(inp)
+    b = piper.alloc_buffers(ctx, backward=True)
+    b.update(dev)
+    if use_chunk_calls:
+        args = piper.chunk_args(b)
+        piper.piper_run_chunk_fwd(ctx, args)
+        if backward:
+            piper.piper_run_chunk_bwd(ctx, args)
+    else:
+        piper.piper_route_topk(ctx, b["logits"], b["topk_idx"], b["gates"], b["counts_global"])
+        piper.piper_dispatch_pack(ctx, b["x"], b["topk_idx"], b["gates"], b["counts"], b["offsets"], b["row_of"],
+                                  b["src_of"], b["gate_rows"], b["xp"])
+        piper.piper_expert_ffn_fwd(ctx, b["xp"], b["offsets"], b["w_gate"], b["w_up"], b["w_down"], b["g_save"],
+                                   b["u_save"], b["h_save"], b["o"])
+        if cfg.I_shared:
+            piper.piper_shared_ffn_fwd(ctx, b["x"], b["ws_gate"], b["ws_up"], b["ws_down"], b["gs_save"], b["us_save"],
+                                       b["hs_save"], b["s"])
+        piper.piper_combine(ctx, b["o"], b["row_of"], b["gates"], b.get("s"), b["y"])
+        if backward:
+            piper.piper_combine_bwd(ctx, b["dy"], b["o"], b["src_of"], b["row_of"], b["gates"], b["offsets"], b["d_o"],
+                                    b["dgates"])
+            piper.piper_expert_ffn_bwd(ctx, b["d_o"], b["xp"], b["g_save"], b["u_save"], b["h_save"], b["offsets"],
+                                       b["w_gate"], b["w_up"], b["w_down"], b["dg"], b["du"], b["dxp"], b["dw_gate"],
+                                       b["dw_up"], b["dw_down"])
+            if cfg.I_shared:
+                piper.piper_shared_ffn_bwd(ctx, b["dy"], b["x"], b["gs_save"], b["us_save"], b["hs_save"], b["ws_gate"],
+                                           b["ws_up"], b["ws_down"], b["dgs"], b["dus"], b["dxs"], b["dws_gate"],
+                                           b["dws_up"], b["dws_down"])
+            piper.piper_dispatch_unpack(ctx, b["dxp"], b["row_of"], b.get("dxs"), b["dx"])
+            piper.piper_route_bwd(ctx, b["logits"], b["topk_idx"], b["gates"], b["dgates"], b["dz_sel"])
+    torch.cuda.synchronize()
+    return ctx, b
+
+
+def _check_routing(cfg, b, ref):
+    A = int(ref["offsets"][-1])
+    for name in ("topk_idx", "counts_global", "counts", "row_of"):
+        assert np.array_equal(util.to_np(b[name]).reshape(-1), ref[name].reshape(-1)), name
+    assert np.array_equal(util.to_np(b["offsets"])[: cfg.e_loc + 1], ref["offsets"])
+    assert np.array_equal(util.to_np(b["src_of"]), ref["src_of"])
+    util.check_close("gates", util.to_np(b["gates"]), ref["gates"], configs.DT_F32)
+    util.check_close("gate_rows", util.to_np(b["gate_rows"])[:A], ref["gate_rows"][:A], configs.DT_F32)
+    return A
+
+
+def _check_all(cfg, b, f, g, label=""):
+    A = _check_routing(cfg, b, f)
+    dt = cfg.dtype
+    assert np.array_equal(util.to_np(b["xp"])[:A], f["xp"][:A]), "xp must be a bit-exact copy"
+    out = {}
+    out["o"] = util.check_close(label + "o", util.to_np(b["o"])[:A], f["o"][:A], dt)
+    out["y"] = util.check_close(label + "y", util.to_np(b["y"]), f["y"], dt)
+    if g is None:
+        return out
+    out["dgates"] = util.check_close(label + "dgates", util.to_np(b["dgates"]), g["dgates"], dt)
+    out["dz"] = util.check_close(label + "dz_sel", util.to_np(b["dz_sel"]), g["dz"], dt)
+    out["dxp"] = util.check_close(label + "dxp", util.to_np(b["dxp"])[:A], g["dxp"][:A], dt)
+    out["dx"] = util.check_close(label + "dx", util.to_np(b["dx"]), g["dx"], dt)
+    for n in ("dw_gate", "dw_up", "dw_down"):
+        out[n] = util.check_close(label + n, util.to_np(b[n]), g[n], dt)
+    if cfg.I_shared:
+        for n in ("dws_gate", "dws_up", "dws_down"):
+            out[n] = util.check_close(label + n, util.to_np(b[n]), g[n][0], dt)
+    # exact zeros for empty experts (Definition 5)
+    for i in np.nonzero(f["counts"] == 0)[0]:
+        for n in ("dw_gate", "dw_up", "dw_down"):
+            assert not util.to_np(b[n][int(i)]).any(), f"{n}[{i}] must be exactly zero for an empty expert"
+    return out
+
+
+@pytest.mark.parametrize("name", SMALL)
+@pytest.mark.parametrize("impl", [piper.GEMM_AUTO, piper.GEMM_SIMT])
+@pytest.mark.parametrize("align", [1, 64])
+def test_small_configs_full_tensor_parity(name, impl, align):
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=align)
+    if cfg.dtype == configs.DT_F32 and impl == piper.GEMM_SIMT:
+        pytest.skip("fp32 already runs the FP32-ALU kernels under GEMM_AUTO")
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp, gemm_impl=impl)
+    _check_all(cfg, b, f, g)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C1", "C3s", "C4s"])
+def test_chunk_calls_equal_step_calls_bitwise(name):
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=64 if name != "C1" else 1)
+    inp = configs.make_inputs(cfg)
+    ctx1, b1 = _run_steps(cfg, inp)
+    ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True)
+    A = int(b1["offsets"][cfg.e_loc])
+    for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y", "dgates", "dz_sel", "dx", "dw_gate", "dw_up",
+              "dw_down"):
+        assert torch.equal(b1[n], b2[n]), n
+    for n in ("xp", "o", "dxp"):
+        assert torch.equal(b1[n][:A], b2[n][:A]), n
+    ctx1.close(), ctx2.close()
+
+
+@pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
+@pytest.mark.parametrize("split", [(132, 16), (100, 48)])
+def test_pair_is_bitwise_equal_to_serial(name, split):
+    """the overlapped, out-of-order plan must respect every dependency -> identical results."""
+    base = configs.BY_NAME[name]
+    cfg_a = dataclasses.replace(base, row_align=64, seed=base.seed + 100)
+    cfg_b = dataclasses.replace(base, row_align=64, seed=base.seed + 200)
+    inp_a, inp_b = configs.make_inputs(cfg_a), configs.make_inputs(cfg_b)
+    # serial: fwd(A) ; fwd(B) (untimed producer of B's saved activations) ; bwd(B)
+    ctx, ba = _run_steps(cfg_a, inp_a, use_chunk_calls=True, backward=False)
+    _, bb = _run_steps(cfg_b, inp_b, use_chunk_calls=True, backward=True)
+    # pair on fresh buffers: B's forward first, then [F(A), B(B)] co-scheduled
+    pa, pb = piper.alloc_buffers(ctx), piper.alloc_buffers(ctx)
+    pa.update(util.upload_inputs(inp_a)), pb.update(util.upload_inputs(inp_b))
+    args_a, args_b = piper.chunk_args(pa), piper.chunk_args(pb)
+    piper.piper_run_chunk_fwd(ctx, args_b)
+    piper.piper_run_chunk_pair(ctx, args_a, args_b, split[0], split[1])
+    torch.cuda.synchronize()
+    assert piper.piper_pair_partition_mode(ctx) in (1, 2)
+    for n in ("topk_idx", "gates", "counts", "offsets", "row_of", "src_of", "y"):
+        assert torch.equal(ba[n], pa[n]), "fwd " + n
+    for n in ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down"):
+        assert torch.equal(bb[n], pb[n]), "bwd " + n
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C4z"])
+def test_full_size_routing_and_permutation_bit_exact(name):
+    cfg = configs.BY_NAME[name]
+    inp = configs.make_inputs(cfg, weights=False, with_dy=False)
+    ref = oracle.routing(cfg, inp)
+    ctx = piper.Context(util.desc_of(cfg))
+    x = util.to_dev(inp["x"])
+    logits = util.to_dev(inp["logits"])
+    A_cap = ctx.a_cap
+    i32 = dict(dtype=torch.int32, device="cuda")
+    topk_idx, row_of = torch.empty((cfg.T, cfg.k), **i32), torch.empty((cfg.T, cfg.k), **i32)
+    cg, counts, offsets = torch.empty(cfg.E, **i32), torch.empty(cfg.e_loc, **i32), torch.empty(cfg.e_loc + 4, **i32)
+    src_of = torch.empty(A_cap, **i32)
+    gates = torch.empty((cfg.T, cfg.k), dtype=torch.float32, device="cuda")
+    gate_rows = torch.empty(A_cap, dtype=torch.float32, device="cuda")
+    xp = torch.empty((A_cap, cfg.d), dtype=ctx.torch_dtype, device="cuda")
+    piper.piper_route_topk(ctx, logits, topk_idx, gates, cg)
+    piper.piper_dispatch_pack(ctx, x, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows, xp)
+    torch.cuda.synchronize()
+    b = dict(topk_idx=topk_idx, counts_global=cg, counts=counts, offsets=offsets, row_of=row_of, src_of=src_of,
+             gates=gates, gate_rows=gate_rows)
+    ref["gate_rows"] = np.where(ref["src_of"] >= 0, ref["gates"].reshape(-1)[np.maximum(ref["src_of"], 0)], 0.0)
+    A = _check_routing(cfg, b, ref)
+    assert int(ref["counts_global"].sum()) == cfg.T * cfg.k
+    # xp is the all-to-all payload: bit-exact rows
+    src = torch.from_numpy(ref["src_of"][:A].astype(np.int64)).cuda()
+    assert torch.equal(xp[:A].view(torch.int16), x[src // cfg.k].view(torch.int16))
+    ctx.close()
+
+
+def test_empty_input_edge_cases():
+    """One token, k = E (every expert selected once), and a local slice that receives nothing."""
+    cfg = configs.MoeConfig("edge1", T=1, d=64, E=4, k=4, I=64, seed=21, dtype=configs.DT_F32)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp)
+    _check_all(cfg, b, f, g)
+    ctx.close()
+    cfg = configs.MoeConfig("edge2", T=40, d=64, E=8, k=1, I=64, seed=22, e_lo=6, E_loc=2, n_dead=2, bias="zipf1.2")
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    assert int(f["offsets"][-1]) == 0  # nothing is routed to the dead local experts
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp)
+    _check_all(cfg, b, f, g)
+    assert not util.to_np(b["y"]).any() and not util.to_np(b["dx"]).any()
+    ctx.close()
