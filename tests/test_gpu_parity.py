@@ -1,6 +1,6 @@
 """GPU parity tests: the CUDA path through the C-ABI (paper_2606_11169_b200.binding) against the CPU
 oracle (oracle/) on the same seeded inputs (inputs/).  Integer / index outputs bit-exact; floating
-point within the north_star tolerances (tests/util.py: TOL)."""
+point within the north_star tolerances (tests/piper_testutil.py: TOL)."""
 import dataclasses
 
 import numpy as np
@@ -10,7 +10,7 @@ import torch
 import paper_2606_11169_b200 as piper
 from inputs import configs
 from oracle import oracle
-from tests import util
+import piper_testutil as util
 
 pytestmark = pytest.mark.gpu
 
