@@ -139,8 +139,10 @@ def test_pair_is_bitwise_equal_to_serial(name, split):
     piper.piper_run_chunk_pair(ctx, args_a, args_b, split[0], split[1])
     torch.cuda.synchronize()
     assert piper.piper_pair_partition_mode(ctx) in (1, 2)
-    for n in ("topk_idx", "gates", "counts", "offsets", "row_of", "src_of", "y"):
+    for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y"):
         assert torch.equal(ba[n], pa[n]), "fwd " + n
+    nofs = base.e_loc + 1  # the offsets buffers are over-allocated; entries past E_loc+1 are never written
+    assert torch.equal(ba["offsets"][:nofs], pa["offsets"][:nofs]), "fwd offsets"
     for n in ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down"):
         assert torch.equal(bb[n], pb[n]), "bwd " + n
     ctx.close()
