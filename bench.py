@@ -1,0 +1,419 @@
+"""bench.py — MoE fwd+bwd tokens/s of the per-device expert-parallel chunk on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2|C3|C4|C4z] [--impl piper|reference] [--pair]
+
+A step = one pass of the whole hot path over one microbatch: forward chunk F1-F5 then backward chunk
+B1-B6 through the C-ABI (piper_run_chunk_fwd + piper_run_chunk_bwd).  Default workload:
+C2 = BASELINE.json configs[1] (Mixtral-8x7B-shaped layer), seeded synthetic inputs (inputs/configs.py).
+Multi-GPU (torchrun): every rank runs its own microbatch (same layer shape, seed + 1000*rank), no
+data-path collective, value = all ranks' tokens / max-over-ranks time: weak scaling.
+
+One JSON line on stdout (rank 0); everything else goes to stderr.  --impl reference times the CPU oracle
+(oracle/) on a bounded sample of the same workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "moe_fwd_bwd_tokens_per_s"
+UNIT = "tokens/s"
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    """MEASURED_PEAKS.json (driver-written) or the fallback of /opt/skills/guides/B200_PROFILING.md."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            m = json.load(f)
+        return dict(hbm=float(m["hbm_gbs"]), tf_burst=float(m["bf16_tflops"]),
+                    tf_sustained=float(m.get("bf16_tflops_sustained", m["bf16_tflops"])), kind="measured")
+    return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, kind="fallback")
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # pragma: no cover
+            log("clock sampler unavailable:", e)
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# --------------------------------------------------------------------------------- reference arm
+def oracle_sample_cfg(cfg, tokens: int):
+    """Bounded sample of the workload for the CPU oracle: the first `tokens` tokens of the same layer
+    (same d, E, k, I, weights and seed; only T shrinks)."""
+    return dataclasses.replace(cfg, T=tokens, name=f"{cfg.name}[first {tokens} tokens]")
+
+
+def time_oracle(cfg, tokens: int, steps: int, warmup: int):
+    """Seconds per fwd+bwd pass of the oracle, as it stands, on `tokens` tokens; threads = host cores."""
+    from inputs import configs
+    from oracle import oracle
+    cores = os.cpu_count() or 1
+    oracle.set_threads(cores)
+    scfg = oracle_sample_cfg(cfg, tokens)
+    inp = configs.make_inputs(scfg)
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        f = oracle.forward(scfg, inp)
+        oracle.backward(scfg, inp, f)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+        log(f"oracle pass {i}: {dt:.2f} s on {tokens} tokens")
+    return sum(times) / len(times), cores, scfg
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return  # rank 0 alone runs the reference arm
+    tokens = args.oracle_tokens or 8
+    sec, cores, scfg = time_oracle(cfg, tokens, args.steps, args.warmup)
+    value = tokens / sec
+    sample = (f"CPU oracle (oracle/, fp64 plain loops, OpenMP over rows) fwd+bwd on the first {tokens} tokens of "
+              f"{cfg.name} (same d/E/k/I and weights), {args.steps} passes after {args.warmup} warm-up")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, extra={"sample_tokens": tokens}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, extra=None):
+    w = {"workload": f"{cfg.name}: one MoE layer fwd+bwd chunk, T={cfg.T} d={cfg.d} E={cfg.E} (local {cfg.e_loc}) "
+                     f"top-{cfg.k} I={cfg.I} I_shared={cfg.I_shared} gate_mode={cfg.gate_mode}",
+         "T": cfg.T, "d": cfg.d, "E": cfg.E, "E_loc": cfg.e_loc, "k": cfg.k, "I": cfg.I, "I_shared": cfg.I_shared,
+         "seed": cfg.seed, "storage": "bf16" if cfg.dtype == 1 else "f32", "accumulate": "f32",
+         "row_align": cfg.row_align,
+         "l2": "working set (weights + dW, GBs) exceeds the 126 MB L2 every step; no explicit flush"}
+    if extra:
+        w.update(extra)
+    return w
+
+
+# ------------------------------------------------------------------------------ algorithmic work
+def task_work(cfg, A: int, t_touched: int):
+    """Algorithmic FLOP (GEMM tasks) or HBM bytes (movers) per task, SURVEY.md §8(d) / DESIGN.md §6."""
+    b = 2 if cfg.dtype == 1 else 4
+    d, I, Is, T, k = cfg.d, cfg.I, cfg.I_shared, cfg.T, cfg.k
+    sh = 1 if Is else 0
+    w = {
+        "F_ROUTE": ("hbm", T * cfg.E * 4 + T * k * 8 + cfg.E * 4),
+        "F_SCAN": ("hbm", 2 * T * k * 4 + A * 4),
+        "F_PACK": ("hbm", (t_touched + A) * d * b + 8 * A),
+        "F_GEMM1": ("tensor", 4.0 * d * I * A),
+        "F_GEMM2": ("tensor", 2.0 * d * I * A),
+        "F_COMBINE": ("hbm", (A + T + sh * T) * d * b + 8 * T * k),
+        "B_CGRAD": ("hbm", (t_touched + 2 * A) * d * b),
+        "B_DGRAD1": ("tensor", 2.0 * d * I * A),
+        "B_DGRAD2": ("tensor", 4.0 * d * I * A),
+        "B_WGRAD": ("tensor", 6.0 * d * I * A),
+        "B_UNPACK": ("hbm", (A + T + sh * T) * d * b),
+        "B_ROUTE_BWD": ("hbm", T * k * 16),
+    }
+    if Is:
+        w["F_SHARED"] = ("tensor", 6.0 * d * Is * T)
+        w["B_SHARED"] = ("tensor", 12.0 * d * Is * T)
+    return w
+
+
+# ----------------------------------------------------------------------------------- piper arm
+INPUT_NAMES = ("logits", "x", "dy", "w_gate", "w_up", "w_down", "ws_gate", "ws_up", "ws_down")
+
+
+def desc_of(piper, cfg):
+    return piper.make_desc(cfg.T, cfg.d, cfg.E, cfg.k, cfg.I, e_lo=cfg.e_lo, E_loc=cfg.e_loc, I_shared=cfg.I_shared,
+                           dtype=cfg.dtype, gate_mode=cfg.gate_mode, row_align=cfg.row_align)
+
+
+def run_piper(args, cfg):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_11169_b200 as piper
+    from inputs import configs
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the piper library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # every rank: its own microbatch of the same layer shape (weak scaling, no data-path collective)
+    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    t0 = time.time()
+    inp = configs.make_inputs(rcfg)
+    log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
+    ctx = piper.Context(desc_of(piper, rcfg), device=local)
+    b = piper.alloc_buffers(ctx)
+    b.update({n: piper.to_tensor(inp[n], dev) for n in INPUT_NAMES if n in inp})
+    cargs = piper.chunk_args(b)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        piper.piper_run_chunk_fwd(ctx, cargs)
+        piper.piper_run_chunk_bwd(ctx, cargs)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    launches0 = piper.piper_kernel_launches(ctx)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    launches = piper.piper_kernel_launches(ctx) - launches0
+    ms = ev0.elapsed_time(ev1)
+    tms = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(tms.item()) / args.steps
+    value = world * cfg.T / (ms_per_step * 1e-3)
+
+    # ---- e2e: pinned host inputs -> device, the same two C-ABI calls, results -> pinned host ----------
+    host_in = {n: piper.to_tensor(inp[n], "cpu").pin_memory() for n in ("logits", "x", "dy")}
+    out_names = ("y", "dx", "dz_sel")
+    host_out = {n: torch.empty(b[n].shape, dtype=b[n].dtype).pin_memory() for n in out_names}
+    h2d = sum(t.numel() * t.element_size() for t in host_in.values())
+    d2h = sum(t.numel() * t.element_size() for t in host_out.values())
+
+    def e2e_step():
+        for n, t in host_in.items():
+            b[n].copy_(t, non_blocking=True)
+        step()
+        for n, t in host_out.items():
+            t.copy_(b[n], non_blocking=True)
+
+    for _ in range(min(args.warmup, 3)):
+        e2e_step()
+    barrier()
+    w0 = time.perf_counter()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        e2e_step()
+    ev1.record(stream)
+    barrier()
+    wall_ms = (time.perf_counter() - w0) * 1e3
+    tms = torch.tensor([max(ev0.elapsed_time(ev1), wall_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    e2e_ms = float(tms.item()) / args.steps
+    e2e = {"value": world * cfg.T / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
+           "what": "pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel -> pinned "
+                   "host; timed as max(CUDA events, host wall clock)"}
+
+    # ---- per-task device times (CUDA events on the launching stream, inside full steps) ---------------
+    tasks = [t for t in piper.TASKS if cfg.I_shared or t not in ("F_SHARED", "B_SHARED")]
+    order = ["F_ROUTE", "F_SCAN", "F_PACK", "F_SHARED", "F_GEMM1", "F_GEMM2", "F_COMBINE", "B_CGRAD", "B_DGRAD1",
+             "B_DGRAD2", "B_WGRAD", "B_SHARED", "B_UNPACK", "B_ROUTE_BWD"]
+    order = [t for t in order if t in tasks]
+    n_prof = max(3, min(args.steps, 10))
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(order) + 1)] for _ in range(n_prof)]
+    for it in range(n_prof):
+        evs[it][0].record(stream)
+        for i, t in enumerate(order):
+            piper.piper_run_task(ctx, t, cargs)
+            evs[it][i + 1].record(stream)
+    torch.cuda.synchronize()
+    task_ms = {t: float(np.mean([evs[it][i].elapsed_time(evs[it][i + 1]) for it in range(n_prof)]))
+               for i, t in enumerate(order)}
+
+    A = int(b["offsets"][rcfg.e_loc].item())
+    t_touched = int((b["row_of"] >= 0).any(dim=1).sum().item())
+    counts = b["counts"].cpu().numpy()
+    peaks = measured_peaks()
+    work = task_work(rcfg, A, t_touched)
+    kernels = {}
+    for t in order:
+        bound, amount = work[t]
+        sec = task_ms[t] * 1e-3
+        if bound == "tensor":
+            ach, peak, unit = amount / sec / 1e12, peaks["tf_sustained"], "TFLOP/s"
+        else:
+            ach, peak, unit = amount / sec / 1e9, peaks["hbm"], "GB/s"
+        kernels[t] = {"ms": round(task_ms[t], 4), "bound": bound, "achieved": round(ach, 2), "unit": unit,
+                      "frac": round(ach / peak, 4)}
+    gemm_tasks = [t for t in order if work[t][0] == "tensor"]
+    gemm_ms = sum(task_ms[t] for t in gemm_tasks)
+    gemm_flop = sum(work[t][1] for t in gemm_tasks)
+    dom = "F_GEMM1"  # one launch per task: the fused gate/up GEMM + SwiGLU kernel (largest single-kernel share)
+    impl = "tcgen05" if (cfg.dtype == 1 and piper.piper_gemm_path(ctx) == 1) else "fp32-alu"
+    roofline = {"bound": "tensor", "kernel": f"{dom} ({impl} grouped GEMM gate|up + SwiGLU epilogue, 1 launch/step)",
+                "achieved": kernels[dom]["achieved"], "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
+                "frac": kernels[dom]["frac"], "traffic": None,
+                "peak_kind": f"bf16_tflops_sustained of {peaks['kind']} (kernel timed inside a long step)",
+                "flop_per_launch": work[dom][1], "ms_per_launch": task_ms[dom],
+                "all_gemm": {"tflops": round(gemm_flop / (gemm_ms * 1e-3) / 1e12, 2),
+                             "frac": round(gemm_flop / (gemm_ms * 1e-3) / 1e12 / peaks["tf_sustained"], 4),
+                             "frac_of_nominal_2250": round(gemm_flop / (gemm_ms * 1e-3) / 1e12 / 2250.0, 4),
+                             "share_of_step": round(gemm_ms / sum(task_ms.values()), 4)}}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if cfg.dtype == 1 else "f32", "data": "synthetic",
+            "config": workload_config(cfg, extra={"A_rows": A, "tokens_touched": t_touched,
+                                                  "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
+                                                  "parallelism": f"replicas x{world} (one microbatch per GPU)"}),
+            "tflops": configs.flops_fwd_bwd(rcfg, A) / (ms_per_step * 1e-3) / 1e12,
+            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "kernels": kernels, "gemm_impl": impl}
+    return line, ctx, b, inp, rcfg
+
+
+def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
+    """Step P on this context's layer shape: forward chunk of microbatch A (the bench inputs) co-scheduled
+    with the backward chunk of microbatch B (seed + 1, own weights: reading c-20) versus the same two
+    chunks back to back on one stream with all SMs."""
+    import torch
+    from inputs import configs
+    cfg_b = dataclasses.replace(cfg, seed=cfg.seed + 1)
+    inp_b = configs.make_inputs(cfg_b)
+    dev = b_a["x"].device
+    b_b = piper.alloc_buffers(ctx)
+    b_b.update({n: piper.to_tensor(inp_b[n], dev) for n in INPUT_NAMES if n in inp_b})
+    args_a, args_b = piper.chunk_args(b_a), piper.chunk_args(b_b)
+    piper.piper_run_chunk_fwd(ctx, args_b)  # untimed producer of B's saved activations
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(iters):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / iters
+
+    t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
+    t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
+    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "splits": {}}
+    for sg, sc in splits:
+        t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
+        out["splits"][f"{sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / (t_f + t_b)}
+    out["partition_mode"] = {1: "green contexts", 2: "bounded grids on plain streams"}.get(
+        piper.piper_pair_partition_mode(ctx), "?")
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--impl", default="piper", choices=["piper", "reference"])
+    ap.add_argument("--row-align", type=int, default=None, help="override the config's row_align")
+    ap.add_argument("--oracle-tokens", type=int, default=0, help="tokens of the CPU-oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pair", action="store_true", help="also time step P (chunk pair vs serial) on this shape")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "piper" else args.warmup
+
+    import __graft_entry__ as ge
+    from inputs import configs
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        ge.build()
+    cfg = configs.BY_NAME[args.config]
+    if cfg.dtype == configs.DT_BF16:
+        cfg = dataclasses.replace(cfg, row_align=args.row_align or 128)  # tcgen05 tiles are 128 rows
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    line, ctx, b, inp, rcfg = run_piper(args, cfg)
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if args.pair and world == 1:
+        import paper_2606_11169_b200 as piper
+        line["pair"] = run_pair(piper, ctx, rcfg, b, inp, [(132, 16), (124, 24), (116, 32), (100, 48)],
+                                max(3, min(args.steps, 10)))
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tokens = args.oracle_tokens or 8
+        sec, cores, _ = time_oracle(cfg, tokens, 1, 0)
+        line["cpu_baseline"] = {"value": tokens / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"CPU oracle fwd+bwd, one pass over the first {tokens} tokens of {cfg.name} "
+                                          f"(same d/E/k/I, weights, seed), {sec:.1f} s"}
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

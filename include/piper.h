@@ -77,6 +77,8 @@ int piper_destroy(piper_ctx* ctx);
 const char* piper_last_cuda_error(const piper_ctx* ctx);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t piper_kernel_launches(const piper_ctx* ctx);
+/* Which GEMM family serves the routed experts of this context: 1 = tcgen05/TMEM/TMA, 0 = FP32 ALUs. */
+int piper_gemm_path(const piper_ctx* ctx);
 /* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */
 int64_t piper_a_cap(const piper_moe_desc* desc);
 
@@ -174,6 +176,25 @@ int piper_run_chunk_bwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream)
  * piper_run_chunk_fwd + piper_run_chunk_bwd. */
 int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const piper_chunk_args* bwd_mb, int sm_gemm,
                          int sm_comm, void* stream);
+/* One task of the pair DAG (SURVEY.md §8c c-sched numbering) on `stream` with all SMs: the unit that
+ * piper_run_chunk_fwd / _bwd / _pair enqueue, exposed so that each step can be timed on its own
+ * (bench.py's roofline block).  F_* tasks read `a` as the forward microbatch, B_* as the backward one. */
+#define PIPER_TASK_F_ROUTE 0
+#define PIPER_TASK_F_SCAN 1
+#define PIPER_TASK_F_PACK 2
+#define PIPER_TASK_F_GEMM1 3
+#define PIPER_TASK_F_GEMM2 4
+#define PIPER_TASK_F_SHARED 5
+#define PIPER_TASK_F_COMBINE 6
+#define PIPER_TASK_B_CGRAD 7
+#define PIPER_TASK_B_DGRAD1 8
+#define PIPER_TASK_B_DGRAD2 9
+#define PIPER_TASK_B_WGRAD 10
+#define PIPER_TASK_B_SHARED 11
+#define PIPER_TASK_B_UNPACK 12
+#define PIPER_TASK_B_ROUTE_BWD 13
+int piper_run_task(piper_ctx* ctx, int task, const piper_chunk_args* a, void* stream);
+
 /* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
  * grids on two plain streams (green contexts unavailable), 0 = never called. */
 int piper_pair_partition_mode(const piper_ctx* ctx);

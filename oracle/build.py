@@ -1,4 +1,5 @@
 """Builds oracle/liboracle.so (plain C++17, no CUDA, no fast-math) in-tree."""
+import fcntl
 import os
 import subprocess
 
@@ -7,11 +8,21 @@ SRC = os.path.join(HERE, "oracle.cpp")
 LIB = os.path.join(HERE, "liboracle.so")
 
 
-def build(force: bool = False) -> str:
+def _build(force: bool = False) -> str:
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
         cmd = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-fopenmp", "-Wall", "-o", LIB, SRC]
         subprocess.run(cmd, check=True)
     return LIB
+
+
+def build(*args, **kwargs) -> str:
+    """Serialised across processes (torchrun ranks share the tree) with a lock file."""
+    with open(os.path.join(HERE, ".build.lock"), "w") as lk:
+        fcntl.flock(lk, fcntl.LOCK_EX)
+        try:
+            return _build(*args, **kwargs)
+        finally:
+            fcntl.flock(lk, fcntl.LOCK_UN)
 
 
 if __name__ == "__main__":

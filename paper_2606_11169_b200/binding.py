@@ -208,6 +208,15 @@ def piper_run_chunk_bwd(ctx, args: ChunkArgs, stream=None):
     ctx.check(lib().piper_run_chunk_bwd(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_bwd")
 
 
+TASKS = ("F_ROUTE", "F_SCAN", "F_PACK", "F_GEMM1", "F_GEMM2", "F_SHARED", "F_COMBINE", "B_CGRAD", "B_DGRAD1",
+         "B_DGRAD2", "B_WGRAD", "B_SHARED", "B_UNPACK", "B_ROUTE_BWD")  # PIPER_TASK_* of include/piper.h
+
+
+def piper_run_task(ctx, task, args: ChunkArgs, stream=None):
+    t = TASKS.index(task) if isinstance(task, str) else int(task)
+    ctx.check(lib().piper_run_task(ctx._h, t, ctypes.byref(args), _stream(stream)), "piper_run_task")
+
+
 def piper_run_chunk_pair(ctx, fwd_args: ChunkArgs, bwd_args: ChunkArgs, sm_gemm: int, sm_comm: int, stream=None):
     ctx.check(lib().piper_run_chunk_pair(ctx._h, ctypes.byref(fwd_args), ctypes.byref(bwd_args), int(sm_gemm),
                                          int(sm_comm), _stream(stream)), "piper_run_chunk_pair")
@@ -232,6 +241,19 @@ def piper_list_schedule(n, edges, stream_of, prio):
 
 
 # ---------------------------------------------------------------------------------- memory plumbing
+def to_tensor(a, device="cuda"):
+    """Generated numpy tensor -> torch tensor on `device` (uint16 bit patterns are reinterpreted as bf16)."""
+    import numpy as np
+    if a.dtype == np.uint16:
+        return torch.from_numpy(a.view(np.int16)).to(device).view(torch.bfloat16)
+    return torch.from_numpy(a).to(device)
+
+
+def piper_gemm_path(ctx: Context) -> int:
+    """1 = the routed-expert GEMMs of this context run on the tcgen05 kernels, 0 = on the FP32 ALUs."""
+    return int(lib().piper_gemm_path(ctx._h))
+
+
 def alloc_buffers(ctx: Context, backward: bool = True) -> dict:
     """Every output / scratch tensor of one microbatch, as torch CUDA tensors (no arithmetic here)."""
     D, dev, dt = ctx.desc, ctx.device, ctx.torch_dtype

@@ -1,4 +1,5 @@
 """Builds paper_2606_11169_b200/libpiper.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+import fcntl
 import os
 import subprocess
 
@@ -20,7 +21,7 @@ def _stale(target: str, deps) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def _build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(INC, "piper.h"))
@@ -44,6 +45,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or procs or _stale(LIB, objs):
         subprocess.run([NVCC, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB] + objs, check=True)
     return LIB
+
+
+def build(*args, **kwargs) -> str:
+    """Serialised across processes (torchrun ranks share the tree) with a lock file."""
+    with open(os.path.join(HERE, ".build.lock"), "w") as lk:
+        fcntl.flock(lk, fcntl.LOCK_EX)
+        try:
+            return _build(*args, **kwargs)
+        finally:
+            fcntl.flock(lk, fcntl.LOCK_UN)
 
 
 if __name__ == "__main__":

@@ -106,6 +106,11 @@ int piper_destroy(piper_ctx* c) {
 
 const char* piper_last_cuda_error(const piper_ctx* c) { return c ? c->err : "null context"; }
 int64_t piper_kernel_launches(const piper_ctx* c) { return c ? c->launches : 0; }
+int piper_gemm_path(const piper_ctx* c) {
+    if (!c || c->D.dtype != PIPER_DTYPE_BF16 || c->D.gemm_impl != PIPER_GEMM_AUTO) return 0;
+    piper_chunk_args a{};
+    return tc_supported(c, routed_problem(c, &a)) ? 1 : 0;
+}
 int piper_pair_partition_mode(const piper_ctx* c) { return c ? c->pair_mode : 0; }
 
 int piper_route_topk(piper_ctx* c, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global,

@@ -206,6 +206,14 @@ int piper_run_chunk_fwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     return PIPER_OK;
 }
 
+int piper_run_task(piper_ctx* c, int task, const piper_chunk_args* a, void* stream) {
+    if (!c || task < 0 || task >= N_TASKS) return PIPER_ERR_INVALID;
+    if (!(task < B_CGRAD ? fwd_args_ok(c, a) : bwd_args_ok(c, a))) return PIPER_ERR_INVALID;
+    if ((task == F_SHARED || task == B_SHARED) && !c->D.I_shared) return PIPER_ERR_INVALID;
+    const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    return run_task(c, task, ln, a, a);
+}
+
 int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
     const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
