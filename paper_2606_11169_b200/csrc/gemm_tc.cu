@@ -1,13 +1,557 @@
-// gemm_tc.cu — placeholder until the tcgen05 kernels land: reports "unsupported" so ffn.cu routes to
-// the FP32-ALU kernels.
+// gemm_tc.cu — grouped SwiGLU expert-FFN GEMMs on the 5th-generation tensor cores (F4, B2-B4 of SURVEY.md
+// §8a; BASELINE.json:north_star part 3).  bf16 x bf16 -> fp32 accumulation in TMEM, one rounding to bf16
+// per stored tensor (SURVEY.md §8c "Error budget").
+//
+// One persistent, warp-specialised kernel template serves the five contractions of the FFN:
+//   warp 0  : TMA producer (cp.async.bulk.tensor, 128-byte swizzle) into a 4-stage shared-memory ring
+//   warp 1  : single-thread tcgen05.mma issuer (M=128, N=256, K=16, cta_group::1), tcgen05.commit hand-off
+//   warp 2  : TMEM allocator (512 columns = two 128x256 fp32 accumulators: the epilogue of tile i overlaps
+//             the main loop of tile i+1)
+//   warps 4-7: epilogue, tcgen05.ld TMEM -> registers -> fused math -> global
+// Operand layouts are taken as they lie in memory (no transposed copies): the descriptors select K-major
+// or MN-major per operand:
+//   fwd1   G|U = Xp Wg | Xp Wu      A K-major  (Xp [rows,d]),   B MN-major (W [d,I], two 128-col halves)
+//   fwd2   O   = H Wd               A K-major  (H  [rows,I]),   B MN-major (Wd [I,d])
+//   dgrad1 dH  = dO Wd^T            A K-major  (dO [rows,d]),   B K-major  (Wd [I,d])
+//   dgrad2 dXp = dG Wg^T + dU Wu^T  A K-major  (dG,dU [rows,I]),B K-major  (Wg,Wu [d,I]); K runs over both
+//   wgrad  dWg|dWu = Xp^T dG|dU ; dWd = H^T dO    A, B MN-major (row buffers), K = the expert's rows
+// Ragged groups: segments are padded to row_align = 128 rows (pad rows are zero in every row buffer), so
+// an M tile never straddles two experts and the ragged K of wgrad is a whole number of tiles; the tile ->
+// expert map is computed on the device from `offsets` (no host read-back).  Tails in d / I / T are
+// handled by TMA zero fill on loads and bounds checks on stores.
 #include "piper_internal.cuh"
+
 namespace piper {
+namespace {
+
+constexpr int BM = 128, BN = 256, BK = 64, UK = 16, STAGES = 4;
+constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int MN_BLOCK_BYTES = 64 * BK * 2;  // one 64(MN) x 64(K) box of an MN-major operand
+constexpr int kThreads = 256;
+constexpr int kMaxGroups = kMaxE;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/ +
+                           (kMaxGroups + 1) * 4 /*tile prefix*/;
+constexpr int PANEL_M = 8;  // M tiles per panel of the tile order (L2 reuse of the weight tile)
+
+enum : int { K_MAJOR = 0, MN_MAJOR = 1 };
+enum : int { EPI_SWIGLU_FWD = 0, EPI_STORE = 1, EPI_SWIGLU_BWD = 2, EPI_WGRAD_SPLIT = 3, EPI_WGRAD = 4 };
+
+struct alignas(64) TcParams {
+    CUtensorMap a[2], b[2];
+    const int32_t* offsets;  // [G+1] device
+    int G;
+    int ragged_m;    // 1: tiles run over the packed rows (fwd / dgrad); 0: over groups (wgrad)
+    int n_tiles;     // tiles along N
+    int m_tiles;     // wgrad: tiles along M per group
+    int kb_per_src;  // ragged_m: K blocks per source
+    int n_src;       // 1, or 2 when K runs over two (A, B) pairs (dgrad2)
+    int b_split;     // B tile = [b[0]: 128 columns | b[1]: 128 columns] (fwd1, wgrad gate|up)
+    int tile_n;      // output columns per tile (128 when split, else 256)
+    int m_limit;     // wgrad: rows of one dW matrix
+    int n_limit;     // columns of the outputs
+    long long ld;            // leading dimension of outputs / epilogue inputs (elements)
+    long long group_stride;  // wgrad: elements between two experts' dW
+    __nv_bfloat16 *out0, *out1, *out2;
+    const __nv_bfloat16 *in0, *in1;
+};
+
+// ---- PTX wrappers ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(cols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem], 128 x 256 x 16, bf16 inputs, fp32 accumulate
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// mbarrier arrives once every tcgen05 operation issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+// 16 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+// wait for the loads above; the registers are in/out operands so that no use is scheduled before the wait
+__device__ __forceinline__ void tmem_ld_wait(uint32_t (&r)[16]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+                 :
+                 : "memory");
+}
+
+// Shared-memory matrix descriptor (tcgen05 "matrix descriptor", version 1, 128-byte swizzle).
+//  K-major : rows of 64 elements (128 B), 8-row swizzle atoms 1024 B apart (SBO); LBO unused.
+//  MN-major: 64(MN) x 8(K) atoms of 1024 B; SBO = 1024 B between 8-K groups, LBO = bytes between 64-wide MN blocks.
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+    d |= (uint64_t)1 << 46;  // descriptor version (Blackwell)
+    d |= (uint64_t)2 << 61;  // SWIZZLE_128B
+    return d;
+}
+// Instruction descriptor: D fp32, A/B bf16, M = 128, N = 256, majors per operand.
+__host__ __device__ constexpr uint32_t make_idesc(int a_major, int b_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_major << 15) | ((uint32_t)b_major << 16) |
+           ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+
+// ---- tile schedule (identical in every role) ----------------------------------------------------------
+struct Tile {
+    int g;    // group (expert)
+    int m0;   // ragged_m: first packed row of the tile; wgrad: first row of dW
+    int n0;   // first output column
+    int k0;   // wgrad: first packed row of the group's K range
+    int nkb;  // K blocks of this tile
+};
+
+// tp[g] = first M tile of group g (ragged_m), tp[G] = number of M tiles.
+__device__ __forceinline__ int total_tiles(const TcParams& P, const int* tp) {
+    return P.ragged_m ? tp[P.G] * P.n_tiles : P.G * P.m_tiles * P.n_tiles;
+}
+
+__device__ __forceinline__ Tile decode_tile(const TcParams& P, const int* tp, const int32_t* __restrict__ offsets, int t) {
+    Tile r;
+    if (P.ragged_m) {
+        // group-major; inside a group panels of PANEL_M M tiles; inside a panel N-major with M fastest, so
+        // the CTAs of one wave share a few weight tiles (L2) and the panel's rows stay L2-resident.
+        int g = 0;
+        while (g + 1 < P.G && tp[g + 1] * P.n_tiles <= t) ++g;
+        const int local = t - tp[g] * P.n_tiles, mg = tp[g + 1] - tp[g];
+        const int per_panel = PANEL_M * P.n_tiles;
+        const int panel = local / per_panel, rem = local - panel * per_panel;
+        const int pm = min(PANEL_M, mg - panel * PANEL_M);
+        const int nt = rem / pm, mt = tp[g] + panel * PANEL_M + (rem - nt * pm);
+        r.g = g, r.m0 = mt * BM, r.n0 = nt * P.tile_n, r.k0 = 0, r.nkb = P.kb_per_src * P.n_src;
+    } else {
+        const int per_group = P.m_tiles * P.n_tiles;
+        const int g = t / per_group, local = t - g * per_group;
+        const int nt = local / P.m_tiles, mt = local - nt * P.m_tiles;
+        const int lo = offsets[g], hi = offsets[g + 1];
+        r.g = g, r.m0 = mt * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + BK - 1) / BK;
+    }
+    return r;
+}
+
+// ---- epilogue helpers ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 pack8(const float* v) {
+    uint4 r;
+    r.x = f2_to_bf2(v[0], v[1]), r.y = f2_to_bf2(v[2], v[3]), r.z = f2_to_bf2(v[4], v[5]), r.w = f2_to_bf2(v[6], v[7]);
+    return r;
+}
+__device__ __forceinline__ void unpack8(const uint4& q, float* v) {
+    float2 f;
+    f = bf2_to_f2(q.x), v[0] = f.x, v[1] = f.y;
+    f = bf2_to_f2(q.y), v[2] = f.x, v[3] = f.y;
+    f = bf2_to_f2(q.z), v[4] = f.x, v[5] = f.y;
+    f = bf2_to_f2(q.w), v[6] = f.x, v[7] = f.y;
+}
+__device__ __forceinline__ float sigmoidf_fast(float x) { return __fdividef(1.f, 1.f + __expf(-x)); }
+
+// 16 output columns [col, col+16) of one row: store the halves that lie below n_limit (n_limit % 8 == 0).
+__device__ __forceinline__ void store16(__nv_bfloat16* row_ptr, int col, int n_limit, const float* v) {
+    if (col < n_limit) *reinterpret_cast<uint4*>(row_ptr + col) = pack8(v);
+    if (col + 8 < n_limit) *reinterpret_cast<uint4*>(row_ptr + col + 8) = pack8(v + 8);
+}
+__device__ __forceinline__ void load16(const __nv_bfloat16* row_ptr, int col, int n_limit, float* v) {
+    uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0;
+    if (col < n_limit) q0 = *reinterpret_cast<const uint4*>(row_ptr + col);
+    if (col + 8 < n_limit) q1 = *reinterpret_cast<const uint4*>(row_ptr + col + 8);
+    unpack8(q0, v), unpack8(q1, v + 8);
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------------
+template <int A_MAJOR, int B_MAJOR, int EPI>
+__global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_constant__ TcParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
+    uint64_t* empty_bar = full_bar + STAGES;
+    uint64_t* tfull_bar = empty_bar + STAGES;  // [2] accumulator ready
+    uint64_t* tempty_bar = tfull_bar + 2;      // [2] accumulator drained
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tempty_bar + 2);
+    int* tp = reinterpret_cast<int*>(smem + STAGES * STAGE_BYTES + 256);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int32_t* __restrict__ offsets = P.offsets;
+
+    if (P.ragged_m)
+        for (int g = threadIdx.x; g <= P.G; g += kThreads) tp[g] = (offsets[g] + BM - 1) / BM;
+    if (warp == 0 && lane == 0) {
+        prefetch_tmap(&P.a[0]), prefetch_tmap(&P.b[0]);
+        if (P.n_src == 2) prefetch_tmap(&P.a[1]);
+        if (P.n_src == 2 || P.b_split) prefetch_tmap(&P.b[1]);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
+        for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 128);
+        fence_barrier_init();
+    }
+    if (warp == 2) tmem_alloc(tmem_ptr, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+    const int n_total = total_tiles(P, tp);
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        int stage = 0, phase = 0;
+        for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
+            const Tile T = decode_tile(P, tp, offsets, t);
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    uint8_t* sa = smem + stage * STAGE_BYTES;
+                    uint8_t* sb = sa + A_BYTES;
+                    uint64_t* bar = &full_bar[stage];
+                    mbar_expect_tx(bar, STAGE_BYTES);
+                    int src = 0, kk = kb;
+                    if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
+                    const int k = T.k0 + kk * BK;
+                    // A: ragged_m -> rows m0.. of a row buffer (z = 0); wgrad -> columns m0.. of a row buffer
+                    if (A_MAJOR == K_MAJOR) {
+                        tma_load_3d(sa, &P.a[src], bar, k, T.m0, 0);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < BM / 64; ++j)
+                            tma_load_3d(sa + j * MN_BLOCK_BYTES, &P.a[src], bar, T.m0 + 64 * j, k, 0);
+                    }
+                    // B: ragged_m -> weights of group g (z = g); wgrad -> columns n0.. of a row buffer (z = 0)
+                    const int bz = P.ragged_m ? T.g : 0;
+                    if (B_MAJOR == K_MAJOR) {
+                        tma_load_3d(sb, &P.b[src], bar, k, T.n0, bz);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < BN / 64; ++j) {
+                            const int half = P.b_split ? (j >> 1) : src;
+                            const int col = P.b_split ? T.n0 + 64 * (j & 1) : T.n0 + 64 * j;
+                            tma_load_3d(sb + j * MN_BLOCK_BYTES, &P.b[half], bar, col, k, bz);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (++stage == STAGES) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread) =====
+        constexpr uint32_t idesc = make_idesc(A_MAJOR, B_MAJOR);
+        constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
+        constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        int stage = 0, phase = 0, as = 0, aphase = 0;
+        for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
+            const Tile T = decode_tile(P, tp, offsets, t);
+            if (lane == 0) {
+                mbar_wait(&tempty_bar[as], aphase ^ 1);
+                tc_fence_after();
+            }
+            __syncwarp();
+            const uint32_t d_tmem = tmem_base + as * BN;
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&full_bar[stage], phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+#pragma unroll
+                    for (int kk = 0; kk < BK / UK; ++kk) {
+                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
+                        const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
+                        umma_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
+                    }
+                    umma_commit(&empty_bar[stage]);  // frees the smem slot when these MMAs have read it
+                }
+                __syncwarp();
+                if (++stage == STAGES) stage = 0, phase ^= 1;
+            }
+            if (lane == 0) umma_commit(&tfull_bar[as]);  // accumulator complete (immediately if nkb == 0)
+            __syncwarp();
+            if (++as == 2) as = 0, aphase ^= 1;
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue: warp w owns TMEM lanes 32 (w % 4) .. +31 = tile rows =====
+        const int wq = warp & 3, row = wq * 32 + lane;
+        int as = 0, aphase = 0;
+        const int rows_total = P.ragged_m ? offsets[P.G] : P.m_limit;
+        for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
+            const Tile T = decode_tile(P, tp, offsets, t);
+            mbar_wait(&tfull_bar[as], aphase);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
+            const int grow = T.m0 + row;
+            const bool row_ok = grow < rows_total;
+            const bool zero = T.nkb == 0;  // empty expert in wgrad: exact zeros, the accumulator is stale
+            const long long base = (P.ragged_m ? 0 : (long long)T.g * P.group_stride) + (long long)grow * P.ld;
+            if (EPI == EPI_SWIGLU_FWD || EPI == EPI_WGRAD_SPLIT) {
+#pragma unroll 1
+                for (int c = 0; c < 128; c += 16) {
+                    uint32_t r0[16], r1[16];
+                    tmem_ld16(taddr + c, r0);
+                    tmem_ld16(taddr + 128 + c, r1);
+                    tmem_ld_wait(r0);
+                    tmem_ld_wait(r1);
+                    float v0[16], v1[16], h[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        v0[i] = zero ? 0.f : __uint_as_float(r0[i]);
+                        v1[i] = zero ? 0.f : __uint_as_float(r1[i]);
+                    }
+                    if (row_ok) {
+                        store16(P.out0 + base, T.n0 + c, P.n_limit, v0);
+                        store16(P.out1 + base, T.n0 + c, P.n_limit, v1);
+                        if (EPI == EPI_SWIGLU_FWD) {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) h[i] = v0[i] * sigmoidf_fast(v0[i]) * v1[i];
+                            store16(P.out2 + base, T.n0 + c, P.n_limit, h);
+                        }
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int c = 0; c < BN; c += 16) {
+                    uint32_t r0[16];
+                    tmem_ld16(taddr + c, r0);
+                    tmem_ld_wait(r0);
+                    float v[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) v[i] = zero ? 0.f : __uint_as_float(r0[i]);
+                    if (row_ok) {
+                        if (EPI == EPI_SWIGLU_BWD) {
+                            // v = dH; dG = dH * U * silu'(G), dU = dH * silu(G)
+                            float gv[16], uv[16], dg[16], du[16];
+                            load16(P.in0 + base, T.n0 + c, P.n_limit, gv);
+                            load16(P.in1 + base, T.n0 + c, P.n_limit, uv);
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                const float s = sigmoidf_fast(gv[i]);
+                                dg[i] = v[i] * uv[i] * (s * (1.f + gv[i] * (1.f - s)));
+                                du[i] = v[i] * (gv[i] * s);
+                            }
+                            store16(P.out0 + base, T.n0 + c, P.n_limit, dg);
+                            store16(P.out1 + base, T.n0 + c, P.n_limit, du);
+                        } else {
+                            store16(P.out0 + base, T.n0 + c, P.n_limit, v);
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(&tempty_bar[as]);
+            if (++as == 2) as = 0, aphase ^= 1;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// ---- host side ------------------------------------------------------------------------------------------
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// bf16 tensor [groups][rows][inner] (row-major), box = 64 inner elements (128 B, swizzled) x box_rows rows.
+int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
+             int box_rows) {
+    const cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)groups};
+    const cuuint64_t strides[2] = {(cuuint64_t)inner * 2, (cuuint64_t)inner * 2 * (cuuint64_t)rows};
+    const cuuint32_t box[3] = {64, (cuuint32_t)box_rows, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = reinterpret_cast<EncodeTiledFn>(c->encode_tiled)(
+        m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled failed (%d): inner %lld rows %lld groups %lld box %d",
+                 (int)r, inner, rows, groups, box_rows);
+        return PIPER_ERR_CUDA;
+    }
+    return PIPER_OK;
+}
+#define PIPER_MAP(...)                                 \
+    do {                                               \
+        const int rc__ = make_map(c, __VA_ARGS__);     \
+        if (rc__ != PIPER_OK) return rc__;             \
+    } while (0)
+
+template <int A_MAJOR, int B_MAJOR, int EPI>
+int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
+    long long grid = tile_bound < ln.sms ? tile_bound : ln.sms;
+    if (grid < 1) grid = 1;
+    tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)grid, kThreads, SMEM_BYTES, ln.stream>>>(P);
+    PIPER_LAUNCHED(c, name);
+    return PIPER_OK;
+}
+
+template <int A_MAJOR, int B_MAJOR, int EPI>
+bool set_smem_attr() {
+    return cudaFuncSetAttribute(tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                SMEM_BYTES) == cudaSuccess;
+}
+
+TcParams base_params(const FfnProblem& p, bool ragged_m) {
+    TcParams P;
+    memset(&P, 0, sizeof(P));
+    P.offsets = p.offsets, P.G = p.G, P.ragged_m = ragged_m ? 1 : 0, P.n_src = 1, P.tile_n = BN;
+    return P;
+}
+inline long long m_tile_bound(const FfnProblem& p) { return cdiv(p.max_rows, BM); }
+
+}  // namespace
+
 size_t tc_scratch_bytes(const piper_moe_desc*) { return 256; }
-int tc_init(piper_ctx*) { return PIPER_OK; }
-bool tc_supported(const piper_ctx*, const FfnProblem&) { return false; }
-int tc_ffn_fwd1(piper_ctx*, Lane, const FfnProblem&) { return PIPER_ERR_UNSUPPORTED; }
-int tc_ffn_fwd2(piper_ctx*, Lane, const FfnProblem&) { return PIPER_ERR_UNSUPPORTED; }
-int tc_ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&) { return PIPER_ERR_UNSUPPORTED; }
-int tc_ffn_dgrad2(piper_ctx*, Lane, const FfnProblem&) { return PIPER_ERR_UNSUPPORTED; }
-int tc_ffn_wgrad(piper_ctx*, Lane, const FfnProblem&) { return PIPER_ERR_UNSUPPORTED; }
+
+int tc_init(piper_ctx* c) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        fn = nullptr;
+    cudaGetLastError();
+    c->encode_tiled = fn;
+    bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
+              set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
+              set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>();
+    if (!ok) {
+        cudaGetLastError();
+        c->encode_tiled = nullptr;  // not an sm_100a device: the FP32-ALU kernels serve every request
+    }
+    return PIPER_OK;
+}
+
+bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
+    if (!c->encode_tiled) return false;
+    if (p.G > kMaxGroups || p.d < 64 || p.I < 64 || p.d % 8 || p.I % 8) return false;
+    if (p.G > 1 && c->D.row_align % BM) return false;  // an M tile must not straddle two experts
+    return true;
+}
+
+// G|U = Xp Wg | Xp Wu, H = silu(G) * U
+int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    TcParams P = base_params(p, true);
+    PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, BM);
+    PIPER_MAP(&P.b[0], p.w_gate, p.I, p.d, p.G, 64);
+    PIPER_MAP(&P.b[1], p.w_up, p.I, p.d, p.G, 64);
+    P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.kb_per_src = cdiv(p.d, BK);
+    P.n_limit = p.I, P.ld = p.I;
+    P.out0 = (__nv_bfloat16*)p.g, P.out1 = (__nv_bfloat16*)p.u, P.out2 = (__nv_bfloat16*)p.h;
+    return launch<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_fwd1");
+}
+
+// O = H Wd
+int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    TcParams P = base_params(p, true);
+    PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, BM);
+    PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, 64);
+    P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
+    P.out0 = (__nv_bfloat16*)p.o;
+    return launch<K_MAJOR, MN_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_fwd2");
+}
+
+// dH = dO Wd^T; dG = dH * U * silu'(G); dU = dH * silu(G)
+int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    TcParams P = base_params(p, true);
+    PIPER_MAP(&P.a[0], p.d_o, p.d, p.max_rows, 1, BM);
+    PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, BN);
+    P.n_tiles = cdiv(p.I, BN), P.kb_per_src = cdiv(p.d, BK), P.n_limit = p.I, P.ld = p.I;
+    P.in0 = (const __nv_bfloat16*)p.g, P.in1 = (const __nv_bfloat16*)p.u;
+    P.out0 = (__nv_bfloat16*)p.dg, P.out1 = (__nv_bfloat16*)p.du;
+    return launch<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_dgrad1");
+}
+
+// dXp = dG Wg^T + dU Wu^T  (one accumulator, K runs over both products)
+int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    TcParams P = base_params(p, true);
+    PIPER_MAP(&P.a[0], p.dg, p.I, p.max_rows, 1, BM);
+    PIPER_MAP(&P.a[1], p.du, p.I, p.max_rows, 1, BM);
+    PIPER_MAP(&P.b[0], p.w_gate, p.I, p.d, p.G, BN);
+    PIPER_MAP(&P.b[1], p.w_up, p.I, p.d, p.G, BN);
+    P.n_src = 2, P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
+    P.out0 = (__nv_bfloat16*)p.dxp;
+    return launch<K_MAJOR, K_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_dgrad2");
+}
+
+// dWg|dWu[e] = Xp^T dG | Xp^T dU ; dWd[e] = H^T dO over the expert's rows (K ragged; zeros for empty experts)
+int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    {
+        TcParams P = base_params(p, false);
+        PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, 64);
+        PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, 64);
+        PIPER_MAP(&P.b[1], p.du, p.I, p.max_rows, 1, 64);
+        P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.m_tiles = cdiv(p.d, BM);
+        P.m_limit = p.d, P.n_limit = p.I, P.ld = p.I, P.group_stride = (long long)p.d * p.I;
+        P.out0 = (__nv_bfloat16*)p.dw_gate, P.out1 = (__nv_bfloat16*)p.dw_up;
+        const int rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * P.m_tiles * P.n_tiles,
+                                                                  "tc_ffn_wgrad_gate_up");
+        if (rc != PIPER_OK) return rc;
+    }
+    TcParams P = base_params(p, false);
+    PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, 64);
+    PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, 64);
+    P.n_tiles = cdiv(p.d, BN), P.m_tiles = cdiv(p.I, BM);
+    P.m_limit = p.I, P.n_limit = p.d, P.ld = p.d, P.group_stride = (long long)p.I * p.d;
+    P.out0 = (__nv_bfloat16*)p.dw_down;
+    return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * P.m_tiles * P.n_tiles, "tc_ffn_wgrad_down");
+}
+
 }  // namespace piper

@@ -92,7 +92,7 @@ def _check_all(cfg, b, f, g, label=""):
 
 @pytest.mark.parametrize("name", SMALL)
 @pytest.mark.parametrize("impl", [piper.GEMM_AUTO, piper.GEMM_SIMT])
-@pytest.mark.parametrize("align", [1, 64])
+@pytest.mark.parametrize("align", [1, 128])  # 128: the tcgen05 kernels; 1: dense packing, FP32-ALU GEMMs
 def test_small_configs_full_tensor_parity(name, impl, align):
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=align)
     if cfg.dtype == configs.DT_F32 and impl == piper.GEMM_SIMT:
@@ -107,7 +107,7 @@ def test_small_configs_full_tensor_parity(name, impl, align):
 
 @pytest.mark.parametrize("name", ["C1", "C3s", "C4s"])
 def test_chunk_calls_equal_step_calls_bitwise(name):
-    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=64 if name != "C1" else 1)
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128 if name != "C1" else 1)
     inp = configs.make_inputs(cfg)
     ctx1, b1 = _run_steps(cfg, inp)
     ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True)
@@ -125,8 +125,8 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
 def test_pair_is_bitwise_equal_to_serial(name, split):
     """the overlapped, out-of-order plan must respect every dependency -> identical results."""
     base = configs.BY_NAME[name]
-    cfg_a = dataclasses.replace(base, row_align=64, seed=base.seed + 100)
-    cfg_b = dataclasses.replace(base, row_align=64, seed=base.seed + 200)
+    cfg_a = dataclasses.replace(base, row_align=128, seed=base.seed + 100)
+    cfg_b = dataclasses.replace(base, row_align=128, seed=base.seed + 200)
     inp_a, inp_b = configs.make_inputs(cfg_a), configs.make_inputs(cfg_b)
     # serial: fwd(A) ; fwd(B) (untimed producer of B's saved activations) ; bwd(B)
     ctx, ba = _run_steps(cfg_a, inp_a, use_chunk_calls=True, backward=False)
