@@ -46,7 +46,7 @@ def measured_peaks():
 
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML every 100 ms while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML every 20 ms while the timed region runs."""
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
@@ -79,7 +79,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(nm)
             except Exception:
                 pass
-            time.sleep(0.1)
+            time.sleep(0.02)
 
     def summary(self):
         s = sorted(self.samples)
@@ -289,7 +289,8 @@ def run_piper(args, cfg):
     task_ms = {t: float(np.mean([evs[it][i].elapsed_time(evs[it][i + 1]) for it in range(n_prof)]))
                for i, t in enumerate(order)}
 
-    A = int(b["offsets"][rcfg.e_loc].item())
+    A_padded = int(b["offsets"][rcfg.e_loc].item())  # rows the kernels process (segments padded to row_align)
+    A = int(b["counts"].sum().item())                # rows the method defines: the algorithmic work
     t_touched = int((b["row_of"] >= 0).any(dim=1).sum().item())
     counts = b["counts"].cpu().numpy()
     peaks = measured_peaks()
@@ -311,7 +312,8 @@ def run_piper(args, cfg):
     impl = "tcgen05" if (cfg.dtype == 1 and piper.piper_gemm_path(ctx) == 1) else "fp32-alu"
     roofline = {"bound": "tensor", "kernel": f"{dom} ({impl} grouped GEMM gate|up + SwiGLU epilogue, 1 launch/step)",
                 "achieved": kernels[dom]["achieved"], "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
-                "frac": kernels[dom]["frac"], "traffic": None,
+                "frac": kernels[dom]["frac"], "frac_of_burst_peak": round(kernels[dom]["achieved"] / peaks["tf_burst"], 4),
+                "frac_of_nominal_2250": round(kernels[dom]["achieved"] / 2250.0, 4), "traffic": None,
                 "peak_kind": f"bf16_tflops_sustained of {peaks['kind']} (kernel timed inside a long step)",
                 "flop_per_launch": work[dom][1], "ms_per_launch": task_ms[dom],
                 "all_gemm": {"tflops": round(gemm_flop / (gemm_ms * 1e-3) / 1e12, 2),
@@ -322,7 +324,7 @@ def run_piper(args, cfg):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16" if cfg.dtype == 1 else "f32", "data": "synthetic",
-            "config": workload_config(cfg, extra={"A_rows": A, "tokens_touched": t_touched,
+            "config": workload_config(cfg, extra={"A_rows": A, "A_rows_padded": A_padded, "tokens_touched": t_touched,
                                                   "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
                                                   "parallelism": f"replicas x{world} (one microbatch per GPU)"}),
             "tflops": configs.flops_fwd_bwd(rcfg, A) / (ms_per_step * 1e-3) / 1e12,

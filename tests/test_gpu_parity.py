@@ -2,6 +2,7 @@
 oracle (oracle/) on the same seeded inputs (inputs/).  Integer / index outputs bit-exact; floating
 point within the north_star tolerances (tests/piper_testutil.py: TOL)."""
 import dataclasses
+import os
 
 import numpy as np
 import pytest
@@ -195,4 +196,61 @@ def test_empty_input_edge_cases():
     ctx, b = _run_steps(cfg, inp)
     _check_all(cfg, b, f, g)
     assert not util.to_np(b["y"]).any() and not util.to_np(b["dx"]).any()
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4z"])
+def test_full_size_sampled_parity_in_bench_configuration(name):
+    """BASELINE.json full sizes in the launch configuration bench.py times (row_align 128, whole-chunk calls,
+    tcgen05 GEMMs): routing / permutation bit-exact on the whole tensors; Y, dX, dgates on sampled tokens and
+    dW on sampled columns of sampled experts, each computed by the oracle one by one from the definition."""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
+    inp = configs.make_inputs(cfg)
+    oracle.set_threads(os.cpu_count() or 1)
+    rt = oracle.routing(cfg, inp)
+    ctx = piper.Context(util.desc_of(cfg))
+    assert piper.piper_gemm_path(ctx) == 1
+    b = piper.alloc_buffers(ctx)
+    b.update(util.upload_inputs(inp))
+    args = piper.chunk_args(b)
+    piper.piper_run_chunk_fwd(ctx, args)
+    piper.piper_run_chunk_bwd(ctx, args)
+    torch.cuda.synchronize()
+    for n in ("topk_idx", "counts_global", "counts", "row_of", "src_of"):
+        assert np.array_equal(util.to_np(b[n]).reshape(-1), rt[n].reshape(-1)), n
+    assert np.array_equal(util.to_np(b["offsets"])[: cfg.e_loc + 1], rt["offsets"])
+    rng = np.random.default_rng(cfg.seed)
+    local_tokens = np.nonzero((rt["row_of"] >= 0).any(axis=1))[0]
+    tokens = np.sort(np.concatenate([rng.choice(local_tokens, 5, replace=False), [0, cfg.T - 1]]))
+    s = oracle.sample_tokens(cfg, inp, rt, tokens)
+    tk = torch.from_numpy(tokens).cuda()
+    rows = torch.from_numpy(s["rows"]).cuda()
+    dt = cfg.dtype
+    util.check_close("o rows", util.to_np(b["o"][rows]), s["o_rows"], dt)
+    util.check_close("y", util.to_np(b["y"][tk]), s["y"], dt)
+    util.check_close("dgates", util.to_np(b["dgates"][tk]), s["dgates"], dt)
+    util.check_close("dxp rows", util.to_np(b["dxp"][rows]), s["dxp_rows"], dt)
+    util.check_close("dx", util.to_np(b["dx"][tk]), s["dx"], dt)
+    # wgrad: the fullest expert, a small one and (C4z) an empty one
+    order = np.argsort(rt["counts"])
+    picks = {int(order[-1]), int(order[len(order) // 4])}
+    J = np.sort(rng.choice(cfg.I, 3, replace=False)).astype(np.int64)
+    Jc = torch.from_numpy(J).cuda()
+    for e in sorted(picks):
+        rg, ru, rd = oracle.sample_wgrad(cfg, inp, rt, e, J)
+        util.check_close(f"dw_gate[{e}][:,J]", util.to_np(b["dw_gate"][e][:, Jc]), rg, dt)
+        util.check_close(f"dw_up[{e}][:,J]", util.to_np(b["dw_up"][e][:, Jc]), ru, dt)
+        util.check_close(f"dw_down[{e}][J,:]", util.to_np(b["dw_down"][e][Jc, :]), rd, dt)
+    for e in np.nonzero(rt["counts"] == 0)[0][:2]:
+        for n in ("dw_gate", "dw_up", "dw_down"):
+            assert not bool(b[n][int(e)].any()), f"{n}[{e}] must be exactly zero for an empty expert"
+    if name == "C4z":
+        assert (rt["counts"] == 0).sum() >= 4
+    if cfg.I_shared:
+        Js = np.sort(rng.choice(cfg.I_shared, 2, replace=False)).astype(np.int64)
+        Jsc = torch.from_numpy(Js).cuda()
+        rg, ru, rd = oracle.sample_wgrad_shared(cfg, inp, Js)
+        util.check_close("dws_gate[:,J]", util.to_np(b["dws_gate"][:, Jsc]), rg, dt)
+        util.check_close("dws_up[:,J]", util.to_np(b["dws_up"][:, Jsc]), ru, dt)
+        util.check_close("dws_down[J,:]", util.to_np(b["dws_down"][Jsc, :]), rd, dt)
     ctx.close()
