@@ -79,6 +79,9 @@ const char* piper_last_cuda_error(const piper_ctx* ctx);
 int64_t piper_kernel_launches(const piper_ctx* ctx);
 /* Which GEMM family serves the routed experts of this context: 1 = tcgen05/TMEM/TMA, 0 = FP32 ALUs. */
 int piper_gemm_path(const piper_ctx* ctx);
+/* Debug (PIPER_TC_PROFILE=1 in the environment at piper_create): device pointer to the wait-cycle counters
+ * the tcgen05 kernels wrote, [16 launches (cycled)][160 CTAs][8] int64; NULL when profiling is off. */
+const void* piper_debug_tc_counters(const piper_ctx* ctx);
 /* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */
 int64_t piper_a_cap(const piper_moe_desc* desc);
 

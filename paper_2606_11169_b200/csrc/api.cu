@@ -111,6 +111,7 @@ int piper_gemm_path(const piper_ctx* c) {
     piper_chunk_args a{};
     return tc_supported(c, routed_problem(c, &a)) ? 1 : 0;
 }
+const void* piper_debug_tc_counters(const piper_ctx* c) { return c && c->tc_prof ? c->tc_scratch : nullptr; }
 int piper_pair_partition_mode(const piper_ctx* c) { return c ? c->pair_mode : 0; }
 
 int piper_route_topk(piper_ctx* c, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global,

@@ -31,6 +31,7 @@ constexpr int kThreads = 256;
 constexpr int kMaxGroups = kMaxE;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/ +
                            (kMaxGroups + 1) * 4 /*tile prefix*/;
+constexpr int kProfSlots = 16, kProfSlotWords = 160 * 8;  // debug counters: 16 launches x 160 CTAs x 8 words
 constexpr int PANEL_M = 8;  // M tiles per panel of the tile order (L2 reuse of the weight tile)
 
 enum : int { K_MAJOR = 0, MN_MAJOR = 1 };
@@ -53,6 +54,7 @@ struct alignas(64) TcParams {
     long long group_stride;  // wgrad: elements between two experts' dW
     __nv_bfloat16 *out0, *out1, *out2;
     const __nv_bfloat16 *in0, *in1;
+    long long* prof;  // debug (PIPER_TC_PROFILE=1): [gridDim.x][8] wait-cycle counters, else NULL
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------------
@@ -254,11 +256,14 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
     if (warp == 0) {
         // ===== TMA producer =====
         int stage = 0, phase = 0;
+        long long w_empty = 0;
         for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
             const Tile T = decode_tile(P, tp, offsets, t);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
+                    if (P.prof) w_empty += clock64() - c0;
                     uint8_t* sa = smem + stage * STAGE_BYTES;
                     uint8_t* sb = sa + A_BYTES;
                     uint64_t* bar = &full_bar[stage];
@@ -291,23 +296,30 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
                 if (++stage == STAGES) stage = 0, phase ^= 1;
             }
         }
+        if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1) {
         // ===== MMA issuer (one thread) =====
         constexpr uint32_t idesc = make_idesc(A_MAJOR, B_MAJOR);
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
         int stage = 0, phase = 0, as = 0, aphase = 0;
+        long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
+        const long long t_begin = P.prof ? clock64() : 0;
         for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
             const Tile T = decode_tile(P, tp, offsets, t);
             if (lane == 0) {
+                const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
+                if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
             __syncwarp();
             const uint32_t d_tmem = tmem_base + as * BN;
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&full_bar[stage], phase);
+                    if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
 #pragma unroll
@@ -325,14 +337,22 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
+        if (P.prof && lane == 0) {
+            long long* q = P.prof + blockIdx.x * 8;
+            q[0] = w_full, q[1] = w_tempty, q[2] = clock64() - t_begin, q[6] = n_tiles_done;
+        }
     } else if (warp >= 4) {
         // ===== epilogue: warp w owns TMEM lanes 32 (w % 4) .. +31 = tile rows =====
         const int wq = warp & 3, row = wq * 32 + lane;
         int as = 0, aphase = 0;
+        long long w_tfull = 0;
+        const long long t_begin = P.prof ? clock64() : 0;
         const int rows_total = P.ragged_m ? offsets[P.G] : P.m_limit;
         for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
             const Tile T = decode_tile(P, tp, offsets, t);
+            const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
+            if (P.prof) w_tfull += clock64() - c0;
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
             const int grow = T.m0 + row;
@@ -396,6 +416,7 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
             mbar_arrive(&tempty_bar[as]);
             if (++as == 2) as = 0, aphase ^= 1;
         }
+        if (P.prof && threadIdx.x == 128) P.prof[blockIdx.x * 8 + 4] = w_tfull, P.prof[blockIdx.x * 8 + 5] = clock64() - t_begin;
     }
     tc_fence_before();
     __syncthreads();
@@ -438,7 +459,12 @@ template <int A_MAJOR, int B_MAJOR, int EPI>
 int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
     long long grid = tile_bound < ln.sms ? tile_bound : ln.sms;
     if (grid < 1) grid = 1;
-    tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)grid, kThreads, SMEM_BYTES, ln.stream>>>(P);
+    TcParams Q = P;
+    if (c->tc_prof) {  // debug: slot per launch, cycled
+        Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
+        c->tc_next_slot += 1;
+    }
+    tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)grid, kThreads, SMEM_BYTES, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
 }
@@ -459,7 +485,7 @@ inline long long m_tile_bound(const FfnProblem& p) { return cdiv(p.max_rows, BM)
 
 }  // namespace
 
-size_t tc_scratch_bytes(const piper_moe_desc*) { return 256; }
+size_t tc_scratch_bytes(const piper_moe_desc*) { return (size_t)kProfSlots * kProfSlotWords * 8; }
 
 int tc_init(piper_ctx* c) {
     void* fn = nullptr;
@@ -469,6 +495,8 @@ int tc_init(piper_ctx* c) {
         fn = nullptr;
     cudaGetLastError();
     c->encode_tiled = fn;
+    const char* pe = getenv("PIPER_TC_PROFILE");
+    c->tc_prof = pe && pe[0] == '1';
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
               set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>();

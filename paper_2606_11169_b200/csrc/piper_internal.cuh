@@ -7,6 +7,7 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -46,6 +47,7 @@ struct piper_ctx {
     piper::GreenPartition* green;
     char* tc_scratch;        // tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
     int tc_next_slot;        // round-robin slot in tc_scratch
+    int tc_prof;             // PIPER_TC_PROFILE=1: the tcgen05 kernels record wait-cycle counters in tc_scratch
     cudaEvent_t events[piper::kMaxEvents];
 };
 
