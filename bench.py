@@ -171,6 +171,26 @@ def task_work(cfg, A: int, t_touched: int):
     return w
 
 
+# ------------------------------------------------------------------------------- multi-rank glue
+def rank_config(cfg, rank: int):
+    """Every rank runs its own microbatch of the same layer shape (replicas, weak scaling): seed + 1000*rank."""
+    return dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+
+
+def max_over_ranks(ms: float, world: int, device):
+    """The slowest rank's time (all-reduce MAX over the default process group; identity at world 1)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_tokens_per_s(cfg, world: int, ms_per_step: float) -> float:
+    return world * cfg.T / (ms_per_step * 1e-3)
+
+
 # ----------------------------------------------------------------------------------- piper arm
 INPUT_NAMES = ("logits", "x", "dy", "w_gate", "w_up", "w_down", "ws_gate", "ws_up", "ws_down")
 
@@ -203,7 +223,7 @@ def run_piper(args, cfg):
         torch.cuda.synchronize()
 
     # every rank: its own microbatch of the same layer shape (weak scaling, no data-path collective)
-    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    rcfg = rank_config(cfg, rank)
     t0 = time.time()
     inp = configs.make_inputs(rcfg)
     log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
@@ -234,11 +254,8 @@ def run_piper(args, cfg):
     sampler.join()
     launches = piper.piper_kernel_launches(ctx) - launches0
     ms = ev0.elapsed_time(ev1)
-    tms = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms_per_step = float(tms.item()) / args.steps
-    value = world * cfg.T / (ms_per_step * 1e-3)
+    ms_per_step = max_over_ranks(ms, world, dev) / args.steps
+    value = whole_job_tokens_per_s(cfg, world, ms_per_step)
 
     # ---- e2e: pinned host inputs -> device, the same two C-ABI calls, results -> pinned host ----------
     host_in = {n: piper.to_tensor(inp[n], "cpu").pin_memory() for n in ("logits", "x", "dy")}
@@ -264,11 +281,8 @@ def run_piper(args, cfg):
     ev1.record(stream)
     barrier()
     wall_ms = (time.perf_counter() - w0) * 1e3
-    tms = torch.tensor([max(ev0.elapsed_time(ev1), wall_ms)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    e2e_ms = float(tms.item()) / args.steps
-    e2e = {"value": world * cfg.T / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+    e2e_ms = max_over_ranks(max(ev0.elapsed_time(ev1), wall_ms), world, dev) / args.steps
+    e2e = {"value": whole_job_tokens_per_s(cfg, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
            "what": "pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel -> pinned "
                    "host; timed as max(CUDA events, host wall clock)"}
