@@ -151,51 +151,60 @@ __device__ __forceinline__ float dot_packets(const int4& a, const int4& b) {
     return s;
 }
 
+// ---- row movers: common shape ----------------------------------------------------------------------
+// Work item = (token, column split): a warp moves `U` 16-byte packets per lane per step (2 KB per warp and
+// source row), with the next source row's packets already in flight while the current ones are consumed.
+// Splitting a row over several items keeps every resident warp busy when T is small (no cross-split
+// reduction exists in pack / combine / unpack; combine_bwd's dot products need the whole row and do not
+// split).  No per-thread arrays indexed at run time: row indices are re-read from row_of (L1 hits).
+constexpr int U = 4;                 // packets per lane per step
+constexpr int kStep = 32 * U;        // packets per warp per step
+
+__device__ __forceinline__ void load_step(int4 (&v)[U], const int4* __restrict__ src, int p0, int lane, int hi) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int p = p0 + u * 32 + lane;
+        v[u] = p < hi ? ld_nc16(src + p) : make_int4(0, 0, 0, 0);
+    }
+}
+
 // ---- F3 dispatch_pack ----------------------------------------------------------------------------
-// Work items [0,T): token t -> copy x[t] into each of its local rows, scatter its gates.
-// Work items [T, T+A_cap): row r -> if it is a pad row inside [0, offsets[E_loc]) zero it.
+// Token items [0, T*S): copy the split's columns of x[t] into each local row of the token; split 0 also
+// scatters the token's gates.  Row items [T*S, T*S + a_cap): zero the pad rows inside [0, offsets[E_loc]).
 __global__ void __launch_bounds__(kMoveWarps * 32)
 pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const int32_t* __restrict__ offsets,
             const int32_t* __restrict__ row_of, const int32_t* __restrict__ src_of, int T, int k, int E_loc, int a_cap,
-            int row_packets, float* __restrict__ gate_rows, int4* __restrict__ xp) {
+            int row_packets, int S, int split_packets, float* __restrict__ gate_rows, int4* __restrict__ xp) {
     const int lane = threadIdx.x & 31;
     const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
     const int nwarps = gridDim.x * kMoveWarps;
     const int used = offsets[E_loc];
-    for (int item = warp; item < T + a_cap; item += nwarps) {
-        if (item < T) {
-            const int t = item;
-            int rows[kMaxK];
-            int n = 0;
-#pragma unroll
-            for (int j = 0; j < kMaxK; ++j)
-                if (j < k) {
-                    const int r = row_of[(size_t)t * k + j];
-                    if (r >= 0) {
-                        rows[n++] = r;
-                        if (lane == 0) gate_rows[r] = gates[(size_t)t * k + j];
-                    }
-                }
-            if (n == 0) continue;
+    const int n_tok_items = T * S;
+    for (int item = warp; item < n_tok_items + a_cap; item += nwarps) {
+        if (item < n_tok_items) {
+            const int t = item / S, sp = item - t * S;
+            const int32_t* ro = row_of + (size_t)t * k;
+            const int my_row = lane < k ? ro[lane] : -1;
+            if (__ballot_sync(0xffffffffu, my_row >= 0) == 0) continue;
+            if (sp == 0 && my_row >= 0) gate_rows[my_row] = gates[(size_t)t * k + lane];
+            const int lo = sp * split_packets, hi = min(row_packets, lo + split_packets);
             const int4* src = x + (size_t)t * row_packets;
-            for (int p0 = 0; p0 < row_packets; p0 += 128) {
-                int4 v[4];
+            for (int p0 = lo; p0 < hi; p0 += kStep) {
+                int4 v[U];
+                load_step(v, src, p0, lane, hi);
+                for (int j = 0; j < k; ++j) {
+                    const int r = __shfl_sync(0xffffffffu, my_row, j);
+                    if (r < 0) continue;
+                    int4* dst = xp + (size_t)r * row_packets;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int p = p0 + u * 32 + lane;
-                    if (p < row_packets) v[u] = ld_nc16(src + p);
-                }
-                for (int q = 0; q < n; ++q) {
-                    int4* dst = xp + (size_t)rows[q] * row_packets;
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
+                    for (int u = 0; u < U; ++u) {
                         const int p = p0 + u * 32 + lane;
-                        if (p < row_packets) st16(dst + p, v[u]);
+                        if (p < hi) st16(dst + p, v[u]);
                     }
                 }
             }
         } else {
-            const int r = item - T;
+            const int r = item - n_tok_items;
             if (r >= used || src_of[r] >= 0) continue;
             if (lane == 0) gate_rows[r] = 0.f;
             int4* dst = xp + (size_t)r * row_packets;
@@ -206,60 +215,68 @@ pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const i
 
 // ---- F5 combine / B5 unpack ------------------------------------------------------------------------
 // y[t] = sum_{j local} w_j * o[row_of[t,j]] (+ s[t]);  WEIGHTED: w_j = gates[t,j], else 1 (unpack).
-// fp32 accumulation, one rounding on store.
+// fp32 accumulation in slot order j = 0..k-1 then s, one rounding on store.
 template <bool BF16, bool WEIGHTED>
 __global__ void __launch_bounds__(kMoveWarps * 32)
 combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, const float* __restrict__ gates,
-               const int4* __restrict__ s, int T, int k, int row_packets, int4* __restrict__ y) {
+               const int4* __restrict__ s, int T, int k, int row_packets, int S, int split_packets,
+               int4* __restrict__ y) {
     const int lane = threadIdx.x & 31;
     const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
     const int nwarps = gridDim.x * kMoveWarps;
-    for (int t = warp; t < T; t += nwarps) {
-        int rows[kMaxK];
-        float w[kMaxK];
-        int n = 0;
+    const int n_src = k + (s != nullptr ? 1 : 0);
+    for (int item = warp; item < T * S; item += nwarps) {
+        const int t = item / S, sp = item - t * S;
+        const int my_row = lane < k ? row_of[(size_t)t * k + lane] : -1;
+        const float my_w = (WEIGHTED && lane < k) ? gates[(size_t)t * k + lane] : 1.f;
+        const int lo = sp * split_packets, hi = min(row_packets, lo + split_packets);
+        for (int p0 = lo; p0 < hi; p0 += kStep) {
+            float acc[U][8];
 #pragma unroll
-        for (int j = 0; j < kMaxK; ++j)
-            if (j < k) {
-                const int r = row_of[(size_t)t * k + j];
-                if (r >= 0) {
-                    w[n] = WEIGHTED ? gates[(size_t)t * k + j] : 1.f;
-                    rows[n++] = r;
-                }
-            }
-        for (int p0 = 0; p0 < row_packets; p0 += 64) {
-            float acc[2][8];
-#pragma unroll
-            for (int u = 0; u < 2; ++u)
+            for (int u = 0; u < U; ++u)
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[u][q] = 0.f;
-            for (int q = 0; q < n; ++q) {
-                const int4* src = o + (size_t)rows[q] * row_packets;
-                int4 v[2];
+            int4 cur[U];
+            float wc = 0.f;
+            bool have = false;
+            for (int j = 0; j < n_src; ++j) {
+                const int4* src;
+                float w = 1.f;
+                if (j < k) {
+                    const int r = __shfl_sync(0xffffffffu, my_row, j);
+                    w = __shfl_sync(0xffffffffu, my_w, j);
+                    if (r < 0) continue;
+                    src = o + (size_t)r * row_packets;
+                } else {
+                    src = s + (size_t)t * row_packets;
+                }
+                int4 nxt[U];
+                load_step(nxt, src, p0, lane, hi);  // in flight while the previous source is accumulated
+                if (have) {
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int p = p0 + u * 32 + lane;
-                    if (p < row_packets) v[u] = ld_nc16(src + p);
+                    for (int u = 0; u < U; ++u) unpack_add<BF16>(cur[u], acc[u], wc);
                 }
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
-                    if (p0 + u * 32 + lane < row_packets) unpack_add<BF16>(v[u], acc[u], w[q]);
+                for (int u = 0; u < U; ++u) cur[u] = nxt[u];
+                wc = w, have = true;
+            }
+            if (have) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) unpack_add<BF16>(cur[u], acc[u], wc);
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < U; ++u) {
                 const int p = p0 + u * 32 + lane;
-                if (p < row_packets) {
-                    if (s != nullptr) unpack_add<BF16>(ld_nc16(s + (size_t)t * row_packets + p), acc[u], 1.f);
-                    st16(y + (size_t)t * row_packets + p, pack_out<BF16>(acc[u]));
-                }
+                if (p < hi) st16(y + (size_t)t * row_packets + p, pack_out<BF16>(acc[u]));
             }
         }
     }
 }
 
 // ---- B1 combine_bwd ---------------------------------------------------------------------------------
-// Token items: d_o[row] = gates[t,j] * dy[t]; dgates[t,j] = <dy[t], o[row]> (0 for non-local slots).
-// Row items: zero the pad rows of d_o inside [0, offsets[E_loc]).
+// Token items: for every local slot j: d_o[row] = gates[t,j] * dy[t]; dgates[t,j] = <dy[t], o[row]> (0 for
+// non-local slots).  Slot-outer loop: dy[t] is re-read per local slot (L1/L2 hits), the dot product stays a
+// scalar.  Row items: zero the pad rows of d_o inside [0, offsets[E_loc]).
 template <bool BF16>
 __global__ void __launch_bounds__(kMoveWarps * 32)
 combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, const int32_t* __restrict__ src_of,
@@ -273,57 +290,39 @@ combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, cons
     for (int item = warp; item < T + a_cap; item += nwarps) {
         if (item < T) {
             const int t = item;
-            int rows[kMaxK], slot[kMaxK];
-            float w[kMaxK], dots[kMaxK];
-            int n = 0;
-#pragma unroll
-            for (int j = 0; j < kMaxK; ++j)
-                if (j < k) {
-                    const int r = row_of[(size_t)t * k + j];
-                    if (r >= 0) {
-                        w[n] = gates[(size_t)t * k + j];
-                        slot[n] = j;
-                        dots[n] = 0.f;
-                        rows[n++] = r;
-                    } else if (lane == 0) {
-                        dgates[(size_t)t * k + j] = 0.f;
-                    }
-                }
-            if (n == 0) continue;
+            const int my_row = lane < k ? row_of[(size_t)t * k + lane] : -1;
+            const float my_w = lane < k ? gates[(size_t)t * k + lane] : 0.f;
+            if (lane < k && my_row < 0) dgates[(size_t)t * k + lane] = 0.f;
             const int4* src = dy + (size_t)t * row_packets;
-            for (int p0 = 0; p0 < row_packets; p0 += 64) {
-                int4 v[2];
+            for (int j = 0; j < k; ++j) {
+                const int r = __shfl_sync(0xffffffffu, my_row, j);
+                const float w = __shfl_sync(0xffffffffu, my_w, j);
+                if (r < 0) continue;
+                const int4* orow = o + (size_t)r * row_packets;
+                int4* drow = d_o + (size_t)r * row_packets;
+                float dot = 0.f;
+                for (int p0 = 0; p0 < row_packets; p0 += kStep) {
+                    int4 v[U], ov[U];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int p = p0 + u * 32 + lane;
-                    if (p < row_packets) v[u] = ld_nc16(src + p);
-                }
-                for (int q = 0; q < n; ++q) {
-                    const int4* orow = o + (size_t)rows[q] * row_packets;
-                    int4* drow = d_o + (size_t)rows[q] * row_packets;
-                    int4 ov[2];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
+                    for (int u = 0; u < U; ++u) {
                         const int p = p0 + u * 32 + lane;
-                        if (p < row_packets) ov[u] = ld_nc16(orow + p);
+                        v[u] = p < row_packets ? __ldg(src + p) : make_int4(0, 0, 0, 0);
                     }
+                    load_step(ov, orow, p0, lane, row_packets);
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
+                    for (int u = 0; u < U; ++u) {
                         const int p = p0 + u * 32 + lane;
                         if (p < row_packets) {
-                            dots[q] += dot_packets<BF16>(v[u], ov[u]);
+                            dot += dot_packets<BF16>(v[u], ov[u]);
                             float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-                            unpack_add<BF16>(v[u], acc, w[q]);
+                            unpack_add<BF16>(v[u], acc, w);
                             st16(drow + p, pack_out<BF16>(acc));
                         }
                     }
                 }
-            }
-            for (int q = 0; q < n; ++q) {
-                float sdot = dots[q];
 #pragma unroll
-                for (int off = 16; off > 0; off >>= 1) sdot += __shfl_xor_sync(0xffffffffu, sdot, off);
-                if (lane == 0) dgates[(size_t)t * k + slot[q]] = sdot;
+                for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, off);
+                if (lane == 0) dgates[(size_t)t * k + j] = dot;
             }
         } else {
             const int r = item - T;
@@ -334,9 +333,23 @@ combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, cons
     }
 }
 
-inline int mover_blocks(Lane ln, int items) {
+// Column splits per token so that about two items exist per resident warp of the lane.
+inline void choose_split(Lane ln, int T, int row_packets, int& S, int& split_packets) {
+    const int warps = ln.sms * 48;
+    int want = (2 * warps + T - 1) / T;
+    const int max_s = (row_packets + kStep - 1) / kStep;
+    if (want > max_s) want = max_s;
+    if (want < 1) want = 1;
+    split_packets = ((row_packets + want - 1) / want + kStep - 1) / kStep * kStep;
+    S = (row_packets + split_packets - 1) / split_packets;
+}
+
+// Grid: one warp per item up to a few waves of resident blocks (more, shorter-lived blocks than fit at once
+// measured faster than an exactly-resident persistent grid: finishing blocks are replaced at once).
+template <typename K>
+inline int mover_blocks(Lane ln, int items, K) {
     int blocks = cdiv(items, kMoveWarps);
-    const int cap = ln.sms * 8;  // 8 blocks x 8 warps = 64 resident warps per SM
+    const int cap = ln.sms * 16;
     return blocks < cap ? (blocks < 1 ? 1 : blocks) : cap;
 }
 
@@ -365,9 +378,11 @@ int launch_pack(piper_ctx* c, Lane ln, const void* x, const float* gates, const 
     const piper_moe_desc& D = c->D;
     const int a_cap = (int)piper_a_cap(&D);
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
-    pack_kernel<<<mover_blocks(ln, D.T + a_cap), kMoveWarps * 32, 0, ln.stream>>>(
-        static_cast<const int4*>(x), gates, offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, gate_rows,
-        static_cast<int4*>(xp));
+    int S, split_packets;
+    choose_split(ln, D.T, row_packets, S, split_packets);
+    pack_kernel<<<mover_blocks(ln, D.T * S + a_cap, pack_kernel), kMoveWarps * 32, 0, ln.stream>>>(
+        static_cast<const int4*>(x), gates, offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, S,
+        split_packets, gate_rows, static_cast<int4*>(xp));
     PIPER_LAUNCHED(c, "pack_kernel");
     return PIPER_OK;
 }
@@ -376,11 +391,13 @@ int launch_combine(piper_ctx* c, Lane ln, const void* o, const int32_t* row_of, 
                    void* y, bool weighted) {
     const piper_moe_desc& D = c->D;
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
-    const int blocks = mover_blocks(ln, D.T);
+    int S, split_packets;
+    choose_split(ln, D.T, row_packets, S, split_packets);
+    const int items = D.T * S;
     const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s);
     int4* y4 = static_cast<int4*>(y);
-#define PIPER_COMBINE(BF, W) \
-    combine_kernel<BF, W><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, D.T, D.k, row_packets, y4)
+#define PIPER_COMBINE(BF, W)                                                                              \
+    combine_kernel<BF, W><<<mover_blocks(ln, items, combine_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, D.T, D.k, row_packets, S, split_packets, y4)
     if (D.dtype == PIPER_DTYPE_BF16) {
         if (weighted) PIPER_COMBINE(true, true); else PIPER_COMBINE(true, false);
     } else {
@@ -396,13 +413,12 @@ int launch_combine_bwd(piper_ctx* c, Lane ln, const void* dy, const void* o, con
     const piper_moe_desc& D = c->D;
     const int a_cap = (int)piper_a_cap(&D);
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
-    const int blocks = mover_blocks(ln, D.T + a_cap);
     if (D.dtype == PIPER_DTYPE_BF16)
-        combine_bwd_kernel<true><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(
+        combine_bwd_kernel<true><<<mover_blocks(ln, D.T + a_cap, combine_bwd_kernel<true>), kMoveWarps * 32, 0, ln.stream>>>(
             static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
             D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
     else
-        combine_bwd_kernel<false><<<blocks, kMoveWarps * 32, 0, ln.stream>>>(
+        combine_bwd_kernel<false><<<mover_blocks(ln, D.T + a_cap, combine_bwd_kernel<false>), kMoveWarps * 32, 0, ln.stream>>>(
             static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
             D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
     PIPER_LAUNCHED(c, "combine_bwd_kernel");
