@@ -219,6 +219,65 @@ __device__ __forceinline__ void load16(const __nv_bfloat16* row_ptr, int col, in
     unpack8(q0, v), unpack8(q1, v + 8);
 }
 
+// One accumulator tile (this thread's TMEM lane = one output row) -> fused math -> global.
+template <int EPI>
+__device__ __forceinline__ void epilogue_tile(const TcParams& P, uint32_t taddr, bool row_ok, bool zero, long long base,
+                                              int n0) {
+                if (EPI == EPI_SWIGLU_FWD || EPI == EPI_WGRAD_SPLIT) {
+    #pragma unroll 1
+                    for (int c = 0; c < 128; c += 16) {
+                        uint32_t r0[16], r1[16];
+                        tmem_ld16(taddr + c, r0);
+                        tmem_ld16(taddr + 128 + c, r1);
+                        tmem_ld_wait(r0);
+                        tmem_ld_wait(r1);
+                        float v0[16], v1[16], h[16];
+    #pragma unroll
+                        for (int i = 0; i < 16; ++i) {
+                            v0[i] = zero ? 0.f : __uint_as_float(r0[i]);
+                            v1[i] = zero ? 0.f : __uint_as_float(r1[i]);
+                        }
+                        if (row_ok) {
+                            store16(P.out0 + base, n0 + c, P.n_limit, v0);
+                            store16(P.out1 + base, n0 + c, P.n_limit, v1);
+                            if (EPI == EPI_SWIGLU_FWD) {
+    #pragma unroll
+                                for (int i = 0; i < 16; ++i) h[i] = v0[i] * sigmoidf_fast(v0[i]) * v1[i];
+                                store16(P.out2 + base, n0 + c, P.n_limit, h);
+                            }
+                        }
+                    }
+                } else {
+    #pragma unroll 1
+                    for (int c = 0; c < BN; c += 16) {
+                        uint32_t r0[16];
+                        tmem_ld16(taddr + c, r0);
+                        tmem_ld_wait(r0);
+                        float v[16];
+    #pragma unroll
+                        for (int i = 0; i < 16; ++i) v[i] = zero ? 0.f : __uint_as_float(r0[i]);
+                        if (row_ok) {
+                            if (EPI == EPI_SWIGLU_BWD) {
+                                // v = dH; dG = dH * U * silu'(G), dU = dH * silu(G)
+                                float gv[16], uv[16], dg[16], du[16];
+                                load16(P.in0 + base, n0 + c, P.n_limit, gv);
+                                load16(P.in1 + base, n0 + c, P.n_limit, uv);
+    #pragma unroll
+                                for (int i = 0; i < 16; ++i) {
+                                    const float s = sigmoidf_fast(gv[i]);
+                                    dg[i] = v[i] * uv[i] * (s * (1.f + gv[i] * (1.f - s)));
+                                    du[i] = v[i] * (gv[i] * s);
+                                }
+                                store16(P.out0 + base, n0 + c, P.n_limit, dg);
+                                store16(P.out1 + base, n0 + c, P.n_limit, du);
+                            } else {
+                                store16(P.out0 + base, n0 + c, P.n_limit, v);
+                            }
+                        }
+                    }
+                }
+}
+
 // ---- the kernel ---------------------------------------------------------------------------------------
 template <int A_MAJOR, int B_MAJOR, int EPI>
 __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_constant__ TcParams P) {
@@ -359,59 +418,7 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
             const bool row_ok = grow < rows_total;
             const bool zero = T.nkb == 0;  // empty expert in wgrad: exact zeros, the accumulator is stale
             const long long base = (P.ragged_m ? 0 : (long long)T.g * P.group_stride) + (long long)grow * P.ld;
-            if (EPI == EPI_SWIGLU_FWD || EPI == EPI_WGRAD_SPLIT) {
-#pragma unroll 1
-                for (int c = 0; c < 128; c += 16) {
-                    uint32_t r0[16], r1[16];
-                    tmem_ld16(taddr + c, r0);
-                    tmem_ld16(taddr + 128 + c, r1);
-                    tmem_ld_wait(r0);
-                    tmem_ld_wait(r1);
-                    float v0[16], v1[16], h[16];
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        v0[i] = zero ? 0.f : __uint_as_float(r0[i]);
-                        v1[i] = zero ? 0.f : __uint_as_float(r1[i]);
-                    }
-                    if (row_ok) {
-                        store16(P.out0 + base, T.n0 + c, P.n_limit, v0);
-                        store16(P.out1 + base, T.n0 + c, P.n_limit, v1);
-                        if (EPI == EPI_SWIGLU_FWD) {
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) h[i] = v0[i] * sigmoidf_fast(v0[i]) * v1[i];
-                            store16(P.out2 + base, T.n0 + c, P.n_limit, h);
-                        }
-                    }
-                }
-            } else {
-#pragma unroll 1
-                for (int c = 0; c < BN; c += 16) {
-                    uint32_t r0[16];
-                    tmem_ld16(taddr + c, r0);
-                    tmem_ld_wait(r0);
-                    float v[16];
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) v[i] = zero ? 0.f : __uint_as_float(r0[i]);
-                    if (row_ok) {
-                        if (EPI == EPI_SWIGLU_BWD) {
-                            // v = dH; dG = dH * U * silu'(G), dU = dH * silu(G)
-                            float gv[16], uv[16], dg[16], du[16];
-                            load16(P.in0 + base, T.n0 + c, P.n_limit, gv);
-                            load16(P.in1 + base, T.n0 + c, P.n_limit, uv);
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                const float s = sigmoidf_fast(gv[i]);
-                                dg[i] = v[i] * uv[i] * (s * (1.f + gv[i] * (1.f - s)));
-                                du[i] = v[i] * (gv[i] * s);
-                            }
-                            store16(P.out0 + base, T.n0 + c, P.n_limit, dg);
-                            store16(P.out1 + base, T.n0 + c, P.n_limit, du);
-                        } else {
-                            store16(P.out0 + base, T.n0 + c, P.n_limit, v);
-                        }
-                    }
-                }
-            }
+            epilogue_tile<EPI>(P, taddr, row_ok, zero, base, T.n0);
             tc_fence_before();
             mbar_arrive(&tempty_bar[as]);
             if (++as == 2) as = 0, aphase ^= 1;
@@ -423,6 +430,267 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
     if (warp == 2) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// =====================================================================================================
+// 2-CTA variant: a cluster of two CTAs (one TPC) works on two M tiles that share one B tile.  The leader CTA
+// issues tcgen05.mma.cta_group::2 (M = 256: rows 0-127 accumulate in the leader's TMEM, 128-255 in the
+// peer's); each CTA stages its own 128 x 64 A tile and one 128-column half of the 256 x 64 B tile, so a
+// stage costs 32 KB per CTA instead of 48 KB: one third less L2 -> SM traffic (the measured limiter of the
+// 1-CTA kernel) and a 6-stage ring.  The two M tiles need not be adjacent: in the ragged problems they are
+// two tiles of the same expert (an odd last tile is paired with a duplicate whose stores are skipped); in
+// wgrad they are two 128-row slices of dW.
+// =====================================================================================================
+constexpr int STAGES2 = 6;
+constexpr int A2_BYTES = BM * BK * 2, B2_BYTES = (BN / 2) * BK * 2, STAGE2_BYTES = A2_BYTES + B2_BYTES;
+constexpr int SMEM2_BYTES = STAGES2 * STAGE2_BYTES + 1024 + 256 + 2 * (kMaxGroups + 1) * 4;
+constexpr int PANEL_PAIRS = 4;
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_alloc2(uint32_t* dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(cols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc2(uint32_t taddr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+// D[tmem of both CTAs] (+)= A * B, 256 x 256 x 16 across the CTA pair
+__device__ __forceinline__ void umma2_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// arrives on the barrier at this offset in BOTH CTAs once the MMAs issued so far have completed
+__device__ __forceinline__ void umma2_commit(uint64_t* bar) {
+    asm volatile(
+        "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+            smem_u32(bar)),
+        "h"((uint16_t)3)
+        : "memory");
+}
+__host__ __device__ constexpr uint32_t make_idesc2(int a_major, int b_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_major << 15) | ((uint32_t)b_major << 16) |
+           ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((2 * BM) >> 4) << 24);
+}
+
+struct Tile2 {
+    int g, m0, n0, k0, nkb;
+    bool store;  // false: this CTA's M tile duplicates the leader's (odd tile count), nothing is stored
+};
+
+// tp[g] = first M tile of group g; tpp[g] = first tile PAIR of group g (ragged_m).
+__device__ __forceinline__ int total_pairs(const TcParams& P, const int* tpp) {
+    return P.ragged_m ? tpp[P.G] * P.n_tiles : P.G * ((P.m_tiles + 1) / 2) * P.n_tiles;
+}
+__device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, const int* tpp,
+                                             const int32_t* __restrict__ offsets, int t, int rank) {
+    Tile2 r;
+    if (P.ragged_m) {
+        int g = 0;
+        while (g + 1 < P.G && tpp[g + 1] * P.n_tiles <= t) ++g;
+        const int local = t - tpp[g] * P.n_tiles, mg = tp[g + 1] - tp[g], pg = tpp[g + 1] - tpp[g];
+        const int per_panel = PANEL_PAIRS * P.n_tiles;
+        const int panel = local / per_panel, rem = local - panel * per_panel;
+        const int pp = min(PANEL_PAIRS, pg - panel * PANEL_PAIRS);
+        const int nt = rem / pp, pair = panel * PANEL_PAIRS + (rem - nt * pp);
+        int mt = 2 * pair + rank;
+        r.store = mt < mg;
+        if (!r.store) mt = 2 * pair;
+        r.g = g, r.m0 = (tp[g] + mt) * BM, r.n0 = nt * P.tile_n, r.k0 = 0, r.nkb = P.kb_per_src * P.n_src;
+    } else {
+        const int pairs = (P.m_tiles + 1) / 2, per_group = pairs * P.n_tiles;
+        const int g = t / per_group, local = t - g * per_group;
+        const int nt = local / pairs, pair = local - nt * pairs;
+        const int lo = offsets[g], hi = offsets[g + 1];
+        r.store = true;  // rows beyond m_limit are clipped by the bounds checks
+        r.g = g, r.m0 = (2 * pair + rank) * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + BK - 1) / BK;
+    }
+    return r;
+}
+
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+// TMA load into this CTA's shared memory, bytes counted on the mbarrier at cluster address `bar_cluster`
+__device__ __forceinline__ void tma_load_3d_pair(void* dst, const CUtensorMap* map, uint32_t bar_cluster, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
+
+template <int A_MAJOR, int B_MAJOR, int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES2 * STAGE2_BYTES);  // used in the leader CTA
+    uint64_t* empty_bar = full_bar + STAGES2;                                          // one set per CTA
+    uint64_t* tfull_bar = empty_bar + STAGES2;                                         // [2] one set per CTA
+    uint64_t* tempty_bar = tfull_bar + 2;                                              // [2] used in the leader CTA
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tempty_bar + 2);
+    int* tp = reinterpret_cast<int*>(smem + STAGES2 * STAGE2_BYTES + 256);
+    int* tpp = tp + (kMaxGroups + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rank = (int)cluster_ctarank();
+    const int pair_id = blockIdx.x >> 1, n_pairs_grid = gridDim.x >> 1;
+    const int32_t* __restrict__ offsets = P.offsets;
+
+    if (P.ragged_m) {
+        for (int g = threadIdx.x; g <= P.G; g += kThreads) tp[g] = (offsets[g] + BM - 1) / BM;
+        __syncthreads();
+        if (warp == 3) {  // exclusive scan of the tile pairs per group
+            int carry = 0;
+            for (int g0 = 0; g0 < P.G; g0 += 32) {
+                const int g = g0 + lane;
+                const int v = g < P.G ? (tp[g + 1] - tp[g] + 1) >> 1 : 0;
+                int x = v;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                if (g < P.G) tpp[g] = carry + x - v;
+                carry += __shfl_sync(0xffffffffu, x, 31);
+            }
+            if (lane == 0) tpp[P.G] = carry;
+        }
+    }
+    if (warp == 0 && lane == 0) {
+        prefetch_tmap(&P.a[0]), prefetch_tmap(&P.b[0]);
+        if (P.n_src == 2) prefetch_tmap(&P.a[1]);
+        if (P.n_src == 2 || P.b_split) prefetch_tmap(&P.b[1]);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES2; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
+        for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
+        fence_barrier_init();
+    }
+    if (warp == 2) tmem_alloc2(tmem_ptr, 512);
+    tc_fence_before();
+    cluster_sync_all();  // barriers of both CTAs initialised before any remote arrive / multicast commit
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+    const int n_total = total_pairs(P, tpp);
+
+    if (warp == 0) {
+        // ===== TMA producer (both CTAs): own A tile + own 128-column half of B, counted on the leader's barrier =====
+        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        int stage = 0, phase = 0;
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    uint8_t* sa = smem + stage * STAGE2_BYTES;
+                    uint8_t* sb = sa + A2_BYTES;
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * STAGE2_BYTES);
+                    const uint32_t bar = leader_full + stage * 8;
+                    int src = 0, kk = kb;
+                    if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
+                    const int k = T.k0 + kk * BK;
+                    if (A_MAJOR == K_MAJOR) {
+                        tma_load_3d_pair(sa, &P.a[src], bar, k, T.m0, 0);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < BM / 64; ++j)
+                            tma_load_3d_pair(sa + j * MN_BLOCK_BYTES, &P.a[src], bar, T.m0 + 64 * j, k, 0);
+                    }
+                    const int bz = P.ragged_m ? T.g : 0;
+                    if (B_MAJOR == K_MAJOR) {
+                        tma_load_3d_pair(sb, &P.b[src], bar, k, T.n0 + rank * (BN / 2), bz);
+                    } else {
+                        const int half = P.b_split ? rank : src;
+                        const int col = P.b_split ? T.n0 : T.n0 + rank * (BN / 2);
+#pragma unroll
+                        for (int j = 0; j < BN / 128; ++j)
+                            tma_load_3d_pair(sb + j * MN_BLOCK_BYTES, &P.b[half], bar, col + 64 * j, k, bz);
+                    }
+                }
+                __syncwarp();
+                if (++stage == STAGES2) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (warp == 1 && rank == 0) {
+        // ===== MMA issuer (one thread of the leader CTA) =====
+        constexpr uint32_t idesc = make_idesc2(A_MAJOR, B_MAJOR);
+        constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
+        constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        int stage = 0, phase = 0, as = 0, aphase = 0;
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0);
+            if (lane == 0) {
+                mbar_wait(&tempty_bar[as], aphase ^ 1);
+                tc_fence_after();
+            }
+            __syncwarp();
+            const uint32_t d_tmem = tmem_base + as * BN;
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&full_bar[stage], phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
+#pragma unroll
+                    for (int kk = 0; kk < BK / UK; ++kk) {
+                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
+                        const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
+                        umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
+                    }
+                    umma2_commit(&empty_bar[stage]);  // frees this stage in both CTAs
+                }
+                __syncwarp();
+                if (++stage == STAGES2) stage = 0, phase ^= 1;
+            }
+            if (lane == 0) umma2_commit(&tfull_bar[as]);  // both CTAs' epilogues
+            __syncwarp();
+            if (++as == 2) as = 0, aphase ^= 1;
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
+        const int wq = warp & 3, row = wq * 32 + lane;
+        const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
+        int as = 0, aphase = 0;
+        const int rows_total = P.ragged_m ? offsets[P.G] : P.m_limit;
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
+            mbar_wait(&tfull_bar[as], aphase);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
+            const int grow = T.m0 + row;
+            const bool row_ok = T.store && grow < rows_total;
+            const bool zero = T.nkb == 0;
+            const long long base = (P.ragged_m ? 0 : (long long)T.g * P.group_stride) + (long long)grow * P.ld;
+            epilogue_tile<EPI>(P, taddr, row_ok, zero, base, T.n0);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(leader_tempty + as * 8);
+            if (++as == 2) as = 0, aphase ^= 1;
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();  // the peer's barriers and TMEM stay alive until the leader's last commit has landed
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc2(tmem_base, 512);
     }
 }
 
@@ -456,10 +724,19 @@ int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, lo
     } while (0)
 
 template <int A_MAJOR, int B_MAJOR, int EPI>
-int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
+int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool two_cta, const char* name) {
+    TcParams Q = P;
+    if (two_cta) {
+        // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
+        long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
+        if (tile_bound < clusters) clusters = tile_bound;
+        if (clusters < 1) clusters = 1;
+        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, SMEM2_BYTES, ln.stream>>>(Q);
+        PIPER_LAUNCHED(c, name);
+        return PIPER_OK;
+    }
     long long grid = tile_bound < ln.sms ? tile_bound : ln.sms;
     if (grid < 1) grid = 1;
-    TcParams Q = P;
     if (c->tc_prof) {  // debug: slot per launch, cycled
         Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
         c->tc_next_slot += 1;
@@ -472,8 +749,19 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const
 template <int A_MAJOR, int B_MAJOR, int EPI>
 bool set_smem_attr() {
     return cudaFuncSetAttribute(tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                SMEM_BYTES) == cudaSuccess;
+                                SMEM_BYTES) == cudaSuccess &&
+           cudaFuncSetAttribute(tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                SMEM2_BYTES) == cudaSuccess;
 }
+
+// Pairing M tiles of one expert costs a duplicate tile per odd group: use the CTA-pair kernel when the groups are
+// long enough for that to be small (host-side expectation; the sizes themselves stay on the device).
+bool pair_ragged(const piper_ctx* c, const FfnProblem& p) {
+    if (c->tc_two_cta == 0) return false;
+    if (c->tc_two_cta == 1) return true;
+    return (long long)p.max_rows >= (long long)p.G * 4 * BM || p.G == 1;
+}
+bool pair_wgrad(const piper_ctx* c) { return c->tc_two_cta != 0; }
 
 TcParams base_params(const FfnProblem& p, bool ragged_m) {
     TcParams P;
@@ -481,7 +769,10 @@ TcParams base_params(const FfnProblem& p, bool ragged_m) {
     P.offsets = p.offsets, P.G = p.G, P.ragged_m = ragged_m ? 1 : 0, P.n_src = 1, P.tile_n = BN;
     return P;
 }
-inline long long m_tile_bound(const FfnProblem& p) { return cdiv(p.max_rows, BM); }
+inline long long m_tile_bound(const FfnProblem& p, bool two) {
+    // pairs: sum_g ceil(tiles_g / 2) <= (tiles + G) / 2
+    return two ? (cdiv(p.max_rows, BM) + p.G + 1) / 2 : cdiv(p.max_rows, BM);
+}
 
 }  // namespace
 
@@ -497,6 +788,9 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     const char* pe = getenv("PIPER_TC_PROFILE");
     c->tc_prof = pe && pe[0] == '1';
+    const char* p2 = getenv("PIPER_TC_2CTA");  // 0: never, 1: always, unset: by expected group length
+    c->tc_two_cta = p2 ? (p2[0] == '0' ? 0 : 1) : 2;
+    c->tc2_max_clusters = c->num_sms / 2;
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
               set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>();
@@ -516,6 +810,7 @@ bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
 
 // G|U = Xp Wg | Xp Wu, H = silu(G) * U
 int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, BM);
     PIPER_MAP(&P.b[0], p.w_gate, p.I, p.d, p.G, 64);
@@ -523,44 +818,48 @@ int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.kb_per_src = cdiv(p.d, BK);
     P.n_limit = p.I, P.ld = p.I;
     P.out0 = (__nv_bfloat16*)p.g, P.out1 = (__nv_bfloat16*)p.u, P.out2 = (__nv_bfloat16*)p.h;
-    return launch<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_fwd1");
+    return launch<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_fwd1");
 }
 
 // O = H Wd
 int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, BM);
     PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, 64);
     P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
     P.out0 = (__nv_bfloat16*)p.o;
-    return launch<K_MAJOR, MN_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_fwd2");
+    return launch<K_MAJOR, MN_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_fwd2");
 }
 
 // dH = dO Wd^T; dG = dH * U * silu'(G); dU = dH * silu(G)
 int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.d_o, p.d, p.max_rows, 1, BM);
-    PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, BN);
+    PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, two ? BN / 2 : BN);
     P.n_tiles = cdiv(p.I, BN), P.kb_per_src = cdiv(p.d, BK), P.n_limit = p.I, P.ld = p.I;
     P.in0 = (const __nv_bfloat16*)p.g, P.in1 = (const __nv_bfloat16*)p.u;
     P.out0 = (__nv_bfloat16*)p.dg, P.out1 = (__nv_bfloat16*)p.du;
-    return launch<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_dgrad1");
+    return launch<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_dgrad1");
 }
 
 // dXp = dG Wg^T + dU Wu^T  (one accumulator, K runs over both products)
 int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.dg, p.I, p.max_rows, 1, BM);
     PIPER_MAP(&P.a[1], p.du, p.I, p.max_rows, 1, BM);
-    PIPER_MAP(&P.b[0], p.w_gate, p.I, p.d, p.G, BN);
-    PIPER_MAP(&P.b[1], p.w_up, p.I, p.d, p.G, BN);
+    PIPER_MAP(&P.b[0], p.w_gate, p.I, p.d, p.G, two ? BN / 2 : BN);
+    PIPER_MAP(&P.b[1], p.w_up, p.I, p.d, p.G, two ? BN / 2 : BN);
     P.n_src = 2, P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
     P.out0 = (__nv_bfloat16*)p.dxp;
-    return launch<K_MAJOR, K_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p) * P.n_tiles, "tc_ffn_dgrad2");
+    return launch<K_MAJOR, K_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_dgrad2");
 }
 
 // dWg|dWu[e] = Xp^T dG | Xp^T dU ; dWd[e] = H^T dO over the expert's rows (K ragged; zeros for empty experts)
 int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    const bool two = pair_wgrad(c);
     {
         TcParams P = base_params(p, false);
         PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, 64);
@@ -569,7 +868,8 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.m_tiles = cdiv(p.d, BM);
         P.m_limit = p.d, P.n_limit = p.I, P.ld = p.I, P.group_stride = (long long)p.d * p.I;
         P.out0 = (__nv_bfloat16*)p.dw_gate, P.out1 = (__nv_bfloat16*)p.dw_up;
-        const int rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * P.m_tiles * P.n_tiles,
+        const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
+        const int rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * mt * P.n_tiles, two,
                                                                   "tc_ffn_wgrad_gate_up");
         if (rc != PIPER_OK) return rc;
     }
@@ -579,7 +879,8 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.n_tiles = cdiv(p.d, BN), P.m_tiles = cdiv(p.I, BM);
     P.m_limit = p.I, P.n_limit = p.d, P.ld = p.d, P.group_stride = (long long)p.I * p.d;
     P.out0 = (__nv_bfloat16*)p.dw_down;
-    return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * P.m_tiles * P.n_tiles, "tc_ffn_wgrad_down");
+    const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
+    return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * mt * P.n_tiles, two, "tc_ffn_wgrad_down");
 }
 
 }  // namespace piper

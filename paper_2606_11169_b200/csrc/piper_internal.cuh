@@ -47,6 +47,8 @@ struct piper_ctx {
     piper::GreenPartition* green;
     char* tc_scratch;        // tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
     int tc_next_slot;        // round-robin slot in tc_scratch
+    int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
+    int tc2_max_clusters;    // co-resident CTA pairs
     int tc_prof;             // PIPER_TC_PROFILE=1: the tcgen05 kernels record wait-cycle counters in tc_scratch
     cudaEvent_t events[piper::kMaxEvents];
 };
