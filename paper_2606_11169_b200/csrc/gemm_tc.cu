@@ -39,6 +39,7 @@ enum : int { EPI_SWIGLU_FWD = 0, EPI_STORE = 1, EPI_SWIGLU_BWD = 2, EPI_WGRAD_SP
 
 struct alignas(64) TcParams {
     CUtensorMap a[2], b[2];
+    CUtensorMap o[3], ein[2];  // CTA-pair kernel: outputs / epilogue inputs as 64-column x 32-row store / load boxes
     const int32_t* offsets;  // [G+1] device
     int G;
     int ragged_m;    // 1: tiles run over the packed rows (fwd / dgrad); 0: over groups (wgrad)
@@ -433,6 +434,49 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
     }
 }
 
+
+// ---- staged epilogue of the CTA-pair kernel: TMEM -> registers -> swizzled shared memory -> TMA store ----------
+// A thread owns one row of the tile; direct row stores cost one L1 wavefront per thread and instruction (32 rows =
+// 32 lines), which made the epilogue the limiter of the short-K tiles.  Each epilogue warp stages 32 rows x 64
+// columns (4 KB, 128-byte rows in the TMA 128-byte swizzle: conflict-free 16-byte st.shared) and one lane issues
+// a bulk tensor store, which also clips rows and columns at the tensor bounds.
+constexpr int STG_BYTES = 32 * 128;  // one staging buffer: 32 rows x 64 bf16
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(r[0]),"=r"(r[1]),"=r"(r[2]),"=r"(r[3]),"=r"(r[4]),"=r"(r[5]),"=r"(r[6]),"=r"(r[7]),"=r"(r[8]),"=r"(r[9]),"=r"(r[10]),"=r"(r[11]),"=r"(r[12]),"=r"(r[13]),"=r"(r[14]),"=r"(r[15]),"=r"(r[16]),"=r"(r[17]),"=r"(r[18]),"=r"(r[19]),"=r"(r[20]),"=r"(r[21]),"=r"(r[22]),"=r"(r[23]),"=r"(r[24]),"=r"(r[25]),"=r"(r[26]),"=r"(r[27]),"=r"(r[28]),"=r"(r[29]),"=r"(r[30]),"=r"(r[31])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait32(uint32_t (&r)[32]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]),"+r"(r[1]),"+r"(r[2]),"+r"(r[3]),"+r"(r[4]),"+r"(r[5]),"+r"(r[6]),"+r"(r[7]),"+r"(r[8]),"+r"(r[9]),"+r"(r[10]),"+r"(r[11]),"+r"(r[12]),"+r"(r[13]),"+r"(r[14]),"+r"(r[15]),"+r"(r[16]),"+r"(r[17]),"+r"(r[18]),"+r"(r[19]),"+r"(r[20]),"+r"(r[21]),"+r"(r[22]),"+r"(r[23]),"+r"(r[24]),"+r"(r[25]),"+r"(r[26]),"+r"(r[27]),"+r"(r[28]),"+r"(r[29]),"+r"(r[30]),"+r"(r[31]) : : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void st_shared16(uint8_t* p, const uint4& v) {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(smem_u32(p)), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ uint4 ld_shared16(const uint8_t* p) {
+    uint4 v;
+    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+// address of 16-byte chunk `ch` (0..7) of row `r` (0..31) in a staging buffer (128-byte swizzle)
+__device__ __forceinline__ uint8_t* stg_at(uint8_t* buf, int r, int ch) { return buf + r * 128 + ((ch ^ (r & 7)) << 4); }
+// 32 fp32 columns -> bf16 -> chunks [4 half, 4 half + 4) of this thread's staging row
+__device__ __forceinline__ void stage32(uint8_t* buf, int r, int half, const float* v) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) st_shared16(stg_at(buf, r, 4 * half + j), pack8(v + 8 * j));
+}
+
 // =====================================================================================================
 // 2-CTA variant: a cluster of two CTAs (one TPC) works on two M tiles that share one B tile.  The leader CTA
 // issues tcgen05.mma.cta_group::2 (M = 256: rows 0-127 accumulate in the leader's TMEM, 128-255 in the
@@ -442,9 +486,15 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
 // two tiles of the same expert (an odd last tile is paired with a duplicate whose stores are skipped); in
 // wgrad they are two 128-row slices of dW.
 // =====================================================================================================
-constexpr int STAGES2 = 6;
 constexpr int A2_BYTES = BM * BK * 2, B2_BYTES = (BN / 2) * BK * 2, STAGE2_BYTES = A2_BYTES + B2_BYTES;
-constexpr int SMEM2_BYTES = STAGES2 * STAGE2_BYTES + 1024 + 256 + 2 * (kMaxGroups + 1) * 4;
+// Ring depth and staging buffers per epilogue warp: the SwiGLU backward epilogue also stages its G, U inputs.
+template <int EPI>
+struct Cfg2 {
+    static constexpr int NST = EPI == EPI_SWIGLU_BWD ? 4 : 5;
+    static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : 3;
+    static constexpr int RING_BYTES = NST * STAGE2_BYTES, STG_TOTAL = 4 * NBUF * STG_BYTES;
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups + 1) * 4;
+};
 constexpr int PANEL_PAIRS = 4;
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -542,12 +592,15 @@ template <int A_MAJOR, int B_MAJOR, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES2 * STAGE2_BYTES);  // used in the leader CTA
-    uint64_t* empty_bar = full_bar + STAGES2;                                          // one set per CTA
-    uint64_t* tfull_bar = empty_bar + STAGES2;                                         // [2] one set per CTA
-    uint64_t* tempty_bar = tfull_bar + 2;                                              // [2] used in the leader CTA
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tempty_bar + 2);
-    int* tp = reinterpret_cast<int*>(smem + STAGES2 * STAGE2_BYTES + 256);
+    constexpr int STAGES2 = Cfg2<EPI>::NST, NBUF = Cfg2<EPI>::NBUF;
+    uint8_t* stg_base = smem + Cfg2<EPI>::RING_BYTES;
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(stg_base + Cfg2<EPI>::STG_TOTAL);  // used in the leader CTA
+    uint64_t* empty_bar = full_bar + STAGES2;                                            // one set per CTA
+    uint64_t* tfull_bar = empty_bar + STAGES2;                                           // [2] one set per CTA
+    uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
+    uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets] epilogue inputs
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
+    int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);
     int* tpp = tp + (kMaxGroups + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -583,6 +636,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES2; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
+        for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -666,25 +720,142 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
-        const int wq = warp & 3, row = wq * 32 + lane;
+        const int wq = warp & 3;
         const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
-        int as = 0, aphase = 0;
-        const int rows_total = P.ragged_m ? offsets[P.G] : P.m_limit;
+        uint8_t* stg = stg_base + wq * NBUF * STG_BYTES;
+        int as = 0, aphase = 0, ring = 0;
+        uint32_t q = 0;  // SwiGLU backward: running chunk number -> input set q & 1, barrier phase (q >> 1) & 1
+        // G, U of 32 rows x 64 columns -> set `set` of this warp's staging buffers (bytes counted on ld_bar)
+        auto load_inputs = [&](const Tile2& Tn, int c, int set) {
+            if (lane == 0) {
+                bulk_wait_read<0>();  // the stores that last read this set are done with it
+                uint64_t* bar = &ld_bar[wq * 2 + set];
+                mbar_expect_tx(bar, 2 * STG_BYTES);
+                tma_load_3d(stg + (2 * set) * STG_BYTES, &P.ein[0], bar, Tn.n0 + 64 * c, Tn.m0 + wq * 32, 0);
+                tma_load_3d(stg + (2 * set + 1) * STG_BYTES, &P.ein[1], bar, Tn.n0 + 64 * c, Tn.m0 + wq * 32, 0);
+            }
+        };
+        if (EPI == EPI_SWIGLU_BWD && pair_id < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, pair_id, rank), 0, 0);
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
             mbar_wait(&tfull_bar[as], aphase);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
-            const int grow = T.m0 + row;
-            const bool row_ok = T.store && grow < rows_total;
-            const bool zero = T.nkb == 0;
-            const long long base = (P.ragged_m ? 0 : (long long)T.g * P.group_stride) + (long long)grow * P.ld;
-            epilogue_tile<EPI>(P, taddr, row_ok, zero, base, T.n0);
+            const int row0 = T.m0 + wq * 32, z = P.ragged_m ? 0 : T.g;
+            const bool zero = T.nkb == 0;  // empty expert in wgrad: exact zeros, the accumulator is stale
+            if (EPI == EPI_SWIGLU_FWD) {
+                // accumulator columns [0,128) = G, [128,256) = U of output columns n0 .. n0+127
+#pragma unroll 1
+                for (int c = 0; c < 2; ++c) {
+                    const int col = T.n0 + 64 * c;
+                    if (col >= P.n_limit) break;
+                    if (lane == 0) bulk_wait_read<0>();
+                    __syncwarp();
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint32_t rg[32], ru[32];
+                        tmem_ld32(taddr + 64 * c + 32 * h, rg);
+                        tmem_ld32(taddr + 128 + 64 * c + 32 * h, ru);
+                        tmem_ld_wait32(rg);
+                        tmem_ld_wait32(ru);
+                        float g[32], u[32];
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) g[i] = __uint_as_float(rg[i]), u[i] = __uint_as_float(ru[i]);
+                        stage32(stg, lane, h, g);
+                        stage32(stg + STG_BYTES, lane, h, u);
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) g[i] = g[i] * sigmoidf_fast(g[i]) * u[i];
+                        stage32(stg + 2 * STG_BYTES, lane, h, g);
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0 && T.store) {
+                        tma_store_3d(&P.o[0], stg, col, row0, z);
+                        tma_store_3d(&P.o[1], stg + STG_BYTES, col, row0, z);
+                        tma_store_3d(&P.o[2], stg + 2 * STG_BYTES, col, row0, z);
+                        bulk_commit();
+                    }
+                }
+            } else if (EPI == EPI_SWIGLU_BWD) {
+                // accumulator = dH; dG = dH * U * silu'(G), dU = dH * silu(G), computed in place over the staged G, U
+#pragma unroll 1
+                for (int c = 0; c < 4; ++c, ++q) {
+                    const int set = q & 1;
+                    uint8_t* bg = stg + (2 * set) * STG_BYTES;
+                    uint8_t* bu = bg + STG_BYTES;
+                    mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
+                    if (c < 3) {
+                        load_inputs(T, c + 1, set ^ 1);
+                    } else if (t + n_pairs_grid < n_total) {
+                        load_inputs(decode_pair(P, tp, tpp, offsets, t + n_pairs_grid, rank), 0, set ^ 1);
+                    }
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint32_t r[32];
+                        tmem_ld32(taddr + 64 * c + 32 * h, r);
+                        tmem_ld_wait32(r);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            uint8_t* pg = stg_at(bg, lane, 4 * h + j);
+                            uint8_t* pu = stg_at(bu, lane, 4 * h + j);
+                            float gv[8], uv[8], dg[8], du[8];
+                            unpack8(ld_shared16(pg), gv);
+                            unpack8(ld_shared16(pu), uv);
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) {
+                                const float v = __uint_as_float(r[8 * j + i]);
+                                const float sg = sigmoidf_fast(gv[i]);
+                                dg[i] = v * uv[i] * (sg * (1.f + gv[i] * (1.f - sg)));
+                                du[i] = v * (gv[i] * sg);
+                            }
+                            st_shared16(pg, pack8(dg));
+                            st_shared16(pu, pack8(du));
+                        }
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0 && T.store) {
+                        tma_store_3d(&P.o[0], bg, T.n0 + 64 * c, row0, z);
+                        tma_store_3d(&P.o[1], bu, T.n0 + 64 * c, row0, z);
+                        bulk_commit();
+                    }
+                }
+            } else {
+                // one output of 256 columns, or (wgrad gate|up) two outputs of 128 columns each
+#pragma unroll 1
+                for (int c = 0; c < 4; ++c) {
+                    const bool split = EPI == EPI_WGRAD_SPLIT;
+                    const CUtensorMap* om = split ? &P.o[c >> 1] : &P.o[0];
+                    const int col = split ? T.n0 + 64 * (c & 1) : T.n0 + 64 * c;
+                    if (col >= P.n_limit) continue;
+                    uint8_t* buf = stg + ring * STG_BYTES;
+                    if (++ring == NBUF) ring = 0;
+                    if (lane == 0) bulk_wait_read<NBUF - 1>();
+                    __syncwarp();
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint32_t r[32];
+                        tmem_ld32(taddr + 64 * c + 32 * h, r);
+                        tmem_ld_wait32(r);
+                        float v[32];
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = zero ? 0.f : __uint_as_float(r[i]);
+                        stage32(buf, lane, h, v);
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0 && T.store) {
+                        tma_store_3d(om, buf, col, row0, z);
+                        bulk_commit();
+                    }
+                }
+            }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(leader_tempty + as * 8);
             if (++as == 2) as = 0, aphase ^= 1;
         }
+        if (lane == 0) bulk_wait_all();
     }
     tc_fence_before();
     cluster_sync_all();  // the peer's barriers and TMEM stay alive until the leader's last commit has landed
@@ -731,7 +902,7 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
         long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
-        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, SMEM2_BYTES, ln.stream>>>(Q);
+        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
     }
@@ -751,7 +922,7 @@ bool set_smem_attr() {
     return cudaFuncSetAttribute(tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 SMEM_BYTES) == cudaSuccess &&
            cudaFuncSetAttribute(tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                SMEM2_BYTES) == cudaSuccess;
+                                Cfg2<EPI>::SMEM) == cudaSuccess;
 }
 
 // Pairing M tiles of one expert costs a duplicate tile per odd group: use the CTA-pair kernel when the groups are
@@ -818,6 +989,11 @@ int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.kb_per_src = cdiv(p.d, BK);
     P.n_limit = p.I, P.ld = p.I;
     P.out0 = (__nv_bfloat16*)p.g, P.out1 = (__nv_bfloat16*)p.u, P.out2 = (__nv_bfloat16*)p.h;
+    if (two) {
+        PIPER_MAP(&P.o[0], p.g, p.I, p.max_rows, 1, 32);
+        PIPER_MAP(&P.o[1], p.u, p.I, p.max_rows, 1, 32);
+        PIPER_MAP(&P.o[2], p.h, p.I, p.max_rows, 1, 32);
+    }
     return launch<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_fwd1");
 }
 
@@ -829,6 +1005,7 @@ int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
     PIPER_MAP(&P.b[0], p.w_down, p.d, p.I, p.G, 64);
     P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
     P.out0 = (__nv_bfloat16*)p.o;
+    if (two) PIPER_MAP(&P.o[0], p.o, p.d, p.max_rows, 1, 32);
     return launch<K_MAJOR, MN_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_fwd2");
 }
 
@@ -841,6 +1018,12 @@ int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.n_tiles = cdiv(p.I, BN), P.kb_per_src = cdiv(p.d, BK), P.n_limit = p.I, P.ld = p.I;
     P.in0 = (const __nv_bfloat16*)p.g, P.in1 = (const __nv_bfloat16*)p.u;
     P.out0 = (__nv_bfloat16*)p.dg, P.out1 = (__nv_bfloat16*)p.du;
+    if (two) {
+        PIPER_MAP(&P.o[0], p.dg, p.I, p.max_rows, 1, 32);
+        PIPER_MAP(&P.o[1], p.du, p.I, p.max_rows, 1, 32);
+        PIPER_MAP(&P.ein[0], p.g, p.I, p.max_rows, 1, 32);
+        PIPER_MAP(&P.ein[1], p.u, p.I, p.max_rows, 1, 32);
+    }
     return launch<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_dgrad1");
 }
 
@@ -854,6 +1037,7 @@ int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
     PIPER_MAP(&P.b[1], p.w_up, p.I, p.d, p.G, two ? BN / 2 : BN);
     P.n_src = 2, P.n_tiles = cdiv(p.d, BN), P.kb_per_src = cdiv(p.I, BK), P.n_limit = p.d, P.ld = p.d;
     P.out0 = (__nv_bfloat16*)p.dxp;
+    if (two) PIPER_MAP(&P.o[0], p.dxp, p.d, p.max_rows, 1, 32);
     return launch<K_MAJOR, K_MAJOR, EPI_STORE>(c, ln, P, m_tile_bound(p, two) * P.n_tiles, two, "tc_ffn_dgrad2");
 }
 
@@ -868,6 +1052,10 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.m_tiles = cdiv(p.d, BM);
         P.m_limit = p.d, P.n_limit = p.I, P.ld = p.I, P.group_stride = (long long)p.d * p.I;
         P.out0 = (__nv_bfloat16*)p.dw_gate, P.out1 = (__nv_bfloat16*)p.dw_up;
+        if (two) {
+            PIPER_MAP(&P.o[0], p.dw_gate, p.I, p.d, p.G, 32);
+            PIPER_MAP(&P.o[1], p.dw_up, p.I, p.d, p.G, 32);
+        }
         const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
         const int rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * mt * P.n_tiles, two,
                                                                   "tc_ffn_wgrad_gate_up");
@@ -879,6 +1067,7 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.n_tiles = cdiv(p.d, BN), P.m_tiles = cdiv(p.I, BM);
     P.m_limit = p.I, P.n_limit = p.d, P.ld = p.d, P.group_stride = (long long)p.I * p.d;
     P.out0 = (__nv_bfloat16*)p.dw_down;
+    if (two) PIPER_MAP(&P.o[0], p.dw_down, p.d, p.I, p.G, 32);
     const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
     return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * mt * P.n_tiles, two, "tc_ffn_wgrad_down");
 }
