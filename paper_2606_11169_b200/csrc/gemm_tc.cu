@@ -585,7 +585,9 @@ __device__ __forceinline__ void tma_load_3d_pair(void* dst, const CUtensorMap* m
         : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+    // default semantics (.release.cta): the .release.cluster form costs a MEMBAR.ALL.GPU per tile; the TMEM reads it must
+    // follow are ordered by tcgen05.fence::before_thread_sync
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
 }
 
 template <int A_MAJOR, int B_MAJOR, int EPI>
@@ -650,11 +652,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         // ===== TMA producer (both CTAs): own A tile + own 128-column half of B, counted on the leader's barrier =====
         const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
         int stage = 0, phase = 0;
+        long long w_empty = 0;
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
+                    if (P.prof) w_empty += clock64() - c0;
                     uint8_t* sa = smem + stage * STAGE2_BYTES;
                     uint8_t* sb = sa + A2_BYTES;
                     if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * STAGE2_BYTES);
@@ -684,23 +689,30 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 if (++stage == STAGES2) stage = 0, phase ^= 1;
             }
         }
+        if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1 && rank == 0) {
         // ===== MMA issuer (one thread of the leader CTA) =====
         constexpr uint32_t idesc = make_idesc2(A_MAJOR, B_MAJOR);
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
         int stage = 0, phase = 0, as = 0, aphase = 0;
+        long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
+        const long long t_begin = P.prof ? clock64() : 0;
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0);
             if (lane == 0) {
+                const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
+                if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
             __syncwarp();
             const uint32_t d_tmem = tmem_base + as * BN;
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&full_bar[stage], phase);
+                    if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
 #pragma unroll
@@ -718,12 +730,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
+        if (P.prof && lane == 0) {
+            long long* pq = P.prof + blockIdx.x * 8;
+            pq[0] = w_full, pq[1] = w_tempty, pq[2] = clock64() - t_begin, pq[6] = n_tiles_done;
+        }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
         const int wq = warp & 3;
         const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
         uint8_t* stg = stg_base + wq * NBUF * STG_BYTES;
         int as = 0, aphase = 0, ring = 0;
+        long long w_tfull = 0, w_stg = 0;
+#ifdef PIPER_EPI_PROBE
+        long long pr_ld = 0, pr_st = 0, pr_fence = 0, pr_tma = 0;
+#endif
+        const long long t_begin = P.prof ? clock64() : 0;
         uint32_t q = 0;  // SwiGLU backward: running chunk number -> input set q & 1, barrier phase (q >> 1) & 1
         // G, U of 32 rows x 64 columns -> set `set` of this warp's staging buffers (bytes counted on ld_bar)
         auto load_inputs = [&](const Tile2& Tn, int c, int set) {
@@ -738,7 +759,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         if (EPI == EPI_SWIGLU_BWD && pair_id < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, pair_id, rank), 0, 0);
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
+            const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
+            if (P.prof) w_tfull += clock64() - c0;
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
             const int row0 = T.m0 + wq * 32, z = P.ragged_m ? 0 : T.g;
@@ -749,8 +772,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 for (int c = 0; c < 2; ++c) {
                     const int col = T.n0 + 64 * c;
                     if (col >= P.n_limit) break;
+                    const long long c1 = P.prof ? clock64() : 0;
                     if (lane == 0) bulk_wait_read<0>();
                     __syncwarp();
+                    if (P.prof) w_stg += clock64() - c1;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         uint32_t rg[32], ru[32];
@@ -783,7 +808,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     const int set = q & 1;
                     uint8_t* bg = stg + (2 * set) * STG_BYTES;
                     uint8_t* bu = bg + STG_BYTES;
+                    const long long c1 = P.prof ? clock64() : 0;
                     mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
+                    if (P.prof) w_stg += clock64() - c1;
                     if (c < 3) {
                         load_inputs(T, c + 1, set ^ 1);
                     } else if (t + n_pairs_grid < n_total) {
@@ -830,24 +857,47 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (col >= P.n_limit) continue;
                     uint8_t* buf = stg + ring * STG_BYTES;
                     if (++ring == NBUF) ring = 0;
+                    const long long c1 = P.prof ? clock64() : 0;
                     if (lane == 0) bulk_wait_read<NBUF - 1>();
                     __syncwarp();
+                    if (P.prof) w_stg += clock64() - c1;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         uint32_t r[32];
+#ifdef PIPER_EPI_PROBE
+                        const long long p0 = clock64();
+#endif
                         tmem_ld32(taddr + 64 * c + 32 * h, r);
                         tmem_ld_wait32(r);
+#ifdef PIPER_EPI_PROBE
+                        const long long p1 = clock64();
+                        pr_ld += p1 - p0;
+#endif
                         float v[32];
 #pragma unroll
                         for (int i = 0; i < 32; ++i) v[i] = zero ? 0.f : __uint_as_float(r[i]);
                         stage32(buf, lane, h, v);
+#ifdef PIPER_EPI_PROBE
+                        pr_st += clock64() - p1;
+#endif
                     }
+#ifdef PIPER_EPI_PROBE
+                    const long long p2 = clock64();
+#endif
                     fence_proxy_async();
                     __syncwarp();
+#ifdef PIPER_EPI_PROBE
+                    const long long p3 = clock64();
+                    pr_fence += p3 - p2;
+#endif
                     if (lane == 0 && T.store) {
                         tma_store_3d(om, buf, col, row0, z);
                         bulk_commit();
                     }
+#ifdef PIPER_EPI_PROBE
+                    __syncwarp();
+                    pr_tma += clock64() - p3;
+#endif
                 }
             }
             tc_fence_before();
@@ -856,6 +906,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             if (++as == 2) as = 0, aphase ^= 1;
         }
         if (lane == 0) bulk_wait_all();
+        if (P.prof && threadIdx.x == 128) {
+            long long* pq = P.prof + blockIdx.x * 8;
+            pq[4] = w_tfull, pq[5] = clock64() - t_begin, pq[7] = w_stg;
+#ifdef PIPER_EPI_PROBE
+            if (EPI == EPI_WGRAD || EPI == EPI_WGRAD_SPLIT || EPI == EPI_STORE) pq[0] = pr_ld, pq[1] = pr_st, pq[3] = pr_fence, pq[6] = pr_tma;
+#endif
+        }
     }
     tc_fence_before();
     cluster_sync_all();  // the peer's barriers and TMEM stay alive until the leader's last commit has landed
@@ -897,6 +954,10 @@ int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, lo
 template <int A_MAJOR, int B_MAJOR, int EPI>
 int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool two_cta, const char* name) {
     TcParams Q = P;
+    if (c->tc_prof) {  // debug: slot per launch, cycled
+        Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
+        c->tc_next_slot += 1;
+    }
     if (two_cta) {
         // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
         long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
@@ -908,10 +969,6 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
     }
     long long grid = tile_bound < ln.sms ? tile_bound : ln.sms;
     if (grid < 1) grid = 1;
-    if (c->tc_prof) {  // debug: slot per launch, cycled
-        Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
-        c->tc_next_slot += 1;
-    }
     tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)grid, kThreads, SMEM_BYTES, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
@@ -930,7 +987,7 @@ bool set_smem_attr() {
 bool pair_ragged(const piper_ctx* c, const FfnProblem& p) {
     if (c->tc_two_cta == 0) return false;
     if (c->tc_two_cta == 1) return true;
-    return (long long)p.max_rows >= (long long)p.G * 4 * BM || p.G == 1;
+    return (long long)p.exp_rows >= (long long)p.G * 4 * BM || p.G == 1;
 }
 bool pair_wgrad(const piper_ctx* c) { return c->tc_two_cta != 0; }
 

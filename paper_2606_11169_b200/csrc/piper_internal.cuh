@@ -97,6 +97,7 @@ struct FfnProblem {
     int G, d, I;
     int max_rows;            // host-side bound on offsets[G] (sizes the tensor maps and SIMT grids)
     int max_group_rows;      // host-side bound on the rows of one group
+    int exp_rows;            // rows expected under uniform routing (kernel-variant choice only)
     const int32_t* offsets;  // device, [G+1]
     const void *xp, *w_gate, *w_up, *w_down;
     void *g, *u, *h, *o;                                 // forward outputs
