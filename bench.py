@@ -377,12 +377,44 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
 
     t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
     t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
-    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "splits": {}}
-    for sg, sc in splits:
-        t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
-        out["splits"][f"{sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / (t_f + t_b)}
+    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "splits": {}, "variants": {}}
+
+    def sweep(split_list):
+        res = {}
+        for sg, sc in split_list:
+            t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
+            res[f"{sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / (t_f + t_b),
+                                 "order": piper.piper_pair_order(ctx, sg, sc)}
+        return res
+
+    # the contract's sweep: Piper's list scheduling on disjoint SM partitions
+    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
+    out["splits"] = sweep(splits)
     out["partition_mode"] = {1: "green contexts", 2: "bounded grids on plain streams"}.get(
         piper.piper_pair_partition_mode(ctx), "?")
+    # measured variants: profile-guided order from per-task times taken here, and SM sharing
+    # (the paper leaves SM allocation to the GPU) where the GEMM grids keep every SM
+    tasks = [t for t in piper.TASKS]
+    task_ms = []
+    for t in tasks:
+        if t in ("F_SHARED", "B_SHARED") and not cfg.I_shared:
+            task_ms.append(0.0)
+            continue
+        a = args_a if t.startswith("F_") else args_b
+        task_ms.append(timed(lambda: piper.piper_run_task(ctx, t, a)))
+    out["task_ms"] = dict(zip(tasks, task_ms))
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE, piper.PART_EXCLUSIVE, task_ms)
+    out["variants"]["profile_order_exclusive"] = sweep(splits)
+    shared_splits = [(n_sm, 16), (n_sm, 32), (n_sm, 48), (n_sm - 16, 16)]
+    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_SHARED, task_ms)
+    out["variants"]["list_order_shared_sms"] = sweep(shared_splits)
+    piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE, piper.PART_SHARED, task_ms)
+    out["variants"]["profile_order_shared_sms"] = sweep(shared_splits)
+    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
+    best = min(((v["ratio_vs_serial"], name, k) for name, d in
+                [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))
+    out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2]}
     return out
 
 
@@ -404,6 +436,8 @@ def main():
     from inputs import configs
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
         ge.build()
+    if args.config == "C5":  # configs[4]: the C3-shaped chunk pair, microbatch seeds 4 (forward) and 5 (backward)
+        args.config, args.pair = "C5a", True
     cfg = configs.BY_NAME[args.config]
     if cfg.dtype == configs.DT_BF16:
         cfg = dataclasses.replace(cfg, row_align=args.row_align or 128)  # tcgen05 tiles are 128 rows

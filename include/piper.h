@@ -179,6 +179,28 @@ int piper_run_chunk_bwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream)
  * piper_run_chunk_fwd + piper_run_chunk_bwd. */
 int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const piper_chunk_args* bwd_mb, int sm_gemm,
                          int sm_comm, void* stream);
+
+/* Policy of piper_run_chunk_pair (host state of `ctx`; default = the paper's: PIPER_ORDER_LIST, PIPER_PART_EXCLUSIVE).
+ *  order     PIPER_ORDER_LIST    Piper's list scheduling, ready task with the most descendants first.
+ *            PIPER_ORDER_PROFILE profile-guided (PAPER.md:273, 420 name it as the way past the simple policy): the
+ *                                static two-stream schedule with the smallest simulated makespan, found by exhaustive
+ *                                search over per-stream sequences (piper_schedule_search) under task durations
+ *                                `task_ms` [14] (PIPER_TASK_* order, milliseconds on the whole device; the library
+ *                                scales them to the partition sizes) or, when task_ms is NULL, under the library's
+ *                                own estimate from the algorithmic FLOPs and bytes of the descriptor.
+ *  partition PIPER_PART_EXCLUSIVE  disjoint SM sets (green contexts; sm_gemm + sm_comm <= SM count).
+ *            PIPER_PART_SHARED     two plain streams, every grid bounded to its side's SM count worth of CTAs; the
+ *                                  sides may overlap (sm_gemm + sm_comm may exceed the SM count): pack/combine CTAs
+ *                                  become co-resident with the persistent GEMM CTAs, as in the paper, which leaves SM
+ *                                  allocation to the GPU.
+ * Either way the results stay bit-identical to the serial chunks.  Returns PIPER_ERR_INVALID on unknown values. */
+#define PIPER_ORDER_LIST 0
+#define PIPER_ORDER_PROFILE 1
+#define PIPER_PART_EXCLUSIVE 0
+#define PIPER_PART_SHARED 1
+int piper_set_pair_policy(piper_ctx* ctx, int order, int partition, const float* task_ms);
+/* The pick sequence (PIPER_TASK_* ids, n <= 14 written to order[14]) the current policy yields for a split. */
+int piper_pair_order(piper_ctx* ctx, int sm_gemm, int sm_comm, int32_t* order, int32_t* n);
 /* One task of the pair DAG (SURVEY.md §8c c-sched numbering) on `stream` with all SMs: the unit that
  * piper_run_chunk_fwd / _bwd / _pair enqueue, exposed so that each step can be timed on its own
  * (bench.py's roofline block).  F_* tasks read `a` as the forward microbatch, B_* as the backward one. */
@@ -199,7 +221,7 @@ int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const p
 int piper_run_task(piper_ctx* ctx, int task, const piper_chunk_args* a, void* stream);
 
 /* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
- * grids on two plain streams (green contexts unavailable), 0 = never called. */
+ * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 0 = never called. */
 int piper_pair_partition_mode(const piper_ctx* ctx);
 
 /* Host-only list scheduler used by piper_run_chunk_pair (reading c-21),
@@ -209,6 +231,12 @@ int piper_pair_partition_mode(const piper_ctx* ctx);
  * event).  Returns PIPER_ERR_INVALID on a cycle or a bad edge. */
 int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const int32_t* prio,
                         int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records);
+/* Profile-guided counterpart (PIPER_ORDER_PROFILE): exhaustive search of the static two-stream schedule (n <= 16,
+ * stream_of in {0,1}) with the smallest makespan under durations dur[n], simulated with the event rule of
+ * PAPER.md:279-286; ties go to the lexicographically smallest pick sequence.  Outputs as piper_list_schedule plus
+ * *makespan (nullable), in the unit of dur. */
+int piper_schedule_search(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const float* dur,
+                          int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records, float* makespan);
 
 #ifdef __cplusplus
 }

@@ -222,6 +222,45 @@ def piper_run_chunk_pair(ctx, fwd_args: ChunkArgs, bwd_args: ChunkArgs, sm_gemm:
                                          int(sm_comm), _stream(stream)), "piper_run_chunk_pair")
 
 
+ORDER_LIST, ORDER_PROFILE = 0, 1
+PART_EXCLUSIVE, PART_SHARED = 0, 1
+
+
+def piper_set_pair_policy(ctx, order: int, partition: int, task_ms=None):
+    """task_ms: 14 floats in TASKS order (ms on the whole device) or None for the library's own estimate."""
+    arr = None
+    if task_ms is not None:
+        arr = (ctypes.c_float * 14)(*[float(v) for v in task_ms])
+    ctx.check(lib().piper_set_pair_policy(ctx._h, int(order), int(partition), arr), "piper_set_pair_policy")
+
+
+def piper_pair_order(ctx, sm_gemm: int, sm_comm: int):
+    """Task names in the pick sequence the current policy yields for this split."""
+    order = (ctypes.c_int32 * 14)()
+    n = _i32(0)
+    ctx.check(lib().piper_pair_order(ctx._h, int(sm_gemm), int(sm_comm), order, ctypes.byref(n)), "piper_pair_order")
+    return [TASKS[order[i]] for i in range(n.value)]
+
+
+def piper_schedule_search(n, edges, stream_of, dur):
+    """Host-only: returns (order, waits[(producer, consumer)], records, makespan)."""
+    import numpy as np
+    edges = np.ascontiguousarray(edges, np.int32).reshape(-1, 2)
+    stream_of = np.ascontiguousarray(stream_of, np.int32)
+    dur = np.ascontiguousarray(dur, np.float32)
+    order = np.empty(n, np.int32)
+    waits = np.empty((max(1, len(edges)), 2), np.int32)
+    records = np.empty(n, np.int32)
+    nw = _i32(0)
+    mk = ctypes.c_float(0)
+    rc = lib().piper_schedule_search(_i32(n), _i32(len(edges)), _vp(edges.ctypes.data), _vp(stream_of.ctypes.data),
+                                     _vp(dur.ctypes.data), _vp(order.ctypes.data), _vp(waits.ctypes.data),
+                                     ctypes.byref(nw), _vp(records.ctypes.data), ctypes.byref(mk))
+    if rc != PIPER_OK:
+        raise PiperError(f"piper_schedule_search: status {rc}")
+    return order, waits[: nw.value].copy(), records, float(mk.value)
+
+
 def piper_list_schedule(n, edges, stream_of, prio):
     """Host-only: returns (order, waits[(producer, consumer)], records)."""
     import numpy as np

@@ -70,11 +70,11 @@ void destroy_partition(GreenPartition* g) {
 }
 
 // Split the device's SMs into {sm_comm, rest}; the gemm side keeps the first sm_gemm of the rest.
-GreenPartition* make_partition(piper_ctx* c, int sm_gemm, int sm_comm) {
+GreenPartition* make_partition(piper_ctx* c, int sm_gemm, int sm_comm, bool want_green) {
     GreenPartition* g = new GreenPartition();
     g->sm_gemm = sm_gemm, g->sm_comm = sm_comm;
     DriverApi& api = driver();
-    bool ok = api.ok;
+    bool ok = api.ok && want_green;
     CUdevice dev = 0;
     CUdevResource all{}, part{}, rest{};
     unsigned int n_groups = 1;
@@ -185,9 +185,20 @@ bool bwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
 
 }  // namespace
 
+struct PairPlan {
+    int32_t n, n_waits;
+    int32_t task_of[N_TASKS], stream_of[N_TASKS], order[N_TASKS], waits[32][2], records[N_TASKS];
+};
+
+void pair_plan_release(piper_ctx* c) {
+    delete static_cast<PairPlan*>(c->pair_plan);
+    c->pair_plan = nullptr;
+}
+
 void pair_release(piper_ctx* c) {
     destroy_partition(c->green);
     c->green = nullptr;
+    pair_plan_release(c);
 }
 
 }  // namespace piper
@@ -226,32 +237,118 @@ int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     return PIPER_OK;
 }
 
+namespace {
+
+// Task durations in ms on the whole device: the caller's profile, else an estimate from the algorithmic work
+// (GEMM tasks at 1.2 PFLOP/s, row movers at 4.5 TB/s, the small routing kernels at a launch-sized 10 us).
+void task_durations(const piper_ctx* c, float* ms) {
+    if (c->pair_have_ms) {
+        for (int t = 0; t < N_TASKS; ++t) ms[t] = c->pair_task_ms[t];
+        return;
+    }
+    const piper_moe_desc& D = c->D;
+    const double A = (double)D.T * D.k * D.E_loc / D.E, b = (double)esize(D.dtype), sh = D.I_shared ? 1.0 : 0.0;
+    const double di = (double)D.d * D.I, dis = (double)D.d * D.I_shared, tf = 1.2e12, bw = 4.5e9;
+    const double rows = (A + D.T + sh * D.T) * D.d * b;
+    ms[F_ROUTE] = ms[F_SCAN] = ms[B_ROUTE_BWD] = 0.01f;
+    ms[F_PACK] = (float)(2 * A * D.d * b / bw), ms[F_COMBINE] = ms[B_UNPACK] = (float)(rows / bw);
+    ms[B_CGRAD] = (float)(3 * A * D.d * b / bw);
+    ms[F_GEMM1] = ms[B_DGRAD2] = (float)(4 * di * A / tf), ms[F_GEMM2] = ms[B_DGRAD1] = (float)(2 * di * A / tf);
+    ms[B_WGRAD] = (float)(6 * di * A / tf);
+    ms[F_SHARED] = (float)(6 * dis * D.T / tf), ms[B_SHARED] = (float)(12 * dis * D.T / tf);
+}
+
+int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl);
+
+// The plan is a pure function of (descriptor, policy, split): computed once and kept (the profile-guided search
+// costs milliseconds of host time, which would otherwise sit between two launches).
+int make_plan(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+    PairPlan* cached = static_cast<PairPlan*>(c->pair_plan);
+    if (cached && c->plan_sm_gemm == sm_gemm && c->plan_sm_comm == sm_comm) {
+        *pl = *cached;
+        return PIPER_OK;
+    }
+    const int rc = make_plan_uncached(c, sm_gemm, sm_comm, pl);
+    if (rc != PIPER_OK) return rc;
+    if (!cached) cached = new (std::nothrow) PairPlan(), c->pair_plan = cached;
+    if (cached) *cached = *pl, c->plan_sm_gemm = sm_gemm, c->plan_sm_comm = sm_comm;
+    return PIPER_OK;
+}
+
+int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+    // task list of this layer (no shared expert -> its two tasks and their edges drop out)
+    const bool shared = c->D.I_shared != 0;
+    int32_t id_of[N_TASKS], n = 0;
+    for (int t = 0; t < N_TASKS; ++t) {
+        id_of[t] = -1;
+        if (!shared && (t == F_SHARED || t == B_SHARED)) continue;
+        id_of[t] = n, pl->task_of[n] = t, ++n;
+    }
+    pl->n = n;
+    int32_t edges[32][2], n_edges = 0, prio[N_TASKS];
+    for (const auto& e : kEdges)
+        if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
+    for (int i = 0; i < n; ++i) pl->stream_of[i] = kStreamOf[pl->task_of[i]], prio[i] = pl->task_of[i] >= B_CGRAD ? 1 : 0;
+    pl->n_waits = 0;
+    if (c->pair_order == PIPER_ORDER_LIST)
+        return piper_list_schedule(n, n_edges, &edges[0][0], pl->stream_of, prio, pl->order, &pl->waits[0][0], &pl->n_waits,
+                                   pl->records);
+    // durations on the partitions: GEMM tasks scale with the SM count; the row movers saturate HBM with about a
+    // third of the SMs, below that they scale with the SM count
+    float full[N_TASKS], dur[N_TASKS];
+    task_durations(c, full);
+    const float fg = (float)c->num_sms / (float)(sm_gemm < c->num_sms ? sm_gemm : c->num_sms);
+    const float fc = sm_comm * 3 >= c->num_sms ? 1.f : (float)c->num_sms / (3.f * (float)sm_comm);
+    for (int i = 0; i < n; ++i) dur[i] = full[pl->task_of[i]] * (pl->stream_of[i] == GEMM ? fg : fc);
+    return piper_schedule_search(n, n_edges, &edges[0][0], pl->stream_of, dur, pl->order, &pl->waits[0][0], &pl->n_waits,
+                                 pl->records, nullptr);
+}
+
+bool split_ok(const piper_ctx* c, int sm_gemm, int sm_comm) {
+    if (sm_gemm < 1 || sm_comm < 8 || sm_comm % 8 || sm_gemm > c->num_sms || sm_comm > c->num_sms) return false;
+    return c->pair_part == PIPER_PART_SHARED || sm_gemm + sm_comm <= c->num_sms;
+}
+
+}  // namespace
+
+int piper_set_pair_policy(piper_ctx* c, int order, int partition, const float* task_ms) {
+    if (!c || (order != PIPER_ORDER_LIST && order != PIPER_ORDER_PROFILE) ||
+        (partition != PIPER_PART_EXCLUSIVE && partition != PIPER_PART_SHARED))
+        return PIPER_ERR_INVALID;
+    if (task_ms)
+        for (int t = 0; t < N_TASKS; ++t)
+            if (!(task_ms[t] >= 0.f)) return PIPER_ERR_INVALID;
+    if (partition != c->pair_part) pair_release(c);
+    pair_plan_release(c);
+    c->pair_order = order, c->pair_part = partition, c->pair_have_ms = task_ms != nullptr;
+    if (task_ms)
+        for (int t = 0; t < N_TASKS; ++t) c->pair_task_ms[t] = task_ms[t];
+    return PIPER_OK;
+}
+
+int piper_pair_order(piper_ctx* c, int sm_gemm, int sm_comm, int32_t* order, int32_t* n) {
+    if (!c || !order || !n || !split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
+    PairPlan pl;
+    const int rc = make_plan(c, sm_gemm, sm_comm, &pl);
+    if (rc != PIPER_OK) return rc;
+    for (int i = 0; i < pl.n; ++i) order[i] = pl.task_of[pl.order[i]];
+    *n = pl.n;
+    return PIPER_OK;
+}
+
 int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_chunk_args* b, int sm_gemm, int sm_comm,
                          void* stream) {
     if (!c || !fwd_args_ok(c, f) || !bwd_args_ok(c, b)) return PIPER_ERR_INVALID;
-    if (sm_gemm < 1 || sm_comm < 8 || sm_comm % 8 || sm_gemm + sm_comm > c->num_sms) return PIPER_ERR_INVALID;
+    if (!split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
     if (!c->green || c->green->sm_gemm != sm_gemm || c->green->sm_comm != sm_comm) {
         pair_release(c);
-        c->green = make_partition(c, sm_gemm, sm_comm);
+        c->green = make_partition(c, sm_gemm, sm_comm, c->pair_part == PIPER_PART_EXCLUSIVE);
         if (!c->green) return cuda_fail(c, cudaErrorUnknown, "make_partition");
     }
     GreenPartition* g = c->green;
     c->pair_mode = g->green ? 1 : 2;
-
-    // task list of this layer (no shared expert -> its two tasks and their edges drop out)
-    const bool shared = c->D.I_shared != 0;
-    int32_t id_of[N_TASKS], task_of[N_TASKS], n = 0;
-    for (int t = 0; t < N_TASKS; ++t) {
-        id_of[t] = -1;
-        if (!shared && (t == F_SHARED || t == B_SHARED)) continue;
-        id_of[t] = n, task_of[n] = t, ++n;
-    }
-    int32_t edges[32][2], n_edges = 0, stream_of[N_TASKS], prio[N_TASKS];
-    for (const auto& e : kEdges)
-        if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
-    for (int i = 0; i < n; ++i) stream_of[i] = kStreamOf[task_of[i]], prio[i] = task_of[i] >= B_CGRAD ? 1 : 0;
-    int32_t order[N_TASKS], waits[32][2], n_waits = 0, records[N_TASKS];
-    int rc = piper_list_schedule(n, n_edges, &edges[0][0], stream_of, prio, order, &waits[0][0], &n_waits, records);
+    PairPlan pl;
+    int rc = make_plan(c, sm_gemm, sm_comm, &pl);
     if (rc != PIPER_OK) return rc;
 
     cudaStream_t user = static_cast<cudaStream_t>(stream);
@@ -261,14 +358,14 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
     PIPER_CUDA(c, cudaEventRecord(fork, user));
     PIPER_CUDA(c, cudaStreamWaitEvent(lanes[0].stream, fork, 0));
     PIPER_CUDA(c, cudaStreamWaitEvent(lanes[1].stream, fork, 0));
-    for (int step = 0; step < n; ++step) {
-        const int v = order[step];
-        const Lane ln = lanes[stream_of[v]];
-        for (int w = 0; w < n_waits; ++w)  // wait for dependencies that ran on another stream
-            if (waits[w][1] == v) PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, c->events[waits[w][0]], 0));
-        rc = run_task(c, task_of[v], ln, f, b);
+    for (int step = 0; step < pl.n; ++step) {
+        const int v = pl.order[step];
+        const Lane ln = lanes[pl.stream_of[v]];
+        for (int w = 0; w < pl.n_waits; ++w)  // wait for dependencies that ran on another stream
+            if (pl.waits[w][1] == v) PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, c->events[pl.waits[w][0]], 0));
+        rc = run_task(c, pl.task_of[v], ln, f, b);
         if (rc != PIPER_OK) return rc;
-        if (records[v]) PIPER_CUDA(c, cudaEventRecord(c->events[v], ln.stream));
+        if (pl.records[v]) PIPER_CUDA(c, cudaEventRecord(c->events[v], ln.stream));
     }
     PIPER_CUDA(c, cudaEventRecord(join0, lanes[0].stream));
     PIPER_CUDA(c, cudaEventRecord(join1, lanes[1].stream));

@@ -42,6 +42,11 @@ struct piper_ctx {
     int32_t* shared_offsets; // [2] = {0, T}: the shared expert as one group
     int64_t launches;
     int pair_mode;
+    int pair_order, pair_part;   // piper_set_pair_policy
+    int pair_have_ms;
+    void* pair_plan;             // cached schedule of the pair for (plan_sm_gemm, plan_sm_comm)
+    int plan_sm_gemm, plan_sm_comm;
+    float pair_task_ms[14];      // caller's task durations on the whole device (PIPER_ORDER_PROFILE)
     char err[256];
     void* encode_tiled;      // cuTensorMapEncodeTiled, resolved at create time
     piper::GreenPartition* green;
@@ -129,6 +134,7 @@ FfnProblem routed_problem(const piper_ctx*, const piper_chunk_args*);
 FfnProblem shared_problem(const piper_ctx*, const piper_chunk_args*);
 // chunk.cu
 void pair_release(piper_ctx*);
+void pair_plan_release(piper_ctx*);
 
 // ---- small device helpers -----------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -122,9 +122,12 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
-@pytest.mark.parametrize("split", [(132, 16), (100, 48)])
-def test_pair_is_bitwise_equal_to_serial(name, split):
-    """the overlapped, out-of-order plan must respect every dependency -> identical results."""
+@pytest.mark.parametrize("split,policy", [((132, 16), "list/exclusive"), ((100, 48), "list/exclusive"),
+                                          ((116, 32), "profile/exclusive"), ((148, 16), "list/shared"),
+                                          ((148, 48), "profile/shared")])
+def test_pair_is_bitwise_equal_to_serial(name, split, policy):
+    """the overlapped, out-of-order plan must respect every dependency -> identical results,
+    for the paper's list order and the profile-guided one, on disjoint and on shared SM partitions."""
     base = configs.BY_NAME[name]
     cfg_a = dataclasses.replace(base, row_align=128, seed=base.seed + 100)
     cfg_b = dataclasses.replace(base, row_align=128, seed=base.seed + 200)
@@ -137,9 +140,20 @@ def test_pair_is_bitwise_equal_to_serial(name, split):
     pa.update(util.upload_inputs(inp_a)), pb.update(util.upload_inputs(inp_b))
     args_a, args_b = piper.chunk_args(pa), piper.chunk_args(pb)
     piper.piper_run_chunk_fwd(ctx, args_b)
-    piper.piper_run_chunk_pair(ctx, args_a, args_b, split[0], split[1])
+    order, part = policy.split("/")
+    piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE if order == "profile" else piper.ORDER_LIST,
+                                piper.PART_SHARED if part == "shared" else piper.PART_EXCLUSIVE)
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    sg = min(split[0], n_sm) if part == "shared" else min(split[0], n_sm - split[1])
+    picked = piper.piper_pair_order(ctx, sg, split[1])
+    assert sorted(picked) == sorted(t for t in piper.TASKS if base.I_shared or t not in ("F_SHARED", "B_SHARED"))
+    piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, split[1])
     torch.cuda.synchronize()
+    assert piper.piper_pair_partition_mode(ctx) == (2 if part == "shared" else piper.piper_pair_partition_mode(ctx))
     assert piper.piper_pair_partition_mode(ctx) in (1, 2)
+    if part == "exclusive":  # sm_gemm + sm_comm beyond the device is refused on disjoint partitions
+        with pytest.raises(piper.PiperError):
+            piper.piper_run_chunk_pair(ctx, args_a, args_b, n_sm, 16)
     for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y"):
         assert torch.equal(ba[n], pa[n]), "fwd " + n
     nofs = base.e_loc + 1  # the offsets buffers are over-allocated; entries past E_loc+1 are never written
