@@ -488,14 +488,16 @@ __device__ __forceinline__ void stage32(uint8_t* buf, int r, int half, const flo
 // =====================================================================================================
 constexpr int A2_BYTES = BM * BK * 2, B2_BYTES = (BN / 2) * BK * 2, STAGE2_BYTES = A2_BYTES + B2_BYTES;
 // Ring depth and staging buffers per epilogue warp: the SwiGLU backward epilogue also stages its G, U inputs.
+constexpr int kMaxGroups2 = 192;  // groups the CTA-pair kernel can index (its tile-prefix arrays share the 227 KB)
 template <int EPI>
 struct Cfg2 {
-    static constexpr int NST = EPI == EPI_SWIGLU_BWD ? 4 : 5;
+    static constexpr int NST = 5;
     static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : 3;
     static constexpr int RING_BYTES = NST * STAGE2_BYTES, STG_TOTAL = 4 * NBUF * STG_BYTES;
-    static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups + 1) * 4;
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups2 + 1) * 4;
+    static_assert(SMEM <= 232448, "shared memory per CTA");
 };
-constexpr int PANEL_PAIRS = 4;
+constexpr int PANEL_PAIRS = 8;
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
     uint32_t r;
@@ -603,7 +605,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets] epilogue inputs
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
     int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);
-    int* tpp = tp + (kMaxGroups + 1);
+    int* tpp = tp + (kMaxGroups2 + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = (int)cluster_ctarank();
@@ -985,11 +987,11 @@ bool set_smem_attr() {
 // Pairing M tiles of one expert costs a duplicate tile per odd group: use the CTA-pair kernel when the groups are
 // long enough for that to be small (host-side expectation; the sizes themselves stay on the device).
 bool pair_ragged(const piper_ctx* c, const FfnProblem& p) {
-    if (c->tc_two_cta == 0) return false;
+    if (c->tc_two_cta == 0 || p.G > kMaxGroups2) return false;
     if (c->tc_two_cta == 1) return true;
     return (long long)p.exp_rows >= (long long)p.G * 4 * BM || p.G == 1;
 }
-bool pair_wgrad(const piper_ctx* c) { return c->tc_two_cta != 0; }
+bool pair_wgrad(const piper_ctx* c, const FfnProblem& p) { return c->tc_two_cta != 0 && p.G <= kMaxGroups2; }
 
 TcParams base_params(const FfnProblem& p, bool ragged_m) {
     TcParams P;
@@ -1100,7 +1102,7 @@ int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
 
 // dWg|dWu[e] = Xp^T dG | Xp^T dU ; dWd[e] = H^T dO over the expert's rows (K ragged; zeros for empty experts)
 int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
-    const bool two = pair_wgrad(c);
+    const bool two = pair_wgrad(c, p);
     {
         TcParams P = base_params(p, false);
         PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, 64);
