@@ -12,7 +12,7 @@ FfnProblem routed_problem(const piper_ctx* c, const piper_chunk_args* a) {
     p.max_rows = (int)piper_a_cap(&D);
     p.max_group_rows = D.T + D.row_align - 1;
     p.exp_rows = (int)((long long)D.T * D.k * D.E_loc / D.E);
-    p.offsets = a->offsets;
+    p.offsets = a->offsets, p.counts = a->counts;
     p.xp = a->xp, p.w_gate = a->w_gate, p.w_up = a->w_up, p.w_down = a->w_down;
     p.g = a->g_save, p.u = a->u_save, p.h = a->h_save, p.o = a->o;
     p.d_o = a->d_o, p.dg = a->dg, p.du = a->du, p.dxp = a->dxp;
@@ -25,7 +25,7 @@ FfnProblem shared_problem(const piper_ctx* c, const piper_chunk_args* a) {
     FfnProblem p{};
     p.G = 1, p.d = D.d, p.I = D.I_shared;
     p.max_rows = D.T, p.max_group_rows = D.T, p.exp_rows = D.T;
-    p.offsets = c->shared_offsets;
+    p.offsets = c->shared_offsets, p.counts = c->shared_offsets + 1;
     p.xp = a->x, p.w_gate = a->ws_gate, p.w_up = a->ws_up, p.w_down = a->ws_down;
     p.g = a->gs_save, p.u = a->us_save, p.h = a->hs_save, p.o = a->s;
     p.d_o = a->dy, p.dg = a->dgs, p.du = a->dus, p.dxp = a->dxs;

@@ -39,6 +39,7 @@ enum : int { EPI_SWIGLU_FWD = 0, EPI_STORE = 1, EPI_SWIGLU_BWD = 2, EPI_WGRAD_SP
 
 struct alignas(64) TcParams {
     CUtensorMap a[2], b[2];
+    CUtensorMap bs[2];         // rows-on-N kernel: the activation operand again with 32-row boxes (short chunks)
     CUtensorMap o[3], ein[2];  // CTA-pair kernel: outputs / epilogue inputs as 64-column x 32-row store / load boxes
     const int32_t* offsets;  // [G+1] device
     int G;
@@ -56,6 +57,12 @@ struct alignas(64) TcParams {
     __nv_bfloat16 *out0, *out1, *out2;
     const __nv_bfloat16 *in0, *in1;
     long long* prof;  // debug (PIPER_TC_PROFILE=1): [gridDim.x][8] wait-cycle counters, else NULL
+    // rows-on-N kernel (tc_gemmT_kernel)
+    const int32_t* counts;  // [G] device: real rows per group
+    int f_tiles;            // tiles along the feature (output column) dimension
+    int f_limit;            // output columns
+    int greedy;             // chunking: 1 = 256-row chunks and a short last one, 0 = equal chunks
+    int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------------
@@ -467,6 +474,20 @@ __device__ __forceinline__ void st_shared16(uint8_t* p, const uint4& v) {
 __device__ __forceinline__ uint4 ld_shared16(const uint8_t* p) {
     uint4 v;
     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ float lds_bf16(uint32_t a) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a) : "memory");
+    return __uint_as_float((uint32_t)v << 16);
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ float lds_f32(uint32_t a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
     return v;
 }
 // address of 16-byte chunk `ch` (0..7) of row `r` (0..31) in a staging buffer (128-byte swizzle)
@@ -924,29 +945,422 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     }
 }
 
+
+// =====================================================================================================
+// Rows-on-N variant of the CTA-pair kernel for the four ragged-M contractions (fwd1, fwd2, dgrad1, dgrad2).
+// The tensor core works on 128 M rows per SM whatever the tile holds, so with the packed rows on M every expert
+// pays for its segment rounded up to 128 rows and, in the CTA pair, to 256.  Here the operands swap roles: the
+// weights are the M operand (256 output features per CTA pair, always full) and the expert's rows are the N
+// operand, which tcgen05.mma takes in multiples of 16 (N <= 256).  An expert's rows are cut into equal chunks of
+// at most 256 rows rounded up to 16, so the tensor work follows the real row counts.  The accumulator holds the
+// transposed tile (TMEM lane = feature, column = row); the epilogue transposes through shared memory and
+// writes the row-major outputs with bulk tensor stores.
+// =====================================================================================================
+enum : int { TEPI_STORE = 0, TEPI_SWIGLU_FWD = 1, TEPI_SWIGLU_BWD = 2 };
+constexpr int TB_BOX_ROWS = 128, TB_SMALL_ROWS = 32;  // rows per activation TMA box (long / short chunks)
+constexpr int T_PANEL = 8;  // chunks per panel of the tile order (the panel's rows stay in L2 across feature tiles)
+//                           // rows per activation TMA box
+constexpr int TA_BYTES = 128 * BK * 2;                     // 128 features x 64 K
+constexpr int TB_BYTES = 128 * BK * 2;                     // up to 128 rows x 64 K per CTA
+constexpr int TSTAGE_BYTES = TA_BYTES + TB_BYTES;
+constexpr int TSTG_BYTES = 32 * 32 * 2;                    // staging block: 32 rows x 32 features bf16
+template <int EPI>
+struct CfgT {
+    static constexpr int NST = 5;
+    static constexpr int NBUF = 4;                         // staging blocks per epilogue warp
+    static constexpr int RING_BYTES = NST * TSTAGE_BYTES, STG_TOTAL = 4 * NBUF * TSTG_BYTES;
+    static constexpr int XCH_BYTES = EPI == TEPI_SWIGLU_FWD ? 2 * 2 * 32 * 32 * 4 : 0;  // fp32 U exchange, 2 pairs x 2
+    static constexpr int ZERO_BYTES = 16 * 32 * 2;         // a zero block for the pad rows
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + XCH_BYTES + ZERO_BYTES + 1024 + 256 + (kMaxGroups2 + 1) * 4;
+    static_assert(SMEM <= 232448, "shared memory per CTA");
+};
+
+struct TileT {
+    int g, f, r0, n;  // group, feature tile, first packed row, rows (multiple of 16, <= 256)
+    int zend;         // last chunk of a group: end of the group's padded segment (rows [r0 + n, zend) are zeroed)
+};
+// An expert's rows are cut into nch chunks of cs rows: about equal, cs a multiple of 16 and <= 256.
+__device__ __forceinline__ void t_plan(int rows, int& nch, int& cs, int greedy) {
+    const int n0 = (rows + 255) >> 8;
+    cs = greedy ? 256 : (n0 ? ((rows + n0 - 1) / n0 + 15) & ~15 : 16);
+    nch = (rows + cs - 1) / cs;
+}
+__device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, const int32_t* __restrict__ offsets,
+                                          const int32_t* __restrict__ counts, int t) {
+    int g = 0;
+    while (g + 1 < P.G && tq[g + 1] <= t) ++g;
+    const int local = t - tq[g], rows = counts[g];
+    int nch, cs;
+    t_plan(rows, nch, cs, P.greedy);
+    // panels of T_PANEL chunks; inside a panel feature-major with the chunk fastest
+    const int per_panel = T_PANEL * P.f_tiles;
+    const int panel = local / per_panel, rem = local - panel * per_panel;
+    const int pc = min(T_PANEL, nch - panel * T_PANEL);
+    const int f = rem / pc, c = panel * T_PANEL + (rem - f * pc);
+    const int left = rows - c * cs;
+    TileT r;
+    r.g = g, r.f = f, r.r0 = offsets[g] + c * cs, r.n = min(cs, (left + 15) & ~15);
+    r.zend = c == nch - 1 ? offsets[g + 1] : r.r0 + r.n;
+    return r;
+}
+__host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_major << 15) | ((uint32_t)K_MAJOR << 16) |
+           ((uint32_t)(n >> 3) << 17) | ((uint32_t)((2 * BM) >> 4) << 24);
+}
+
+
+template <int A_MAJOR, int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemmT_kernel(const __grid_constant__ TcParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    constexpr int NST = CfgT<EPI>::NST, NBUF = CfgT<EPI>::NBUF;
+    uint8_t* stg_base = smem + CfgT<EPI>::RING_BYTES;
+    uint8_t* xch_base = stg_base + CfgT<EPI>::STG_TOTAL;
+    uint8_t* zero_blk = xch_base + CfgT<EPI>::XCH_BYTES;
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(zero_blk + CfgT<EPI>::ZERO_BYTES);  // used in the leader CTA
+    uint64_t* empty_bar = full_bar + NST;                                                // one set per CTA
+    uint64_t* tfull_bar = empty_bar + NST;                                               // [2] one set per CTA
+    uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
+    uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets]
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
+    int* tq = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);       // first tile of each group
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rank = (int)cluster_ctarank();
+    const int pair_id = blockIdx.x >> 1, n_pairs_grid = gridDim.x >> 1;
+    const int32_t* __restrict__ offsets = P.offsets;
+    const int32_t* __restrict__ counts = P.counts;
+
+    if (warp == 3) {  // zero block; exclusive scan of the tiles per group
+        for (int i = lane; i < CfgT<EPI>::ZERO_BYTES / 16; i += 32) st_shared16(zero_blk + 16 * i, make_uint4(0, 0, 0, 0));
+        fence_proxy_async();
+        int carry = 0;
+        for (int g0 = 0; g0 < P.G; g0 += 32) {
+            const int g = g0 + lane;
+            int nch = 0, cs;
+            if (g < P.G) t_plan(counts[g], nch, cs, P.greedy);
+            const int v = nch * P.f_tiles;
+            int x = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            if (g < P.G) tq[g] = carry + x - v;
+            carry += __shfl_sync(0xffffffffu, x, 31);
+        }
+        if (lane == 0) tq[P.G] = carry;
+    }
+    if (warp == 0 && lane == 0) {
+        prefetch_tmap(&P.a[0]), prefetch_tmap(&P.b[0]);
+        if (P.n_src == 2 || EPI == TEPI_SWIGLU_FWD) prefetch_tmap(&P.a[1]);
+        if (P.n_src == 2) prefetch_tmap(&P.b[1]), prefetch_tmap(&P.bs[1]);
+        prefetch_tmap(&P.bs[0]);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
+        for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
+        for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
+        fence_barrier_init();
+    }
+    if (warp == 2) tmem_alloc2(tmem_ptr, 512);
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+    const int n_total = tq[P.G];
+    const int nkb = P.kb_per_src * P.n_src;
+
+    if (warp == 0) {
+        // ===== TMA producer (both CTAs): own 128 features of the weights + own half of the rows =====
+        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        int stage = 0, phase = 0;
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const TileT T = decode_t(P, tq, offsets, counts, t);
+            const int nb = T.n >> 1, rb = T.r0 + rank * nb;
+            const bool small = nb <= P.small_rows;
+            const int nbox = small ? (nb + TB_SMALL_ROWS - 1) / TB_SMALL_ROWS : 1;
+            const int box_bytes = (small ? TB_SMALL_ROWS : TB_BOX_ROWS) * BK * 2;
+            for (int kb = 0; kb < nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    uint8_t* sa = smem + stage * TSTAGE_BYTES;
+                    uint8_t* sb = sa + TA_BYTES;
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * (TA_BYTES + nbox * box_bytes));
+                    const uint32_t bar = leader_full + stage * 8;
+                    int src = 0, kk = kb;
+                    if (kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
+                    const int k = kk * BK;
+                    if (EPI == TEPI_SWIGLU_FWD) {  // 64 gate features | the same 64 up features
+                        const int fc = T.f * 128 + rank * 64;
+                        tma_load_3d_pair(sa, &P.a[0], bar, fc, k, T.g);
+                        tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[1], bar, fc, k, T.g);
+                    } else if (A_MAJOR == MN_MAJOR) {
+                        const int fc = T.f * 256 + rank * 128;
+                        tma_load_3d_pair(sa, &P.a[src], bar, fc, k, T.g);
+                        tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[src], bar, fc + 64, k, T.g);
+                    } else {
+                        tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + rank * 128, T.g);
+                    }
+                    if (small) {
+                        for (int i = 0; i < nbox; ++i)
+                            tma_load_3d_pair(sb + i * box_bytes, &P.bs[src], bar, k, rb + i * TB_SMALL_ROWS, 0);
+                    } else {
+                        tma_load_3d_pair(sb, &P.b[src], bar, k, rb, 0);
+                    }
+                }
+                __syncwarp();
+                if (++stage == NST) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (warp == 1 && rank == 0) {
+        // ===== MMA issuer (one thread of the leader CTA): D^T[256 features, n rows] += W-tile * rows^T =====
+        constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
+        constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        int stage = 0, phase = 0, as = 0, aphase = 0;
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const TileT T = decode_t(P, tq, offsets, counts, t);
+            const uint32_t idesc = make_idesc_t(A_MAJOR, T.n);
+            if (lane == 0) {
+                mbar_wait(&tempty_bar[as], aphase ^ 1);
+                tc_fence_after();
+            }
+            __syncwarp();
+            const uint32_t d_tmem = tmem_base + as * BN;
+            for (int kb = 0; kb < nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&full_bar[stage], phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_u32(smem + stage * TSTAGE_BYTES), sb = sa + TA_BYTES;
+#pragma unroll
+                    for (int kk = 0; kk < BK / UK; ++kk) {
+                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
+                        const uint64_t bd = make_desc(sb + kk * UK * 2, 16, 1024);
+                        umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
+                    }
+                    umma2_commit(&empty_bar[stage]);
+                }
+                __syncwarp();
+                if (++stage == NST) stage = 0, phase ^= 1;
+            }
+            if (lane == 0) umma2_commit(&tfull_bar[as]);
+            __syncwarp();
+            if (++as == 2) as = 0, aphase ^= 1;
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue (both CTAs): TMEM lane = feature, column = row; transposed through shared memory =====
+        const int wq = warp & 3;
+        const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
+        uint8_t* stg = stg_base + wq * NBUF * TSTG_BYTES;
+        int as = 0, aphase = 0, ring = 0;
+        uint32_t q = 0;  // running 32-row block number (SwiGLU epilogues: exchange slot / input set q & 1)
+        // one staged block [32 rows][32 features] -> out rows row.. (the second 16-row half only if `both`)
+        auto store_block = [&](const CUtensorMap* om, const uint8_t* buf, int fcol, int row, bool both) {
+            tma_store_3d(om, buf, fcol, row, 0);
+            if (both) tma_store_3d(om, buf + TSTG_BYTES / 2, fcol, row + 16, 0);
+        };
+        auto stage_col = [&](uint8_t* buf, const float* v) {  // this thread's feature: 32 rows of one column
+            const uint32_t a = smem_u32(buf) + lane * 2;
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) {
+                const uint32_t pk = f2_to_bf2(v[i], v[i + 1]);
+                sts_u16(a + i * 64, pk & 0xffffu);
+                sts_u16(a + (i + 1) * 64, pk >> 16);
+            }
+        };
+        auto next_buf = [&]() {
+            uint8_t* buf = stg + ring * TSTG_BYTES;
+            if (++ring == NBUF) ring = 0;
+            return buf;
+        };
+        // SwiGLU backward: G, U of 32 rows x 32 features -> input set `set` (two staging blocks)
+        auto load_inputs = [&](int fcol, int row, int set) {
+            if (lane == 0) {
+                bulk_wait_read<0>();
+                uint64_t* bar = &ld_bar[wq * 2 + set];
+                mbar_expect_tx(bar, 2 * TSTG_BYTES);
+                tma_load_3d(stg + (2 * set) * TSTG_BYTES, &P.ein[0], bar, fcol, row, 0);
+                tma_load_3d(stg + (2 * set + 1) * TSTG_BYTES, &P.ein[1], bar, fcol, row, 0);
+            }
+        };
+        const int pr = wq & 1;  // SwiGLU forward: warps pr (G lanes) and pr + 2 (U lanes) hold the same 32 features
+        auto feat_col = [&](const TileT& T) {
+            return EPI == TEPI_SWIGLU_FWD ? T.f * 128 + rank * 64 + 32 * pr : T.f * 256 + rank * 128 + 32 * wq;
+        };
+        if (EPI == TEPI_SWIGLU_BWD && pair_id < n_total) {
+            const TileT T0 = decode_t(P, tq, offsets, counts, pair_id);
+            load_inputs(feat_col(T0), T0.r0, 0);
+        }
+        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+            const TileT T = decode_t(P, tq, offsets, counts, t);
+            mbar_wait(&tfull_bar[as], aphase);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
+            const int fcol = feat_col(T);
+            const bool f_ok = fcol < P.f_limit;
+#pragma unroll 1
+            for (int j = 0; j < T.n; j += 32, ++q) {
+                const bool both = j + 16 < T.n;
+                uint32_t r[32];
+                float v[32];
+                if (EPI == TEPI_STORE) {
+                    if (!f_ok) break;
+                    uint8_t* buf = next_buf();
+                    if (lane == 0) bulk_wait_read<NBUF - 1>();
+                    __syncwarp();
+                    tmem_ld32(taddr + j, r);
+                    tmem_ld_wait32(r);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+                    stage_col(buf, v);
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) {
+                        store_block(&P.o[0], buf, fcol, T.r0 + j, both);
+                        bulk_commit();
+                    }
+                } else if (EPI == TEPI_SWIGLU_FWD) {
+                    const uint32_t xch = smem_u32(xch_base) + (pr * 2 + (q & 1)) * 4096 + lane * 4;
+                    tmem_ld32(taddr + j, r);
+                    tmem_ld_wait32(r);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+                    if (wq >= 2) {  // U lanes: hand the fp32 values to the G warp, store U
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) sts_f32(xch + i * 128, v[i]);
+                        asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
+                        uint8_t* buf = next_buf();
+                        if (lane == 0) bulk_wait_read<NBUF - 1>();
+                        __syncwarp();
+                        stage_col(buf, v);
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0 && f_ok) {
+                            store_block(&P.o[1], buf, fcol, T.r0 + j, both);
+                            bulk_commit();
+                        }
+                    } else {  // G lanes: store G, H = silu(G) * U
+                        uint8_t* bg = next_buf();
+                        uint8_t* bh = next_buf();
+                        if (lane == 0) bulk_wait_read<1>();  // two blocks per commit group, ring of four
+                        __syncwarp();
+                        stage_col(bg, v);
+                        asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = v[i] * sigmoidf_fast(v[i]) * lds_f32(xch + i * 128);
+                        stage_col(bh, v);
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0 && f_ok) {
+                            store_block(&P.o[0], bg, fcol, T.r0 + j, both);
+                            store_block(&P.o[2], bh, fcol, T.r0 + j, both);
+                            bulk_commit();
+                        }
+                    }
+                } else {
+                    // accumulator = dH; dG = dH * U * silu'(G), dU = dH * silu(G), in place over the staged G, U
+                    const int set = q & 1;
+                    const uint32_t bg = smem_u32(stg + (2 * set) * TSTG_BYTES) + lane * 2, bu = bg + TSTG_BYTES;
+                    mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
+                    if (j + 32 < T.n) {
+                        load_inputs(fcol, T.r0 + j + 32, set ^ 1);
+                    } else if (t + n_pairs_grid < n_total) {
+                        const TileT Tn = decode_t(P, tq, offsets, counts, t + n_pairs_grid);
+                        load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
+                    }
+                    tmem_ld32(taddr + j, r);
+                    tmem_ld_wait32(r);
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) {
+                        float dg[2], du[2];
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const float dh = __uint_as_float(r[i + e]);
+                            const float gv = lds_bf16(bg + (i + e) * 64), uv = lds_bf16(bu + (i + e) * 64);
+                            const float sg = sigmoidf_fast(gv);
+                            dg[e] = dh * uv * (sg * (1.f + gv * (1.f - sg)));
+                            du[e] = dh * (gv * sg);
+                        }
+                        const uint32_t pg = f2_to_bf2(dg[0], dg[1]), pu = f2_to_bf2(du[0], du[1]);
+                        sts_u16(bg + i * 64, pg & 0xffffu), sts_u16(bg + (i + 1) * 64, pg >> 16);
+                        sts_u16(bu + i * 64, pu & 0xffffu), sts_u16(bu + (i + 1) * 64, pu >> 16);
+                    }
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0 && f_ok) {
+                        store_block(&P.o[0], stg + (2 * set) * TSTG_BYTES, fcol, T.r0 + j, both);
+                        store_block(&P.o[1], stg + (2 * set + 1) * TSTG_BYTES, fcol, T.r0 + j, both);
+                        bulk_commit();
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(leader_tempty + as * 8);
+            if (++as == 2) as = 0, aphase ^= 1;
+            // pad rows behind the group's last chunk: exact zeros (wgrad reads them as part of its K range)
+            if (lane == 0 && f_ok && T.r0 + T.n < T.zend) {
+                for (int row = T.r0 + T.n; row < T.zend; row += 16) {
+                    if (EPI == TEPI_STORE) {
+                        tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
+                    } else if (EPI == TEPI_SWIGLU_FWD) {
+                        if (wq >= 2) {
+                            tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
+                        } else {
+                            tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
+                            tma_store_3d(&P.o[2], zero_blk, fcol, row, 0);
+                        }
+                    } else {
+                        tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
+                        tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
+                    }
+                }
+                bulk_commit();
+            }
+        }
+        if (lane == 0) bulk_wait_all();
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc2(tmem_base, 512);
+    }
+}
+
 // ---- host side ------------------------------------------------------------------------------------------
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// bf16 tensor [groups][rows][inner] (row-major), box = 64 inner elements (128 B, swizzled) x box_rows rows.
-int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
-             int box_rows) {
+// bf16 tensor [groups][rows][inner] (row-major), box = box_inner elements x box_rows rows; 128-byte swizzle when the
+// box is 64 elements (128 B) wide, else none.
+int make_map2(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
+              int box_inner, int box_rows) {
     const cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)groups};
     const cuuint64_t strides[2] = {(cuuint64_t)inner * 2, (cuuint64_t)inner * 2 * (cuuint64_t)rows};
-    const cuuint32_t box[3] = {64, (cuuint32_t)box_rows, 1};
+    const cuuint32_t box[3] = {(cuuint32_t)box_inner, (cuuint32_t)box_rows, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = reinterpret_cast<EncodeTiledFn>(c->encode_tiled)(
         m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
-        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        CU_TENSOR_MAP_INTERLEAVE_NONE, box_inner == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
-        snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled failed (%d): inner %lld rows %lld groups %lld box %d",
-                 (int)r, inner, rows, groups, box_rows);
+        snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled failed (%d): inner %lld rows %lld groups %lld box %dx%d",
+                 (int)r, inner, rows, groups, box_inner, box_rows);
         return PIPER_ERR_CUDA;
     }
     return PIPER_OK;
 }
+int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
+             int box_rows) {
+    return make_map2(c, m, base, inner, rows, groups, 64, box_rows);
+}
+#define PIPER_MAP2(...)                                \
+    do {                                               \
+        const int rc__ = make_map2(c, __VA_ARGS__);    \
+        if (rc__ != PIPER_OK) return rc__;             \
+    } while (0)
 #define PIPER_MAP(...)                                 \
     do {                                               \
         const int rc__ = make_map(c, __VA_ARGS__);     \
@@ -984,6 +1398,35 @@ bool set_smem_attr() {
                                 Cfg2<EPI>::SMEM) == cudaSuccess;
 }
 
+template <int A_MAJOR, int EPI>
+int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
+    long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
+    if (tile_bound < clusters) clusters = tile_bound;
+    if (clusters < 1) clusters = 1;
+    tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(P);
+    PIPER_LAUNCHED(c, name);
+    return PIPER_OK;
+}
+template <int A_MAJOR, int EPI>
+bool set_smem_attr_t() {
+    return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                CfgT<EPI>::SMEM) == cudaSuccess;
+}
+// rows-on-N kernel for the ragged-M contractions (PIPER_TC_ROWS_ON_N=0 switches it off)
+bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2 && p.counts; }
+TcParams t_params(const FfnProblem& p, int F, int K, int f_tile) {
+    TcParams P;
+    memset(&P, 0, sizeof(P));
+    P.offsets = p.offsets, P.counts = p.counts, P.G = p.G, P.n_src = 1;
+    P.f_tiles = cdiv(F, f_tile), P.f_limit = F, P.kb_per_src = cdiv(K, BK);
+    const char* e = getenv("PIPER_T_SMALL");
+    P.small_rows = e ? atoi(e) : TB_SMALL_ROWS;
+    const char* e2 = getenv("PIPER_T_GREEDY");
+    P.greedy = e2 ? atoi(e2) : 1;
+    return P;
+}
+inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
+
 // Pairing M tiles of one expert costs a duplicate tile per odd group: use the CTA-pair kernel when the groups are
 // long enough for that to be small (host-side expectation; the sizes themselves stay on the device).
 bool pair_ragged(const piper_ctx* c, const FfnProblem& p) {
@@ -1018,12 +1461,16 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     const char* pe = getenv("PIPER_TC_PROFILE");
     c->tc_prof = pe && pe[0] == '1';
+    const char* pt = getenv("PIPER_TC_ROWS_ON_N");
+    c->tc_rows_on_n = !(pt && pt[0] == '0');
     const char* p2 = getenv("PIPER_TC_2CTA");  // 0: never, 1: always, unset: by expected group length
     c->tc_two_cta = p2 ? (p2[0] == '0' ? 0 : 1) : 2;
     c->tc2_max_clusters = c->num_sms / 2;
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
-              set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>();
+              set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>() &&
+              set_smem_attr_t<MN_MAJOR, TEPI_SWIGLU_FWD>() && set_smem_attr_t<MN_MAJOR, TEPI_STORE>() &&
+              set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD>() && set_smem_attr_t<K_MAJOR, TEPI_STORE>();
     if (!ok) {
         cudaGetLastError();
         c->encode_tiled = nullptr;  // not an sm_100a device: the FP32-ALU kernels serve every request
@@ -1040,6 +1487,17 @@ bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
 
 // G|U = Xp Wg | Xp Wu, H = silu(G) * U
 int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    if (rows_on_n(c, p)) {
+        TcParams P = t_params(p, p.I, p.d, 128);
+        PIPER_MAP(&P.a[0], p.w_gate, p.I, p.d, p.G, 64);
+        PIPER_MAP(&P.a[1], p.w_up, p.I, p.d, p.G, 64);
+        PIPER_MAP(&P.b[0], p.xp, p.d, p.max_rows, 1, TB_BOX_ROWS);
+        PIPER_MAP(&P.bs[0], p.xp, p.d, p.max_rows, 1, TB_SMALL_ROWS);
+        PIPER_MAP2(&P.o[0], p.g, p.I, p.max_rows, 1, 32, 16);
+        PIPER_MAP2(&P.o[1], p.u, p.I, p.max_rows, 1, 32, 16);
+        PIPER_MAP2(&P.o[2], p.h, p.I, p.max_rows, 1, 32, 16);
+        return launch_t<MN_MAJOR, TEPI_SWIGLU_FWD>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd1_t");
+    }
     const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, BM);
@@ -1058,6 +1516,14 @@ int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
 
 // O = H Wd
 int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    if (rows_on_n(c, p)) {
+        TcParams P = t_params(p, p.d, p.I, 256);
+        PIPER_MAP(&P.a[0], p.w_down, p.d, p.I, p.G, 64);
+        PIPER_MAP(&P.b[0], p.h, p.I, p.max_rows, 1, TB_BOX_ROWS);
+        PIPER_MAP(&P.bs[0], p.h, p.I, p.max_rows, 1, TB_SMALL_ROWS);
+        PIPER_MAP2(&P.o[0], p.o, p.d, p.max_rows, 1, 32, 16);
+        return launch_t<MN_MAJOR, TEPI_STORE>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd2_t");
+    }
     const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, BM);
@@ -1070,6 +1536,17 @@ int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
 
 // dH = dO Wd^T; dG = dH * U * silu'(G); dU = dH * silu(G)
 int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    if (rows_on_n(c, p)) {
+        TcParams P = t_params(p, p.I, p.d, 256);
+        PIPER_MAP(&P.a[0], p.w_down, p.d, p.I, p.G, 128);
+        PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, TB_BOX_ROWS);
+        PIPER_MAP(&P.bs[0], p.d_o, p.d, p.max_rows, 1, TB_SMALL_ROWS);
+        PIPER_MAP2(&P.o[0], p.dg, p.I, p.max_rows, 1, 32, 16);
+        PIPER_MAP2(&P.o[1], p.du, p.I, p.max_rows, 1, 32, 16);
+        PIPER_MAP2(&P.ein[0], p.g, p.I, p.max_rows, 1, 32, 32);
+        PIPER_MAP2(&P.ein[1], p.u, p.I, p.max_rows, 1, 32, 32);
+        return launch_t<K_MAJOR, TEPI_SWIGLU_BWD>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad1_t");
+    }
     const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.d_o, p.d, p.max_rows, 1, BM);
@@ -1088,6 +1565,18 @@ int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
 
 // dXp = dG Wg^T + dU Wu^T  (one accumulator, K runs over both products)
 int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    if (rows_on_n(c, p)) {
+        TcParams P = t_params(p, p.d, p.I, 256);
+        PIPER_MAP(&P.a[0], p.w_gate, p.I, p.d, p.G, 128);
+        PIPER_MAP(&P.a[1], p.w_up, p.I, p.d, p.G, 128);
+        PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, TB_BOX_ROWS);
+        PIPER_MAP(&P.b[1], p.du, p.I, p.max_rows, 1, TB_BOX_ROWS);
+        PIPER_MAP(&P.bs[0], p.dg, p.I, p.max_rows, 1, TB_SMALL_ROWS);
+        PIPER_MAP(&P.bs[1], p.du, p.I, p.max_rows, 1, TB_SMALL_ROWS);
+        P.n_src = 2;
+        PIPER_MAP2(&P.o[0], p.dxp, p.d, p.max_rows, 1, 32, 16);
+        return launch_t<K_MAJOR, TEPI_STORE>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad2_t");
+    }
     const bool two = pair_ragged(c, p);
     TcParams P = base_params(p, true);
     PIPER_MAP(&P.a[0], p.dg, p.I, p.max_rows, 1, BM);

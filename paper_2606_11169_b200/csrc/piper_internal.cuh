@@ -54,6 +54,7 @@ struct piper_ctx {
     int tc_next_slot;        // round-robin slot in tc_scratch
     int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
     int tc2_max_clusters;    // co-resident CTA pairs
+    int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_TC_ROWS_ON_N, default on)
     int tc_prof;             // PIPER_TC_PROFILE=1: the tcgen05 kernels record wait-cycle counters in tc_scratch
     cudaEvent_t events[piper::kMaxEvents];
 };
@@ -104,6 +105,7 @@ struct FfnProblem {
     int max_group_rows;      // host-side bound on the rows of one group
     int exp_rows;            // rows expected under uniform routing (kernel-variant choice only)
     const int32_t* offsets;  // device, [G+1]
+    const int32_t* counts;   // device, [G]: real rows per group (offsets are padded to row_align)
     const void *xp, *w_gate, *w_up, *w_down;
     void *g, *u, *h, *o;                                 // forward outputs
     const void* d_o;                                     // backward inputs / outputs
