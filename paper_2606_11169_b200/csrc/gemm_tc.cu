@@ -507,14 +507,21 @@ __device__ __forceinline__ void stage32(uint8_t* buf, int r, int half, const flo
 // two tiles of the same expert (an odd last tile is paired with a duplicate whose stores are skipped); in
 // wgrad they are two 128-row slices of dW.
 // =====================================================================================================
-constexpr int A2_BYTES = BM * BK * 2, B2_BYTES = (BN / 2) * BK * 2, STAGE2_BYTES = A2_BYTES + B2_BYTES;
+#ifndef PIPER_WGRAD_BK
+#define PIPER_WGRAD_BK 128
+#endif
 // Ring depth and staging buffers per epilogue warp: the SwiGLU backward epilogue also stages its G, U inputs.
 constexpr int kMaxGroups2 = 192;  // groups the CTA-pair kernel can index (its tile-prefix arrays share the 227 KB)
 template <int EPI>
 struct Cfg2 {
-    static constexpr int NST = 5;
-    static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : 3;
-    static constexpr int RING_BYTES = NST * STAGE2_BYTES, STG_TOTAL = 4 * NBUF * STG_BYTES;
+    // wgrad (both operands MN-major: TMA boxes of 64 columns x BK rows) takes K blocks of 128 rows, so that a box is
+    // 16 KB like the K-major ones (8 KB boxes measured slower), in a 3-stage ring
+    static constexpr bool WG = EPI == EPI_WGRAD || EPI == EPI_WGRAD_SPLIT;
+    static constexpr int BKc = WG ? PIPER_WGRAD_BK : BK;
+    static constexpr int NST = BKc == 128 ? 3 : 5;
+    static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : (BKc == 128 ? 2 : 3);
+    static constexpr int A_B = BM * BKc * 2, B_B = (BN / 2) * BKc * 2, STAGE_B = A_B + B_B, MNB = 64 * BKc * 2;
+    static constexpr int RING_BYTES = NST * STAGE_B, STG_TOTAL = 4 * NBUF * STG_BYTES;
     static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups2 + 1) * 4;
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
@@ -569,7 +576,7 @@ __device__ __forceinline__ int total_pairs(const TcParams& P, const int* tpp) {
     return P.ragged_m ? tpp[P.G] * P.n_tiles : P.G * ((P.m_tiles + 1) / 2) * P.n_tiles;
 }
 __device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, const int* tpp,
-                                             const int32_t* __restrict__ offsets, int t, int rank) {
+                                             const int32_t* __restrict__ offsets, int t, int rank, int bk = BK) {
     Tile2 r;
     if (P.ragged_m) {
         int g = 0;
@@ -589,7 +596,7 @@ __device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, c
         const int nt = local / pairs, pair = local - nt * pairs;
         const int lo = offsets[g], hi = offsets[g + 1];
         r.store = true;  // rows beyond m_limit are clipped by the bounds checks
-        r.g = g, r.m0 = (2 * pair + rank) * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + BK - 1) / BK;
+        r.g = g, r.m0 = (2 * pair + rank) * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + bk - 1) / bk;
     }
     return r;
 }
@@ -617,7 +624,8 @@ template <int A_MAJOR, int B_MAJOR, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    constexpr int STAGES2 = Cfg2<EPI>::NST, NBUF = Cfg2<EPI>::NBUF;
+    constexpr int STAGES2 = Cfg2<EPI>::NST, NBUF = Cfg2<EPI>::NBUF, BKc = Cfg2<EPI>::BKc, MNB = Cfg2<EPI>::MNB;
+    constexpr int A2_BYTES = Cfg2<EPI>::A_B, STAGE2_BYTES = Cfg2<EPI>::STAGE_B;
     uint8_t* stg_base = smem + Cfg2<EPI>::RING_BYTES;
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(stg_base + Cfg2<EPI>::STG_TOTAL);  // used in the leader CTA
     uint64_t* empty_bar = full_bar + STAGES2;                                            // one set per CTA
@@ -677,7 +685,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         int stage = 0, phase = 0;
         long long w_empty = 0;
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
                     const long long c0 = P.prof ? clock64() : 0;
@@ -689,13 +697,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
-                    const int k = T.k0 + kk * BK;
+                    const int k = T.k0 + kk * BKc;
                     if (A_MAJOR == K_MAJOR) {
                         tma_load_3d_pair(sa, &P.a[src], bar, k, T.m0, 0);
                     } else {
 #pragma unroll
                         for (int j = 0; j < BM / 64; ++j)
-                            tma_load_3d_pair(sa + j * MN_BLOCK_BYTES, &P.a[src], bar, T.m0 + 64 * j, k, 0);
+                            tma_load_3d_pair(sa + j * MNB, &P.a[src], bar, T.m0 + 64 * j, k, 0);
                     }
                     const int bz = P.ragged_m ? T.g : 0;
                     if (B_MAJOR == K_MAJOR) {
@@ -705,7 +713,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                         const int col = P.b_split ? T.n0 : T.n0 + rank * (BN / 2);
 #pragma unroll
                         for (int j = 0; j < BN / 128; ++j)
-                            tma_load_3d_pair(sb + j * MN_BLOCK_BYTES, &P.b[half], bar, col + 64 * j, k, bz);
+                            tma_load_3d_pair(sb + j * MNB, &P.b[half], bar, col + 64 * j, k, bz);
                     }
                 }
                 __syncwarp();
@@ -716,13 +724,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     } else if (warp == 1 && rank == 0) {
         // ===== MMA issuer (one thread of the leader CTA) =====
         constexpr uint32_t idesc = make_idesc2(A_MAJOR, B_MAJOR);
-        constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
+        constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MNB, b_lbo = B_MAJOR == K_MAJOR ? 16 : MNB;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
         int stage = 0, phase = 0, as = 0, aphase = 0;
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc);
             if (lane == 0) {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
@@ -739,7 +747,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
 #pragma unroll
-                    for (int kk = 0; kk < BK / UK; ++kk) {
+                    for (int kk = 0; kk < BKc / UK; ++kk) {
                         const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
                         const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
                         umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
@@ -779,9 +787,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 tma_load_3d(stg + (2 * set + 1) * STG_BYTES, &P.ein[1], bar, Tn.n0 + 64 * c, Tn.m0 + wq * 32, 0);
             }
         };
-        if (EPI == EPI_SWIGLU_BWD && pair_id < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, pair_id, rank), 0, 0);
+        if (EPI == EPI_SWIGLU_BWD && pair_id < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, pair_id, rank, BKc), 0, 0);
         for (int t = pair_id; t < n_total; t += n_pairs_grid) {
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
             const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
             if (P.prof) w_tfull += clock64() - c0;
@@ -837,7 +845,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (c < 3) {
                         load_inputs(T, c + 1, set ^ 1);
                     } else if (t + n_pairs_grid < n_total) {
-                        load_inputs(decode_pair(P, tp, tpp, offsets, t + n_pairs_grid, rank), 0, set ^ 1);
+                        load_inputs(decode_pair(P, tp, tpp, offsets, t + n_pairs_grid, rank, BKc), 0, set ^ 1);
                     }
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -1594,9 +1602,10 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     const bool two = pair_wgrad(c, p);
     {
         TcParams P = base_params(p, false);
-        PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, 64);
-        PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, 64);
-        PIPER_MAP(&P.b[1], p.du, p.I, p.max_rows, 1, 64);
+        const int kbox = two ? Cfg2<EPI_WGRAD_SPLIT>::BKc : BK;
+        PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, kbox);
+        PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, kbox);
+        PIPER_MAP(&P.b[1], p.du, p.I, p.max_rows, 1, kbox);
         P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.m_tiles = cdiv(p.d, BM);
         P.m_limit = p.d, P.n_limit = p.I, P.ld = p.I, P.group_stride = (long long)p.d * p.I;
         P.out0 = (__nv_bfloat16*)p.dw_gate, P.out1 = (__nv_bfloat16*)p.dw_up;
@@ -1610,8 +1619,9 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         if (rc != PIPER_OK) return rc;
     }
     TcParams P = base_params(p, false);
-    PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, 64);
-    PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, 64);
+    const int kbox = two ? Cfg2<EPI_WGRAD>::BKc : BK;
+    PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, kbox);
+    PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, kbox);
     P.n_tiles = cdiv(p.d, BN), P.m_tiles = cdiv(p.I, BM);
     P.m_limit = p.I, P.n_limit = p.d, P.ld = p.d, P.group_stride = (long long)p.I * p.d;
     P.out0 = (__nv_bfloat16*)p.dw_down;
