@@ -364,16 +364,21 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     stream = torch.cuda.current_stream()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
-    def timed(fn):
+    def timed(fn, repeats=3):
+        """Median over `repeats` timings of `iters` back-to-back calls (the pair's time moves by several % from one
+        timing to the next: which SMs a partition gets and how the two streams interleave is not ours to fix)."""
         for _ in range(2):
             fn()
-        torch.cuda.synchronize()
-        e0.record(stream)
-        for _ in range(iters):
-            fn()
-        e1.record(stream)
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / iters
+        ts = []
+        for _ in range(repeats):
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(iters):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) / iters)
+        return sorted(ts)[len(ts) // 2]
 
     t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
     t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))

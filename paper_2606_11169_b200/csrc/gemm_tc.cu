@@ -772,9 +772,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         uint8_t* stg = stg_base + wq * NBUF * STG_BYTES;
         int as = 0, aphase = 0, ring = 0;
         long long w_tfull = 0, w_stg = 0;
-#ifdef PIPER_EPI_PROBE
-        long long pr_ld = 0, pr_st = 0, pr_fence = 0, pr_tma = 0;
-#endif
         const long long t_begin = P.prof ? clock64() : 0;
         uint32_t q = 0;  // SwiGLU backward: running chunk number -> input set q & 1, barrier phase (q >> 1) & 1
         // G, U of 32 rows x 64 columns -> set `set` of this warp's staging buffers (bytes counted on ld_bar)
@@ -895,40 +892,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         uint32_t r[32];
-#ifdef PIPER_EPI_PROBE
-                        const long long p0 = clock64();
-#endif
                         tmem_ld32(taddr + 64 * c + 32 * h, r);
                         tmem_ld_wait32(r);
-#ifdef PIPER_EPI_PROBE
-                        const long long p1 = clock64();
-                        pr_ld += p1 - p0;
-#endif
                         float v[32];
 #pragma unroll
                         for (int i = 0; i < 32; ++i) v[i] = zero ? 0.f : __uint_as_float(r[i]);
                         stage32(buf, lane, h, v);
-#ifdef PIPER_EPI_PROBE
-                        pr_st += clock64() - p1;
-#endif
                     }
-#ifdef PIPER_EPI_PROBE
-                    const long long p2 = clock64();
-#endif
                     fence_proxy_async();
                     __syncwarp();
-#ifdef PIPER_EPI_PROBE
-                    const long long p3 = clock64();
-                    pr_fence += p3 - p2;
-#endif
                     if (lane == 0 && T.store) {
                         tma_store_3d(om, buf, col, row0, z);
                         bulk_commit();
                     }
-#ifdef PIPER_EPI_PROBE
-                    __syncwarp();
-                    pr_tma += clock64() - p3;
-#endif
                 }
             }
             tc_fence_before();
@@ -940,9 +916,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         if (P.prof && threadIdx.x == 128) {
             long long* pq = P.prof + blockIdx.x * 8;
             pq[4] = w_tfull, pq[5] = clock64() - t_begin, pq[7] = w_stg;
-#ifdef PIPER_EPI_PROBE
-            if (EPI == EPI_WGRAD || EPI == EPI_WGRAD_SPLIT || EPI == EPI_STORE) pq[0] = pr_ld, pq[1] = pr_st, pq[3] = pr_fence, pq[6] = pr_tma;
-#endif
         }
     }
     tc_fence_before();
@@ -1375,6 +1348,36 @@ int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, lo
         if (rc__ != PIPER_OK) return rc__;             \
     } while (0)
 
+// Co-resident CTA pairs of a cluster kernel on the lane's stream (a green-context partition may hold fewer whole
+// pairs than sms / 2): the persistent grids stride over this many pairs, so it must not exceed what fits at once.
+// Queried once per (kernel, SM count of the lane) and kept.
+template <typename K>
+int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes) {
+    constexpr int kSlots = 128;
+    static struct { const void* fn; cudaStream_t stream; int sms; int n; } cache[kSlots];
+    static int used = 0;
+    const void* key = reinterpret_cast<const void*>(kernel);
+    for (int i = 0; i < (used < kSlots ? used : kSlots); ++i)
+        if (cache[i].fn == key && cache[i].sms == ln.sms && cache[i].stream == ln.stream) return cache[i].n;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2, attr.val.clusterDim.y = 1, attr.val.clusterDim.z = 1;
+    cfg.gridDim = dim3(2 * (ln.sms / 2)), cfg.blockDim = dim3(kThreads), cfg.dynamicSmemBytes = smem_bytes;
+    cfg.stream = ln.stream, cfg.attrs = &attr, cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kernel, &cfg) != cudaSuccess || n < 1) {
+        cudaGetLastError();
+        n = ln.sms / 2;
+    }
+    if (n > ln.sms / 2) n = ln.sms / 2;
+    if (getenv("PIPER_DEBUG")) fprintf(stderr, "[piper] resident clusters: lane of %d SMs -> %d pairs\n", ln.sms, n);
+    const int slot = used++ % kSlots;
+    cache[slot].fn = key, cache[slot].stream = ln.stream, cache[slot].sms = ln.sms, cache[slot].n = n;
+    return n;
+}
+
 template <int A_MAJOR, int B_MAJOR, int EPI>
 int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool two_cta, const char* name) {
     TcParams Q = P;
@@ -1384,7 +1387,7 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
     }
     if (two_cta) {
         // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
-        long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
+        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
         tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
@@ -1408,7 +1411,7 @@ bool set_smem_attr() {
 
 template <int A_MAJOR, int EPI>
 int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
-    long long clusters = ln.sms / 2 < c->tc2_max_clusters ? ln.sms / 2 : c->tc2_max_clusters;
+    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI>, CfgT<EPI>::SMEM);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
     tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(P);
