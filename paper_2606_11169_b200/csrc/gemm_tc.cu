@@ -2,23 +2,30 @@
 // §8a; BASELINE.json:north_star part 3).  bf16 x bf16 -> fp32 accumulation in TMEM, one rounding to bf16
 // per stored tensor (SURVEY.md §8c "Error budget").
 //
-// One persistent, warp-specialised kernel template serves the five contractions of the FFN:
-//   warp 0  : TMA producer (cp.async.bulk.tensor, 128-byte swizzle) into a 4-stage shared-memory ring
-//   warp 1  : single-thread tcgen05.mma issuer (M=128, N=256, K=16, cta_group::1), tcgen05.commit hand-off
-//   warp 2  : TMEM allocator (512 columns = two 128x256 fp32 accumulators: the epilogue of tile i overlaps
-//             the main loop of tile i+1)
+// Three persistent, warp-specialised kernel templates, all with
+//   warp 0  : TMA producer (cp.async.bulk.tensor, 128-byte swizzle) into a shared-memory ring
+//   warp 1  : single-thread tcgen05.mma issuer, tcgen05.commit hand-off to the ring and to the epilogue
+//   warp 2  : TMEM allocator (512 columns = two fp32 accumulators: the epilogue of tile i overlaps the main
+//             loop of tile i+1)
 //   warps 4-7: epilogue, tcgen05.ld TMEM -> registers -> fused math -> global
+//  tc_gemmT_kernel  rows-on-N CTA pair (cta_group::2): fwd1, fwd2, dgrad1, dgrad2.  Weights on M (256 features per
+//                   pair), the expert's rows on N in multiples of 16; transposing TMA-store epilogues.
+//  tc_gemm2_kernel  CTA pair, 256 x 256 tiles: wgrad (K = the expert's rows, both operands MN-major, K blocks of
+//                   128); TMEM -> swizzled shared memory -> TMA-store epilogue.  Also the rows-on-M form of the
+//                   four contractions above (PIPER_TC_ROWS_ON_N=0).
+//  tc_gemm_kernel   1-CTA 128 x 256 tiles, direct-store epilogue: fallback (> 192 groups, PIPER_TC_2CTA=0).
 // Operand layouts are taken as they lie in memory (no transposed copies): the descriptors select K-major
-// or MN-major per operand:
+// or MN-major per operand.  In the rows-on-M form:
 //   fwd1   G|U = Xp Wg | Xp Wu      A K-major  (Xp [rows,d]),   B MN-major (W [d,I], two 128-col halves)
 //   fwd2   O   = H Wd               A K-major  (H  [rows,I]),   B MN-major (Wd [I,d])
 //   dgrad1 dH  = dO Wd^T            A K-major  (dO [rows,d]),   B K-major  (Wd [I,d])
 //   dgrad2 dXp = dG Wg^T + dU Wu^T  A K-major  (dG,dU [rows,I]),B K-major  (Wg,Wu [d,I]); K runs over both
 //   wgrad  dWg|dWu = Xp^T dG|dU ; dWd = H^T dO    A, B MN-major (row buffers), K = the expert's rows
+// (rows-on-N: the same products transposed, the weight operand first.)
 // Ragged groups: segments are padded to row_align = 128 rows (pad rows are zero in every row buffer), so
 // an M tile never straddles two experts and the ragged K of wgrad is a whole number of tiles; the tile ->
-// expert map is computed on the device from `offsets` (no host read-back).  Tails in d / I / T are
-// handled by TMA zero fill on loads and bounds checks on stores.
+// expert map is computed on the device from `offsets` / `counts` (no host read-back).  Tails in d / I / T are
+// handled by TMA zero fill on loads and TMA clipping / bounds checks on stores.
 #include "piper_internal.cuh"
 
 namespace piper {
