@@ -106,6 +106,35 @@ def test_small_configs_full_tensor_parity(name, impl, align):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s"])
+def test_poisoned_buffers_and_untouched_capacity(name):
+    """No result may depend on what a buffer held before (pad rows are written, never assumed), and no kernel may
+    write past the used rows: every output / scratch buffer starts as NaN (0x7FC1 / int 0x7FC17FC1 patterns), the
+    chunk calls run, the results match the oracle, dW is finite, and the rows of the row buffers beyond
+    offsets[E_loc] still hold the poison.  (compute-sanitizer is closed on this pool; this is the bounds check.)"""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx = piper.Context(util.desc_of(cfg))
+    b = piper.alloc_buffers(ctx, backward=True)
+    for t in b.values():
+        t.view(torch.int16).fill_(0x7FC1)
+    b.update(util.upload_inputs(inp))
+    args = piper.chunk_args(b)
+    piper.piper_run_chunk_fwd(ctx, args)
+    piper.piper_run_chunk_bwd(ctx, args)
+    torch.cuda.synchronize()
+    A = _check_all(cfg, b, f, g) and int(f["offsets"][-1])
+    poison = torch.tensor(0x7FC1, dtype=torch.int16, device=b["xp"].device)
+    for n in ("xp", "g_save", "u_save", "h_save", "o", "d_o", "dg", "du", "dxp"):
+        assert bool((b[n][A:].view(torch.int16) == poison).all()), f"{n}: rows beyond offsets[E_loc] were written"
+        assert bool(torch.isfinite(b[n][:A].float()).all()), f"{n}: non-finite value inside the used rows"
+    for n in ("dw_gate", "dw_up", "dw_down", "y", "dx"):
+        assert bool(torch.isfinite(b[n].float()).all()), n
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["C1", "C3s", "C4s"])
 def test_chunk_calls_equal_step_calls_bitwise(name):
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128 if name != "C1" else 1)
