@@ -63,7 +63,7 @@ typedef struct {
     int32_t dtype;     /* PIPER_DTYPE_*                                                             */
     int32_t gate_mode; /* PIPER_GATE_*                                                              */
     int32_t row_align; /* >= 1: each expert's row segment is padded to a multiple; pad rows are 0   */
-    int32_t dw_dtype;  /* element type of dW outputs; must equal dtype in this build                */
+    int32_t dw_dtype;  /* element type of dW outputs: = dtype, or F32 on a BF16 layer (main-grad style) */
     int32_t gemm_impl; /* PIPER_GEMM_*                                                              */
 } piper_moe_desc;
 
@@ -126,8 +126,10 @@ int piper_combine_bwd(piper_ctx* ctx, const void* dy, const void* o, const int32
 /* B2-B4 expert_ffn_bwd (SURVEY.md §8a B2/B3/B4, §8c Definition 5; north_star part 3 "dgrad and
  * wgrad").  dh = d_o W_down^T; dg = dh*u*silu'(g); du = dh*silu(g); dxp = dg W_gate^T + du W_up^T;
  * dw_down[e] = h^T d_o, dw_gate[e] = xp^T dg, dw_up[e] = xp^T du summed over the expert's rows
- * (exact zeros for empty experts).  dg, du [A_cap,I] are opaque scratch.  accumulate must be 0 in
- * this build. */
+ * (exact zeros for empty experts).  dg, du [A_cap,I] are opaque scratch.  accumulate = 1 adds the
+ * sums into dw_* instead of overwriting them (reading c-17: main-grad style; Piper reduces after every backward,
+ * PAPER.md:384): needs dw_dtype = F32 on a BF16 layer (the whole ragged-K sum is accumulated in fp32 in TMEM and
+ * added to dW by a bulk tensor reduction), PIPER_ERR_UNSUPPORTED otherwise. */
 int piper_expert_ffn_bwd(piper_ctx* ctx, const void* d_o, const void* xp, const void* g_save, const void* u_save,
                          const void* h_save, const int32_t* offsets, const void* w_gate, const void* w_up,
                          const void* w_down, void* dg, void* du, void* dxp, void* dw_gate, void* dw_up, void* dw_down,
@@ -219,6 +221,10 @@ int piper_pair_order(piper_ctx* ctx, int sm_gemm, int sm_comm, int32_t* order, i
 #define PIPER_TASK_B_UNPACK 12
 #define PIPER_TASK_B_ROUTE_BWD 13
 int piper_run_task(piper_ctx* ctx, int task, const piper_chunk_args* a, void* stream);
+
+/* accumulate flag of the wgrad inside piper_run_chunk_bwd / piper_run_chunk_pair / piper_run_task (host state of
+ * `ctx`, default 0); PIPER_ERR_UNSUPPORTED unless dw_dtype = F32. */
+int piper_set_wgrad_accumulate(piper_ctx* ctx, int accumulate);
 
 /* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
  * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 0 = never called. */

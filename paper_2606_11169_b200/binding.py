@@ -76,9 +76,10 @@ def _stream(stream):
 
 
 def make_desc(T, d, E, k, I, e_lo=0, E_loc=-1, I_shared=0, dtype=DT_BF16, gate_mode=0, row_align=1,
-              gemm_impl=GEMM_AUTO) -> MoeDesc:
-    return MoeDesc(T, d, E, k, e_lo, E if E_loc < 0 else E_loc, I, I_shared, dtype, gate_mode, row_align, dtype,
-                   gemm_impl)
+              gemm_impl=GEMM_AUTO, dw_dtype=None) -> MoeDesc:
+    """dw_dtype: element type of the dW outputs (default = dtype; DT_F32 on a bf16 layer = main-grad style fp32 dW)."""
+    return MoeDesc(T, d, E, k, e_lo, E if E_loc < 0 else E_loc, I, I_shared, dtype, gate_mode, row_align,
+                   dtype if dw_dtype is None else dw_dtype, gemm_impl)
 
 
 class Context:
@@ -128,6 +129,10 @@ class Context:
 
 def piper_kernel_launches(ctx: Context) -> int:
     return int(lib().piper_kernel_launches(ctx._h))
+
+
+def piper_set_wgrad_accumulate(ctx: Context, accumulate: int):
+    ctx.check(lib().piper_set_wgrad_accumulate(ctx._h, int(accumulate)), "piper_set_wgrad_accumulate")
 
 
 def piper_pair_partition_mode(ctx: Context) -> int:
@@ -311,12 +316,13 @@ def alloc_buffers(ctx: Context, backward: bool = True) -> dict:
         b.update(gs_save=e((D.T, D.I_shared), dt), us_save=e((D.T, D.I_shared), dt), hs_save=e((D.T, D.I_shared), dt),
                  s=e((D.T, D.d), dt))
     if backward:
+        wt = torch.bfloat16 if D.dw_dtype == DT_BF16 else torch.float32
         b.update(dgates=e((D.T, D.k), f32), dz_sel=e((D.T, D.E if D.gate_mode == 2 else D.k), f32),
                  d_o=e((A, D.d), dt), dg=e((A, D.I), dt), du=e((A, D.I), dt), dxp=e((A, D.d), dt),
-                 dx=e((D.T, D.d), dt), dw_gate=e((D.E_loc, D.d, D.I), dt), dw_up=e((D.E_loc, D.d, D.I), dt),
-                 dw_down=e((D.E_loc, D.I, D.d), dt))
+                 dx=e((D.T, D.d), dt), dw_gate=e((D.E_loc, D.d, D.I), wt), dw_up=e((D.E_loc, D.d, D.I), wt),
+                 dw_down=e((D.E_loc, D.I, D.d), wt))
         if D.I_shared:
             b.update(dgs=e((D.T, D.I_shared), dt), dus=e((D.T, D.I_shared), dt), dxs=e((D.T, D.d), dt),
-                     dws_gate=e((D.d, D.I_shared), dt), dws_up=e((D.d, D.I_shared), dt),
-                     dws_down=e((D.I_shared, D.d), dt))
+                     dws_gate=e((D.d, D.I_shared), wt), dws_up=e((D.d, D.I_shared), wt),
+                     dws_down=e((D.I_shared, D.d), wt))
     return b

@@ -15,7 +15,7 @@ bool desc_ok(const piper_moe_desc* D) {
     if (D->dtype != PIPER_DTYPE_F32 && D->dtype != PIPER_DTYPE_BF16) return false;
     if (D->gate_mode < 0 || D->gate_mode > 2) return false;
     if (D->row_align < 1 || D->row_align > 1024) return false;
-    if (D->dw_dtype != D->dtype) return false;
+    if (D->dw_dtype != D->dtype && !(D->dtype == PIPER_DTYPE_BF16 && D->dw_dtype == PIPER_DTYPE_F32)) return false;
     if (D->gemm_impl != PIPER_GEMM_AUTO && D->gemm_impl != PIPER_GEMM_SIMT) return false;
     if ((int64_t)D->T * D->k > (1ll << 30)) return false;
     return true;
@@ -113,6 +113,12 @@ int piper_gemm_path(const piper_ctx* c) {
 }
 const void* piper_debug_tc_counters(const piper_ctx* c) { return c && c->tc_prof ? c->tc_scratch : nullptr; }
 int piper_pair_partition_mode(const piper_ctx* c) { return c ? c->pair_mode : 0; }
+int piper_set_wgrad_accumulate(piper_ctx* c, int accumulate) {
+    if (!c || (accumulate != 0 && accumulate != 1)) return PIPER_ERR_INVALID;
+    if (accumulate && c->D.dw_dtype != PIPER_DTYPE_F32) return PIPER_ERR_UNSUPPORTED;
+    c->wgrad_accumulate = accumulate;
+    return PIPER_OK;
+}
 
 int piper_route_topk(piper_ctx* c, const float* logits, int32_t* topk_idx, float* gates, int32_t* counts_global,
                      void* stream) {
@@ -174,13 +180,14 @@ int piper_expert_ffn_bwd(piper_ctx* c, const void* d_o, const void* xp, const vo
     if (!c || !all_aligned(d_o, xp, g_save, u_save, h_save, offsets, w_gate, w_up, w_down, dg, du, dxp, dw_gate, dw_up,
                            dw_down))
         return PIPER_ERR_INVALID;
-    if (accumulate) return PIPER_ERR_UNSUPPORTED;
+    if (accumulate != 0 && accumulate != 1) return PIPER_ERR_INVALID;
     piper_chunk_args a{};
     a.d_o = const_cast<void*>(d_o), a.xp = const_cast<void*>(xp), a.offsets = const_cast<int32_t*>(offsets);
     a.g_save = const_cast<void*>(g_save), a.u_save = const_cast<void*>(u_save), a.h_save = const_cast<void*>(h_save);
     a.w_gate = w_gate, a.w_up = w_up, a.w_down = w_down;
     a.dg = dg, a.du = du, a.dxp = dxp, a.dw_gate = dw_gate, a.dw_up = dw_up, a.dw_down = dw_down;
-    const FfnProblem p = routed_problem(c, &a);
+    FfnProblem p = routed_problem(c, &a);
+    p.accumulate = accumulate;
     const Lane ln = full_lane(c, stream);
     int rc = ffn_dgrad1(c, ln, p);
     if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
@@ -195,13 +202,14 @@ int piper_shared_ffn_bwd(piper_ctx* c, const void* dy, const void* x, const void
     if (!c || c->D.I_shared == 0 ||
         !all_aligned(dy, x, g_save, u_save, h_save, ws_gate, ws_up, ws_down, dgs, dus, dxs, dws_gate, dws_up, dws_down))
         return PIPER_ERR_INVALID;
-    if (accumulate) return PIPER_ERR_UNSUPPORTED;
+    if (accumulate != 0 && accumulate != 1) return PIPER_ERR_INVALID;
     piper_chunk_args a{};
     a.dy = dy, a.x = x;
     a.gs_save = const_cast<void*>(g_save), a.us_save = const_cast<void*>(u_save), a.hs_save = const_cast<void*>(h_save);
     a.ws_gate = ws_gate, a.ws_up = ws_up, a.ws_down = ws_down;
     a.dgs = dgs, a.dus = dus, a.dxs = dxs, a.dws_gate = dws_gate, a.dws_up = dws_up, a.dws_down = dws_down;
-    const FfnProblem p = shared_problem(c, &a);
+    FfnProblem p = shared_problem(c, &a);
+    p.accumulate = accumulate;
     const Lane ln = full_lane(c, stream);
     int rc = ffn_dgrad1(c, ln, p);
     if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);

@@ -12,6 +12,7 @@ FfnProblem routed_problem(const piper_ctx* c, const piper_chunk_args* a) {
     p.max_rows = (int)piper_a_cap(&D);
     p.max_group_rows = D.T + D.row_align - 1;
     p.exp_rows = (int)((long long)D.T * D.k * D.E_loc / D.E);
+    p.accumulate = c->wgrad_accumulate;
     p.offsets = a->offsets, p.counts = a->counts;
     p.xp = a->xp, p.w_gate = a->w_gate, p.w_up = a->w_up, p.w_down = a->w_down;
     p.g = a->g_save, p.u = a->u_save, p.h = a->h_save, p.o = a->o;
@@ -25,6 +26,7 @@ FfnProblem shared_problem(const piper_ctx* c, const piper_chunk_args* a) {
     FfnProblem p{};
     p.G = 1, p.d = D.d, p.I = D.I_shared;
     p.max_rows = D.T, p.max_group_rows = D.T, p.exp_rows = D.T;
+    p.accumulate = c->wgrad_accumulate;
     p.offsets = c->shared_offsets, p.counts = c->shared_offsets + 1;
     p.xp = a->x, p.w_gate = a->ws_gate, p.w_up = a->ws_up, p.w_down = a->ws_down;
     p.g = a->gs_save, p.u = a->us_save, p.h = a->hs_save, p.o = a->s;
@@ -41,6 +43,10 @@ int ffn_gemm1(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) 
 int ffn_gemm2(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_fwd2(c, ln, p) : simt_ffn_fwd(c, ln, p, 2); }
 int ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_dgrad1(c, ln, p) : simt_ffn_dgrad(c, ln, p, 1); }
 int ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_dgrad2(c, ln, p) : simt_ffn_dgrad(c, ln, p, 2); }
-int ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_wgrad(c, ln, p) : simt_ffn_wgrad(c, ln, p); }
+int ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
+    if (use_tc(c, p)) return tc_ffn_wgrad(c, ln, p);
+    if (p.accumulate || c->D.dw_dtype != c->D.dtype) return PIPER_ERR_UNSUPPORTED;  // fp32 dW of bf16 layers: tcgen05 only
+    return simt_ffn_wgrad(c, ln, p);
+}
 
 }  // namespace piper

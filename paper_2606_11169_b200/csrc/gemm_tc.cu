@@ -68,6 +68,8 @@ struct alignas(64) TcParams {
     const int32_t* counts;  // [G] device: real rows per group
     int f_tiles;            // tiles along the feature (output column) dimension
     int f_limit;            // output columns
+    int out_f32;            // wgrad: dW is fp32 (o[] are fp32 maps, 32-column boxes); accum: add into dW (TMA reduce)
+    int accum;
     int greedy;             // chunking: 1 = 256-row chunks and a short last one, 0 = equal chunks
     int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
 };
@@ -466,6 +468,11 @@ __device__ __forceinline__ void tmem_ld_wait32(uint32_t (&r)[32]) {
 }
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
+    asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
                  "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2)
                  : "memory");
 }
@@ -890,6 +897,36 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     const CUtensorMap* om = split ? &P.o[c >> 1] : &P.o[0];
                     const int col = split ? T.n0 + 64 * (c & 1) : T.n0 + 64 * c;
                     if (col >= P.n_limit) continue;
+                    if (P.out_f32) {
+                        // fp32 dW (main-grad style): two blocks of 32 columns x 32 rows fp32, stored or added into
+                        // dW by the TMA (cp.reduce.async.bulk.tensor .add: no read-modify-write on the SM)
+#pragma unroll 1
+                        for (int h = 0; h < 2; ++h) {
+                            if (col + 32 * h >= P.n_limit) break;
+                            uint8_t* fbuf = stg + ring * STG_BYTES;
+                            if (++ring == NBUF) ring = 0;
+                            if (lane == 0) bulk_wait_read<NBUF - 1>();
+                            __syncwarp();
+                            uint32_t r[32];
+                            tmem_ld32(taddr + 64 * c + 32 * h, r);
+                            tmem_ld_wait32(r);
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                uint4 q4;
+                                q4.x = zero ? 0u : r[4 * j], q4.y = zero ? 0u : r[4 * j + 1];
+                                q4.z = zero ? 0u : r[4 * j + 2], q4.w = zero ? 0u : r[4 * j + 3];
+                                st_shared16(stg_at(fbuf, lane, j), q4);
+                            }
+                            fence_proxy_async();
+                            __syncwarp();
+                            if (lane == 0 && T.store) {
+                                if (P.accum) tma_reduce_add_3d(om, fbuf, col + 32 * h, row0, z);
+                                else tma_store_3d(om, fbuf, col + 32 * h, row0, z);
+                                bulk_commit();
+                            }
+                        }
+                        continue;
+                    }
                     uint8_t* buf = stg + ring * STG_BYTES;
                     if (++ring == NBUF) ring = 0;
                     const long long c1 = P.prof ? clock64() : 0;
@@ -977,7 +1014,7 @@ __device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, cons
                                           const int32_t* __restrict__ counts, int t) {
     int g = 0;
     while (g + 1 < P.G && tq[g + 1] <= t) ++g;
-    const int local = t - tq[g], rows = counts[g];
+    const int local = t - tq[g], rows = counts ? counts[g] : offsets[g + 1] - offsets[g];
     int nch, cs;
     t_plan(rows, nch, cs, P.greedy);
     // panels of T_PANEL chunks; inside a panel feature-major with the chunk fastest
@@ -1026,7 +1063,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         for (int g0 = 0; g0 < P.G; g0 += 32) {
             const int g = g0 + lane;
             int nch = 0, cs;
-            if (g < P.G) t_plan(counts[g], nch, cs, P.greedy);
+            if (g < P.G) t_plan(counts ? counts[g] : offsets[g + 1] - offsets[g], nch, cs, P.greedy);
             const int v = nch * P.f_tiles;
             int x = v;
 #pragma unroll
@@ -1344,6 +1381,23 @@ int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, lo
              int box_rows) {
     return make_map2(c, m, base, inner, rows, groups, 64, box_rows);
 }
+// fp32 tensor [groups][rows][inner], box = 32 columns (128 B, swizzled) x 32 rows: the fp32 dW outputs of wgrad
+int make_map_f32(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups) {
+    const cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)groups};
+    const cuuint64_t strides[2] = {(cuuint64_t)inner * 4, (cuuint64_t)inner * 4 * (cuuint64_t)rows};
+    const cuuint32_t box[3] = {32, 32, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = reinterpret_cast<EncodeTiledFn>(c->encode_tiled)(
+        m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(base), dims, strides, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled (fp32) failed (%d): inner %lld rows %lld groups %lld", (int)r,
+                 inner, rows, groups);
+        return PIPER_ERR_CUDA;
+    }
+    return PIPER_OK;
+}
 #define PIPER_MAP2(...)                                \
     do {                                               \
         const int rc__ = make_map2(c, __VA_ARGS__);    \
@@ -1431,7 +1485,7 @@ bool set_smem_attr_t() {
                                 CfgT<EPI>::SMEM) == cudaSuccess;
 }
 // rows-on-N kernel for the ragged-M contractions (PIPER_TC_ROWS_ON_N=0 switches it off)
-bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2 && p.counts; }
+bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2; }
 TcParams t_params(const FfnProblem& p, int F, int K, int f_tile) {
     TcParams P;
     memset(&P, 0, sizeof(P));
@@ -1610,6 +1664,8 @@ int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
 // dWg|dWu[e] = Xp^T dG | Xp^T dU ; dWd[e] = H^T dO over the expert's rows (K ragged; zeros for empty experts)
 int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     const bool two = pair_wgrad(c, p);
+    const bool f32 = c->D.dw_dtype == PIPER_DTYPE_F32;  // fp32 dW from bf16 operands: the CTA-pair kernel only
+    if ((f32 || p.accumulate) && !(two && f32)) return PIPER_ERR_UNSUPPORTED;
     {
         TcParams P = base_params(p, false);
         const int kbox = two ? Cfg2<EPI_WGRAD_SPLIT>::BKc : BK;
@@ -1619,7 +1675,12 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         P.b_split = 1, P.tile_n = 128, P.n_tiles = cdiv(p.I, 128), P.m_tiles = cdiv(p.d, BM);
         P.m_limit = p.d, P.n_limit = p.I, P.ld = p.I, P.group_stride = (long long)p.d * p.I;
         P.out0 = (__nv_bfloat16*)p.dw_gate, P.out1 = (__nv_bfloat16*)p.dw_up;
-        if (two) {
+        if (f32) {
+            int rc = make_map_f32(c, &P.o[0], p.dw_gate, p.I, p.d, p.G);
+            if (rc == PIPER_OK) rc = make_map_f32(c, &P.o[1], p.dw_up, p.I, p.d, p.G);
+            if (rc != PIPER_OK) return rc;
+            P.out_f32 = 1, P.accum = p.accumulate;
+        } else if (two) {
             PIPER_MAP(&P.o[0], p.dw_gate, p.I, p.d, p.G, 32);
             PIPER_MAP(&P.o[1], p.dw_up, p.I, p.d, p.G, 32);
         }
@@ -1635,7 +1696,13 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     P.n_tiles = cdiv(p.d, BN), P.m_tiles = cdiv(p.I, BM);
     P.m_limit = p.I, P.n_limit = p.d, P.ld = p.d, P.group_stride = (long long)p.I * p.d;
     P.out0 = (__nv_bfloat16*)p.dw_down;
-    if (two) PIPER_MAP(&P.o[0], p.dw_down, p.d, p.I, p.G, 32);
+    if (f32) {
+        const int rc = make_map_f32(c, &P.o[0], p.dw_down, p.d, p.I, p.G);
+        if (rc != PIPER_OK) return rc;
+        P.out_f32 = 1, P.accum = p.accumulate;
+    } else if (two) {
+        PIPER_MAP(&P.o[0], p.dw_down, p.d, p.I, p.G, 32);
+    }
     const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
     return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * mt * P.n_tiles, two, "tc_ffn_wgrad_down");
 }

@@ -42,6 +42,7 @@ struct piper_ctx {
     int32_t* shared_offsets; // [2] = {0, T}: the shared expert as one group
     int64_t launches;
     int pair_mode;
+    int wgrad_accumulate;        // piper_set_wgrad_accumulate: the chunk calls' wgrad adds into dW
     int pair_order, pair_part;   // piper_set_pair_policy
     int pair_have_ms;
     void* pair_plan;             // cached schedule of the pair for (plan_sm_gemm, plan_sm_comm)
@@ -104,6 +105,7 @@ struct FfnProblem {
     int max_rows;            // host-side bound on offsets[G] (sizes the tensor maps and SIMT grids)
     int max_group_rows;      // host-side bound on the rows of one group
     int exp_rows;            // rows expected under uniform routing (kernel-variant choice only)
+    int accumulate;          // wgrad adds into dW (fp32 dW only)
     const int32_t* offsets;  // device, [G+1]
     const int32_t* counts;   // device, [G]: real rows per group (offsets are padded to row_align)
     const void *xp, *w_gate, *w_up, *w_down;

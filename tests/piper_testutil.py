@@ -9,9 +9,10 @@ from inputs import configs
 TOL = {configs.DT_BF16: (5e-3, 2e-2), configs.DT_F32: (1e-5, 1e-5)}
 
 
-def desc_of(cfg, gemm_impl=piper.GEMM_AUTO):
+def desc_of(cfg, gemm_impl=piper.GEMM_AUTO, dw_dtype=None):
     return piper.make_desc(cfg.T, cfg.d, cfg.E, cfg.k, cfg.I, e_lo=cfg.e_lo, E_loc=cfg.e_loc, I_shared=cfg.I_shared,
-                           dtype=cfg.dtype, gate_mode=cfg.gate_mode, row_align=cfg.row_align, gemm_impl=gemm_impl)
+                           dtype=cfg.dtype, gate_mode=cfg.gate_mode, row_align=cfg.row_align, gemm_impl=gemm_impl,
+                           dw_dtype=dw_dtype)
 
 
 def to_dev(a: np.ndarray, device="cuda"):

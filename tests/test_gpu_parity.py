@@ -135,6 +135,51 @@ def test_poisoned_buffers_and_untouched_capacity(name):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s"])
+def test_fp32_dw_and_accumulate(name):
+    """Reading c-17: dW accumulated in fp32 over the whole ragged K; with dw_dtype = F32 it is written unrounded, and
+    accumulate = 1 adds it into dW (main-grad style).  Two backward passes over the same microbatch, the second
+    accumulating, must give twice the oracle's dW; empty experts stay exactly zero."""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx = piper.Context(util.desc_of(cfg, dw_dtype=piper.DT_F32))
+    b = piper.alloc_buffers(ctx, backward=True)
+    assert b["dw_gate"].dtype == torch.float32
+    b.update(util.upload_inputs(inp))
+    args = piper.chunk_args(b)
+    piper.piper_run_chunk_fwd(ctx, args)
+    piper.piper_run_chunk_bwd(ctx, args)
+    torch.cuda.synchronize()
+    names = ["dw_gate", "dw_up", "dw_down"] + (["dws_gate", "dws_up", "dws_down"] if cfg.I_shared else [])
+    ref = {n: (g[n] if n.startswith("dw_") else g[n][0]) for n in names}
+    for n in names:
+        util.check_close(n + " fp32", util.to_np(b[n]), ref[n], cfg.dtype)
+    first = {n: b[n].clone() for n in names}
+    piper.piper_set_wgrad_accumulate(ctx, 1)
+    piper.piper_run_chunk_bwd(ctx, args)
+    torch.cuda.synchronize()
+    for n in names:
+        assert torch.equal(b[n], first[n] + first[n]), n + ": accumulate must add the same fp32 sums"
+        util.check_close(n + " accumulated", util.to_np(b[n]), 2.0 * ref[n], cfg.dtype)
+    for i in np.nonzero(f["counts"] == 0)[0]:
+        assert not util.to_np(b["dw_gate"][int(i)]).any()
+    # the step call takes the flag as an argument
+    piper.piper_set_wgrad_accumulate(ctx, 0)
+    piper.piper_expert_ffn_bwd(ctx, b["d_o"], b["xp"], b["g_save"], b["u_save"], b["h_save"], b["offsets"], b["w_gate"],
+                               b["w_up"], b["w_down"], b["dg"], b["du"], b["dxp"], b["dw_gate"], b["dw_up"], b["dw_down"],
+                               accumulate=1)
+    torch.cuda.synchronize()
+    assert torch.equal(b["dw_down"], first["dw_down"] * 3.0)
+    ctx.close()
+    # bf16 dW cannot accumulate
+    ctx2 = piper.Context(util.desc_of(cfg))
+    with pytest.raises(piper.PiperError):
+        piper.piper_set_wgrad_accumulate(ctx2, 1)
+    ctx2.close()
+
+
 @pytest.mark.parametrize("name", ["C1", "C3s", "C4s"])
 def test_chunk_calls_equal_step_calls_bitwise(name):
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128 if name != "C1" else 1)
