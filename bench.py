@@ -195,9 +195,10 @@ def whole_job_tokens_per_s(cfg, world: int, ms_per_step: float) -> float:
 INPUT_NAMES = ("logits", "x", "dy", "w_gate", "w_up", "w_down", "ws_gate", "ws_up", "ws_down")
 
 
-def desc_of(piper, cfg):
+def desc_of(piper, cfg, dw_f32=False):
     return piper.make_desc(cfg.T, cfg.d, cfg.E, cfg.k, cfg.I, e_lo=cfg.e_lo, E_loc=cfg.e_loc, I_shared=cfg.I_shared,
-                           dtype=cfg.dtype, gate_mode=cfg.gate_mode, row_align=cfg.row_align)
+                           dtype=cfg.dtype, gate_mode=cfg.gate_mode, row_align=cfg.row_align,
+                           dw_dtype=piper.DT_F32 if dw_f32 else None)
 
 
 def run_piper(args, cfg):
@@ -227,8 +228,14 @@ def run_piper(args, cfg):
     t0 = time.time()
     inp = configs.make_inputs(rcfg)
     log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
-    ctx = piper.Context(desc_of(piper, rcfg), device=local)
+    ctx = piper.Context(desc_of(piper, rcfg, dw_f32=args.main_grad), device=local)
+    if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
+        piper.piper_set_wgrad_accumulate(ctx, 1)
     b = piper.alloc_buffers(ctx)
+    if getattr(args, "main_grad", False):
+        for n in ("dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down"):
+            if n in b:
+                b[n].zero_()
     b.update({n: piper.to_tensor(inp[n], dev) for n in INPUT_NAMES if n in inp})
     cargs = piper.chunk_args(b)
     stream = torch.cuda.current_stream()
@@ -344,6 +351,8 @@ def run_piper(args, cfg):
             "tflops": configs.flops_fwd_bwd(rcfg, A) / (ms_per_step * 1e-3) / 1e12,
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "kernels": kernels, "gemm_impl": impl}
+    if args.main_grad:
+        line["config"]["dw"] = "fp32, accumulated across steps (accumulate = 1)"
     return line, ctx, b, inp, rcfg
 
 
@@ -434,6 +443,8 @@ def main():
     ap.add_argument("--oracle-tokens", type=int, default=0, help="tokens of the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pair", action="store_true", help="also time step P (chunk pair vs serial) on this shape")
+    ap.add_argument("--main-grad", action="store_true",
+                    help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "piper" else args.warmup
 

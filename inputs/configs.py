@@ -68,7 +68,10 @@ C4S = MoeConfig("C4s", T=1000, d=256, E=16, k=6, I=448, seed=13, bias="zipf1.2",
 C1S = MoeConfig("C1s", T=200, d=72, E=6, k=3, I=88, seed=14, dtype=DT_F32, I_shared=40, e_lo=1, E_loc=4,
                 gate_mode=GATE_SIGMOID_RENORM, bias="normal0.5")
 
-BY_NAME = {c.name: c for c in (C1, C2, C3, C4, C4Z, C5A, C5B, C2S, C3S, C4S, C1S)}
+# d, I, I_shared that are multiples of 8 only (ragged K blocks and feature tiles), experts of ~450 rows (two row chunks)
+C6S = MoeConfig("C6s", T=900, d=328, E=4, k=2, I=296, seed=15, I_shared=200)
+
+BY_NAME = {c.name: c for c in (C1, C2, C3, C4, C4Z, C5A, C5B, C2S, C3S, C4S, C1S, C6S)}
 
 
 def router_bias(cfg: MoeConfig) -> np.ndarray:

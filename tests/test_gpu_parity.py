@@ -15,7 +15,7 @@ import piper_testutil as util
 
 pytestmark = pytest.mark.gpu
 
-SMALL = ["C1", "C1s", "C2s", "C3s", "C4s"]
+SMALL = ["C1", "C1s", "C2s", "C3s", "C4s", "C6s"]
 
 
 def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True):
@@ -106,7 +106,7 @@ def test_small_configs_full_tensor_parity(name, impl, align):
     ctx.close()
 
 
-@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s"])
+@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s", "C6s"])
 def test_poisoned_buffers_and_untouched_capacity(name):
     """No result may depend on what a buffer held before (pad rows are written, never assumed), and no kernel may
     write past the used rows: every output / scratch buffer starts as NaN (0x7FC1 / int 0x7FC17FC1 patterns), the
@@ -135,7 +135,7 @@ def test_poisoned_buffers_and_untouched_capacity(name):
     ctx.close()
 
 
-@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s"])
+@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s", "C6s"])
 def test_fp32_dw_and_accumulate(name):
     """Reading c-17: dW accumulated in fp32 over the whole ragged K; with dw_dtype = F32 it is written unrounded, and
     accumulate = 1 adds it into dW (main-grad style).  Two backward passes over the same microbatch, the second
