@@ -44,6 +44,17 @@ def measured_peaks():
     return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, kind="fallback")
 
 
+def ncu_traffic(config_name: str, task: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the task's kernel from the committed `ncu --set full`
+    capture (profiles/r1c_traffic.json.txt names its source), or None when no capture exists for this workload."""
+    p = os.path.join(ROOT, "profiles", "r1c_traffic.json.txt")
+    try:
+        with open(p) as f:
+            return json.load(f).get(config_name, {}).get(task)
+    except (OSError, ValueError):
+        return None
+
+
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML every 20 ms while the timed region runs."""
@@ -334,7 +345,8 @@ def run_piper(args, cfg):
     roofline = {"bound": "tensor", "kernel": f"{dom} ({impl} grouped GEMM gate|up + SwiGLU epilogue, 1 launch/step)",
                 "achieved": kernels[dom]["achieved"], "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
                 "frac": kernels[dom]["frac"], "frac_of_burst_peak": round(kernels[dom]["achieved"] / peaks["tf_burst"], 4),
-                "frac_of_nominal_2250": round(kernels[dom]["achieved"] / 2250.0, 4), "traffic": None,
+                "frac_of_nominal_2250": round(kernels[dom]["achieved"] / 2250.0, 4),
+                "traffic": ncu_traffic(cfg.name, dom),
                 "peak_kind": f"bf16_tflops_sustained of {peaks['kind']} (kernel timed inside a long step)",
                 "flop_per_launch": work[dom][1], "ms_per_launch": task_ms[dom],
                 "all_gemm": {"tflops": round(gemm_flop / (gemm_ms * 1e-3) / 1e12, 2),
