@@ -282,28 +282,57 @@ def run_piper(args, cfg):
     h2d = sum(t.numel() * t.element_size() for t in host_in.values())
     d2h = sum(t.numel() * t.element_size() for t in host_out.values())
 
-    def e2e_step():
-        for n, t in host_in.items():
-            b[n].copy_(t, non_blocking=True)
-        step()
-        for n, t in host_out.items():
-            t.copy_(b[n], non_blocking=True)
+    # Software pipeline over three streams (what a training loop's data loader does): the inputs of step i+1 go up
+    # and the results of step i-1 come down while step i computes; two sets of input / output device buffers, the
+    # scratch and the weights are shared (the compute stream is serial).  Every step's copies are inside the timed
+    # region.
+    sets = [b, dict(b)]
+    for n in ("logits", "x", "dy") + out_names:
+        sets[1][n] = torch.empty_like(b[n])
+    set_args = [cargs, piper.chunk_args(sets[1])]
+    s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    in_ready = [torch.cuda.Event() for _ in range(2)]
+    comp_done = [torch.cuda.Event() for _ in range(2)]
+    out_done = [torch.cuda.Event() for _ in range(2)]
 
-    for _ in range(min(args.warmup, 3)):
-        e2e_step()
+    def e2e_steps(n_steps):
+        for i in range(n_steps):
+            k = i & 1
+            with torch.cuda.stream(s_in):
+                if i >= 2:
+                    s_in.wait_event(comp_done[k])  # step i-2 has consumed this input set
+                for n, t in host_in.items():
+                    sets[k][n].copy_(t, non_blocking=True)
+                in_ready[k].record(s_in)
+            stream.wait_event(in_ready[k])
+            if i >= 2:
+                stream.wait_event(out_done[k])  # step i-2's results have left this output set
+            piper.piper_run_chunk_fwd(ctx, set_args[k])
+            piper.piper_run_chunk_bwd(ctx, set_args[k])
+            comp_done[k].record(stream)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(comp_done[k])
+                for n, t in host_out.items():
+                    t.copy_(sets[k][n], non_blocking=True)
+                out_done[k].record(s_out)
+        stream.wait_event(out_done[0])
+        stream.wait_event(out_done[1])
+
+    e2e_steps(min(args.warmup, 3))
+    torch.cuda.synchronize(dev)
     barrier()
     w0 = time.perf_counter()
     ev0.record(stream)
-    for _ in range(args.steps):
-        e2e_step()
+    e2e_steps(args.steps)
     ev1.record(stream)
     barrier()
     wall_ms = (time.perf_counter() - w0) * 1e3
     e2e_ms = max_over_ranks(max(ev0.elapsed_time(ev1), wall_ms), world, dev) / args.steps
     e2e = {"value": whole_job_tokens_per_s(cfg, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
-           "what": "pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel -> pinned "
-                   "host; timed as max(CUDA events, host wall clock)"}
+           "what": "every step: pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel "
+                   "-> pinned host, as a 3-stream pipeline (copies of steps i+1 / i-1 overlap the compute of step i); "
+                   "timed as max(CUDA events, host wall clock) over the whole pipeline"}
 
     # ---- per-task device times (CUDA events on the launching stream, inside full steps) ---------------
     tasks = [t for t in piper.TASKS if cfg.I_shared or t not in ("F_SHARED", "B_SHARED")]
