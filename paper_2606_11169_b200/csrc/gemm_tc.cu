@@ -38,6 +38,7 @@ constexpr int kThreads = 256;
 constexpr int kMaxGroups = kMaxE;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/ +
                            (kMaxGroups + 1) * 4 /*tile prefix*/;
+constexpr int kSchedSlots = 32;  // {next tile, clusters done} counter pairs of the dynamically scheduled kernels
 constexpr int kProfSlots = 16, kProfSlotWords = 160 * 8;  // debug counters: 16 launches x 160 CTAs x 8 words
 constexpr int PANEL_M = 8;  // M tiles per panel of the tile order (L2 reuse of the weight tile)
 
@@ -68,6 +69,7 @@ struct alignas(64) TcParams {
     const int32_t* counts;  // [G] device: real rows per group
     int f_tiles;            // tiles along the feature (output column) dimension
     int f_limit;            // output columns
+    int* sched;             // rows-on-N kernel: {next tile, clusters done} counters of this launch (both 0 between launches)
     int out_f32;            // wgrad: dW is fp32 (o[] are fp32 maps, 32-column boxes); accum: add into dW (TMA reduce)
     int accum;
     int greedy;             // chunking: 1 = 256-row chunks and a short last one, 0 = equal chunks
@@ -996,7 +998,8 @@ struct CfgT {
     static constexpr int RING_BYTES = NST * TSTAGE_BYTES, STG_TOTAL = 4 * NBUF * TSTG_BYTES;
     static constexpr int XCH_BYTES = EPI == TEPI_SWIGLU_FWD ? 2 * 2 * 32 * 32 * 4 : 0;  // fp32 U exchange, 2 pairs x 2
     static constexpr int ZERO_BYTES = 16 * 32 * 2;         // a zero block for the pad rows
-    static constexpr int SMEM = RING_BYTES + STG_TOTAL + XCH_BYTES + ZERO_BYTES + 1024 + 256 + (kMaxGroups2 + 1) * 4;
+    static constexpr int SCHED_BYTES = 256;                // tile feed: 8 ids + 2 x 8 mbarriers
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + XCH_BYTES + ZERO_BYTES + SCHED_BYTES + 1024 + 256 + (kMaxGroups2 + 1) * 4;
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 
@@ -1034,6 +1037,31 @@ __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
 }
 
 
+// Tile feed of the rows-on-N kernel: tiles are handed out dynamically (a static stride leaves whole tiles of imbalance
+// when a cluster draws the long chunks, and stalls when a co-scheduled kernel slows one SM).  One thread of the leader
+// CTA draws tile numbers from a global counter and publishes them, in order, in a ring of kFeed slots in both CTAs'
+// shared memory; every consumer warp (producer, MMA issuer, 4 epilogue warps per CTA) reads slot it % kFeed for its
+// it-th tile and releases it to the feeder.  A number >= the tile count ends every loop.  The ring is two deep and the
+// first tile of a cluster is its own index, so the clusters start on neighbouring tiles (shared weight tiles in L2)
+// and every later tile is drawn only when the cluster is about to need it.
+constexpr int kFeed = 2, kFeedConsumers = 2 * 5 + 1;
+struct TileFeed {
+    int* ids;             // [kFeed] this CTA
+    uint64_t* full;       // [kFeed] this CTA
+    uint32_t empty_addr;  // cluster address of the leader's empty barriers [kFeed]
+    __device__ __forceinline__ int peek(int it) const {
+        mbar_wait(&full[it & (kFeed - 1)], (it / kFeed) & 1);
+        return *reinterpret_cast<volatile int*>(&ids[it & (kFeed - 1)]);
+    }
+    // all lanes of a consumer warp call this
+    __device__ __forceinline__ int take(int it, int lane) const {
+        const int t = peek(it);
+        __syncwarp();
+        if (lane == 0 && t >= 0) mbar_arrive_cluster(empty_addr + (it & (kFeed - 1)) * 8);
+        return t;
+    }
+};
+
 template <int A_MAJOR, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemmT_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
@@ -1042,7 +1070,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     uint8_t* stg_base = smem + CfgT<EPI>::RING_BYTES;
     uint8_t* xch_base = stg_base + CfgT<EPI>::STG_TOTAL;
     uint8_t* zero_blk = xch_base + CfgT<EPI>::XCH_BYTES;
-    uint64_t* full_bar = reinterpret_cast<uint64_t*>(zero_blk + CfgT<EPI>::ZERO_BYTES);  // used in the leader CTA
+    uint64_t* feed_full = reinterpret_cast<uint64_t*>(zero_blk + CfgT<EPI>::ZERO_BYTES);  // [kFeed] one set per CTA
+    uint64_t* feed_empty = feed_full + kFeed;                                              // [kFeed] used in the leader CTA
+    int* feed_ids = reinterpret_cast<int*>(feed_empty + kFeed);                            // [kFeed] one set per CTA
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(feed_full) + CfgT<EPI>::SCHED_BYTES);
     uint64_t* empty_bar = full_bar + NST;                                                // one set per CTA
     uint64_t* tfull_bar = empty_bar + NST;                                               // [2] one set per CTA
     uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
@@ -1086,6 +1117,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
+        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers);
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -1095,12 +1127,38 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     const uint32_t tmem_base = *tmem_ptr;
     const int n_total = tq[P.G];
     const int nkb = P.kb_per_src * P.n_src;
+    TileFeed feed;
+    feed.ids = feed_ids, feed.full = feed_full, feed.empty_addr = mapa_u32(smem_u32(feed_empty), 0);
+
+    if (warp == 3 && rank == 0 && lane == 0) {
+        // ===== tile feeder (one thread of the leader CTA) =====
+        const uint32_t peer_ids = mapa_u32(smem_u32(feed_ids), 1), peer_full = mapa_u32(smem_u32(feed_full), 1);
+        for (int it = 0;; ++it) {
+            const int slot = it & (kFeed - 1);
+            mbar_wait(&feed_empty[slot], ((it / kFeed) & 1) ^ 1);
+            const int t = it == 0 ? pair_id : n_pairs_grid + atomicAdd(P.sched, 1);
+            *reinterpret_cast<volatile int*>(&feed_ids[slot]) = t;
+            asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(peer_ids + slot * 4), "r"(t) : "memory");
+            mbar_arrive(&feed_full[slot]);
+            // the peer must see the id before the arrival: cluster-scope release (a membar on this otherwise idle thread)
+            asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(peer_full + slot * 8) : "memory");
+            if (t >= n_total) break;
+        }
+        // the last cluster to finish re-arms the counters for the next launch that uses this slot
+        __threadfence();
+        if (atomicAdd(P.sched + 1, 1) == n_pairs_grid - 1) {
+            __threadfence();
+            P.sched[0] = 0, P.sched[1] = 0;
+        }
+    }
 
     if (warp == 0) {
         // ===== TMA producer (both CTAs): own 128 features of the weights + own half of the rows =====
         const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
         int stage = 0, phase = 0;
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        for (int it = 0;; ++it) {
+            const int t = feed.take(it, lane);
+            if (t >= n_total) break;
             const TileT T = decode_t(P, tq, offsets, counts, t);
             const int nb = T.n >> 1, rb = T.r0 + rank * nb;
             const bool small = nb <= P.small_rows;
@@ -1143,7 +1201,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
         int stage = 0, phase = 0, as = 0, aphase = 0;
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        for (int it = 0;; ++it) {
+            const int t = feed.take(it, lane);
+            if (t >= n_total) break;
             const TileT T = decode_t(P, tq, offsets, counts, t);
             const uint32_t idesc = make_idesc_t(A_MAJOR, T.n);
             if (lane == 0) {
@@ -1212,11 +1272,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         auto feat_col = [&](const TileT& T) {
             return EPI == TEPI_SWIGLU_FWD ? T.f * 128 + rank * 64 + 32 * pr : T.f * 256 + rank * 128 + 32 * wq;
         };
-        if (EPI == TEPI_SWIGLU_BWD && pair_id < n_total) {
-            const TileT T0 = decode_t(P, tq, offsets, counts, pair_id);
-            load_inputs(feat_col(T0), T0.r0, 0);
+        if (EPI == TEPI_SWIGLU_BWD) {
+            const int t0 = feed.peek(0);
+            if (t0 < n_total) {
+                const TileT T0 = decode_t(P, tq, offsets, counts, t0);
+                load_inputs(feat_col(T0), T0.r0, 0);
+            }
         }
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        for (int it = 0;; ++it) {
+            const int t = feed.take(it, lane);
+            if (t >= n_total) break;
             const TileT T = decode_t(P, tq, offsets, counts, t);
             mbar_wait(&tfull_bar[as], aphase);
             tc_fence_after();
@@ -1289,9 +1354,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
                     if (j + 32 < T.n) {
                         load_inputs(fcol, T.r0 + j + 32, set ^ 1);
-                    } else if (t + n_pairs_grid < n_total) {
-                        const TileT Tn = decode_t(P, tq, offsets, counts, t + n_pairs_grid);
-                        load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
+                    } else {
+                        const int tn = feed.peek(it + 1);
+                        if (tn < n_total) {
+                            const TileT Tn = decode_t(P, tq, offsets, counts, tn);
+                            load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
+                        }
                     }
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
@@ -1475,7 +1543,9 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
     long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI>, CfgT<EPI>::SMEM);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
-    tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(P);
+    TcParams Q = P;  // tile counters of this launch: one of kSchedSlots pairs, cycled (kernels in flight never share one)
+    Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
+    tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
 }
@@ -1521,7 +1591,7 @@ inline long long m_tile_bound(const FfnProblem& p, bool two) {
 
 }  // namespace
 
-size_t tc_scratch_bytes(const piper_moe_desc*) { return (size_t)kProfSlots * kProfSlotWords * 8; }
+size_t tc_scratch_bytes(const piper_moe_desc*) { return (size_t)kProfSlots * kProfSlotWords * 8 + kSchedSlots * 8; }
 
 int tc_init(piper_ctx* c) {
     void* fn = nullptr;
@@ -1531,6 +1601,7 @@ int tc_init(piper_ctx* c) {
         fn = nullptr;
     cudaGetLastError();
     c->encode_tiled = fn;
+    if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     const char* pe = getenv("PIPER_TC_PROFILE");
     c->tc_prof = pe && pe[0] == '1';
     const char* pt = getenv("PIPER_TC_ROWS_ON_N");

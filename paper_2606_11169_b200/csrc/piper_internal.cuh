@@ -52,6 +52,7 @@ struct piper_ctx {
     void* encode_tiled;      // cuTensorMapEncodeTiled, resolved at create time
     piper::GreenPartition* green;
     char* tc_scratch;        // tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
+    int tc_sched_slot;       // round-robin tile-counter pair in tc_scratch
     int tc_next_slot;        // round-robin slot in tc_scratch
     int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
     int tc2_max_clusters;    // co-resident CTA pairs
