@@ -106,6 +106,50 @@ def test_small_configs_full_tensor_parity(name, impl, align):
     ctx.close()
 
 
+def _random_config(i):
+    """Seeded random layer shapes: every dimension a multiple of 8 only, experts from empty to several row chunks,
+    local slices, shared expert or not, all three gate modes."""
+    rng = np.random.default_rng(1000 + i)
+    E = int(rng.choice([2, 5, 8, 24]))
+    k = int(rng.integers(1, min(E, 6) + 1))
+    e_loc = int(rng.integers(1, E + 1))
+    e_lo = int(rng.integers(0, E - e_loc + 1))
+    return configs.MoeConfig(f"R{i}", T=int(rng.integers(1, 1400)), d=8 * int(rng.integers(8, 70)), E=E, k=k,
+                             I=8 * int(rng.integers(8, 70)), seed=2000 + i, e_lo=e_lo, E_loc=e_loc,
+                             I_shared=int(rng.choice([0, 8 * int(rng.integers(8, 40))])),
+                             gate_mode=int(rng.integers(0, 3)), bias=str(rng.choice(["none", "normal0.5", "zipf1.2"])),
+                             n_dead=int(rng.integers(0, 2)) if E > k + 1 else 0, row_align=128)
+
+
+@pytest.mark.parametrize("i", range(8))
+def test_random_shapes_full_tensor_parity(i):
+    cfg = _random_config(i)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True)
+    _check_all(cfg, b, f, g, label=f"{cfg} ")
+    assert piper.piper_gemm_path(ctx) == 1
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
+@pytest.mark.parametrize("env", [{"PIPER_TC_ROWS_ON_N": "0"}, {"PIPER_TC_ROWS_ON_N": "0", "PIPER_TC_2CTA": "0"}])
+def test_fallback_kernel_families(name, env, monkeypatch):
+    """The rows-on-M CTA-pair kernels and the 1-CTA kernels (DESIGN.md section 5.1 b, c) stay correct: they serve
+    layers with more than 192 local experts.  The switches are read when a context is created."""
+    for k_, v_ in env.items():
+        monkeypatch.setenv(k_, v_)
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True)
+    _check_all(cfg, b, f, g)
+    assert piper.piper_gemm_path(ctx) == 1
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["C2s", "C3s", "C4s", "C6s"])
 def test_poisoned_buffers_and_untouched_capacity(name):
     """No result may depend on what a buffer held before (pad rows are written, never assumed), and no kernel may
