@@ -44,6 +44,16 @@ def measured_peaks():
     return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, kind="fallback")
 
 
+def ncu_mover_us(config_name: str):
+    """Per-launch gpu__time_duration of the row movers from the committed ncu launch lists (a CUDA-event pair around one
+    ~20 us launch also counts ~6 us of launch latency), or {}."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1c_traffic.json.txt")) as f:
+            return json.load(f).get("ncu_us", {}).get(config_name, {})
+    except (OSError, ValueError):
+        return {}
+
+
 def ncu_traffic(config_name: str, task: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the task's kernel from the committed `ncu --set full`
     capture (profiles/r1c_traffic.json.txt names its source), or None when no capture exists for this workload."""
@@ -366,6 +376,10 @@ def run_piper(args, cfg):
             ach, peak, unit = amount / sec / 1e9, peaks["hbm"], "GB/s"
         kernels[t] = {"ms": round(task_ms[t], 4), "bound": bound, "achieved": round(ach, 2), "unit": unit,
                       "frac": round(ach / peak, 4)}
+        us = ncu_mover_us(cfg.name).get(t)
+        if us:  # the same algorithmic bytes over the kernel's own duration from the committed ncu launch list
+            kernels[t]["ncu_us"] = us
+            kernels[t]["ncu_frac"] = round(amount / (us * 1e-6) / 1e9 / peak, 4)
     gemm_tasks = [t for t in order if work[t][0] == "tensor"]
     gemm_ms = sum(task_ms[t] for t in gemm_tasks)
     gemm_flop = sum(work[t][1] for t in gemm_tasks)

@@ -8,7 +8,16 @@
 namespace piper {
 namespace {
 
-constexpr int kMoveWarps = 8;  // warps per block of the row movers
+#ifndef PIPER_MOVE_WARPS
+#define PIPER_MOVE_WARPS 8
+#endif
+#ifndef PIPER_MOVE_U
+#define PIPER_MOVE_U 4
+#endif
+#ifndef PIPER_MOVE_CAP
+#define PIPER_MOVE_CAP 16
+#endif
+constexpr int kMoveWarps = PIPER_MOVE_WARPS;  // warps per block of the row movers
 
 // ---- F2 phase 1: per-chunk histogram of local experts ------------------------------------------
 __global__ void __launch_bounds__(kScanChunk)
@@ -157,7 +166,7 @@ __device__ __forceinline__ float dot_packets(const int4& a, const int4& b) {
 // Splitting a row over several items keeps every resident warp busy when T is small (no cross-split
 // reduction exists in pack / combine / unpack; combine_bwd's dot products need the whole row and do not
 // split).  No per-thread arrays indexed at run time: row indices are re-read from row_of (L1 hits).
-constexpr int U = 4;                 // packets per lane per step
+constexpr int U = PIPER_MOVE_U;       // packets per lane per step
 constexpr int kStep = 32 * U;        // packets per warp per step
 
 __device__ __forceinline__ void load_step(int4 (&v)[U], const int4* __restrict__ src, int p0, int lane, int hi) {
@@ -349,7 +358,7 @@ inline void choose_split(Lane ln, int T, int row_packets, int& S, int& split_pac
 template <typename K>
 inline int mover_blocks(Lane ln, int items, K) {
     int blocks = cdiv(items, kMoveWarps);
-    const int cap = ln.sms * 16;
+    const int cap = ln.sms * PIPER_MOVE_CAP;
     return blocks < cap ? (blocks < 1 ? 1 : blocks) : cap;
 }
 
