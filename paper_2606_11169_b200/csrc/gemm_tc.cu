@@ -636,6 +636,31 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
 }
 
+// Tile feed of the CTA-pair kernels: tiles are handed out dynamically (a static stride leaves whole tiles of imbalance
+// when a cluster draws the long chunks, and stalls when a co-scheduled kernel slows one SM).  One thread of the leader
+// CTA draws tile numbers from a global counter and publishes them, in order, in a ring of kFeed slots in both CTAs'
+// shared memory; every consumer warp (producer, MMA issuer, 4 epilogue warps per CTA) reads slot it % kFeed for its
+// it-th tile and releases it to the feeder.  A number >= the tile count ends every loop.  The ring is two deep and the
+// first tile of a cluster is its own index, so the clusters start on neighbouring tiles (shared weight tiles in L2)
+// and every later tile is drawn only when the cluster is about to need it.
+constexpr int kFeed = 2, kFeedConsumers = 2 * 5 + 1;
+struct TileFeed {
+    int* ids;             // [kFeed] this CTA
+    uint64_t* full;       // [kFeed] this CTA
+    uint32_t empty_addr;  // cluster address of the leader's empty barriers [kFeed]
+    __device__ __forceinline__ int peek(int it) const {
+        mbar_wait(&full[it & (kFeed - 1)], (it / kFeed) & 1);
+        return *reinterpret_cast<volatile int*>(&ids[it & (kFeed - 1)]);
+    }
+    // all lanes of a consumer warp call this
+    __device__ __forceinline__ int take(int it, int lane) const {
+        const int t = peek(it);
+        __syncwarp();
+        if (lane == 0 && t >= 0) mbar_arrive_cluster(empty_addr + (it & (kFeed - 1)) * 8);
+        return t;
+    }
+};
+
 template <int A_MAJOR, int B_MAJOR, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
@@ -649,6 +674,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
     uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets] epilogue inputs
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
+    uint64_t* feed_full = ld_bar + 9;         // [kFeed] one set per CTA
+    uint64_t* feed_empty = feed_full + kFeed;  // [kFeed] used in the leader CTA
+    int* feed_ids = reinterpret_cast<int*>(feed_empty + kFeed);
     int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);
     int* tpp = tp + (kMaxGroups2 + 1);
 
@@ -686,6 +714,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         for (int s = 0; s < STAGES2; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
+        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers);
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -694,13 +723,49 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
     const int n_total = total_pairs(P, tpp);
+    TileFeed feed;
+    feed.ids = feed_ids, feed.full = feed_full, feed.empty_addr = mapa_u32(smem_u32(feed_empty), 0);
+
+    // wgrad: draw tiles from the counter only when the experts' K ranges are long and uneven (C4: one expert holds 16% of
+    // the rows, so a static stride leaves some clusters two of its tiles); equal or short tiles keep the static stride
+    // (the draw costs an atomic and a cluster-scope release per tile: -2% on C2, -7% on C3's 2-3 K-block tiles).
+    bool dynamic = true;  // computed by every warp (same data, same answer): static tiles bypass the feed altogether
+    if (!P.ragged_m) {
+        int mx = 0;
+        for (int g = lane; g < P.G; g += 32) mx = max(mx, offsets[g + 1] - offsets[g]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        const int total = offsets[P.G];
+        dynamic = total >= 512 * P.G && (long long)mx * P.G > 2ll * total;
+    }
+    if (dynamic && warp == 3 && rank == 0 && lane == 0) {
+        // ===== tile feeder (one thread of the leader CTA), see TileFeed =====
+        const uint32_t peer_ids = mapa_u32(smem_u32(feed_ids), 1), peer_full = mapa_u32(smem_u32(feed_full), 1);
+        for (int it = 0;; ++it) {
+            const int slot = it & (kFeed - 1);
+            mbar_wait(&feed_empty[slot], ((it / kFeed) & 1) ^ 1);
+            const int t = it == 0 ? pair_id : n_pairs_grid + atomicAdd(P.sched, 1);
+            *reinterpret_cast<volatile int*>(&feed_ids[slot]) = t;
+            asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(peer_ids + slot * 4), "r"(t) : "memory");
+            mbar_arrive(&feed_full[slot]);
+            asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(peer_full + slot * 8) : "memory");
+            if (t >= n_total) break;
+        }
+        __threadfence();
+        if (atomicAdd(P.sched + 1, 1) == n_pairs_grid - 1) {
+            __threadfence();
+            P.sched[0] = 0, P.sched[1] = 0;
+        }
+    }
 
     if (warp == 0) {
         // ===== TMA producer (both CTAs): own A tile + own 128-column half of B, counted on the leader's barrier =====
         const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
         int stage = 0, phase = 0;
         long long w_empty = 0;
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        for (int it = 0;; ++it) {
+            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
@@ -745,7 +810,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         int stage = 0, phase = 0, as = 0, aphase = 0;
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        for (int it = 0;; ++it) {
+            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc);
             if (lane == 0) {
                 const long long c0 = P.prof ? clock64() : 0;
@@ -800,8 +867,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 tma_load_3d(stg + (2 * set + 1) * STG_BYTES, &P.ein[1], bar, Tn.n0 + 64 * c, Tn.m0 + wq * 32, 0);
             }
         };
-        if (EPI == EPI_SWIGLU_BWD && pair_id < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, pair_id, rank, BKc), 0, 0);
-        for (int t = pair_id; t < n_total; t += n_pairs_grid) {
+        if (EPI == EPI_SWIGLU_BWD) {
+            const int t0 = dynamic ? feed.peek(0) : pair_id;
+            if (t0 < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, t0, rank, BKc), 0, 0);
+        }
+        for (int it = 0;; ++it) {
+            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
             const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
@@ -857,8 +929,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (P.prof) w_stg += clock64() - c1;
                     if (c < 3) {
                         load_inputs(T, c + 1, set ^ 1);
-                    } else if (t + n_pairs_grid < n_total) {
-                        load_inputs(decode_pair(P, tp, tpp, offsets, t + n_pairs_grid, rank, BKc), 0, set ^ 1);
+                    } else {
+                        const int tn = dynamic ? feed.peek(it + 1) : t + n_pairs_grid;
+                        if (tn < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, tn, rank, BKc), 0, set ^ 1);
                     }
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -1036,31 +1109,6 @@ __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)((2 * BM) >> 4) << 24);
 }
 
-
-// Tile feed of the rows-on-N kernel: tiles are handed out dynamically (a static stride leaves whole tiles of imbalance
-// when a cluster draws the long chunks, and stalls when a co-scheduled kernel slows one SM).  One thread of the leader
-// CTA draws tile numbers from a global counter and publishes them, in order, in a ring of kFeed slots in both CTAs'
-// shared memory; every consumer warp (producer, MMA issuer, 4 epilogue warps per CTA) reads slot it % kFeed for its
-// it-th tile and releases it to the feeder.  A number >= the tile count ends every loop.  The ring is two deep and the
-// first tile of a cluster is its own index, so the clusters start on neighbouring tiles (shared weight tiles in L2)
-// and every later tile is drawn only when the cluster is about to need it.
-constexpr int kFeed = 2, kFeedConsumers = 2 * 5 + 1;
-struct TileFeed {
-    int* ids;             // [kFeed] this CTA
-    uint64_t* full;       // [kFeed] this CTA
-    uint32_t empty_addr;  // cluster address of the leader's empty barriers [kFeed]
-    __device__ __forceinline__ int peek(int it) const {
-        mbar_wait(&full[it & (kFeed - 1)], (it / kFeed) & 1);
-        return *reinterpret_cast<volatile int*>(&ids[it & (kFeed - 1)]);
-    }
-    // all lanes of a consumer warp call this
-    __device__ __forceinline__ int take(int it, int lane) const {
-        const int t = peek(it);
-        __syncwarp();
-        if (lane == 0 && t >= 0) mbar_arrive_cluster(empty_addr + (it & (kFeed - 1)) * 8);
-        return t;
-    }
-};
 
 template <int A_MAJOR, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemmT_kernel(const __grid_constant__ TcParams P) {
@@ -1519,6 +1567,7 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
         long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
+        Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
         tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
