@@ -814,6 +814,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
             if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc);
+            // wgrad: the K range ends with the expert's zero pad rows; K slices (16 rows) that hold only pad rows are
+            // not issued (C2: 640 of 8832 rows, 7% of the tensor work)
+            const int k_valid = (!P.ragged_m && P.counts) ? P.counts[T.g] : 0x3fffffff;
             if (lane == 0) {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
@@ -829,8 +832,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
+                    const int kk_end = (k_valid - kb * BKc + UK - 1) / UK;  // >= 1 in block 0 of a non-empty expert
 #pragma unroll
                     for (int kk = 0; kk < BKc / UK; ++kk) {
+                        if (kk >= kk_end) break;
                         const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
                         const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
                         umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
@@ -1204,6 +1209,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         // ===== TMA producer (both CTAs): own 128 features of the weights + own half of the rows =====
         const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
         int stage = 0, phase = 0;
+        long long w_empty = 0;
         for (int it = 0;; ++it) {
             const int t = feed.take(it, lane);
             if (t >= n_total) break;
@@ -1214,7 +1220,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             const int box_bytes = (small ? TB_SMALL_ROWS : TB_BOX_ROWS) * BK * 2;
             for (int kb = 0; kb < nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
+                    if (P.prof) w_empty += clock64() - c0;
                     uint8_t* sa = smem + stage * TSTAGE_BYTES;
                     uint8_t* sb = sa + TA_BYTES;
                     if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * (TA_BYTES + nbox * box_bytes));
@@ -1244,25 +1252,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 if (++stage == NST) stage = 0, phase ^= 1;
             }
         }
+        if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1 && rank == 0) {
         // ===== MMA issuer (one thread of the leader CTA): D^T[256 features, n rows] += W-tile * rows^T =====
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
         int stage = 0, phase = 0, as = 0, aphase = 0;
+        long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
+        const long long t_begin = P.prof ? clock64() : 0;
         for (int it = 0;; ++it) {
             const int t = feed.take(it, lane);
             if (t >= n_total) break;
             const TileT T = decode_t(P, tq, offsets, counts, t);
             const uint32_t idesc = make_idesc_t(A_MAJOR, T.n);
             if (lane == 0) {
+                const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
+                if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
             __syncwarp();
             const uint32_t d_tmem = tmem_base + as * BN;
             for (int kb = 0; kb < nkb; ++kb) {
                 if (lane == 0) {
+                    const long long c0 = P.prof ? clock64() : 0;
                     mbar_wait(&full_bar[stage], phase);
+                    if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * TSTAGE_BYTES), sb = sa + TA_BYTES;
 #pragma unroll
@@ -1280,12 +1295,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
+        if (P.prof && lane == 0) {
+            long long* pq = P.prof + blockIdx.x * 8;
+            pq[0] = w_full, pq[1] = w_tempty, pq[2] = clock64() - t_begin, pq[6] = n_tiles_done;
+        }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): TMEM lane = feature, column = row; transposed through shared memory =====
         const int wq = warp & 3;
         const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
         uint8_t* stg = stg_base + wq * NBUF * TSTG_BYTES;
         int as = 0, aphase = 0, ring = 0;
+        long long w_tfull = 0, w_stg = 0;
+        const long long t_begin = P.prof ? clock64() : 0;
         uint32_t q = 0;  // running 32-row block number (SwiGLU epilogues: exchange slot / input set q & 1)
         // one staged block [32 rows][32 features] -> out rows row.. (the second 16-row half only if `both`)
         auto store_block = [&](const CUtensorMap* om, const uint8_t* buf, int fcol, int row, bool both) {
@@ -1331,7 +1352,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             const int t = feed.take(it, lane);
             if (t >= n_total) break;
             const TileT T = decode_t(P, tq, offsets, counts, t);
+            const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
+            if (P.prof) w_tfull += clock64() - c0;
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
             const int fcol = feat_col(T);
@@ -1399,7 +1422,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     // accumulator = dH; dG = dH * U * silu'(G), dU = dH * silu(G), in place over the staged G, U
                     const int set = q & 1;
                     const uint32_t bg = smem_u32(stg + (2 * set) * TSTG_BYTES) + lane * 2, bu = bg + TSTG_BYTES;
+                    const long long c1 = P.prof ? clock64() : 0;
                     mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
+                    if (P.prof) w_stg += clock64() - c1;
                     if (j + 32 < T.n) {
                         load_inputs(fcol, T.r0 + j + 32, set ^ 1);
                     } else {
@@ -1460,6 +1485,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             }
         }
         if (lane == 0) bulk_wait_all();
+        if (P.prof && threadIdx.x == 128) {
+            long long* pq = P.prof + blockIdx.x * 8;
+            pq[4] = w_tfull, pq[5] = clock64() - t_begin, pq[7] = w_stg;
+        }
     }
     tc_fence_before();
     cluster_sync_all();
@@ -1593,6 +1622,10 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
     TcParams Q = P;  // tile counters of this launch: one of kSchedSlots pairs, cycled (kernels in flight never share one)
+    if (c->tc_prof) {  // debug: slot per launch, cycled
+        Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
+        c->tc_next_slot += 1;
+    }
     Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
     tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
@@ -1788,6 +1821,7 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     if ((f32 || p.accumulate) && !(two && f32)) return PIPER_ERR_UNSUPPORTED;
     {
         TcParams P = base_params(p, false);
+        P.counts = p.counts;
         const int kbox = two ? Cfg2<EPI_WGRAD_SPLIT>::BKc : BK;
         PIPER_MAP(&P.a[0], p.xp, p.d, p.max_rows, 1, kbox);
         PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, kbox);
@@ -1810,6 +1844,7 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         if (rc != PIPER_OK) return rc;
     }
     TcParams P = base_params(p, false);
+    P.counts = p.counts;
     const int kbox = two ? Cfg2<EPI_WGRAD>::BKc : BK;
     PIPER_MAP(&P.a[0], p.h, p.I, p.max_rows, 1, kbox);
     PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, kbox);
