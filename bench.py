@@ -480,6 +480,9 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     out["variants"]["list_order_shared_sms"] = sweep(shared_splits)
     piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE, piper.PART_SHARED, task_ms)
     out["variants"]["profile_order_shared_sms"] = sweep(shared_splits)
+    # the paper's own setting: one stream per chunk, SM allocation left to the GPU
+    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_CHUNK_STREAMS, task_ms)
+    out["variants"]["chunk_streams_gpu_allocates_sms"] = sweep([(n_sm, 16)])
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
     best = min(((v["ratio_vs_serial"], name, k) for name, d in
                 [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))

@@ -195,9 +195,15 @@ int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const p
  *                                  sides may overlap (sm_gemm + sm_comm may exceed the SM count): pack/combine CTAs
  *                                  become co-resident with the persistent GEMM CTAs, as in the paper, which leaves SM
  *                                  allocation to the GPU.
+ *            PIPER_PART_CHUNK_STREAMS  one plain stream per chunk (forward chunk / backward chunk, each in its serial
+ *                                  task order, `order` and the SM counts are not used), every grid sized for the whole
+ *                                  device: SM allocation is left entirely to the GPU.  The chunks'
+ *                                  GEMM kernels follow one another SM by SM as clusters retire and the row movers
+ *                                  run beside them.
  * Either way the results stay bit-identical to the serial chunks.  Returns PIPER_ERR_INVALID on unknown values. */
 #define PIPER_ORDER_LIST 0
 #define PIPER_ORDER_PROFILE 1
+#define PIPER_PART_CHUNK_STREAMS 2
 #define PIPER_PART_EXCLUSIVE 0
 #define PIPER_PART_SHARED 1
 int piper_set_pair_policy(piper_ctx* ctx, int order, int partition, const float* task_ms);
@@ -227,7 +233,8 @@ int piper_run_task(piper_ctx* ctx, int task, const piper_chunk_args* a, void* st
 int piper_set_wgrad_accumulate(piper_ctx* ctx, int accumulate);
 
 /* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
- * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 0 = never called. */
+ * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 3 = one stream per chunk
+ * (PIPER_PART_CHUNK_STREAMS), 0 = never called. */
 int piper_pair_partition_mode(const piper_ctx* ctx);
 
 /* Host-only list scheduler used by piper_run_chunk_pair (reading c-21),

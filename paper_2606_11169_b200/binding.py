@@ -228,7 +228,7 @@ def piper_run_chunk_pair(ctx, fwd_args: ChunkArgs, bwd_args: ChunkArgs, sm_gemm:
 
 
 ORDER_LIST, ORDER_PROFILE = 0, 1
-PART_EXCLUSIVE, PART_SHARED = 0, 1
+PART_EXCLUSIVE, PART_SHARED, PART_CHUNK_STREAMS = 0, 1, 2
 
 
 def piper_set_pair_policy(ctx, order: int, partition: int, task_ms=None):

@@ -306,14 +306,14 @@ int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
 
 bool split_ok(const piper_ctx* c, int sm_gemm, int sm_comm) {
     if (sm_gemm < 1 || sm_comm < 8 || sm_comm % 8 || sm_gemm > c->num_sms || sm_comm > c->num_sms) return false;
-    return c->pair_part == PIPER_PART_SHARED || sm_gemm + sm_comm <= c->num_sms;
+    return c->pair_part != PIPER_PART_EXCLUSIVE || sm_gemm + sm_comm <= c->num_sms;
 }
 
 }  // namespace
 
 int piper_set_pair_policy(piper_ctx* c, int order, int partition, const float* task_ms) {
     if (!c || (order != PIPER_ORDER_LIST && order != PIPER_ORDER_PROFILE) ||
-        (partition != PIPER_PART_EXCLUSIVE && partition != PIPER_PART_SHARED))
+        (partition != PIPER_PART_EXCLUSIVE && partition != PIPER_PART_SHARED && partition != PIPER_PART_CHUNK_STREAMS))
         return PIPER_ERR_INVALID;
     if (task_ms)
         for (int t = 0; t < N_TASKS; ++t)
@@ -346,12 +346,41 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
         if (!c->green) return cuda_fail(c, cudaErrorUnknown, "make_partition");
     }
     GreenPartition* g = c->green;
-    c->pair_mode = g->green ? 1 : 2;
+    c->pair_mode = c->pair_part == PIPER_PART_CHUNK_STREAMS ? 3 : (g->green ? 1 : 2);
     PairPlan pl;
     int rc = make_plan(c, sm_gemm, sm_comm, &pl);
     if (rc != PIPER_OK) return rc;
 
     cudaStream_t user = static_cast<cudaStream_t>(stream);
+    if (c->pair_part == PIPER_PART_CHUNK_STREAMS) {
+        // One stream per chunk, every grid sized for the whole device, no cross-stream edge (the two microbatches are
+        // independent): which SM runs what is left to the GPU's block scheduler, as in the paper.  The
+        // persistent GEMM grids of the two chunks cannot be co-resident (one CTA fills an SM's shared memory), so a
+        // chunk's next GEMM moves in SM by SM as the other's clusters retire (the tile feeds are dynamic or strided:
+        // no kernel waits on a CTA that is not resident), and the row movers run beside whichever GEMM is resident.
+        const Lane lf{g->stream[0], c->num_sms}, lb{g->stream[1], c->num_sms};
+        cudaEvent_t fork = c->events[kMaxEvents - 1], join0 = c->events[kMaxEvents - 2], join1 = c->events[kMaxEvents - 3];
+        PIPER_CUDA(c, cudaEventRecord(fork, user));
+        PIPER_CUDA(c, cudaStreamWaitEvent(lf.stream, fork, 0));
+        PIPER_CUDA(c, cudaStreamWaitEvent(lb.stream, fork, 0));
+        const int fseq[] = {F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE};
+        const int bseq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+        for (int i = 0; i < 7; ++i) {  // enqueued alternately, each chunk in its serial order
+            if (fseq[i] != F_SHARED || c->D.I_shared) {
+                rc = run_task(c, fseq[i], lf, f, b);
+                if (rc != PIPER_OK) return rc;
+            }
+            if (bseq[i] != B_SHARED || c->D.I_shared) {
+                rc = run_task(c, bseq[i], lb, f, b);
+                if (rc != PIPER_OK) return rc;
+            }
+        }
+        PIPER_CUDA(c, cudaEventRecord(join0, lf.stream));
+        PIPER_CUDA(c, cudaEventRecord(join1, lb.stream));
+        PIPER_CUDA(c, cudaStreamWaitEvent(user, join0, 0));
+        PIPER_CUDA(c, cudaStreamWaitEvent(user, join1, 0));
+        return PIPER_OK;
+    }
     const Lane lanes[2] = {{g->stream[COMM], sm_comm}, {g->stream[GEMM], sm_gemm}};
     // fork: both partitions start after the work already queued on the caller's stream
     cudaEvent_t fork = c->events[kMaxEvents - 1], join0 = c->events[kMaxEvents - 2], join1 = c->events[kMaxEvents - 3];

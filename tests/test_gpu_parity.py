@@ -242,7 +242,7 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
 @pytest.mark.parametrize("split,policy", [((132, 16), "list/exclusive"), ((100, 48), "list/exclusive"),
                                           ((116, 32), "profile/exclusive"), ((148, 16), "list/shared"),
-                                          ((148, 48), "profile/shared")])
+                                          ((148, 48), "profile/shared"), ((148, 16), "list/chunks")])
 def test_pair_is_bitwise_equal_to_serial(name, split, policy):
     """the overlapped, out-of-order plan must respect every dependency -> identical results,
     for the paper's list order and the profile-guided one, on disjoint and on shared SM partitions."""
@@ -260,15 +260,15 @@ def test_pair_is_bitwise_equal_to_serial(name, split, policy):
     piper.piper_run_chunk_fwd(ctx, args_b)
     order, part = policy.split("/")
     piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE if order == "profile" else piper.ORDER_LIST,
-                                piper.PART_SHARED if part == "shared" else piper.PART_EXCLUSIVE)
+                                {"shared": piper.PART_SHARED, "chunks": piper.PART_CHUNK_STREAMS}.get(part, piper.PART_EXCLUSIVE))
     n_sm = torch.cuda.get_device_properties(0).multi_processor_count
-    sg = min(split[0], n_sm) if part == "shared" else min(split[0], n_sm - split[1])
+    sg = min(split[0], n_sm) if part != "exclusive" else min(split[0], n_sm - split[1])
     picked = piper.piper_pair_order(ctx, sg, split[1])
     assert sorted(picked) == sorted(t for t in piper.TASKS if base.I_shared or t not in ("F_SHARED", "B_SHARED"))
     piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, split[1])
     torch.cuda.synchronize()
-    assert piper.piper_pair_partition_mode(ctx) == (2 if part == "shared" else piper.piper_pair_partition_mode(ctx))
-    assert piper.piper_pair_partition_mode(ctx) in (1, 2)
+    mode = piper.piper_pair_partition_mode(ctx)
+    assert mode == {"shared": 2, "chunks": 3}.get(part, mode) and mode in (1, 2, 3)
     if part == "exclusive":  # sm_gemm + sm_comm beyond the device is refused on disjoint partitions
         with pytest.raises(piper.PiperError):
             piper.piper_run_chunk_pair(ctx, args_a, args_b, n_sm, 16)
