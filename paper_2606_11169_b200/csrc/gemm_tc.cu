@@ -526,6 +526,9 @@ __device__ __forceinline__ void stage32(uint8_t* buf, int r, int half, const flo
 #ifndef PIPER_WGRAD_BK
 #define PIPER_WGRAD_BK 128
 #endif
+#ifndef PIPER_WGRAD_EPI_WARPS
+#define PIPER_WGRAD_EPI_WARPS 4
+#endif
 // Ring depth and staging buffers per epilogue warp: the SwiGLU backward epilogue also stages its G, U inputs.
 constexpr int kMaxGroups2 = 192;  // groups the CTA-pair kernel can index (its tile-prefix arrays share the 227 KB)
 template <int EPI>
@@ -535,9 +538,14 @@ struct Cfg2 {
     static constexpr bool WG = EPI == EPI_WGRAD || EPI == EPI_WGRAD_SPLIT;
     static constexpr int BKc = WG ? PIPER_WGRAD_BK : BK;
     static constexpr int NST = BKc == 128 ? 3 : 5;
-    static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : (BKc == 128 ? 2 : 3);
+    // wgrad: PIPER_WGRAD_EPI_WARPS = 8 gives two epilogue warps per TMEM lane quarter (each half of the tile's columns,
+    // one staging buffer each).  Measured: C3 wgrad (2-3 K blocks per tile) 0.840 -> 0.824 ms, C2 2.10 -> 2.13 ms, so
+    // the epilogue's dependent chain is not what bounds the short-K tiles; default 4.
+    static constexpr int EPI_WARPS = WG ? PIPER_WGRAD_EPI_WARPS : 4;
+    static constexpr int THREADS = 128 + 32 * EPI_WARPS;
+    static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : (BKc == 128 ? (EPI_WARPS == 8 ? 1 : 2) : 3);
     static constexpr int A_B = BM * BKc * 2, B_B = (BN / 2) * BKc * 2, STAGE_B = A_B + B_B, MNB = 64 * BKc * 2;
-    static constexpr int RING_BYTES = NST * STAGE_B, STG_TOTAL = 4 * NBUF * STG_BYTES;
+    static constexpr int RING_BYTES = NST * STAGE_B, STG_TOTAL = EPI_WARPS * NBUF * STG_BYTES;
     static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups2 + 1) * 4;
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
@@ -662,7 +670,7 @@ struct TileFeed {
 };
 
 template <int A_MAJOR, int B_MAJOR, int EPI>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     constexpr int STAGES2 = Cfg2<EPI>::NST, NBUF = Cfg2<EPI>::NBUF, BKc = Cfg2<EPI>::BKc, MNB = Cfg2<EPI>::MNB;
@@ -686,7 +694,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     const int32_t* __restrict__ offsets = P.offsets;
 
     if (P.ragged_m) {
-        for (int g = threadIdx.x; g <= P.G; g += kThreads) tp[g] = (offsets[g] + BM - 1) / BM;
+        for (int g = threadIdx.x; g <= P.G; g += Cfg2<EPI>::THREADS) tp[g] = (offsets[g] + BM - 1) / BM;
         __syncthreads();
         if (warp == 3) {  // exclusive scan of the tile pairs per group
             int carry = 0;
@@ -712,9 +720,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES2; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
-        for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
+        for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 2 * Cfg2<EPI>::EPI_WARPS);  // both CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
-        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers);
+        for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1);
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -855,9 +864,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
-        const int wq = warp & 3;
+        const int wq = warp & 3;            // TMEM lane quarter of this warp
+        const int chalf = (warp - 4) >> 2;  // 8 epilogue warps: the second warp of a quarter takes the tile's upper columns
+        constexpr int C_PER_WARP = 4 / (Cfg2<EPI>::EPI_WARPS / 4);
         const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
-        uint8_t* stg = stg_base + wq * NBUF * STG_BYTES;
+        uint8_t* stg = stg_base + (warp - 4) * NBUF * STG_BYTES;
         int as = 0, aphase = 0, ring = 0;
         long long w_tfull = 0, w_stg = 0;
         const long long t_begin = P.prof ? clock64() : 0;
@@ -972,7 +983,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             } else {
                 // one output of 256 columns, or (wgrad gate|up) two outputs of 128 columns each
 #pragma unroll 1
-                for (int c = 0; c < 4; ++c) {
+                for (int c = chalf * C_PER_WARP; c < (chalf + 1) * C_PER_WARP; ++c) {
                     const bool split = EPI == EPI_WGRAD_SPLIT;
                     const CUtensorMap* om = split ? &P.o[c >> 1] : &P.o[0];
                     const int col = split ? T.n0 + 64 * (c & 1) : T.n0 + 64 * c;
@@ -1167,10 +1178,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         prefetch_tmap(&P.bs[0]);
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
+        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], 2), mbar_init(&empty_bar[s], 1);  // two producer warps
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
-        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers);
+        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers + 2);  // + the second producer warp of each CTA
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -1205,8 +1216,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     }
 
-    if (warp == 0) {
-        // ===== TMA producer (both CTAs): own 128 features of the weights + own half of the rows =====
+    if (warp == 0 || warp == 2) {
+        // ===== TMA producers (both CTAs): warp 0 loads the CTA's 128 features of the weights, warp 2 (idle after the
+        // TMEM allocation) its half of the rows.  One thread issuing every box of a stage spent most of its time inside
+        // the issue of the bulk tensor instructions, not waiting for free stages. =====
+        const bool load_a = warp == 0;
         const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
         int stage = 0, phase = 0;
         long long w_empty = 0;
@@ -1225,12 +1239,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (P.prof) w_empty += clock64() - c0;
                     uint8_t* sa = smem + stage * TSTAGE_BYTES;
                     uint8_t* sb = sa + TA_BYTES;
-                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * (TA_BYTES + nbox * box_bytes));
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], load_a ? 2 * TA_BYTES : 2 * nbox * box_bytes);
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
                     const int k = kk * BK;
-                    if (EPI == TEPI_SWIGLU_FWD) {  // 64 gate features | the same 64 up features
+                    if (!load_a) {
+                        if (small) {
+                            for (int i = 0; i < nbox; ++i)
+                                tma_load_3d_pair(sb + i * box_bytes, &P.bs[src], bar, k, rb + i * TB_SMALL_ROWS, 0);
+                        } else {
+                            tma_load_3d_pair(sb, &P.b[src], bar, k, rb, 0);
+                        }
+                    } else if (EPI == TEPI_SWIGLU_FWD) {  // 64 gate features | the same 64 up features
                         const int fc = T.f * 128 + rank * 64;
                         tma_load_3d_pair(sa, &P.a[0], bar, fc, k, T.g);
                         tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[1], bar, fc, k, T.g);
@@ -1241,18 +1262,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     } else {
                         tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + rank * 128, T.g);
                     }
-                    if (small) {
-                        for (int i = 0; i < nbox; ++i)
-                            tma_load_3d_pair(sb + i * box_bytes, &P.bs[src], bar, k, rb + i * TB_SMALL_ROWS, 0);
-                    } else {
-                        tma_load_3d_pair(sb, &P.b[src], bar, k, rb, 0);
-                    }
                 }
                 __syncwarp();
                 if (++stage == NST) stage = 0, phase ^= 1;
             }
         }
-        if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
+        if (P.prof && lane == 0 && load_a) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1 && rank == 0) {
         // ===== MMA issuer (one thread of the leader CTA): D^T[256 features, n rows] += W-tile * rows^T =====
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
@@ -1558,7 +1573,7 @@ int make_map_f32(piper_ctx* c, CUtensorMap* m, const void* base, long long inner
 // pairs than sms / 2): the persistent grids stride over this many pairs, so it must not exceed what fits at once.
 // Queried once per (kernel, SM count of the lane) and kept.
 template <typename K>
-int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes) {
+int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes, int threads = kThreads) {
     constexpr int kSlots = 128;
     static struct { const void* fn; cudaStream_t stream; int sms; int n; } cache[kSlots];
     static int used = 0;
@@ -1570,7 +1585,7 @@ int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes) {
     cudaLaunchAttribute attr;
     attr.id = cudaLaunchAttributeClusterDimension;
     attr.val.clusterDim.x = 2, attr.val.clusterDim.y = 1, attr.val.clusterDim.z = 1;
-    cfg.gridDim = dim3(2 * (ln.sms / 2)), cfg.blockDim = dim3(kThreads), cfg.dynamicSmemBytes = smem_bytes;
+    cfg.gridDim = dim3(2 * (ln.sms / 2)), cfg.blockDim = dim3(threads), cfg.dynamicSmemBytes = smem_bytes;
     cfg.stream = ln.stream, cfg.attrs = &attr, cfg.numAttrs = 1;
     int n = 0;
     if (cudaOccupancyMaxActiveClusters(&n, kernel, &cfg) != cudaSuccess || n < 1) {
@@ -1593,11 +1608,11 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
     }
     if (two_cta) {
         // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
-        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM);
+        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM, Cfg2<EPI>::THREADS);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
         Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
-        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
+        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), Cfg2<EPI>::THREADS, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
     }
