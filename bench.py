@@ -301,7 +301,9 @@ def run_piper(args, cfg):
         sets[1][n] = torch.empty_like(b[n])
     set_args = [cargs, piper.chunk_args(sets[1])]
     s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
-    in_ready = [torch.cuda.Event() for _ in range(2)]
+    in_ready = [torch.cuda.Event() for _ in range(2)]   # logits and x are up (what the forward chunk reads)
+    dy_ready = [torch.cuda.Event() for _ in range(2)]   # dY is up (first read by the backward chunk)
+    fwd_done = [torch.cuda.Event() for _ in range(2)]   # y can go down while the backward chunk runs
     comp_done = [torch.cuda.Event() for _ in range(2)]
     out_done = [torch.cuda.Event() for _ in range(2)]
 
@@ -311,19 +313,25 @@ def run_piper(args, cfg):
             with torch.cuda.stream(s_in):
                 if i >= 2:
                     s_in.wait_event(comp_done[k])  # step i-2 has consumed this input set
-                for n, t in host_in.items():
-                    sets[k][n].copy_(t, non_blocking=True)
+                for n in ("logits", "x"):
+                    sets[k][n].copy_(host_in[n], non_blocking=True)
                 in_ready[k].record(s_in)
+                sets[k]["dy"].copy_(host_in["dy"], non_blocking=True)
+                dy_ready[k].record(s_in)
             stream.wait_event(in_ready[k])
             if i >= 2:
                 stream.wait_event(out_done[k])  # step i-2's results have left this output set
             piper.piper_run_chunk_fwd(ctx, set_args[k])
+            fwd_done[k].record(stream)
+            stream.wait_event(dy_ready[k])
             piper.piper_run_chunk_bwd(ctx, set_args[k])
             comp_done[k].record(stream)
             with torch.cuda.stream(s_out):
+                s_out.wait_event(fwd_done[k])
+                host_out["y"].copy_(sets[k]["y"], non_blocking=True)
                 s_out.wait_event(comp_done[k])
-                for n, t in host_out.items():
-                    t.copy_(sets[k][n], non_blocking=True)
+                for n in ("dx", "dz_sel"):
+                    host_out[n].copy_(sets[k][n], non_blocking=True)
                 out_done[k].record(s_out)
         stream.wait_event(out_done[0])
         stream.wait_event(out_done[1])
@@ -341,7 +349,8 @@ def run_piper(args, cfg):
     e2e = {"value": whole_job_tokens_per_s(cfg, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
            "what": "every step: pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel "
-                   "-> pinned host, as a 3-stream pipeline (copies of steps i+1 / i-1 overlap the compute of step i); "
+                   "-> pinned host, as a 3-stream pipeline (copies of steps i+1 / i-1 overlap the compute of step i; dY goes up "
+                   "behind x and y comes down while the backward chunk runs); "
                    "timed as max(CUDA events, host wall clock) over the whole pipeline"}
 
     # ---- per-task device times (CUDA events on the launching stream, inside full steps) ---------------
