@@ -248,6 +248,8 @@ def run_piper(args, cfg):
     rcfg = rank_config(cfg, rank)
     t0 = time.time()
     inp = configs.make_inputs(rcfg)
+    if getattr(args, "uniform_rows", 0):
+        inp["logits"] = configs.uniform_logits(rcfg)
     log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
     ctx = piper.Context(desc_of(piper, rcfg, dw_f32=args.main_grad), device=local)
     if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
@@ -509,6 +511,9 @@ def main():
     ap.add_argument("--row-align", type=int, default=None, help="override the config's row_align")
     ap.add_argument("--oracle-tokens", type=int, default=0, help="tokens of the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--uniform-rows", type=int, default=0,
+                    help="microbenchmark: C3's routed layer shape with exactly this many rows in each of 32 experts "
+                         "(overrides --config; use with --no-cpu-baseline)")
     ap.add_argument("--pair", action="store_true", help="also time step P (chunk pair vs serial) on this shape")
     ap.add_argument("--main-grad", action="store_true",
                     help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")
@@ -521,7 +526,7 @@ def main():
         ge.build()
     if args.config == "C5":  # configs[4]: the C3-shaped chunk pair, microbatch seeds 4 (forward) and 5 (backward)
         args.config, args.pair = "C5a", True
-    cfg = configs.BY_NAME[args.config]
+    cfg = configs.uniform_config(args.uniform_rows) if args.uniform_rows else configs.BY_NAME[args.config]
     if cfg.dtype == configs.DT_BF16:
         cfg = dataclasses.replace(cfg, row_align=args.row_align or 128)  # tcgen05 tiles are 128 rows
     if args.impl == "reference":

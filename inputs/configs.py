@@ -129,3 +129,20 @@ def make_inputs(cfg: MoeConfig, weights: bool = True, with_dy: bool = True) -> d
 def flops_fwd_bwd(cfg: MoeConfig, a_rows: int) -> float:
     """18*d*I per routed row + 18*d*I_sh per token."""
     return 18.0 * cfg.d * cfg.I * a_rows + 18.0 * cfg.d * cfg.I_shared * cfg.T
+
+
+def uniform_config(rows_per_expert: int) -> MoeConfig:
+    """Microbenchmark workload (bench.py --uniform-rows): C3's routed layer shape (d = 7168, I = 2048, 32 local
+    experts, top-8, no shared expert) with exactly `rows_per_expert` rows in every expert, so that a GEMM's rate can be
+    read as a function of the group length alone."""
+    E, k = 32, 8
+    return MoeConfig(f"U{rows_per_expert}", T=rows_per_expert * E // k, d=7168, E=E, k=k, I=2048, seed=7, row_align=128)
+
+
+def uniform_logits(cfg: MoeConfig) -> np.ndarray:
+    """Logits that send token t to experts (t k + j) mod E, j < k, in that order of preference."""
+    lg = np.full((cfg.T, cfg.E), -10.0, dtype=np.float32)
+    t = np.arange(cfg.T)
+    for j in range(cfg.k):
+        lg[t, (t * cfg.k + j) % cfg.E] = np.float32(1.0 - 0.01 * j)
+    return lg
