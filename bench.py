@@ -252,6 +252,7 @@ def run_piper(args, cfg):
         inp["logits"] = configs.uniform_logits(rcfg)
     log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
     ctx = piper.Context(desc_of(piper, rcfg, dw_f32=args.main_grad), device=local)
+    piper.piper_set_chunk_overlap(ctx, 1 if getattr(args, "chunk_overlap", False) else 0)
     if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
         piper.piper_set_wgrad_accumulate(ctx, 1)
     b = piper.alloc_buffers(ctx)
@@ -455,9 +456,19 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
             ts.append(e0.elapsed_time(e1) / iters)
         return sorted(ts)[len(ts) // 2]
 
+    # the serial baseline: every task of both chunks on one stream, all SMs; beside it the same two
+    # calls with the library's intra-chunk overlap (piper_set_chunk_overlap), a measured variant
+    piper.piper_set_chunk_overlap(ctx, 1)
+    t_fo = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
+    t_bo = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
+    piper.piper_set_chunk_overlap(ctx, 0)
     t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
     t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
-    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "splits": {}, "variants": {}}
+    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b,
+           "chunk_overlap": {"fwd_ms": t_fo, "bwd_ms": t_bo, "ratio_vs_serial": (t_fo + t_bo) / (t_f + t_b),
+                             "what": "the two chunks one after the other, each with its row movers on a side stream "
+                                     "beside the shared expert's GEMMs (fwd) / the routed wgrad (bwd)"},
+           "splits": {}, "variants": {}}
 
     def sweep(split_list):
         res = {}
@@ -514,6 +525,10 @@ def main():
     ap.add_argument("--uniform-rows", type=int, default=0,
                     help="microbenchmark: C3's routed layer shape with exactly this many rows in each of 32 experts "
                          "(overrides --config; use with --no-cpu-baseline)")
+    ap.add_argument("--chunk-overlap", action="store_true",
+                    help="measured variant: piper_set_chunk_overlap(1), the chunks' row movers on the library's side "
+                         "stream beside the shared expert's GEMMs / the routed wgrad (default: one stream; measured "
+                         "neutral, C2 6.67 -> 6.82 ms, C3 4.22 -> 4.23 ms: the GEMM beside them slows by what they hide)")
     ap.add_argument("--pair", action="store_true", help="also time step P (chunk pair vs serial) on this shape")
     ap.add_argument("--main-grad", action="store_true",
                     help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")

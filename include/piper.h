@@ -232,6 +232,14 @@ int piper_run_task(piper_ctx* ctx, int task, const piper_chunk_args* a, void* st
  * `ctx`, default 0); PIPER_ERR_UNSUPPORTED unless dw_dtype = F32. */
 int piper_set_wgrad_accumulate(piper_ctx* ctx, int accumulate);
 
+/* Intra-chunk overlap of piper_run_chunk_fwd / piper_run_chunk_bwd (host state of `ctx`, default 0 = every task on the
+ * caller's stream, one after the other: the serial baseline the pair is compared with).  on = 1: the forward chunk runs
+ * route / scan / pack on a side stream of the library beside the shared expert's GEMMs (layers with a shared expert),
+ * the backward chunk runs unpack and route_bwd on the side stream beside the routed wgrad (the shared expert's backward
+ * moves in front of it).  The side stream forks from and joins into the caller's stream inside the call; results are
+ * bit-identical.  Returns PIPER_ERR_INVALID for other values, PIPER_ERR_CUDA if the stream cannot be created. */
+int piper_set_chunk_overlap(piper_ctx* ctx, int on);
+
 /* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
  * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 3 = one stream per chunk
  * (PIPER_PART_CHUNK_STREAMS), 0 = never called. */

@@ -131,6 +131,10 @@ def piper_kernel_launches(ctx: Context) -> int:
     return int(lib().piper_kernel_launches(ctx._h))
 
 
+def piper_set_chunk_overlap(ctx: Context, on: int):
+    ctx.check(lib().piper_set_chunk_overlap(ctx._h, int(on)), "piper_set_chunk_overlap")
+
+
 def piper_set_wgrad_accumulate(ctx: Context, accumulate: int):
     ctx.check(lib().piper_set_wgrad_accumulate(ctx._h, int(accumulate)), "piper_set_wgrad_accumulate")
 

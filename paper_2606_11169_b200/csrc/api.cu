@@ -98,6 +98,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
 int piper_destroy(piper_ctx* c) {
     if (!c) return PIPER_ERR_INVALID;
     pair_release(c);
+    if (c->side_stream) cudaStreamDestroy(c->side_stream);
     for (int i = 0; i < kMaxEvents; ++i)
         if (c->events[i]) cudaEventDestroy(c->events[i]);
     delete c;

@@ -205,9 +205,38 @@ void pair_release(piper_ctx* c) {
 
 extern "C" {
 
+int piper_set_chunk_overlap(piper_ctx* c, int on) {
+    if (!c || (on != 0 && on != 1)) return PIPER_ERR_INVALID;
+    if (on && !c->side_stream && cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess)
+        return cuda_fail(c, cudaGetLastError(), "cudaStreamCreateWithFlags");
+    c->chunk_overlap = on;
+    return PIPER_OK;
+}
+
 int piper_run_chunk_fwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     if (!c || !fwd_args_ok(c, a)) return PIPER_ERR_INVALID;
     const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    if (c->chunk_overlap && c->D.I_shared) {
+        // The shared expert does not depend on the routing: route / scan / pack run on the side stream beside its
+        // (compute-bound) GEMMs, the same two-stream rule as the pair inside one chunk.
+        const Lane side{c->side_stream, c->num_sms};
+        cudaEvent_t fork = c->events[14], packed = c->events[15];
+        PIPER_CUDA(c, cudaEventRecord(fork, ln.stream));
+        PIPER_CUDA(c, cudaStreamWaitEvent(side.stream, fork, 0));
+        for (int t : {F_ROUTE, F_SCAN, F_PACK}) {
+            const int rc = run_task(c, t, side, a, nullptr);
+            if (rc != PIPER_OK) return rc;
+        }
+        PIPER_CUDA(c, cudaEventRecord(packed, side.stream));
+        int rc = run_task(c, F_SHARED, ln, a, nullptr);
+        if (rc != PIPER_OK) return rc;
+        PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, packed, 0));
+        for (int t : {F_GEMM1, F_GEMM2, F_COMBINE}) {
+            rc = run_task(c, t, ln, a, nullptr);
+            if (rc != PIPER_OK) return rc;
+        }
+        return PIPER_OK;
+    }
     const int seq[] = {F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE};
     for (int t : seq) {
         if (t == F_SHARED && !c->D.I_shared) continue;
@@ -228,6 +257,27 @@ int piper_run_task(piper_ctx* c, int task, const piper_chunk_args* a, void* stre
 int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
     const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    if (c->chunk_overlap) {
+        // unpack and route_bwd need no wgrad output: they run on the side stream beside the routed wgrad
+        const Lane side{c->side_stream, c->num_sms};
+        cudaEvent_t fork = c->events[14], joined = c->events[16];
+        for (int t : {B_CGRAD, B_DGRAD1, B_DGRAD2, B_SHARED}) {
+            if (t == B_SHARED && !c->D.I_shared) continue;
+            const int rc = run_task(c, t, ln, nullptr, a);
+            if (rc != PIPER_OK) return rc;
+        }
+        PIPER_CUDA(c, cudaEventRecord(fork, ln.stream));
+        PIPER_CUDA(c, cudaStreamWaitEvent(side.stream, fork, 0));
+        int rc = run_task(c, B_WGRAD, ln, nullptr, a);
+        if (rc != PIPER_OK) return rc;
+        for (int t : {B_UNPACK, B_ROUTE_BWD}) {
+            rc = run_task(c, t, side, nullptr, a);
+            if (rc != PIPER_OK) return rc;
+        }
+        PIPER_CUDA(c, cudaEventRecord(joined, side.stream));
+        PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, joined, 0));
+        return PIPER_OK;
+    }
     const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD};
     for (int t : seq) {
         if (t == B_SHARED && !c->D.I_shared) continue;

@@ -43,6 +43,8 @@ struct piper_ctx {
     int64_t launches;
     int pair_mode;
     int wgrad_accumulate;        // piper_set_wgrad_accumulate: the chunk calls' wgrad adds into dW
+    int chunk_overlap;           // piper_set_chunk_overlap: the chunk calls run their row movers on a side stream
+    cudaStream_t side_stream;    // created on first use
     int pair_order, pair_part;   // piper_set_pair_policy
     int pair_have_ms;
     void* pair_plan;             // cached schedule of the pair for (plan_sm_gemm, plan_sm_comm)

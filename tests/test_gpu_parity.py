@@ -18,9 +18,11 @@ pytestmark = pytest.mark.gpu
 SMALL = ["C1", "C1s", "C2s", "C3s", "C4s", "C6s"]
 
 
-def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True):
+def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True, overlap=False):
     """Runs the whole path; returns (ctx, dict of device tensors)."""
     ctx = piper.Context(util.desc_of(cfg, gemm_impl))
+    if overlap:
+        piper.piper_set_chunk_overlap(ctx, 1)
     dev = util.upload_inputs(inp)
     b = piper.alloc_buffers(ctx, backward=True)
     b.update(dev)
@@ -229,14 +231,16 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128 if name != "C1" else 1)
     inp = configs.make_inputs(cfg)
     ctx1, b1 = _run_steps(cfg, inp)
-    ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True)
     A = int(b1["offsets"][cfg.e_loc])
-    for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y", "dgates", "dz_sel", "dx", "dw_gate", "dw_up",
-              "dw_down"):
-        assert torch.equal(b1[n], b2[n]), n
-    for n in ("xp", "o", "dxp"):
-        assert torch.equal(b1[n][:A], b2[n][:A]), n
-    ctx1.close(), ctx2.close()
+    for overlap in (False, True):  # piper_set_chunk_overlap: row movers on the library's side stream
+        ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True, overlap=overlap)
+        for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y", "dgates", "dz_sel", "dx", "dw_gate", "dw_up",
+                  "dw_down") + (("dws_gate", "dws_up", "dws_down") if cfg.I_shared else ()):
+            assert torch.equal(b1[n], b2[n]), (n, overlap)
+        for n in ("xp", "o", "dxp"):
+            assert torch.equal(b1[n][:A], b2[n][:A]), (n, overlap)
+        ctx2.close()
+    ctx1.close()
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
