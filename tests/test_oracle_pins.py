@@ -365,3 +365,17 @@ def test_list_scheduler_golden_order():
         assert pos[s] < pos[t]
         if so[s] != so[t]:
             assert (s, t) in {tuple(w) for w in waits.tolist()} and records[s] == 1
+
+
+# ------------------------------------------------------------------------------------ input recipe of the microbenchmark
+@pytest.mark.parametrize("rows", [16, 64, 200])
+def test_uniform_logits_give_every_expert_the_same_rows(rows):
+    """bench.py --uniform-rows: the crafted logits must route exactly `rows` rows to each of the 32 experts, token t to
+    experts (t k + j) mod E in that order (checked with the oracle's routing, the definition of SURVEY.md §8c-1)."""
+    cfg = C.uniform_config(rows)
+    z = C.uniform_logits(cfg)
+    idx, gates, cg = O.route_topk(cfg, z)
+    assert (cg == rows).all() and cg.sum() == cfg.T * cfg.k
+    t = np.arange(cfg.T)[:, None]
+    assert (idx == (t * cfg.k + np.arange(cfg.k)[None, :]) % cfg.E).all()
+    assert (np.diff(gates, axis=1) < 0).all()  # descending preference -> descending gates
