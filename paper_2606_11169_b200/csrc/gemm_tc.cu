@@ -1653,15 +1653,12 @@ bool set_smem_attr_t() {
 }
 // rows-on-N kernel for the ragged-M contractions (PIPER_TC_ROWS_ON_N=0 switches it off)
 bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2; }
-TcParams t_params(const FfnProblem& p, int F, int K, int f_tile) {
+TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_tile) {
     TcParams P;
     memset(&P, 0, sizeof(P));
     P.offsets = p.offsets, P.counts = p.counts, P.G = p.G, P.n_src = 1;
     P.f_tiles = cdiv(F, f_tile), P.f_limit = F, P.kb_per_src = cdiv(K, BK);
-    const char* e = getenv("PIPER_T_SMALL");
-    P.small_rows = e ? atoi(e) : TB_SMALL_ROWS;
-    const char* e2 = getenv("PIPER_T_GREEDY");
-    P.greedy = e2 ? atoi(e2) : 1;
+    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy;
     return P;
 }
 inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
@@ -1703,6 +1700,10 @@ int tc_init(piper_ctx* c) {
     c->tc_prof = pe && pe[0] == '1';
     const char* pt = getenv("PIPER_TC_ROWS_ON_N");
     c->tc_rows_on_n = !(pt && pt[0] == '0');
+    const char* ps = getenv("PIPER_T_SMALL");   // tuning knobs of the rows-on-N kernels, read once
+    c->tc_small_rows = ps ? atoi(ps) : TB_SMALL_ROWS;
+    const char* pg = getenv("PIPER_T_GREEDY");
+    c->tc_greedy = pg ? atoi(pg) : 1;
     const char* p2 = getenv("PIPER_TC_2CTA");  // 0: never, 1: always, unset: by expected group length
     c->tc_two_cta = p2 ? (p2[0] == '0' ? 0 : 1) : 2;
     c->tc2_max_clusters = c->num_sms / 2;
@@ -1728,7 +1729,7 @@ bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
 // G|U = Xp Wg | Xp Wu, H = silu(G) * U
 int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
     if (rows_on_n(c, p)) {
-        TcParams P = t_params(p, p.I, p.d, 128);
+        TcParams P = t_params(c, p, p.I, p.d, 128);
         PIPER_MAP(&P.a[0], p.w_gate, p.I, p.d, p.G, 64);
         PIPER_MAP(&P.a[1], p.w_up, p.I, p.d, p.G, 64);
         PIPER_MAP(&P.b[0], p.xp, p.d, p.max_rows, 1, TB_BOX_ROWS);
@@ -1757,7 +1758,7 @@ int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
 // O = H Wd
 int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
     if (rows_on_n(c, p)) {
-        TcParams P = t_params(p, p.d, p.I, 256);
+        TcParams P = t_params(c, p, p.d, p.I, 256);
         PIPER_MAP(&P.a[0], p.w_down, p.d, p.I, p.G, 64);
         PIPER_MAP(&P.b[0], p.h, p.I, p.max_rows, 1, TB_BOX_ROWS);
         PIPER_MAP(&P.bs[0], p.h, p.I, p.max_rows, 1, TB_SMALL_ROWS);
@@ -1777,7 +1778,7 @@ int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
 // dH = dO Wd^T; dG = dH * U * silu'(G); dU = dH * silu(G)
 int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
     if (rows_on_n(c, p)) {
-        TcParams P = t_params(p, p.I, p.d, 256);
+        TcParams P = t_params(c, p, p.I, p.d, 256);
         PIPER_MAP(&P.a[0], p.w_down, p.d, p.I, p.G, 128);
         PIPER_MAP(&P.b[0], p.d_o, p.d, p.max_rows, 1, TB_BOX_ROWS);
         PIPER_MAP(&P.bs[0], p.d_o, p.d, p.max_rows, 1, TB_SMALL_ROWS);
@@ -1806,7 +1807,7 @@ int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
 // dXp = dG Wg^T + dU Wu^T  (one accumulator, K runs over both products)
 int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
     if (rows_on_n(c, p)) {
-        TcParams P = t_params(p, p.d, p.I, 256);
+        TcParams P = t_params(c, p, p.d, p.I, 256);
         PIPER_MAP(&P.a[0], p.w_gate, p.I, p.d, p.G, 128);
         PIPER_MAP(&P.a[1], p.w_up, p.I, p.d, p.G, 128);
         PIPER_MAP(&P.b[0], p.dg, p.I, p.max_rows, 1, TB_BOX_ROWS);

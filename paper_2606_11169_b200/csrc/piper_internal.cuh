@@ -59,6 +59,7 @@ struct piper_ctx {
     int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
     int tc2_max_clusters;    // co-resident CTA pairs
     int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_TC_ROWS_ON_N, default on)
+    int tc_small_rows, tc_greedy;  // PIPER_T_SMALL / PIPER_T_GREEDY: row chunking of the rows-on-N kernels
     int tc_prof;             // PIPER_TC_PROFILE=1: the tcgen05 kernels record wait-cycle counters in tc_scratch
     cudaEvent_t events[piper::kMaxEvents];
 };

@@ -135,6 +135,19 @@ def test_random_shapes_full_tensor_parity(i):
     ctx.close()
 
 
+def test_more_local_experts_than_the_cta_pair_kernels_index():
+    """256 local experts (> 192, the group bound of the CTA-pair kernels' tile-prefix arrays): every GEMM takes the
+    1-CTA tcgen05 kernels without any switch; many experts are short or empty."""
+    cfg = configs.MoeConfig("many", T=1500, d=128, E=256, k=4, I=192, seed=31, bias="zipf1.2", row_align=128)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True)
+    _check_all(cfg, b, f, g)
+    assert piper.piper_gemm_path(ctx) == 1
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
 @pytest.mark.parametrize("env", [{"PIPER_TC_ROWS_ON_N": "0"}, {"PIPER_TC_ROWS_ON_N": "0", "PIPER_TC_2CTA": "0"}])
 def test_fallback_kernel_families(name, env, monkeypatch):
