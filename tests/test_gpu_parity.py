@@ -135,6 +135,31 @@ def test_random_shapes_full_tensor_parity(i):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["C3s", "C4s"])
+def test_chunk_calls_capture_into_a_cuda_graph(name):
+    """The chunk calls only enqueue work on the caller's stream (no host read-back, no allocation), so a step can be
+    captured in a CUDA graph; the replay is bit-identical to the eager run (the tile counters of the persistent
+    kernels re-arm themselves)."""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
+    inp = configs.make_inputs(cfg)
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True)
+    names = ("y", "dx", "dz_sel", "dw_gate", "dw_up", "dw_down", "row_of")
+    ref = {n: b[n].clone() for n in names}
+    args = piper.chunk_args(b)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        piper.piper_run_chunk_fwd(ctx, args)
+        piper.piper_run_chunk_bwd(ctx, args)
+    for rep in range(2):
+        for n in names:
+            b[n].fill_(-1 if b[n].dtype == torch.int32 else 7.0)
+        graph.replay()
+        torch.cuda.synchronize()
+        for n in names:
+            assert torch.equal(ref[n], b[n]), (n, rep)
+    ctx.close()
+
+
 def test_more_local_experts_than_the_cta_pair_kernels_index():
     """256 local experts (> 192, the group bound of the CTA-pair kernels' tile-prefix arrays): every GEMM takes the
     1-CTA tcgen05 kernels without any switch; many experts are short or empty."""
