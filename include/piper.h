@@ -18,7 +18,7 @@
  *    frees caller memory; `workspace` (device, caller-owned) must outlive the context;
  *  - `stream` is a cudaStream_t passed as void*; calls only enqueue work: no host synchronisation,
  *    no host read-back of device data (the packed row count A lives on the device in
- *    offsets[E_loc]);
+ *    offsets[E_loc]), so a sequence of calls can be captured in a CUDA graph and replayed;
  *  - activation / weight element type is `desc.dtype` (0 = fp32, 1 = bf16 with fp32 accumulation);
  *    logits, gates, gate_rows, dgates, dz_sel are always fp32; indices are int32;
  *  - row buffers (xp, o, d_o, dxp, g_save, u_save, h_save, src_of, gate_rows) hold
