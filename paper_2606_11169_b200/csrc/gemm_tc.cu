@@ -615,10 +615,12 @@ __device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, c
         if (!r.store) mt = 2 * pair;
         r.g = g, r.m0 = (tp[g] + mt) * BM, r.n0 = nt * P.tile_n, r.k0 = 0, r.nkb = P.kb_per_src * P.n_src;
     } else {
+        // wgrad: tp[] holds the groups' offsets (copied to shared memory in the prologue: a tile of 2-8 K blocks is too
+        // short to hide two dependent global loads of the issuing thread between tiles)
         const int pairs = (P.m_tiles + 1) / 2, per_group = pairs * P.n_tiles;
         const int g = t / per_group, local = t - g * per_group;
         const int nt = local / pairs, pair = local - nt * pairs;
-        const int lo = offsets[g], hi = offsets[g + 1];
+        const int lo = tp[g], hi = tp[g + 1];
         r.store = true;  // rows beyond m_limit are clipped by the bounds checks
         r.g = g, r.m0 = (2 * pair + rank) * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + bk - 1) / bk;
     }
@@ -652,13 +654,22 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
 // first tile of a cluster is its own index, so the clusters start on neighbouring tiles (shared weight tiles in L2)
 // and every later tile is drawn only when the cluster is about to need it.
 constexpr int kFeed = 2, kFeedConsumers = 2 * 5 + 1;
+constexpr int kFeedWords = 8;  // rows-on-N kernels: a slot holds the decoded tile {t, g, f, r0, n, zend}
 struct TileFeed {
-    int* ids;             // [kFeed] this CTA
+    int* ids;             // [kFeed][stride] this CTA
     uint64_t* full;       // [kFeed] this CTA
     uint32_t empty_addr;  // cluster address of the leader's empty barriers [kFeed]
+    int stride = 1;       // ints per slot
     __device__ __forceinline__ int peek(int it) const {
         mbar_wait(&full[it & (kFeed - 1)], (it / kFeed) & 1);
-        return *reinterpret_cast<volatile int*>(&ids[it & (kFeed - 1)]);
+        return *reinterpret_cast<volatile int*>(&ids[(it & (kFeed - 1)) * stride]);
+    }
+    // words 1.. of the slot of tile `it` (valid between peek(it) and this warp's release in take(it))
+    __device__ __forceinline__ const volatile int* slot(int it) const { return ids + (it & (kFeed - 1)) * stride; }
+    // all lanes of a consumer warp: done with slot `it` (after every lane has read what it needs from it)
+    __device__ __forceinline__ void release(int it, int lane) const {
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(empty_addr + (it & (kFeed - 1)) * 8);
     }
     // all lanes of a consumer warp call this
     __device__ __forceinline__ int take(int it, int lane) const {
@@ -693,6 +704,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
     const int pair_id = blockIdx.x >> 1, n_pairs_grid = gridDim.x >> 1;
     const int32_t* __restrict__ offsets = P.offsets;
 
+    if (!P.ragged_m) {  // wgrad: offsets and real row counts of the groups (read by decode_pair / the MMA issuer)
+        for (int g = threadIdx.x; g <= P.G; g += Cfg2<EPI>::THREADS) {
+            tp[g] = offsets[g];
+            if (g < P.G) tpp[g] = P.counts ? P.counts[g] : offsets[g + 1] - offsets[g];
+        }
+    }
     if (P.ragged_m) {
         for (int g = threadIdx.x; g <= P.G; g += Cfg2<EPI>::THREADS) tp[g] = (offsets[g] + BM - 1) / BM;
         __syncthreads();
@@ -825,7 +842,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc);
             // wgrad: the K range ends with the expert's zero pad rows; K slices (16 rows) that hold only pad rows are
             // not issued (C2: 640 of 8832 rows, 7% of the tensor work)
-            const int k_valid = (!P.ragged_m && P.counts) ? P.counts[T.g] : 0x3fffffff;
+            const int k_valid = !P.ragged_m ? tpp[T.g] : 0x3fffffff;
             if (lane == 0) {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
@@ -1088,7 +1105,7 @@ struct CfgT {
     static constexpr int XCH_BYTES = EPI == TEPI_SWIGLU_FWD ? 2 * 2 * 32 * 32 * 4 : 0;  // fp32 U exchange, 2 pairs x 2
     static constexpr int ZERO_BYTES = 16 * 32 * 2;         // a zero block for the pad rows
     static constexpr int SCHED_BYTES = 256;                // tile feed: 8 ids + 2 x 8 mbarriers
-    static constexpr int SMEM = RING_BYTES + STG_TOTAL + XCH_BYTES + ZERO_BYTES + SCHED_BYTES + 1024 + 256 + (kMaxGroups2 + 1) * 4;
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + XCH_BYTES + ZERO_BYTES + SCHED_BYTES + 1024 + 256 + 3 * (kMaxGroups2 + 1) * 4;
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 
@@ -1102,11 +1119,12 @@ __device__ __forceinline__ void t_plan(int rows, int& nch, int& cs, int greedy) 
     cs = greedy ? 256 : (n0 ? ((rows + n0 - 1) / n0 + 15) & ~15 : 16);
     nch = (rows + cs - 1) / cs;
 }
-__device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, const int32_t* __restrict__ offsets,
-                                          const int32_t* __restrict__ counts, int t) {
+// tq / so / sc: first tile, first packed row and real row count of each group, in shared memory
+__device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, const int* so, const int* sc, int t) {
     int g = 0;
     while (g + 1 < P.G && tq[g + 1] <= t) ++g;
-    const int local = t - tq[g], rows = counts ? counts[g] : offsets[g + 1] - offsets[g];
+    const int local = t - tq[g], rows = sc[g];
+    const int* offsets = so;
     int nch, cs;
     t_plan(rows, nch, cs, P.greedy);
     // panels of T_PANEL chunks; inside a panel feature-major with the chunk fastest
@@ -1144,6 +1162,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets]
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
     int* tq = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);       // first tile of each group
+    int* so = tq + (kMaxGroups2 + 1);                                                    // offsets of the groups
+    int* sc = so + (kMaxGroups2 + 1);                                                    // real rows of the groups
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = (int)cluster_ctarank();
@@ -1155,10 +1175,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         for (int i = lane; i < CfgT<EPI>::ZERO_BYTES / 16; i += 32) st_shared16(zero_blk + 16 * i, make_uint4(0, 0, 0, 0));
         fence_proxy_async();
         int carry = 0;
+        if (lane == 0) so[P.G] = offsets[P.G];
         for (int g0 = 0; g0 < P.G; g0 += 32) {
             const int g = g0 + lane;
             int nch = 0, cs;
-            if (g < P.G) t_plan(counts ? counts[g] : offsets[g + 1] - offsets[g], nch, cs, P.greedy);
+            if (g < P.G) {
+                const int lo = offsets[g], rows = counts ? counts[g] : offsets[g + 1] - lo;
+                so[g] = lo, sc[g] = rows;
+                t_plan(rows, nch, cs, P.greedy);
+            }
             const int v = nch * P.f_tiles;
             int x = v;
 #pragma unroll
@@ -1193,16 +1218,33 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     const int nkb = P.kb_per_src * P.n_src;
     TileFeed feed;
     feed.ids = feed_ids, feed.full = feed_full, feed.empty_addr = mapa_u32(smem_u32(feed_empty), 0);
+    feed.stride = kFeedWords;
+    // the tile of iteration `it` as the feeder decoded it (all lanes of a consumer warp; after feed.peek / before the release)
+    auto tile_of = [&](int it) {
+        const volatile int* w = feed.slot(it);
+        TileT T;
+        T.g = w[1], T.f = w[2], T.r0 = w[3], T.n = w[4], T.zend = w[5];
+        return T;
+    };
 
     if (warp == 3 && rank == 0 && lane == 0) {
-        // ===== tile feeder (one thread of the leader CTA) =====
+        // ===== tile feeder (one thread of the leader CTA): draws the tile and decodes it once for every consumer warp
+        // of both CTAs (the issuing thread's own decode cost 1500-2000 cycles between two tiles) =====
         const uint32_t peer_ids = mapa_u32(smem_u32(feed_ids), 1), peer_full = mapa_u32(smem_u32(feed_full), 1);
         for (int it = 0;; ++it) {
             const int slot = it & (kFeed - 1);
             mbar_wait(&feed_empty[slot], ((it / kFeed) & 1) ^ 1);
             const int t = it == 0 ? pair_id : n_pairs_grid + atomicAdd(P.sched, 1);
-            *reinterpret_cast<volatile int*>(&feed_ids[slot]) = t;
-            asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(peer_ids + slot * 4), "r"(t) : "memory");
+            int w[6] = {t, 0, 0, 0, 0, 0};
+            if (t < n_total) {
+                const TileT T = decode_t(P, tq, so, sc, t);
+                w[1] = T.g, w[2] = T.f, w[3] = T.r0, w[4] = T.n, w[5] = T.zend;
+            }
+#pragma unroll
+            for (int i = 0; i < 6; ++i) {
+                *reinterpret_cast<volatile int*>(&feed_ids[slot * kFeedWords + i]) = w[i];
+                asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(peer_ids + (slot * kFeedWords + i) * 4), "r"(w[i]) : "memory");
+            }
             mbar_arrive(&feed_full[slot]);
             // the peer must see the id before the arrival: cluster-scope release (a membar on this otherwise idle thread)
             asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(peer_full + slot * 8) : "memory");
@@ -1225,9 +1267,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         int stage = 0, phase = 0;
         long long w_empty = 0;
         for (int it = 0;; ++it) {
-            const int t = feed.take(it, lane);
+            const int t = feed.peek(it);
+            const TileT T = tile_of(it);
+            feed.release(it, lane);
             if (t >= n_total) break;
-            const TileT T = decode_t(P, tq, offsets, counts, t);
             const int nb = T.n >> 1, rb = T.r0 + rank * nb;
             const bool small = nb <= P.small_rows;
             const int nbox = small ? (nb + TB_SMALL_ROWS - 1) / TB_SMALL_ROWS : 1;
@@ -1276,9 +1319,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         for (int it = 0;; ++it) {
-            const int t = feed.take(it, lane);
+            const int t = feed.peek(it);
+            const TileT T = tile_of(it);
+            feed.release(it, lane);
             if (t >= n_total) break;
-            const TileT T = decode_t(P, tq, offsets, counts, t);
             const uint32_t idesc = make_idesc_t(A_MAJOR, T.n);
             if (lane == 0) {
                 const long long c0 = P.prof ? clock64() : 0;
@@ -1359,14 +1403,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         if (EPI == TEPI_SWIGLU_BWD) {
             const int t0 = feed.peek(0);
             if (t0 < n_total) {
-                const TileT T0 = decode_t(P, tq, offsets, counts, t0);
+                const TileT T0 = tile_of(0);
                 load_inputs(feat_col(T0), T0.r0, 0);
             }
         }
         for (int it = 0;; ++it) {
-            const int t = feed.take(it, lane);
+            const int t = feed.peek(it);
+            const TileT T = tile_of(it);
+            feed.release(it, lane);
             if (t >= n_total) break;
-            const TileT T = decode_t(P, tq, offsets, counts, t);
             const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
             if (P.prof) w_tfull += clock64() - c0;
@@ -1445,7 +1490,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     } else {
                         const int tn = feed.peek(it + 1);
                         if (tn < n_total) {
-                            const TileT Tn = decode_t(P, tq, offsets, counts, tn);
+                            const TileT Tn = tile_of(it + 1);
                             load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
                         }
                     }
