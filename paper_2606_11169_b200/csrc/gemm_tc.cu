@@ -599,8 +599,19 @@ struct Tile2 {
 __device__ __forceinline__ int total_pairs(const TcParams& P, const int* tpp) {
     return P.ragged_m ? tpp[P.G] * P.n_tiles : P.G * ((P.m_tiles + 1) / 2) * P.n_tiles;
 }
+// t / d for 0 <= t < 2^22, 0 < d < 2^22 with the reciprocal of d hoisted out of the tile loop (one correction step makes
+// the float estimate exact); an integer division costs the issuing thread ~100 cycles between two short wgrad tiles
+__device__ __forceinline__ int div_rcp(int t, int d, float rcp, int& rem) {
+    int q = __float2int_rz(__int2float_rz(t) * rcp);
+    int r = t - q * d;
+    if (r < 0) --q, r += d;
+    else if (r >= d) ++q, r -= d;
+    rem = r;
+    return q;
+}
 __device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, const int* tpp,
-                                             const int32_t* __restrict__ offsets, int t, int rank, int bk = BK) {
+                                             const int32_t* __restrict__ offsets, int t, int rank, int bk = BK,
+                                             float rcp_group = 0.f, float rcp_pairs = 0.f) {
     Tile2 r;
     if (P.ragged_m) {
         int g = 0;
@@ -618,8 +629,14 @@ __device__ __forceinline__ Tile2 decode_pair(const TcParams& P, const int* tp, c
         // wgrad: tp[] holds the groups' offsets (copied to shared memory in the prologue: a tile of 2-8 K blocks is too
         // short to hide two dependent global loads of the issuing thread between tiles)
         const int pairs = (P.m_tiles + 1) / 2, per_group = pairs * P.n_tiles;
-        const int g = t / per_group, local = t - g * per_group;
-        const int nt = local / pairs, pair = local - nt * pairs;
+        int g, local, nt, pair;
+        if (rcp_group != 0.f) {
+            g = div_rcp(t, per_group, rcp_group, local);
+            nt = div_rcp(local, pairs, rcp_pairs, pair);
+        } else {
+            g = t / per_group, local = t - g * per_group;
+            nt = local / pairs, pair = local - nt * pairs;
+        }
         const int lo = tp[g], hi = tp[g + 1];
         r.store = true;  // rows beyond m_limit are clipped by the bounds checks
         r.g = g, r.m0 = (2 * pair + rank) * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + bk - 1) / bk;
@@ -749,6 +766,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
     const int n_total = total_pairs(P, tpp);
+    // wgrad tile decode: reciprocals of the two divisors (0: plain integer division, ragged problems / huge tile counts)
+    const int wg_pairs = (P.m_tiles + 1) / 2, wg_group = wg_pairs * P.n_tiles;
+    const bool wg_fast = !P.ragged_m && n_total < (1 << 22);
+    const float rcp_group = wg_fast ? 1.f / (float)wg_group : 0.f, rcp_pairs = wg_fast ? 1.f / (float)wg_pairs : 0.f;
     TileFeed feed;
     feed.ids = feed_ids, feed.full = feed_full, feed.empty_addr = mapa_u32(smem_u32(feed_empty), 0);
 
@@ -792,7 +813,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
         for (int it = 0;; ++it) {
             const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
             if (t >= n_total) break;
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
                     const long long c0 = P.prof ? clock64() : 0;
@@ -839,7 +860,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
         for (int it = 0;; ++it) {
             const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
             if (t >= n_total) break;
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc, rcp_group, rcp_pairs);
             // wgrad: the K range ends with the expert's zero pad rows; K slices (16 rows) that hold only pad rows are
             // not issued (C2: 640 of 8832 rows, 7% of the tensor work)
             const int k_valid = !P.ragged_m ? tpp[T.g] : 0x3fffffff;
@@ -902,12 +923,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
         };
         if (EPI == EPI_SWIGLU_BWD) {
             const int t0 = dynamic ? feed.peek(0) : pair_id;
-            if (t0 < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, t0, rank, BKc), 0, 0);
+            if (t0 < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, t0, rank, BKc, rcp_group, rcp_pairs), 0, 0);
         }
         for (int it = 0;; ++it) {
             const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
             if (t >= n_total) break;
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc);
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
             const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
             if (P.prof) w_tfull += clock64() - c0;
@@ -964,7 +985,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                         load_inputs(T, c + 1, set ^ 1);
                     } else {
                         const int tn = dynamic ? feed.peek(it + 1) : t + n_pairs_grid;
-                        if (tn < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, tn, rank, BKc), 0, set ^ 1);
+                        if (tn < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, tn, rank, BKc, rcp_group, rcp_pairs), 0, set ^ 1);
                     }
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
