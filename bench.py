@@ -48,7 +48,7 @@ def ncu_mover_us(config_name: str):
     """Per-launch gpu__time_duration of the row movers from the committed ncu launch lists (a CUDA-event pair around one
     ~20 us launch also counts ~6 us of launch latency), or {}."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r1d_traffic.json.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r1e_traffic.json.txt")) as f:
             return json.load(f).get("ncu_us", {}).get(config_name, {})
     except (OSError, ValueError):
         return {}
@@ -56,8 +56,8 @@ def ncu_mover_us(config_name: str):
 
 def ncu_traffic(config_name: str, task: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the task's kernel from the committed `ncu --set full`
-    capture (profiles/r1d_traffic.json.txt names its source), or None when no capture exists for this workload."""
-    p = os.path.join(ROOT, "profiles", "r1d_traffic.json.txt")
+    capture (profiles/r1e_traffic.json.txt names its source), or None when no capture exists for this workload."""
+    p = os.path.join(ROOT, "profiles", "r1e_traffic.json.txt")
     try:
         with open(p) as f:
             return json.load(f).get(config_name, {}).get(task)
