@@ -100,6 +100,19 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             : "memory");
     } while (!done);
 }
+// the same wait with cluster-scope acquire: pairs with a peer CTA's st.shared::cluster + mbarrier.arrive.release.cluster
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -678,7 +691,7 @@ struct TileFeed {
     uint32_t empty_addr;  // cluster address of the leader's empty barriers [kFeed]
     int stride = 1;       // ints per slot
     __device__ __forceinline__ int peek(int it) const {
-        mbar_wait(&full[it & (kFeed - 1)], (it / kFeed) & 1);
+        mbar_wait_cluster(&full[it & (kFeed - 1)], (it / kFeed) & 1);
         return *reinterpret_cast<volatile int*>(&ids[(it & (kFeed - 1)) * stride]);
     }
     // words 1.. of the slot of tile `it` (valid between peek(it) and this warp's release in take(it))
