@@ -14,8 +14,11 @@
  * Conventions (all entry points):
  *  - return value: PIPER_OK or a negative PIPER_ERR_* code; never throws, never aborts;
  *  - every tensor pointer is a DEVICE pointer owned by the caller, 16-byte aligned, row-major,
- *    contiguous; the library never allocates or frees device memory after piper_create() and never
- *    frees caller memory; `workspace` (device, caller-owned) must outlive the context;
+ *    contiguous; the library never allocates or frees device memory and never frees caller memory;
+ *    `workspace` (device, caller-owned) must outlive the context.  Host-side CUDA objects (events, the
+ *    side stream of piper_set_chunk_overlap) are created in piper_create(); the SM partitions and
+ *    streams of step P are created by piper_pair_prepare() (or by the first piper_run_chunk_pair() of a
+ *    split, which therefore must not run inside a stream capture); no other call creates anything;
  *  - `stream` is a cudaStream_t passed as void*; calls only enqueue work: no host synchronisation,
  *    no host read-back of device data (the packed row count A lives on the device in
  *    offsets[E_loc]), so a sequence of calls can be captured in a CUDA graph and replayed;
@@ -27,7 +30,10 @@
  *  - preconditions checked on the host: shapes > 0, k <= E, k <= 8, E <= 512, d % 8 == 0, I % 8 == 0,
  *    I_shared % 8 == 0, pointers non-null and 16-byte aligned.  Logits must be finite (or -inf with
  *    at least k finite entries per row, reading c-7); the device does not validate data;
- *  - a piper_ctx is not thread-safe.
+ *  - a piper_ctx is not thread-safe.  Calls of one context may go to different streams and run
+ *    concurrently on the device (every GEMM launch takes the tile counters of its own stream; up to 64
+ *    streams / captured graphs per context are tracked, the least recently used entry is recycled
+ *    beyond that).
  */
 #ifndef PIPER_H_
 #define PIPER_H_
@@ -52,8 +58,11 @@ extern "C" {
 #define PIPER_GATE_SIGMOID_RENORM 1 /* s_j = 1/(1+exp(-z_j)); g_j = s_j / sum_{j'<k} s_j'           */
 #define PIPER_GATE_SOFTMAX_FULL 2   /* g_j = exp(z_j - m) / sum_{e<E} exp(z_e - m)                  */
 
-#define PIPER_GEMM_AUTO 0 /* bf16: tcgen05/TMEM/TMA kernels; fp32: FP32-ALU kernels (1e-5 bar)     */
-#define PIPER_GEMM_SIMT 1 /* force the FP32-ALU grouped GEMM (debug cross-check of the tcgen05 path) */
+#define PIPER_GEMM_AUTO 0 /* bf16: tcgen05/TMEM/TMA kernels; fp32: FP32-ALU kernels (1e-5 bar).  A bf16 layer the
+                           * tcgen05 kernels cannot take (row_align % 16 != 0 with more than one local expert,
+                           * d or I < 64) is refused by piper_create with PIPER_ERR_UNSUPPORTED instead of
+                           * silently running ~100x slower: ask for PIPER_GEMM_SIMT explicitly.               */
+#define PIPER_GEMM_SIMT 1 /* the FP32-ALU grouped GEMM for any dtype / row_align (cross-check of the tcgen05 path) */
 
 typedef struct piper_ctx piper_ctx;
 
@@ -79,9 +88,28 @@ const char* piper_last_cuda_error(const piper_ctx* ctx);
 int64_t piper_kernel_launches(const piper_ctx* ctx);
 /* Which GEMM family serves the routed experts of this context: 1 = tcgen05/TMEM/TMA, 0 = FP32 ALUs. */
 int piper_gemm_path(const piper_ctx* ctx);
-/* Debug (PIPER_TC_PROFILE=1 in the environment at piper_create): device pointer to the wait-cycle counters
- * the tcgen05 kernels wrote, [16 launches (cycled)][160 CTAs][8] int64; NULL when profiling is off. */
+/* Debug (PIPER_OPT_TC_PROFILE = 1): device pointer to the wait-cycle counters the tcgen05 kernels wrote,
+ * [16 launches (cycled)][160 CTAs][8] int64; NULL when profiling is off. */
 const void* piper_debug_tc_counters(const piper_ctx* ctx);
+/* Kernel-variant switches of a context (host state; nothing is read from the environment).  Defaults in brackets.
+ *  PIPER_OPT_TC_ROWS_ON_N [1]  rows-on-N CTA-pair kernels for fwd / dgrad; 0 = rows-on-M kernels (row_align % 128 only)
+ *  PIPER_OPT_TC_2CTA      [2]  CTA-pair kernels: 0 never (1-CTA kernels; bf16 dW, row_align % 128 only), 1 always,
+ *                              2 by expected group length
+ *  PIPER_OPT_T_SMALL_ROWS [32] rows-on-N: chunks of at most this many rows per CTA load 32-row boxes
+ *  PIPER_OPT_T_GREEDY     [1]  rows-on-N: 1 = 256-row chunks and a short last one, 0 = equal chunks
+ *  PIPER_OPT_TC_PROFILE   [0]  1 = the tcgen05 kernels record wait-cycle counters (piper_debug_tc_counters)
+ *  PIPER_OPT_FUSED_GATHER [1]  chunk calls on tcgen05 layers: 1 = the GEMMs gather x / dY rows themselves
+ *                              (N2 fusion), 0 = they read the packed buffers xp / d_o
+ * Returns PIPER_ERR_INVALID for unknown options / values, PIPER_ERR_UNSUPPORTED when the layer cannot run the
+ * variant (e.g. fp32 dW without the CTA-pair wgrad). */
+#define PIPER_OPT_TC_ROWS_ON_N 0
+#define PIPER_OPT_TC_2CTA 1
+#define PIPER_OPT_T_SMALL_ROWS 2
+#define PIPER_OPT_T_GREEDY 3
+#define PIPER_OPT_TC_PROFILE 4
+#define PIPER_OPT_FUSED_GATHER 5
+int piper_set_option(piper_ctx* ctx, int option, int value);
+int piper_get_option(const piper_ctx* ctx, int option, int* value);
 /* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */
 int64_t piper_a_cap(const piper_moe_desc* desc);
 
@@ -169,6 +197,13 @@ typedef struct {
  * the serial baseline of step P. */
 int piper_run_chunk_fwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
 int piper_run_chunk_bwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
+/* The backward chunk split into the paper's two passes (PASS = Bi, Bw; Fig. 3; SURVEY.md
+ * §8f N3): _input runs everything the upstream layer waits for (combine_bwd, dgrad-1, dgrad-2, the shared expert's
+ * dgrads, unpack, route_bwd -> dX, dgates, dz_sel), _weight the weight gradients (routed and shared wgrad -> dW_*), which
+ * a schedule may delay to fill bubbles.  _weight needs the scratch _input left in `a` (d_o / dg / du / dgs / dus).
+ * _input followed by _weight is bit-identical to piper_run_chunk_bwd. */
+int piper_run_chunk_bwd_input(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
+int piper_run_chunk_bwd_weight(piper_ctx* ctx, const piper_chunk_args* a, void* stream);
 
 /* P run_chunk_pair (SURVEY.md §8a P, §8c c-sched; north_star part 5).  Enqueues the forward chunk of
  * `fwd_mb` and the backward chunk of `bwd_mb` as the 14-task DAG of SURVEY.md §8c on two logical
@@ -181,6 +216,17 @@ int piper_run_chunk_bwd(piper_ctx* ctx, const piper_chunk_args* a, void* stream)
  * piper_run_chunk_fwd + piper_run_chunk_bwd. */
 int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const piper_chunk_args* bwd_mb, int sm_gemm,
                          int sm_comm, void* stream);
+/* Creates the SM partitions (green contexts), their streams and the schedule for a split ahead of time, so that
+ * piper_run_chunk_pair with the same split and policy creates nothing (and can be captured in a CUDA graph).  The last
+ * prepared split is kept; another split, or another partition policy, releases it.  PIPER_ERR_UNSUPPORTED when
+ * PIPER_PART_EXCLUSIVE cannot be honoured (no green contexts, or the driver cannot split off these SM counts). */
+int piper_pair_prepare(piper_ctx* ctx, int sm_gemm, int sm_comm);
+/* Which pass of microbatch B the pair overlaps with the forward chunk (host state, default PIPER_PASS_B):
+ * PIPER_PASS_BI runs F || Bi (Fig. 3b) and leaves the weight gradients to a later
+ * piper_run_chunk_bwd_weight(bwd_mb). */
+#define PIPER_PASS_B 0
+#define PIPER_PASS_BI 1
+int piper_set_pair_bwd_pass(piper_ctx* ctx, int pass);
 
 /* Policy of piper_run_chunk_pair (host state of `ctx`; default = the paper's: PIPER_ORDER_LIST, PIPER_PART_EXCLUSIVE).
  *  order     PIPER_ORDER_LIST    Piper's list scheduling, ready task with the most descendants first.
@@ -190,7 +236,9 @@ int piper_run_chunk_pair(piper_ctx* ctx, const piper_chunk_args* fwd_mb, const p
  *                                `task_ms` [14] (PIPER_TASK_* order, milliseconds on the whole device; the library
  *                                scales them to the partition sizes) or, when task_ms is NULL, under the library's
  *                                own estimate from the algorithmic FLOPs and bytes of the descriptor.
- *  partition PIPER_PART_EXCLUSIVE  disjoint SM sets (green contexts; sm_gemm + sm_comm <= SM count).
+ *  partition PIPER_PART_EXCLUSIVE  disjoint SM sets (green contexts; sm_gemm + sm_comm <= SM count; sm_comm a multiple
+ *                                  of 8, sm_gemm a multiple of 8 or the whole remainder).  When the driver cannot
+ *                                  provide them the call fails with PIPER_ERR_UNSUPPORTED: no silent fallback.
  *            PIPER_PART_SHARED     two plain streams, every grid bounded to its side's SM count worth of CTAs; the
  *                                  sides may overlap (sm_gemm + sm_comm may exceed the SM count): pack/combine CTAs
  *                                  become co-resident with the persistent GEMM CTAs, as in the paper, which leaves SM
@@ -240,9 +288,9 @@ int piper_set_wgrad_accumulate(piper_ctx* ctx, int accumulate);
  * bit-identical.  Returns PIPER_ERR_INVALID for other values, PIPER_ERR_CUDA if the stream cannot be created. */
 int piper_set_chunk_overlap(piper_ctx* ctx, int on);
 
-/* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts, 2 = bounded persistent
- * grids on two plain streams (green contexts unavailable, or PIPER_PART_SHARED), 3 = one stream per chunk
- * (PIPER_PART_CHUNK_STREAMS), 0 = never called. */
+/* How the last piper_run_chunk_pair partitioned the SMs: 1 = green contexts (PIPER_PART_EXCLUSIVE), 2 = bounded
+ * persistent grids on two plain streams (PIPER_PART_SHARED), 3 = one stream per chunk (PIPER_PART_CHUNK_STREAMS),
+ * 0 = never called. */
 int piper_pair_partition_mode(const piper_ctx* ctx);
 
 /* Host-only list scheduler used by piper_run_chunk_pair (reading c-21),

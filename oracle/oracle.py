@@ -296,6 +296,33 @@ def sample_tokens(cfg, inp, rt, tokens, backward_too=True):
     return out
 
 
+def sample_rows(cfg, inp, rt, rows, backward_too=True):
+    """O[r] (and dXp[r], dG[r], dU[r]) for the listed non-pad packed rows, each from the definition directly:
+    row r holds token src_of[r] // k at expert topk_idx[src_of[r]]; dO[r] = gates[src_of[r]] * dY[token]."""
+    rows = np.asarray(rows, np.int64)
+    a = rt["src_of"][rows].astype(np.int64)
+    assert (a >= 0).all(), "sample_rows wants non-pad rows"
+    tok = a // cfg.k
+    ex = (rt["topk_idx"].reshape(-1)[a] - cfg.e_lo).astype(np.int32)
+    X = _f64(inp["x"][tok])
+    f = ffn_fwd_rows(cfg, cfg.I, X, ex, inp["w_gate"], inp["w_up"], inp["w_down"])
+    out = {"rows": rows, "tokens": tok, "o": f["O"], "g": f["G"], "u": f["U"], "h": f["H"]}
+    if backward_too:
+        dO = rt["gates"].reshape(-1)[a][:, None] * _f64(inp["dy"][tok])
+        dXp, dG, dU, _ = ffn_bwd_rows(cfg, cfg.I, X, ex, dO, inp["w_gate"], inp["w_up"], inp["w_down"])
+        out.update(dxp=dXp, dg=dG, du=dU)
+    return out
+
+
+def sample_route_bwd(cfg, inp, rt, tokens, dgates):
+    """dz_sel[t] for the listed tokens from the oracle's dgates[t] (gate backward is per token)."""
+    import dataclasses
+    tokens = np.asarray(tokens, np.int64)
+    sub = dataclasses.replace(cfg, T=len(tokens))
+    return route_bwd(sub, np.ascontiguousarray(inp["logits"][tokens]), np.ascontiguousarray(rt["topk_idx"][tokens]),
+                     np.ascontiguousarray(dgates))
+
+
 def sample_wgrad(cfg, inp, rt, e_local, J):
     """dW_gate[e][:, J], dW_up[e][:, J] ([d, nJ]) and dW_down[e][J, :] ([nJ, d]) for local expert e_local."""
     lo, cnt = int(rt["offsets"][e_local]), int(rt["counts"][e_local])

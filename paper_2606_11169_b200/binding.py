@@ -58,6 +58,7 @@ def lib() -> ctypes.CDLL:
         L.piper_a_cap.restype = ctypes.c_int64
         L.piper_kernel_launches.restype = ctypes.c_int64
         L.piper_last_cuda_error.restype = ctypes.c_char_p
+        L.piper_debug_tc_counters.restype = ctypes.c_void_p
         _lib = L
     return _lib
 
@@ -123,7 +124,7 @@ class Context:
 
     def check(self, rc: int, what: str):
         if rc != PIPER_OK:
-            msg = lib().piper_last_cuda_error(self._h).decode() if rc == -4 else ""
+            msg = lib().piper_last_cuda_error(self._h).decode() if rc in (-4, -2) else ""
             raise PiperError(f"{what}: status {rc} {msg}")
 
 
@@ -215,6 +216,38 @@ def piper_run_chunk_fwd(ctx, args: ChunkArgs, stream=None):
 
 def piper_run_chunk_bwd(ctx, args: ChunkArgs, stream=None):
     ctx.check(lib().piper_run_chunk_bwd(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_bwd")
+
+
+def piper_run_chunk_bwd_input(ctx, args: ChunkArgs, stream=None):
+    ctx.check(lib().piper_run_chunk_bwd_input(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_bwd_input")
+
+
+def piper_run_chunk_bwd_weight(ctx, args: ChunkArgs, stream=None):
+    ctx.check(lib().piper_run_chunk_bwd_weight(ctx._h, ctypes.byref(args), _stream(stream)), "piper_run_chunk_bwd_weight")
+
+
+PASS_B, PASS_BI = 0, 1
+
+
+def piper_set_pair_bwd_pass(ctx, bwd_pass: int):
+    ctx.check(lib().piper_set_pair_bwd_pass(ctx._h, int(bwd_pass)), "piper_set_pair_bwd_pass")
+
+
+def piper_pair_prepare(ctx, sm_gemm: int, sm_comm: int):
+    ctx.check(lib().piper_pair_prepare(ctx._h, int(sm_gemm), int(sm_comm)), "piper_pair_prepare")
+
+
+OPT_TC_ROWS_ON_N, OPT_TC_2CTA, OPT_T_SMALL_ROWS, OPT_T_GREEDY, OPT_TC_PROFILE, OPT_FUSED_GATHER = range(6)
+
+
+def piper_set_option(ctx, option: int, value: int):
+    ctx.check(lib().piper_set_option(ctx._h, int(option), int(value)), "piper_set_option")
+
+
+def piper_get_option(ctx, option: int) -> int:
+    v = _i32(0)
+    ctx.check(lib().piper_get_option(ctx._h, int(option), ctypes.byref(v)), "piper_get_option")
+    return int(v.value)
 
 
 TASKS = ("F_ROUTE", "F_SCAN", "F_PACK", "F_GEMM1", "F_GEMM2", "F_SHARED", "F_COMBINE", "B_CGRAD", "B_DGRAD1",

@@ -25,14 +25,13 @@ inline int n_chunks_of(const piper_moe_desc* D) { return cdiv(D->T * D->k, kScan
 inline size_t round256(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t chunk_counts, chunk_base, shared_offsets, tc_scratch, total;
+    size_t chunk_counts, chunk_counts_per, shared_offsets, tc_scratch, total;
 };
 WsLayout ws_layout(const piper_moe_desc* D) {
     WsLayout L{};
     const size_t per = round256(sizeof(int32_t) * (size_t)n_chunks_of(D) * D->E_loc);
     size_t at = 0;
-    L.chunk_counts = at, at += per;
-    L.chunk_base = at, at += per;
+    L.chunk_counts = at, L.chunk_counts_per = per, at += per * kSchedSlots;
     L.shared_offsets = at, at += 256;
     L.tc_scratch = at, at += tc_scratch_bytes(D);
     L.total = at;
@@ -46,7 +45,51 @@ bool all_aligned(P... ptrs) {
 
 inline Lane full_lane(piper_ctx* c, void* stream) { return Lane{static_cast<cudaStream_t>(stream), c->num_sms}; }
 
+// Can this context's kernel variants serve its layer?  A bf16 layer under PIPER_GEMM_AUTO must run on the tcgen05
+// kernels (no silent ~100x slower path), and fp32 dW of a bf16 layer exists only in the CTA-pair wgrad.
+int variant_ok(const piper_ctx* c) {
+    if (c->D.dtype != PIPER_DTYPE_BF16) return PIPER_OK;
+    piper_chunk_args a{};
+    const FfnProblem p = routed_problem(c, &a);
+    const bool tc = c->D.gemm_impl == PIPER_GEMM_AUTO && tc_supported(c, p);
+    if (c->D.gemm_impl == PIPER_GEMM_AUTO && !tc) return PIPER_ERR_UNSUPPORTED;
+    if (c->D.dw_dtype == PIPER_DTYPE_F32 && !(tc && tc_wgrad_f32_ok(c, p))) return PIPER_ERR_UNSUPPORTED;
+    return PIPER_OK;
+}
+
 }  // namespace
+
+namespace piper {
+
+int stream_slot(piper_ctx* c, cudaStream_t stream) {
+    unsigned long long cap_id = 0;
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamGetCaptureInfo(stream, &st, &cap_id) != cudaSuccess) cudaGetLastError(), st = cudaStreamCaptureStatusNone;
+    if (st != cudaStreamCaptureStatusActive) cap_id = 0;
+    int match = -1, free_slot = -1, lru = 0;
+    for (int i = 0; i < kSchedSlots; ++i) {
+        const SchedSlot& e = c->sched_slots[i];
+        if (!e.used) {
+            if (free_slot < 0) free_slot = i;
+        } else if (e.stream == stream && e.capture_id == cap_id) {
+            match = i;
+            break;
+        } else if (e.last_use < c->sched_slots[lru].last_use || !c->sched_slots[lru].used) {
+            lru = i;
+        }
+    }
+    // no entry yet: a free one, else the least recently used stream / graph gives up its slot
+    const int pick = match >= 0 ? match : (free_slot >= 0 ? free_slot : lru);
+    SchedSlot& e = c->sched_slots[pick];
+    e.used = true, e.stream = stream, e.capture_id = cap_id, e.last_use = ++c->sched_clock;
+    return pick;
+}
+
+int32_t* scan_scratch(piper_ctx* c, cudaStream_t stream) {
+    return c->chunk_counts + (size_t)stream_slot(c, stream) * c->chunk_counts_stride;
+}
+
+}  // namespace piper
 
 extern "C" {
 
@@ -77,7 +120,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
     c->ws_bytes = workspace_bytes;
     c->n_chunks = n_chunks_of(D);
     c->chunk_counts = reinterpret_cast<int32_t*>(c->ws + L.chunk_counts);
-    c->chunk_base = reinterpret_cast<int32_t*>(c->ws + L.chunk_base);
+    c->chunk_counts_stride = L.chunk_counts_per / sizeof(int32_t);
     c->shared_offsets = reinterpret_cast<int32_t*>(c->ws + L.shared_offsets);
     c->tc_scratch = c->ws + L.tc_scratch;
     bool ok = cudaSetDevice(device) == cudaSuccess &&
@@ -86,10 +129,17 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
     ok = ok && cudaMemcpy(c->shared_offsets, so, sizeof(so), cudaMemcpyHostToDevice) == cudaSuccess;
     for (int i = 0; ok && i < kMaxEvents; ++i)
         ok = cudaEventCreateWithFlags(&c->events[i], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && tc_init(c) == PIPER_OK;
     if (!ok) {
         piper_destroy(c);
         return PIPER_ERR_CUDA;
+    }
+    c->fused_gather = 1;
+    const int rc = variant_ok(c);
+    if (rc != PIPER_OK) {
+        piper_destroy(c);
+        return rc;
     }
     *out = c;
     return PIPER_OK;
@@ -98,6 +148,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
 int piper_destroy(piper_ctx* c) {
     if (!c) return PIPER_ERR_INVALID;
     pair_release(c);
+    tc_release(c);
     if (c->side_stream) cudaStreamDestroy(c->side_stream);
     for (int i = 0; i < kMaxEvents; ++i)
         if (c->events[i]) cudaEventDestroy(c->events[i]);
@@ -113,10 +164,41 @@ int piper_gemm_path(const piper_ctx* c) {
     return tc_supported(c, routed_problem(c, &a)) ? 1 : 0;
 }
 const void* piper_debug_tc_counters(const piper_ctx* c) { return c && c->tc_prof ? c->tc_scratch : nullptr; }
+
+int piper_get_option(const piper_ctx* c, int option, int* value) {
+    if (!c || !value) return PIPER_ERR_INVALID;
+    switch (option) {
+        case PIPER_OPT_TC_ROWS_ON_N: *value = c->tc_rows_on_n; return PIPER_OK;
+        case PIPER_OPT_TC_2CTA: *value = c->tc_two_cta; return PIPER_OK;
+        case PIPER_OPT_T_SMALL_ROWS: *value = c->tc_small_rows; return PIPER_OK;
+        case PIPER_OPT_T_GREEDY: *value = c->tc_greedy; return PIPER_OK;
+        case PIPER_OPT_TC_PROFILE: *value = c->tc_prof; return PIPER_OK;
+        case PIPER_OPT_FUSED_GATHER: *value = c->fused_gather; return PIPER_OK;
+    }
+    return PIPER_ERR_INVALID;
+}
+
+int piper_set_option(piper_ctx* c, int option, int value) {
+    int old = 0;
+    if (piper_get_option(c, option, &old) != PIPER_OK) return PIPER_ERR_INVALID;
+    int* field = nullptr;
+    switch (option) {
+        case PIPER_OPT_TC_ROWS_ON_N: field = &c->tc_rows_on_n; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_TC_2CTA: field = &c->tc_two_cta; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_T_SMALL_ROWS: field = &c->tc_small_rows; if (value < 0 || value > 128) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_T_GREEDY: field = &c->tc_greedy; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_TC_PROFILE: field = &c->tc_prof; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+    }
+    *field = value;
+    const int rc = variant_ok(c);  // e.g. row_align 16 needs the rows-on-N + CTA-pair kernels, fp32 dW the CTA-pair wgrad
+    if (rc != PIPER_OK) *field = old;
+    return rc;
+}
 int piper_pair_partition_mode(const piper_ctx* c) { return c ? c->pair_mode : 0; }
 int piper_set_wgrad_accumulate(piper_ctx* c, int accumulate) {
     if (!c || (accumulate != 0 && accumulate != 1)) return PIPER_ERR_INVALID;
-    if (accumulate && c->D.dw_dtype != PIPER_DTYPE_F32) return PIPER_ERR_UNSUPPORTED;
+    if (accumulate && (c->D.dw_dtype != PIPER_DTYPE_F32 || c->D.dtype != PIPER_DTYPE_BF16)) return PIPER_ERR_UNSUPPORTED;
     c->wgrad_accumulate = accumulate;
     return PIPER_OK;
 }

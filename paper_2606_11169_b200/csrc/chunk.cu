@@ -60,10 +60,10 @@ DriverApi& driver() {
     return d;
 }
 
-void destroy_partition(GreenPartition* g) {
+void destroy_partition(piper_ctx* c, GreenPartition* g) {
     if (!g) return;
     for (int i = 0; i < 2; ++i) {
-        if (g->stream[i]) cudaStreamDestroy(g->stream[i]);
+        if (g->stream[i]) tc_forget_stream(c, g->stream[i]), cudaStreamDestroy(g->stream[i]);
         if (g->gctx[i] && driver().ok) driver().GreenCtxDestroy(g->gctx[i]);
     }
     delete g;
@@ -102,15 +102,19 @@ GreenPartition* make_partition(piper_ctx* c, int sm_gemm, int sm_comm, bool want
         g->green = true;
         return g;
     }
-    // fallback: plain streams, grids bounded by Lane::sms
     for (int i = 0; i < 2; ++i) {
         if (g->stream[i]) cudaStreamDestroy(g->stream[i]), g->stream[i] = nullptr;
         if (g->gctx[i] && api.ok) api.GreenCtxDestroy(g->gctx[i]), g->gctx[i] = nullptr;
     }
     cudaGetLastError();
+    if (want_green) {  // disjoint SM sets were asked for and cannot be had: no silent fallback
+        delete g;
+        return nullptr;
+    }
+    // PIPER_PART_SHARED / _CHUNK_STREAMS: plain streams, grids bounded by Lane::sms
     for (int i = 0; i < 2; ++i)
         if (cudaStreamCreateWithFlags(&g->stream[i], cudaStreamNonBlocking) != cudaSuccess) {
-            destroy_partition(g);
+            destroy_partition(c, g);
             return nullptr;
         }
     g->green = false;
@@ -129,7 +133,9 @@ const int kEdges[][2] = {{F_ROUTE, F_SCAN},   {F_SCAN, F_PACK},    {F_PACK, F_GE
                          {B_CGRAD, B_DGRAD1},  {B_DGRAD1, B_DGRAD2}, {B_DGRAD2, B_UNPACK},  {B_CGRAD, B_WGRAD},
                          {B_DGRAD1, B_WGRAD},  {B_SHARED, B_UNPACK}, {B_CGRAD, B_ROUTE_BWD}};
 
-int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b) {
+// `parts` of the backward tasks that hold both passes (B_SHARED): bit 0 = input gradients (Bi), bit 1 = weight gradients (Bw)
+constexpr int PART_BI = 1, PART_BW = 2, PART_ALL = 3;
+int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b, int parts = PART_ALL) {
     switch (task) {
         case F_ROUTE: return launch_route_topk(c, ln, f->logits, f->topk_idx, f->gates, f->counts_global);
         case F_SCAN: return launch_scan_rank(c, ln, f->topk_idx, f->counts, f->offsets, f->row_of, f->src_of);
@@ -150,9 +156,12 @@ int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const p
         case B_WGRAD: return ffn_wgrad(c, ln, routed_problem(c, b));
         case B_SHARED: {
             const FfnProblem p = shared_problem(c, b);
-            int rc = ffn_dgrad1(c, ln, p);
-            if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
-            if (rc == PIPER_OK) rc = ffn_wgrad(c, ln, p);
+            int rc = PIPER_OK;
+            if (parts & PART_BI) {
+                rc = ffn_dgrad1(c, ln, p);
+                if (rc == PIPER_OK) rc = ffn_dgrad2(c, ln, p);
+            }
+            if (rc == PIPER_OK && (parts & PART_BW)) rc = ffn_wgrad(c, ln, p);
             return rc;
         }
         case B_UNPACK:
@@ -196,7 +205,7 @@ void pair_plan_release(piper_ctx* c) {
 }
 
 void pair_release(piper_ctx* c) {
-    destroy_partition(c->green);
+    destroy_partition(c, c->green);
     c->green = nullptr;
     pair_plan_release(c);
 }
@@ -207,9 +216,7 @@ extern "C" {
 
 int piper_set_chunk_overlap(piper_ctx* c, int on) {
     if (!c || (on != 0 && on != 1)) return PIPER_ERR_INVALID;
-    if (on && !c->side_stream && cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess)
-        return cuda_fail(c, cudaGetLastError(), "cudaStreamCreateWithFlags");
-    c->chunk_overlap = on;
+    c->chunk_overlap = on;  // the side stream exists since piper_create
     return PIPER_OK;
 }
 
@@ -287,6 +294,33 @@ int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     return PIPER_OK;
 }
 
+int piper_run_chunk_bwd_input(piper_ctx* c, const piper_chunk_args* a, void* stream) {
+    if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
+    const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+    for (int t : seq) {
+        if (t == B_SHARED && !c->D.I_shared) continue;
+        const int rc = run_task(c, t, ln, nullptr, a, PART_BI);
+        if (rc != PIPER_OK) return rc;
+    }
+    return PIPER_OK;
+}
+
+int piper_run_chunk_bwd_weight(piper_ctx* c, const piper_chunk_args* a, void* stream) {
+    if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
+    const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
+    int rc = run_task(c, B_WGRAD, ln, nullptr, a);
+    if (rc == PIPER_OK && c->D.I_shared) rc = run_task(c, B_SHARED, ln, nullptr, a, PART_BW);
+    return rc;
+}
+
+int piper_set_pair_bwd_pass(piper_ctx* c, int pass) {
+    if (!c || (pass != PIPER_PASS_B && pass != PIPER_PASS_BI)) return PIPER_ERR_INVALID;
+    if (pass != c->pair_bwd_pass) pair_plan_release(c);
+    c->pair_bwd_pass = pass;
+    return PIPER_OK;
+}
+
 namespace {
 
 // Task durations in ms on the whole device: the caller's profile, else an estimate from the algorithmic work
@@ -332,6 +366,7 @@ int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
     for (int t = 0; t < N_TASKS; ++t) {
         id_of[t] = -1;
         if (!shared && (t == F_SHARED || t == B_SHARED)) continue;
+        if (t == B_WGRAD && c->pair_bwd_pass == PIPER_PASS_BI) continue;  // F || Bi: the weight gradients run later
         id_of[t] = n, pl->task_of[n] = t, ++n;
     }
     pl->n = n;
@@ -350,13 +385,31 @@ int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
     const float fg = (float)c->num_sms / (float)(sm_gemm < c->num_sms ? sm_gemm : c->num_sms);
     const float fc = sm_comm * 3 >= c->num_sms ? 1.f : (float)c->num_sms / (3.f * (float)sm_comm);
     for (int i = 0; i < n; ++i) dur[i] = full[pl->task_of[i]] * (pl->stream_of[i] == GEMM ? fg : fc);
+    if (c->pair_bwd_pass == PIPER_PASS_BI && id_of[B_SHARED] >= 0) dur[id_of[B_SHARED]] *= 2.f / 3.f;  // dgrads only
     return piper_schedule_search(n, n_edges, &edges[0][0], pl->stream_of, dur, pl->order, &pl->waits[0][0], &pl->n_waits,
                                  pl->records, nullptr);
 }
 
 bool split_ok(const piper_ctx* c, int sm_gemm, int sm_comm) {
     if (sm_gemm < 1 || sm_comm < 8 || sm_comm % 8 || sm_gemm > c->num_sms || sm_comm > c->num_sms) return false;
-    return c->pair_part != PIPER_PART_EXCLUSIVE || sm_gemm + sm_comm <= c->num_sms;
+    if (c->pair_part != PIPER_PART_EXCLUSIVE) return true;
+    // disjoint green-context partitions come in multiples of 8 SMs; the GEMM side may instead take the whole remainder
+    return sm_gemm + sm_comm <= c->num_sms && (sm_gemm % 8 == 0 || sm_gemm + sm_comm == c->num_sms);
+}
+
+// Partition + streams + schedule of a split (created once, kept until the split or the partition policy changes).
+int pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+    if (!split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
+    if (!c->green || c->green->sm_gemm != sm_gemm || c->green->sm_comm != sm_comm) {
+        pair_release(c);
+        c->green = make_partition(c, sm_gemm, sm_comm, c->pair_part == PIPER_PART_EXCLUSIVE);
+        if (!c->green) {
+            snprintf(c->err, sizeof(c->err), "SM partition %d:%d unavailable (%s)", sm_gemm, sm_comm,
+                     c->pair_part == PIPER_PART_EXCLUSIVE ? "green contexts" : "stream creation");
+            return c->pair_part == PIPER_PART_EXCLUSIVE ? PIPER_ERR_UNSUPPORTED : PIPER_ERR_CUDA;
+        }
+    }
+    return make_plan(c, sm_gemm, sm_comm, pl);
 }
 
 }  // namespace
@@ -386,20 +439,21 @@ int piper_pair_order(piper_ctx* c, int sm_gemm, int sm_comm, int32_t* order, int
     return PIPER_OK;
 }
 
+int piper_pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm) {
+    if (!c) return PIPER_ERR_INVALID;
+    PairPlan pl;
+    return pair_prepare(c, sm_gemm, sm_comm, &pl);
+}
+
 int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_chunk_args* b, int sm_gemm, int sm_comm,
                          void* stream) {
     if (!c || !fwd_args_ok(c, f) || !bwd_args_ok(c, b)) return PIPER_ERR_INVALID;
-    if (!split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
-    if (!c->green || c->green->sm_gemm != sm_gemm || c->green->sm_comm != sm_comm) {
-        pair_release(c);
-        c->green = make_partition(c, sm_gemm, sm_comm, c->pair_part == PIPER_PART_EXCLUSIVE);
-        if (!c->green) return cuda_fail(c, cudaErrorUnknown, "make_partition");
-    }
+    PairPlan pl;
+    int rc = pair_prepare(c, sm_gemm, sm_comm, &pl);
+    if (rc != PIPER_OK) return rc;
     GreenPartition* g = c->green;
     c->pair_mode = c->pair_part == PIPER_PART_CHUNK_STREAMS ? 3 : (g->green ? 1 : 2);
-    PairPlan pl;
-    int rc = make_plan(c, sm_gemm, sm_comm, &pl);
-    if (rc != PIPER_OK) return rc;
+    const int parts = c->pair_bwd_pass == PIPER_PASS_BI ? PART_BI : PART_ALL;
 
     cudaStream_t user = static_cast<cudaStream_t>(stream);
     if (c->pair_part == PIPER_PART_CHUNK_STREAMS) {
@@ -420,8 +474,8 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
                 rc = run_task(c, fseq[i], lf, f, b);
                 if (rc != PIPER_OK) return rc;
             }
-            if (bseq[i] != B_SHARED || c->D.I_shared) {
-                rc = run_task(c, bseq[i], lb, f, b);
+            if ((bseq[i] != B_SHARED || c->D.I_shared) && !(bseq[i] == B_WGRAD && parts == PART_BI)) {
+                rc = run_task(c, bseq[i], lb, f, b, parts);
                 if (rc != PIPER_OK) return rc;
             }
         }
@@ -442,7 +496,7 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
         const Lane ln = lanes[pl.stream_of[v]];
         for (int w = 0; w < pl.n_waits; ++w)  // wait for dependencies that ran on another stream
             if (pl.waits[w][1] == v) PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, c->events[pl.waits[w][0]], 0));
-        rc = run_task(c, pl.task_of[v], ln, f, b);
+        rc = run_task(c, pl.task_of[v], ln, f, b, parts);
         if (rc != PIPER_OK) return rc;
         if (pl.records[v]) PIPER_CUDA(c, cudaEventRecord(c->events[v], ln.stream));
     }

@@ -12,8 +12,8 @@
 //                   pair), the expert's rows on N in multiples of 16; transposing TMA-store epilogues.
 //  tc_gemm2_kernel  CTA pair, 256 x 256 tiles: wgrad (K = the expert's rows, both operands MN-major, K blocks of
 //                   128); TMEM -> swizzled shared memory -> TMA-store epilogue.  Also the rows-on-M form of the
-//                   four contractions above (PIPER_TC_ROWS_ON_N=0).
-//  tc_gemm_kernel   1-CTA 128 x 256 tiles, direct-store epilogue: fallback (> 192 groups, PIPER_TC_2CTA=0).
+//                   four contractions above (PIPER_OPT_TC_ROWS_ON_N = 0).
+//  tc_gemm_kernel   1-CTA 128 x 256 tiles, direct-store epilogue: fallback (> 192 groups, PIPER_OPT_TC_2CTA = 0).
 // Operand layouts are taken as they lie in memory (no transposed copies): the descriptors select K-major
 // or MN-major per operand.  In the rows-on-M form:
 //   fwd1   G|U = Xp Wg | Xp Wu      A K-major  (Xp [rows,d]),   B MN-major (W [d,I], two 128-col halves)
@@ -38,7 +38,6 @@ constexpr int kThreads = 256;
 constexpr int kMaxGroups = kMaxE;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/ +
                            (kMaxGroups + 1) * 4 /*tile prefix*/;
-constexpr int kSchedSlots = 32;  // {next tile, clusters done} counter pairs of the dynamically scheduled kernels
 constexpr int kProfSlots = 16, kProfSlotWords = 160 * 8;  // debug counters: 16 launches x 160 CTAs x 8 words
 constexpr int PANEL_M = 8;  // M tiles per panel of the tile order (L2 reuse of the weight tile)
 
@@ -64,7 +63,7 @@ struct alignas(64) TcParams {
     long long group_stride;  // wgrad: elements between two experts' dW
     __nv_bfloat16 *out0, *out1, *out2;
     const __nv_bfloat16 *in0, *in1;
-    long long* prof;  // debug (PIPER_TC_PROFILE=1): [gridDim.x][8] wait-cycle counters, else NULL
+    long long* prof;  // debug (PIPER_OPT_TC_PROFILE): [gridDim.x][8] wait-cycle counters, else NULL
     // rows-on-N kernel (tc_gemmT_kernel)
     const int32_t* counts;  // [G] device: real rows per group
     int f_tiles;            // tiles along the feature (output column) dimension
@@ -1599,8 +1598,43 @@ using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
 
 // bf16 tensor [groups][rows][inner] (row-major), box = box_inner elements x box_rows rows; 128-byte swizzle when the
 // box is 64 elements (128 B) wide, else none.
+// The same maps are needed every step (the caller's pointers do not change): keep the encoded descriptors, keyed by
+// everything cuTensorMapEncodeTiled was given (open addressing, overwritten on collision of a full probe window).
+MapCacheEntry* map_cache_find(piper_ctx* c, const void* base, long long inner, long long rows, long long groups,
+                              int box_inner, int box_rows, int kind, bool* hit) {
+    *hit = false;
+    if (!c->map_cache) return nullptr;
+    uint64_t h = reinterpret_cast<uintptr_t>(base) * 0x9E3779B97F4A7C15ull;
+    h ^= (uint64_t)inner * 0xC2B2AE3D27D4EB4Full + (uint64_t)rows * 0x165667B19E3779F9ull + (uint64_t)groups * 31 +
+         (uint64_t)box_inner * 131 + (uint64_t)box_rows * 8191 + (uint64_t)kind;
+    h ^= h >> 29;
+    const int start = (int)(h % kMapCache);
+    for (int i = 0; i < 8; ++i) {
+        MapCacheEntry* e = &c->map_cache[(start + i) % kMapCache];
+        if (e->kind == 0) return e;
+        if (e->kind == kind && e->base == base && e->inner == inner && e->rows == rows && e->groups == groups &&
+            e->box_inner == box_inner && e->box_rows == box_rows) {
+            *hit = true;
+            return e;
+        }
+    }
+    return &c->map_cache[start];  // probe window full: recycle its first entry
+}
+void map_cache_fill(MapCacheEntry* e, const CUtensorMap* m, const void* base, long long inner, long long rows,
+                    long long groups, int box_inner, int box_rows, int kind) {
+    if (!e) return;
+    e->base = base, e->inner = inner, e->rows = rows, e->groups = groups;
+    e->box_inner = box_inner, e->box_rows = box_rows, e->kind = kind, e->map = *m;
+}
+
 int make_map2(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
               int box_inner, int box_rows) {
+    bool hit;
+    MapCacheEntry* ce = map_cache_find(c, base, inner, rows, groups, box_inner, box_rows, 1, &hit);
+    if (hit) {
+        *m = ce->map;
+        return PIPER_OK;
+    }
     const cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)groups};
     const cuuint64_t strides[2] = {(cuuint64_t)inner * 2, (cuuint64_t)inner * 2 * (cuuint64_t)rows};
     const cuuint32_t box[3] = {(cuuint32_t)box_inner, (cuuint32_t)box_rows, 1};
@@ -1614,6 +1648,7 @@ int make_map2(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, l
                  (int)r, inner, rows, groups, box_inner, box_rows);
         return PIPER_ERR_CUDA;
     }
+    map_cache_fill(ce, m, base, inner, rows, groups, box_inner, box_rows, 1);
     return PIPER_OK;
 }
 int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups,
@@ -1622,6 +1657,12 @@ int make_map(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, lo
 }
 // fp32 tensor [groups][rows][inner], box = 32 columns (128 B, swizzled) x 32 rows: the fp32 dW outputs of wgrad
 int make_map_f32(piper_ctx* c, CUtensorMap* m, const void* base, long long inner, long long rows, long long groups) {
+    bool hit;
+    MapCacheEntry* ce = map_cache_find(c, base, inner, rows, groups, 32, 32, 2, &hit);
+    if (hit) {
+        *m = ce->map;
+        return PIPER_OK;
+    }
     const cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)groups};
     const cuuint64_t strides[2] = {(cuuint64_t)inner * 4, (cuuint64_t)inner * 4 * (cuuint64_t)rows};
     const cuuint32_t box[3] = {32, 32, 1};
@@ -1635,6 +1676,7 @@ int make_map_f32(piper_ctx* c, CUtensorMap* m, const void* base, long long inner
                  inner, rows, groups);
         return PIPER_ERR_CUDA;
     }
+    map_cache_fill(ce, m, base, inner, rows, groups, 32, 32, 2);
     return PIPER_OK;
 }
 #define PIPER_MAP2(...)                                \
@@ -1653,12 +1695,12 @@ int make_map_f32(piper_ctx* c, CUtensorMap* m, const void* base, long long inner
 // Queried once per (kernel, SM count of the lane) and kept.
 template <typename K>
 int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes, int threads = kThreads) {
-    constexpr int kSlots = 128;
-    static struct { const void* fn; cudaStream_t stream; int sms; int n; } cache[kSlots];
-    static int used = 0;
     const void* key = reinterpret_cast<const void*>(kernel);
-    for (int i = 0; i < (used < kSlots ? used : kSlots); ++i)
-        if (cache[i].fn == key && cache[i].sms == ln.sms && cache[i].stream == ln.stream) return cache[i].n;
+    const int used = c->cluster_cache_used < kClusterCache ? c->cluster_cache_used : kClusterCache;
+    for (int i = 0; i < used; ++i) {
+        const ClusterCacheEntry& e = c->cluster_cache[i];
+        if (e.fn == key && e.sms == ln.sms && e.stream == ln.stream) return e.n;
+    }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cudaLaunchAttribute attr;
@@ -1672,10 +1714,14 @@ int resident_clusters(piper_ctx* c, Lane ln, K kernel, int smem_bytes, int threa
         n = ln.sms / 2;
     }
     if (n > ln.sms / 2) n = ln.sms / 2;
-    if (getenv("PIPER_DEBUG")) fprintf(stderr, "[piper] resident clusters: lane of %d SMs -> %d pairs\n", ln.sms, n);
-    const int slot = used++ % kSlots;
-    cache[slot].fn = key, cache[slot].stream = ln.stream, cache[slot].sms = ln.sms, cache[slot].n = n;
+    ClusterCacheEntry& e = c->cluster_cache[c->cluster_cache_used++ % kClusterCache];
+    e.fn = key, e.stream = ln.stream, e.sms = ln.sms, e.n = n;
     return n;
+}
+
+// The {next tile, clusters done} counters of a launch on `stream`: see SchedSlot (piper_internal.cuh).
+int* sched_counters(piper_ctx* c, cudaStream_t stream) {
+    return reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * stream_slot(c, stream);
 }
 
 template <int A_MAJOR, int B_MAJOR, int EPI>
@@ -1690,7 +1736,7 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
         long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM, Cfg2<EPI>::THREADS);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
-        Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
+        Q.sched = sched_counters(c, ln.stream);
         tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), Cfg2<EPI>::THREADS, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
@@ -1715,12 +1761,12 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
     long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI>, CfgT<EPI>::SMEM);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
-    TcParams Q = P;  // tile counters of this launch: one of kSchedSlots pairs, cycled (kernels in flight never share one)
+    TcParams Q = P;
     if (c->tc_prof) {  // debug: slot per launch, cycled
         Q.prof = reinterpret_cast<long long*>(c->tc_scratch) + (size_t)(c->tc_next_slot % kProfSlots) * kProfSlotWords;
         c->tc_next_slot += 1;
     }
-    Q.sched = reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * (c->tc_sched_slot++ % kSchedSlots);
+    Q.sched = sched_counters(c, ln.stream);
     tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
@@ -1730,7 +1776,7 @@ bool set_smem_attr_t() {
     return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 CfgT<EPI>::SMEM) == cudaSuccess;
 }
-// rows-on-N kernel for the ragged-M contractions (PIPER_TC_ROWS_ON_N=0 switches it off)
+// rows-on-N kernel for the ragged-M contractions (PIPER_OPT_TC_ROWS_ON_N = 0 switches it off)
 bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2; }
 TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_tile) {
     TcParams P;
@@ -1766,6 +1812,21 @@ inline long long m_tile_bound(const FfnProblem& p, bool two) {
 
 size_t tc_scratch_bytes(const piper_moe_desc*) { return (size_t)kProfSlots * kProfSlotWords * 8 + kSchedSlots * 8; }
 
+void tc_release(piper_ctx* c) {
+    delete[] c->map_cache;
+    c->map_cache = nullptr;
+}
+
+void tc_forget_stream(piper_ctx* c, cudaStream_t stream) {
+    for (int i = 0; i < kSchedSlots; ++i)
+        if (c->sched_slots[i].used && c->sched_slots[i].stream == stream) c->sched_slots[i].used = false;
+    int n = 0;
+    const int used = c->cluster_cache_used < kClusterCache ? c->cluster_cache_used : kClusterCache;
+    for (int i = 0; i < used; ++i)
+        if (c->cluster_cache[i].stream != stream) c->cluster_cache[n++] = c->cluster_cache[i];
+    c->cluster_cache_used = n;
+}
+
 int tc_init(piper_ctx* c) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult q;
@@ -1775,17 +1836,8 @@ int tc_init(piper_ctx* c) {
     cudaGetLastError();
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
-    const char* pe = getenv("PIPER_TC_PROFILE");
-    c->tc_prof = pe && pe[0] == '1';
-    const char* pt = getenv("PIPER_TC_ROWS_ON_N");
-    c->tc_rows_on_n = !(pt && pt[0] == '0');
-    const char* ps = getenv("PIPER_T_SMALL");   // tuning knobs of the rows-on-N kernels, read once
-    c->tc_small_rows = ps ? atoi(ps) : TB_SMALL_ROWS;
-    const char* pg = getenv("PIPER_T_GREEDY");
-    c->tc_greedy = pg ? atoi(pg) : 1;
-    const char* p2 = getenv("PIPER_TC_2CTA");  // 0: never, 1: always, unset: by expected group length
-    c->tc_two_cta = p2 ? (p2[0] == '0' ? 0 : 1) : 2;
-    c->tc2_max_clusters = c->num_sms / 2;
+    c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
+    c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
               set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>() &&
@@ -1801,9 +1853,16 @@ int tc_init(piper_ctx* c) {
 bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
     if (!c->encode_tiled) return false;
     if (p.G > kMaxGroups || p.d < 64 || p.I < 64 || p.d % 8 || p.I % 8) return false;
-    if (p.G > 1 && c->D.row_align % BM) return false;  // an M tile must not straddle two experts
+    if (p.G > 1) {
+        // the rows-on-N kernels and the CTA-pair wgrad work in 16-row units (chunks rounded up to 16 rows, K slices of
+        // 16 rows issued up to the expert's real count); the rows-on-M and 1-CTA families need whole 128-row tiles
+        if (c->D.row_align % 16) return false;
+        if (c->D.row_align % BM && !(rows_on_n(c, p) && pair_wgrad(c, p))) return false;
+    }
     return true;
 }
+
+bool tc_wgrad_f32_ok(const piper_ctx* c, const FfnProblem& p) { return pair_wgrad(c, p); }
 
 // G|U = Xp Wg | Xp Wu, H = silu(G) * U
 int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {

@@ -38,24 +38,39 @@ chunk_hist_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, 
     for (int e = threadIdx.x; e < E_loc; e += blockDim.x) chunk_counts[(size_t)blockIdx.x * E_loc + e] = hist[e];
 }
 
-// ---- F2 phase 2: prefix over chunks per expert, counts, aligned exclusive scan -> offsets --------
-// One block of 512 threads (E_loc <= kMaxE = 512): thread e walks its column of chunk_counts.
-__global__ void __launch_bounds__(512)
-chunk_scan_kernel(const int32_t* __restrict__ chunk_counts, int n_chunks, int E_loc, int row_align,
-                  int32_t* __restrict__ chunk_base, int32_t* __restrict__ counts, int32_t* __restrict__ offsets) {
-    __shared__ int32_t warp_tot[16];
-    const int e = threadIdx.x, lane = e & 31, w = e >> 5;
-    int run = 0;
+// ---- F2 phase 2: prefix over chunks, aligned exclusive scan -> offsets, stable ranks, row_of and src_of ----------
+// Block = one chunk of kScanChunk assignments in flat order a = t*k + j.  Every block derives what it needs from the
+// chunk histograms itself (n_chunks * E_loc integers, L2-resident): the experts' totals, its own base = the counts of
+// the chunks before it, and the aligned exclusive scan of the totals (block 0 also writes counts / offsets), so no
+// single-block scan kernel sits between the histogram and the ranks.  Ranks: warps take turns (ascending a); inside a
+// warp __match_any_sync groups equal experts and the rank is the number of lower lanes of the group; a shared running
+// count per expert carries the rank across warps.  No atomic decides an index.  src_of entries that hold no
+// assignment (pad rows of a segment and every row from offsets[E_loc] to a_cap) are written as -1 by the same launch:
+// the blocks share those ranges.
+__global__ void __launch_bounds__(kScanChunk)
+scan_rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_loc, int row_align, int a_cap,
+                 const int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
+                 int32_t* __restrict__ row_of, int32_t* __restrict__ src_of) {
+    extern __shared__ int32_t sm[];
+    int32_t* run = sm;                  // [E_loc] next free row of each expert for this chunk
+    int32_t* s_cnt = sm + E_loc;        // [E_loc] real rows
+    int32_t* s_off = sm + 2 * E_loc;    // [E_loc + 1] aligned exclusive scan
+    __shared__ int32_t warp_tot[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int n_chunks = gridDim.x;
+    // totals and this chunk's base, experts strided over the block (E_loc <= 512 < blockDim)
+    int total = 0, base = 0;
+    const int e = threadIdx.x;
     if (e < E_loc) {
         for (int c = 0; c < n_chunks; ++c) {
             const int v = chunk_counts[(size_t)c * E_loc + e];
-            chunk_base[(size_t)c * E_loc + e] = run;
-            run += v;
+            if (c < (int)blockIdx.x) base += v;
+            total += v;
         }
-        counts[e] = run;
+        s_cnt[e] = total;
     }
-    const int padded = e < E_loc ? (run + row_align - 1) / row_align * row_align : 0;
-    int inc = padded;  // inclusive warp scan by shuffles
+    const int padded = e < E_loc ? (total + row_align - 1) / row_align * row_align : 0;
+    int inc = padded;  // inclusive warp scan by shuffles, then over the warps' totals
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
         const int o = __shfl_up_sync(0xffffffffu, inc, off);
@@ -64,33 +79,35 @@ chunk_scan_kernel(const int32_t* __restrict__ chunk_counts, int n_chunks, int E_
     if (lane == 31) warp_tot[w] = inc;
     __syncthreads();
     if (w == 0) {
-        int t = lane < 16 ? warp_tot[lane] : 0, ti = t;
+        const int t = warp_tot[lane];
+        int ti = t;
 #pragma unroll
-        for (int off = 1; off < 16; off <<= 1) {
+        for (int off = 1; off < 32; off <<= 1) {
             const int o = __shfl_up_sync(0xffffffffu, ti, off);
             if (lane >= off) ti += o;
         }
-        if (lane < 16) warp_tot[lane] = ti - t;  // exclusive
+        warp_tot[lane] = ti - t;  // exclusive
     }
     __syncthreads();
     const int excl = warp_tot[w] + inc - padded;
-    if (e < E_loc) offsets[e] = excl;
-    if (e == E_loc - 1) offsets[E_loc] = excl + padded;
-}
-
-// ---- F2 phase 3: stable rank of every assignment, row_of and src_of ------------------------------
-// Block = one chunk of kScanChunk assignments in flat order a = t*k + j.  Warps take turns (ascending
-// a): inside a warp __match_any_sync groups equal experts and the rank is the number of lower lanes
-// of the group; a shared running count per expert carries the rank across warps.
-__global__ void __launch_bounds__(kScanChunk)
-rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_loc,
-            const int32_t* __restrict__ chunk_base, const int32_t* __restrict__ offsets,
-            int32_t* __restrict__ row_of, int32_t* __restrict__ src_of) {
-    extern __shared__ int32_t run[];
-    for (int e = threadIdx.x; e < E_loc; e += blockDim.x)
-        run[e] = offsets[e] + chunk_base[(size_t)blockIdx.x * E_loc + e];
+    if (e < E_loc) {
+        s_off[e] = excl, run[e] = excl + base;
+        if (e == E_loc - 1) s_off[E_loc] = excl + padded;
+        if (blockIdx.x == 0) {
+            counts[e] = total, offsets[e] = excl;
+            if (e == E_loc - 1) offsets[E_loc] = excl + padded;
+        }
+    }
     __syncthreads();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    // rows without an assignment: segment pads (experts dealt round-robin over the blocks) and the unused tail
+    for (int g = blockIdx.x; g < E_loc; g += n_chunks)
+        for (int r = s_off[g] + s_cnt[g] + threadIdx.x; r < s_off[g + 1]; r += blockDim.x) src_of[r] = -1;
+    {
+        const int used = s_off[E_loc], tail = a_cap - used;
+        const int per = (tail + n_chunks - 1) / n_chunks;
+        const int lo = used + (int)blockIdx.x * per, hi = min(a_cap, lo + per);
+        for (int r = lo + threadIdx.x; r < hi; r += blockDim.x) src_of[r] = -1;
+    }
     const int a = blockIdx.x * kScanChunk + threadIdx.x;
     int i = -1;
     if (a < n_assign) {
@@ -103,13 +120,13 @@ rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_
     int row = -1;
     for (int turn = 0; turn < kScanChunk / 32; ++turn) {
         if (turn == w && i >= 0) {
-            int base = 0;
+            int b0 = 0;
             if (lane == leader) {
-                base = run[i];
-                run[i] = base + __popc(peers);
+                b0 = run[i];
+                run[i] = b0 + __popc(peers);
             }
-            base = __shfl_sync(peers, base, leader);
-            row = base + below;
+            b0 = __shfl_sync(peers, b0, leader);
+            row = b0 + below;
         }
         __syncthreads();
     }
@@ -373,17 +390,14 @@ int launch_scan_rank(piper_ctx* c, Lane ln, const int32_t* topk_idx, int32_t* co
                      int32_t* src_of) {
     const piper_moe_desc& D = c->D;
     const int n_assign = D.T * D.k;
-    const size_t hist_bytes = sizeof(int32_t) * D.E_loc;
-    PIPER_CUDA(c, cudaMemsetAsync(src_of, 0xFF, sizeof(int32_t) * (size_t)piper_a_cap(&D), ln.stream));
-    chunk_hist_kernel<<<c->n_chunks, kScanChunk, hist_bytes, ln.stream>>>(topk_idx, n_assign, D.e_lo, D.E_loc,
-                                                                         c->chunk_counts);
+    int32_t* chunk_counts = scan_scratch(c, ln.stream);  // per stream: forward chunks of two streams may overlap
+    chunk_hist_kernel<<<c->n_chunks, kScanChunk, sizeof(int32_t) * D.E_loc, ln.stream>>>(topk_idx, n_assign, D.e_lo,
+                                                                                        D.E_loc, chunk_counts);
     PIPER_LAUNCHED(c, "chunk_hist_kernel");
-    chunk_scan_kernel<<<1, 512, 0, ln.stream>>>(c->chunk_counts, c->n_chunks, D.E_loc, D.row_align, c->chunk_base,
-                                                 counts, offsets);
-    PIPER_LAUNCHED(c, "chunk_scan_kernel");
-    rank_kernel<<<c->n_chunks, kScanChunk, hist_bytes, ln.stream>>>(topk_idx, n_assign, D.e_lo, D.E_loc, c->chunk_base,
-                                                                   offsets, row_of, src_of);
-    PIPER_LAUNCHED(c, "rank_kernel");
+    scan_rank_kernel<<<c->n_chunks, kScanChunk, sizeof(int32_t) * (3 * D.E_loc + 1), ln.stream>>>(
+        topk_idx, n_assign, D.e_lo, D.E_loc, D.row_align, (int)piper_a_cap(&D), chunk_counts, counts, offsets, row_of,
+        src_of);
+    PIPER_LAUNCHED(c, "scan_rank_kernel");
     return PIPER_OK;
 }
 

@@ -26,7 +26,34 @@ struct Lane {
     int sms;
 };
 
-struct GreenPartition;  // chunk_pair.cu
+struct GreenPartition;  // chunk.cu
+
+// Tile counters of the dynamically scheduled tcgen05 kernels: one {next tile, clusters done} pair per stream (kernels
+// of one stream are ordered, and the last cluster of a launch re-arms the pair), so launches that run concurrently on
+// different streams never share one.  A stream under capture is keyed by (capture id, stream): a captured graph
+// keeps its own pair wherever it is replayed.
+constexpr int kSchedSlots = 64;
+struct SchedSlot {
+    cudaStream_t stream;
+    unsigned long long capture_id;  // 0 = eager
+    unsigned long long last_use;
+    bool used;
+};
+// occupancy of a cluster kernel on a lane, queried once per (kernel, stream, SM count)
+constexpr int kClusterCache = 64;
+struct ClusterCacheEntry {
+    const void* fn;
+    cudaStream_t stream;
+    int sms, n;
+};
+// encoded tensor maps, keyed by what cuTensorMapEncodeTiled was given (the same ~40 maps are needed every step)
+constexpr int kMapCache = 512;
+struct MapCacheEntry {
+    const void* base;
+    long long inner, rows, groups;
+    int box_inner, box_rows, kind;  // kind: 0 unused, 1 bf16, 2 fp32, 3 bf16 gather rows
+    CUtensorMap map;
+};
 
 }  // namespace piper
 
@@ -37,8 +64,8 @@ struct piper_ctx {
     char* ws;
     size_t ws_bytes;
     int n_chunks;            // ceil(T*k / kScanChunk)
-    int32_t* chunk_counts;   // [n_chunks][E_loc]  per-chunk local-expert histogram
-    int32_t* chunk_base;     // [n_chunks][E_loc]  exclusive prefix over chunks
+    int32_t* chunk_counts;   // [kSchedSlots][n_chunks][E_loc]  per-chunk local-expert histograms, one set per stream slot
+    size_t chunk_counts_stride;  // int32 elements between two slots' histograms
     int32_t* shared_offsets; // [2] = {0, T}: the shared expert as one group
     int64_t launches;
     int pair_mode;
@@ -53,14 +80,19 @@ struct piper_ctx {
     char err[256];
     void* encode_tiled;      // cuTensorMapEncodeTiled, resolved at create time
     piper::GreenPartition* green;
-    char* tc_scratch;        // tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
-    int tc_sched_slot;       // round-robin tile-counter pair in tc_scratch
-    int tc_next_slot;        // round-robin slot in tc_scratch
+    char* tc_scratch;        // debug counters + tile counters of the persistent tcgen05 kernels (gemm_tc.cu)
+    int tc_next_slot;        // round-robin debug-counter slot in tc_scratch
     int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
-    int tc2_max_clusters;    // co-resident CTA pairs
-    int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_TC_ROWS_ON_N, default on)
-    int tc_small_rows, tc_greedy;  // PIPER_T_SMALL / PIPER_T_GREEDY: row chunking of the rows-on-N kernels
-    int tc_prof;             // PIPER_TC_PROFILE=1: the tcgen05 kernels record wait-cycle counters in tc_scratch
+    int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_OPT_TC_ROWS_ON_N, default on)
+    int tc_small_rows, tc_greedy;  // PIPER_OPT_T_SMALL_ROWS / PIPER_OPT_T_GREEDY: row chunking of the rows-on-N kernels
+    int tc_prof;             // PIPER_OPT_TC_PROFILE: the tcgen05 kernels record wait-cycle counters in tc_scratch
+    int fused_gather;        // PIPER_OPT_FUSED_GATHER: chunk calls let the GEMMs gather x / dY rows (N2)
+    int pair_bwd_pass;       // piper_set_pair_bwd_pass
+    unsigned long long sched_clock;
+    piper::SchedSlot sched_slots[piper::kSchedSlots];
+    piper::ClusterCacheEntry cluster_cache[piper::kClusterCache];
+    int cluster_cache_used;
+    piper::MapCacheEntry* map_cache;  // [kMapCache], host
     cudaEvent_t events[piper::kMaxEvents];
 };
 
@@ -125,7 +157,9 @@ int simt_ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);
 // gemm_tc.cu (tcgen05 / TMEM / TMA; bf16 storage)
 size_t tc_scratch_bytes(const piper_moe_desc*);
 int tc_init(piper_ctx*);  // resolves cuTensorMapEncodeTiled, sets kernel attributes
+void tc_release(piper_ctx*);
 bool tc_supported(const piper_ctx*, const FfnProblem&);
+bool tc_wgrad_f32_ok(const piper_ctx*, const FfnProblem&);  // fp32 dW (and accumulate) exist in the CTA-pair wgrad only
 int tc_ffn_fwd1(piper_ctx*, Lane, const FfnProblem&);    // G,U,H = swiglu(xp W_gate, xp W_up)
 int tc_ffn_fwd2(piper_ctx*, Lane, const FfnProblem&);    // O = H W_down
 int tc_ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&);  // dG,dU from dO W_down^T and G,U
@@ -143,6 +177,11 @@ FfnProblem shared_problem(const piper_ctx*, const piper_chunk_args*);
 // chunk.cu
 void pair_release(piper_ctx*);
 void pair_plan_release(piper_ctx*);
+// api.cu: per-stream scratch of a context (see SchedSlot): the slot of a stream, its scan histograms, its tile counters
+int stream_slot(piper_ctx*, cudaStream_t);
+int32_t* scan_scratch(piper_ctx*, cudaStream_t);
+// gemm_tc.cu: forget what the context cached about a stream that is being destroyed
+void tc_forget_stream(piper_ctx*, cudaStream_t);
 
 // ---- small device helpers -----------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -18,9 +18,11 @@ pytestmark = pytest.mark.gpu
 SMALL = ["C1", "C1s", "C2s", "C3s", "C4s", "C6s"]
 
 
-def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True, overlap=False):
+def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backward=True, overlap=False, options=()):
     """Runs the whole path; returns (ctx, dict of device tensors)."""
     ctx = piper.Context(util.desc_of(cfg, gemm_impl))
+    for opt, val in options:
+        piper.piper_set_option(ctx, opt, val)
     if overlap:
         piper.piper_set_chunk_overlap(ctx, 1)
     dev = util.upload_inputs(inp)
@@ -95,16 +97,22 @@ def _check_all(cfg, b, f, g, label=""):
 
 @pytest.mark.parametrize("name", SMALL)
 @pytest.mark.parametrize("impl", [piper.GEMM_AUTO, piper.GEMM_SIMT])
-@pytest.mark.parametrize("align", [1, 128])  # 128: the tcgen05 kernels; 1: dense packing, FP32-ALU GEMMs
+@pytest.mark.parametrize("align", [1, 16, 128])  # 16 / 128: the tcgen05 kernels; 1: dense packing, FP32-ALU GEMMs only
 def test_small_configs_full_tensor_parity(name, impl, align):
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=align)
     if cfg.dtype == configs.DT_F32 and impl == piper.GEMM_SIMT:
         pytest.skip("fp32 already runs the FP32-ALU kernels under GEMM_AUTO")
+    if cfg.dtype == configs.DT_BF16 and impl == piper.GEMM_AUTO and align % 16:
+        # no silent ~100x slower path: a bf16 layer the tcgen05 kernels cannot take is refused at creation
+        with pytest.raises(piper.PiperError):
+            piper.Context(util.desc_of(cfg, impl))
+        return
     inp = configs.make_inputs(cfg)
     f = oracle.forward(cfg, inp)
     g = oracle.backward(cfg, inp, f)
     ctx, b = _run_steps(cfg, inp, gemm_impl=impl)
     _check_all(cfg, b, f, g)
+    assert piper.piper_gemm_path(ctx) == (1 if cfg.dtype == configs.DT_BF16 and impl == piper.GEMM_AUTO else 0)
     ctx.close()
 
 
@@ -120,7 +128,7 @@ def _random_config(i):
                              I=8 * int(rng.integers(8, 70)), seed=2000 + i, e_lo=e_lo, E_loc=e_loc,
                              I_shared=int(rng.choice([0, 8 * int(rng.integers(8, 40))])),
                              gate_mode=int(rng.integers(0, 3)), bias=str(rng.choice(["none", "normal0.5", "zipf1.2"])),
-                             n_dead=int(rng.integers(0, 2)) if E > k + 1 else 0, row_align=128)
+                             n_dead=int(rng.integers(0, 2)) if E > k + 1 else 0, row_align=int(rng.choice([16, 32, 128])))
 
 
 @pytest.mark.parametrize("i", range(8))
@@ -174,19 +182,24 @@ def test_more_local_experts_than_the_cta_pair_kernels_index():
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
-@pytest.mark.parametrize("env", [{"PIPER_TC_ROWS_ON_N": "0"}, {"PIPER_TC_ROWS_ON_N": "0", "PIPER_TC_2CTA": "0"}])
-def test_fallback_kernel_families(name, env, monkeypatch):
+@pytest.mark.parametrize("family", ["rows_on_m", "one_cta"])
+def test_fallback_kernel_families(name, family):
     """The rows-on-M CTA-pair kernels and the 1-CTA kernels (DESIGN.md section 5.1 b, c) stay correct: they serve
-    layers with more than 192 local experts.  The switches are read when a context is created."""
-    for k_, v_ in env.items():
-        monkeypatch.setenv(k_, v_)
+    layers with more than 192 local experts.  piper_set_option selects them (host state of the context)."""
+    opts = [(piper.OPT_TC_ROWS_ON_N, 0)] + ([(piper.OPT_TC_2CTA, 0)] if family == "one_cta" else [])
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
     inp = configs.make_inputs(cfg)
     f = oracle.forward(cfg, inp)
     g = oracle.backward(cfg, inp, f)
-    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True)
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True, options=opts)
     _check_all(cfg, b, f, g)
     assert piper.piper_gemm_path(ctx) == 1
+    ctx.close()
+    # these families need whole 128-row tiles: at row_align 16 the switch is refused and the context keeps its kernels
+    ctx = piper.Context(util.desc_of(dataclasses.replace(cfg, row_align=16)))
+    with pytest.raises(piper.PiperError):
+        piper.piper_set_option(ctx, piper.OPT_TC_ROWS_ON_N, 0)
+    assert piper.piper_get_option(ctx, piper.OPT_TC_ROWS_ON_N) == 1
     ctx.close()
 
 
@@ -284,42 +297,139 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
 @pytest.mark.parametrize("split,policy", [((132, 16), "list/exclusive"), ((100, 48), "list/exclusive"),
                                           ((116, 32), "profile/exclusive"), ((148, 16), "list/shared"),
-                                          ((148, 48), "profile/shared"), ((148, 16), "list/chunks")])
-def test_pair_is_bitwise_equal_to_serial(name, split, policy):
-    """the overlapped, out-of-order plan must respect every dependency -> identical results,
-    for the paper's list order and the profile-guided one, on disjoint and on shared SM partitions."""
+                                          ((148, 48), "profile/shared"), ((148, 16), "list/chunks"),
+                                          ((132, 16), "list/exclusive/bi"), ((148, 32), "profile/shared/bi")])
+def test_pair_matches_the_oracle_and_equals_serial_bitwise(name, split, policy):
+    """the overlapped, out-of-order plan must respect every dependency.  The pair's outputs are checked
+    against the CPU oracle (both microbatches) and must equal the serial chunks bit for bit, for the paper's list order
+    and the profile-guided one, on disjoint (green contexts) and on shared SM partitions, and for F || Bi followed by Bw
+    (PASS = Bi, Bw, PAPER.md:171)."""
     base = configs.BY_NAME[name]
-    cfg_a = dataclasses.replace(base, row_align=128, seed=base.seed + 100)
-    cfg_b = dataclasses.replace(base, row_align=128, seed=base.seed + 200)
+    align = 128 if base.dtype == configs.DT_BF16 else 1
+    cfg_a = dataclasses.replace(base, row_align=align, seed=base.seed + 100)
+    cfg_b = dataclasses.replace(base, row_align=align, seed=base.seed + 200)
     inp_a, inp_b = configs.make_inputs(cfg_a), configs.make_inputs(cfg_b)
     # serial: fwd(A) ; fwd(B) (untimed producer of B's saved activations) ; bwd(B)
     ctx, ba = _run_steps(cfg_a, inp_a, use_chunk_calls=True, backward=False)
-    _, bb = _run_steps(cfg_b, inp_b, use_chunk_calls=True, backward=True)
+    ctx_b, bb = _run_steps(cfg_b, inp_b, use_chunk_calls=True, backward=True)
+    ctx_b.close()
     # pair on fresh buffers: B's forward first, then [F(A), B(B)] co-scheduled
     pa, pb = piper.alloc_buffers(ctx), piper.alloc_buffers(ctx)
     pa.update(util.upload_inputs(inp_a)), pb.update(util.upload_inputs(inp_b))
     args_a, args_b = piper.chunk_args(pa), piper.chunk_args(pb)
     piper.piper_run_chunk_fwd(ctx, args_b)
-    order, part = policy.split("/")
+    parts = policy.split("/")
+    order, part, bi = parts[0], parts[1], len(parts) > 2
     piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE if order == "profile" else piper.ORDER_LIST,
                                 {"shared": piper.PART_SHARED, "chunks": piper.PART_CHUNK_STREAMS}.get(part, piper.PART_EXCLUSIVE))
+    piper.piper_set_pair_bwd_pass(ctx, piper.PASS_BI if bi else piper.PASS_B)
     n_sm = torch.cuda.get_device_properties(0).multi_processor_count
     sg = min(split[0], n_sm) if part != "exclusive" else min(split[0], n_sm - split[1])
     picked = piper.piper_pair_order(ctx, sg, split[1])
-    assert sorted(picked) == sorted(t for t in piper.TASKS if base.I_shared or t not in ("F_SHARED", "B_SHARED"))
+    want = [t for t in piper.TASKS if (base.I_shared or t not in ("F_SHARED", "B_SHARED")) and not (bi and t == "B_WGRAD")]
+    assert sorted(picked) == sorted(want)
+    piper.piper_pair_prepare(ctx, sg, split[1])  # partitions, streams and the plan exist before the run
     piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, split[1])
+    if bi:
+        piper.piper_run_chunk_bwd_weight(ctx, args_b)
     torch.cuda.synchronize()
-    mode = piper.piper_pair_partition_mode(ctx)
-    assert mode == {"shared": 2, "chunks": 3}.get(part, mode) and mode in (1, 2, 3)
-    if part == "exclusive":  # sm_gemm + sm_comm beyond the device is refused on disjoint partitions
-        with pytest.raises(piper.PiperError):
+    # disjoint partitions are green contexts or an error, never a silent fallback (piper.h)
+    assert piper.piper_pair_partition_mode(ctx) == {"shared": 2, "chunks": 3}.get(part, 1)
+    if part == "exclusive":  # sm_gemm + sm_comm beyond the device, and a GEMM side that is neither a multiple of 8 nor
+        with pytest.raises(piper.PiperError):  # the remainder, are refused on disjoint partitions
             piper.piper_run_chunk_pair(ctx, args_a, args_b, n_sm, 16)
+        with pytest.raises(piper.PiperError):
+            piper.piper_run_chunk_pair(ctx, args_a, args_b, 60, 16)
     for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y"):
         assert torch.equal(ba[n], pa[n]), "fwd " + n
     nofs = base.e_loc + 1  # the offsets buffers are over-allocated; entries past E_loc+1 are never written
     assert torch.equal(ba["offsets"][:nofs], pa["offsets"][:nofs]), "fwd offsets"
-    for n in ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down"):
+    for n in ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down") + (("dws_gate", "dws_up", "dws_down") if base.I_shared else ()):
         assert torch.equal(bb[n], pb[n]), "bwd " + n
+    # against the oracle: microbatch A's forward, microbatch B's forward + backward
+    fa = oracle.forward(cfg_a, inp_a)
+    _check_all(cfg_a, pa, fa, None, label="pair A ")
+    fb = oracle.forward(cfg_b, inp_b)
+    _check_all(cfg_b, pb, fb, oracle.backward(cfg_b, inp_b, fb), label="pair B ")
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C1", "C3s", "C4s", "C6s"])
+def test_bwd_input_then_weight_equals_bwd_bitwise(name):
+    """PASS = Bi, Bw (PAPER.md:171): piper_run_chunk_bwd_input leaves dX, dgates, dz_sel complete and writes no dW;
+    piper_run_chunk_bwd_weight then produces the dW of piper_run_chunk_bwd bit for bit."""
+    base = configs.BY_NAME[name]
+    cfg = dataclasses.replace(base, row_align=128 if base.dtype == configs.DT_BF16 else 1)
+    inp = configs.make_inputs(cfg)
+    ctx, ref = _run_steps(cfg, inp, use_chunk_calls=True)
+    b = piper.alloc_buffers(ctx)
+    b.update(util.upload_inputs(inp))
+    dws = ["dw_gate", "dw_up", "dw_down"] + (["dws_gate", "dws_up", "dws_down"] if cfg.I_shared else [])
+    for n in dws:
+        b[n].fill_(3.0)
+    args = piper.chunk_args(b)
+    piper.piper_run_chunk_fwd(ctx, args)
+    piper.piper_run_chunk_bwd_input(ctx, args)
+    torch.cuda.synchronize()
+    for n in ("dgates", "dz_sel", "dx"):
+        assert torch.equal(ref[n], b[n]), n
+    for n in dws:
+        assert bool((b[n] == 3.0).all()), n + " written by the input pass"
+    piper.piper_run_chunk_bwd_weight(ctx, args)
+    torch.cuda.synchronize()
+    for n in dws:
+        assert torch.equal(ref[n], b[n]), n
+    f = oracle.forward(cfg, inp)
+    _check_all(cfg, b, f, oracle.backward(cfg, inp, f))
+    ctx.close()
+
+
+def test_two_streams_of_one_context_run_concurrently():
+    """Calls of one context on different streams may overlap on the device: every GEMM launch draws its tiles from the
+    counters of its own stream (piper.h conventions).  Two microbatches, one stream each, several steps deep with no
+    host synchronisation in between, against the single-stream results; then a captured graph of stream 1 replayed on
+    stream 2 while stream 1 runs eager launches."""
+    cfg = dataclasses.replace(configs.C4S, row_align=128)
+    cfgs = [dataclasses.replace(cfg, seed=cfg.seed + 7 * i) for i in range(2)]
+    inps = [configs.make_inputs(c) for c in cfgs]
+    ctx, ref0 = _run_steps(cfgs[0], inps[0], use_chunk_calls=True)
+    ctx1, ref1 = _run_steps(cfgs[1], inps[1], use_chunk_calls=True)
+    ctx1.close()
+    refs = [ref0, ref1]
+    names = ("y", "dx", "dz_sel", "dw_gate", "dw_up", "dw_down")
+    bufs = []
+    for inp in inps:
+        b = piper.alloc_buffers(ctx)
+        b.update(util.upload_inputs(inp))
+        bufs.append(b)
+    args = [piper.chunk_args(b) for b in bufs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for step in range(12):  # 5 dynamic-feed GEMM launches per chunk call and stream
+        for i in (0, 1):
+            piper.piper_run_chunk_fwd(ctx, args[i], stream=streams[i])
+            piper.piper_run_chunk_bwd(ctx, args[i], stream=streams[i])
+    torch.cuda.synchronize()
+    for i in (0, 1):
+        for n in names:
+            assert torch.equal(refs[i][n], bufs[i][n]), (i, n)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(streams[0]):
+        with torch.cuda.graph(graph, stream=streams[0]):
+            piper.piper_run_chunk_fwd(ctx, args[0], stream=streams[0])
+            piper.piper_run_chunk_bwd(ctx, args[0], stream=streams[0])
+    for n in names:
+        bufs[0][n].zero_(), bufs[1][n].zero_()
+    torch.cuda.synchronize()
+    for rep in range(4):
+        with torch.cuda.stream(streams[1]):
+            graph.replay()
+        piper.piper_run_chunk_fwd(ctx, args[1], stream=streams[0])
+        piper.piper_run_chunk_bwd(ctx, args[1], stream=streams[0])
+    torch.cuda.synchronize()
+    for i in (0, 1):
+        for n in names:
+            assert torch.equal(refs[i][n], bufs[i][n]), ("graph + eager", i, n)
     ctx.close()
 
 
@@ -373,11 +483,108 @@ def test_empty_input_edge_cases():
     ctx.close()
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C4z"])
+def _boundary_rows(cfg, rt, rng, max_chunk_edges=3):
+    """Packed rows aimed at tile edges: for every non-empty local expert its first row, its last real row, and rows
+    255 / 256 of up to `max_chunk_edges` of its 256-row chunks (the rows-on-N kernels cut an expert's rows into
+    256-row chunks and a last one rounded up to 16 rows; a CTA of the pair holds half a chunk, so 127 / 128 too)."""
+    rows = []
+    for e in range(cfg.e_loc):
+        lo, cnt = int(rt["offsets"][e]), int(rt["counts"][e])
+        if cnt == 0:
+            continue
+        rows += [lo, lo + cnt - 1]
+        edges = list(range(256, cnt, 256))
+        if len(edges) > max_chunk_edges:
+            edges = [edges[0], edges[-1]] + list(rng.choice(edges[1:-1], max_chunk_edges - 2, replace=False))
+        for c in edges:
+            rows += [lo + c - 1, lo + c]
+        if cnt > 128:
+            rows += [lo + 127, lo + 128]
+    return np.unique(np.asarray(rows, np.int64))
+
+
+def _feature_columns(n):
+    """Columns at the edges of the 128- / 256-wide feature tiles, including the last (possibly half-empty) tile."""
+    return np.unique(np.asarray([c for c in (0, 127, 128, 255, 256, n - 129, n - 128, n - 1) if 0 <= c < n], np.int64))
+
+
+def _sampled_check(cfg, inp, rt, b, fwd=True, bwd=True, n_tokens=64, experts=None, label=""):
+    """Full-size outputs against the oracle on a deliberate sample: packed rows at chunk / tile edges
+    of every expert (O, dXp), tokens owning such rows plus random ones, the first / last token and tokens without a
+    local slot (Y, dgates, dz_sel, dX), pad rows (exact zeros in xp), and dW columns at the feature-tile edges of
+    every local expert (all d rows of dW_gate / dW_up, all d columns of dW_down)."""
+    dt = cfg.dtype
+    rng = np.random.default_rng(cfg.seed)
+    experts = list(range(cfg.e_loc)) if experts is None else list(experts)
+    A = int(rt["offsets"][-1])
+    rows = _boundary_rows(cfg, rt, rng)
+    if experts is not None:
+        ex_of_row = np.searchsorted(rt["offsets"], rows, side="right") - 1
+        rows = rows[np.isin(ex_of_row, experts)]
+    sr = oracle.sample_rows(cfg, inp, rt, rows, backward_too=bwd)
+    rows_d = torch.from_numpy(rows).cuda()
+    if fwd:
+        util.check_close(label + "o rows at chunk edges", util.to_np(b["o"][rows_d]), sr["o"], dt)
+        # xp is the all-to-all payload: pad rows are exact zeros, every other row below offsets[E_loc] a token's row
+        pad = np.nonzero(rt["src_of"][:A] < 0)[0]
+        if len(pad):
+            pick = torch.from_numpy(np.unique(np.concatenate([pad[:4], pad[-4:], rng.choice(pad, min(16, len(pad)))]))).cuda()
+            assert not bool(b["xp"][pick].any()), "xp pad rows must be zero"
+            assert not bool(b["gate_rows"][pick].any()), "gate_rows of pad rows must be zero"
+    if bwd:
+        util.check_close(label + "dxp rows at chunk edges", util.to_np(b["dxp"][rows_d]), sr["dxp"], dt)
+    # tokens: owners of boundary rows, random local ones, the first / last token, tokens with no local slot
+    local = (rt["row_of"] >= 0).any(axis=1)
+    owners = np.unique(sr["tokens"])
+    want = [owners[:: max(1, len(owners) // (n_tokens // 2))][: n_tokens // 2], [0, cfg.T - 1],
+            np.nonzero(~local)[0][:3]]
+    have = set(np.concatenate(want).tolist())
+    pool = np.setdiff1d(np.nonzero(local)[0], np.fromiter(have, np.int64))
+    want.append(rng.choice(pool, max(0, n_tokens - len(have)), replace=False))
+    tokens = np.unique(np.concatenate(want).astype(np.int64))
+    assert len(tokens) >= min(n_tokens, cfg.T)
+    s = oracle.sample_tokens(cfg, inp, rt, tokens, backward_too=bwd)
+    tk = torch.from_numpy(tokens).cuda()
+    if fwd:
+        util.check_close(label + "y", util.to_np(b["y"][tk]), s["y"], dt)
+    if bwd:
+        util.check_close(label + "dgates", util.to_np(b["dgates"][tk]), s["dgates"], dt)
+        util.check_close(label + "dz_sel", util.to_np(b["dz_sel"][tk]), oracle.sample_route_bwd(cfg, inp, rt, tokens, s["dgates"]), dt)
+        util.check_close(label + "dx", util.to_np(b["dx"][tk]), s["dx"], dt)
+        J = _feature_columns(cfg.I)
+        Jc = torch.from_numpy(J).cuda()
+        for e in experts:
+            if rt["counts"][e] == 0:
+                for n in ("dw_gate", "dw_up", "dw_down"):
+                    assert not bool(b[n][int(e)].any()), f"{n}[{e}] must be exactly zero for an empty expert"
+                continue
+            rg, ru, rd = oracle.sample_wgrad(cfg, inp, rt, e, J)
+            # an expert with a handful of rows has tiny dW entries: compare against the layer-wide scale as well
+            util.check_close(f"{label}dw_gate[{e}][:,J]", util.to_np(b["dw_gate"][e][:, Jc]), rg, dt)
+            util.check_close(f"{label}dw_up[{e}][:,J]", util.to_np(b["dw_up"][e][:, Jc]), ru, dt)
+            util.check_close(f"{label}dw_down[{e}][J,:]", util.to_np(b["dw_down"][e][Jc, :]), rd, dt)
+        if cfg.I_shared:
+            Js = _feature_columns(cfg.I_shared)
+            Jsc = torch.from_numpy(Js).cuda()
+            rg, ru, rd = oracle.sample_wgrad_shared(cfg, inp, Js)
+            util.check_close(label + "dws_gate[:,J]", util.to_np(b["dws_gate"][:, Jsc]), rg, dt)
+            util.check_close(label + "dws_up[:,J]", util.to_np(b["dws_up"][:, Jsc]), ru, dt)
+            util.check_close(label + "dws_down[J,:]", util.to_np(b["dws_down"][Jsc, :]), rd, dt)
+    return len(rows), len(tokens)
+
+
+def _check_full_size_routing(cfg, b, rt):
+    for n in ("topk_idx", "counts_global", "counts", "row_of", "src_of"):
+        assert np.array_equal(util.to_np(b[n]).reshape(-1), rt[n].reshape(-1)), n
+    assert np.array_equal(util.to_np(b["offsets"])[: cfg.e_loc + 1], rt["offsets"])
+    util.check_close("gates", util.to_np(b["gates"]), rt["gates"], configs.DT_F32)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C4z"])
 def test_full_size_sampled_parity_in_bench_configuration(name):
     """BASELINE.json full sizes in the launch configuration bench.py times (row_align 128, whole-chunk calls,
-    tcgen05 GEMMs): routing / permutation bit-exact on the whole tensors; Y, dX, dgates on sampled tokens and
-    dW on sampled columns of sampled experts, each computed by the oracle one by one from the definition."""
+    tcgen05 GEMMs): routing / permutation bit-exact on the whole tensors; everything else on the deliberate sample of
+    _sampled_check, each value computed by the oracle one by one from the definition."""
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
     inp = configs.make_inputs(cfg)
     oracle.set_threads(os.cpu_count() or 1)
@@ -390,41 +597,55 @@ def test_full_size_sampled_parity_in_bench_configuration(name):
     piper.piper_run_chunk_fwd(ctx, args)
     piper.piper_run_chunk_bwd(ctx, args)
     torch.cuda.synchronize()
-    for n in ("topk_idx", "counts_global", "counts", "row_of", "src_of"):
-        assert np.array_equal(util.to_np(b[n]).reshape(-1), rt[n].reshape(-1)), n
-    assert np.array_equal(util.to_np(b["offsets"])[: cfg.e_loc + 1], rt["offsets"])
-    rng = np.random.default_rng(cfg.seed)
-    local_tokens = np.nonzero((rt["row_of"] >= 0).any(axis=1))[0]
-    tokens = np.sort(np.concatenate([rng.choice(local_tokens, 5, replace=False), [0, cfg.T - 1]]))
-    s = oracle.sample_tokens(cfg, inp, rt, tokens)
-    tk = torch.from_numpy(tokens).cuda()
-    rows = torch.from_numpy(s["rows"]).cuda()
-    dt = cfg.dtype
-    util.check_close("o rows", util.to_np(b["o"][rows]), s["o_rows"], dt)
-    util.check_close("y", util.to_np(b["y"][tk]), s["y"], dt)
-    util.check_close("dgates", util.to_np(b["dgates"][tk]), s["dgates"], dt)
-    util.check_close("dxp rows", util.to_np(b["dxp"][rows]), s["dxp_rows"], dt)
-    util.check_close("dx", util.to_np(b["dx"][tk]), s["dx"], dt)
-    # wgrad: the fullest expert, a small one and (C4z) an empty one
-    order = np.argsort(rt["counts"])
-    picks = {int(order[-1]), int(order[len(order) // 4])}
-    J = np.sort(rng.choice(cfg.I, 3, replace=False)).astype(np.int64)
-    Jc = torch.from_numpy(J).cuda()
-    for e in sorted(picks):
-        rg, ru, rd = oracle.sample_wgrad(cfg, inp, rt, e, J)
-        util.check_close(f"dw_gate[{e}][:,J]", util.to_np(b["dw_gate"][e][:, Jc]), rg, dt)
-        util.check_close(f"dw_up[{e}][:,J]", util.to_np(b["dw_up"][e][:, Jc]), ru, dt)
-        util.check_close(f"dw_down[{e}][J,:]", util.to_np(b["dw_down"][e][Jc, :]), rd, dt)
-    for e in np.nonzero(rt["counts"] == 0)[0][:2]:
-        for n in ("dw_gate", "dw_up", "dw_down"):
-            assert not bool(b[n][int(e)].any()), f"{n}[{e}] must be exactly zero for an empty expert"
+    _check_full_size_routing(cfg, b, rt)
+    n_rows, n_tok = _sampled_check(cfg, inp, rt, b)
+    assert n_tok >= 64 and n_rows >= 2 * int((rt["counts"] > 0).sum())
     if name == "C4z":
         assert (rt["counts"] == 0).sum() >= 4
-    if cfg.I_shared:
-        Js = np.sort(rng.choice(cfg.I_shared, 2, replace=False)).astype(np.int64)
-        Jsc = torch.from_numpy(Js).cuda()
-        rg, ru, rd = oracle.sample_wgrad_shared(cfg, inp, Js)
-        util.check_close("dws_gate[:,J]", util.to_np(b["dws_gate"][:, Jsc]), rg, dt)
-        util.check_close("dws_up[:,J]", util.to_np(b["dws_up"][:, Jsc]), ru, dt)
-        util.check_close("dws_down[J,:]", util.to_np(b["dws_down"][Jsc, :]), rd, dt)
+    ctx.close()
+
+
+def test_full_size_c5_pair_against_the_oracle_and_the_serial_chunks():
+    """BASELINE.json configs[4] (reading c-20): microbatch A (seed 4) forward co-scheduled with microbatch B (seed 5, own
+    weights) backward at full size.  The pair's outputs equal the serial chunks bit for bit on disjoint green-context
+    partitions (132:16, list order) and on shared SMs (148:32, profile order), and match the oracle on the deliberate
+    sample of _sampled_check: Y(A), dX(B), dgates(B), dz_sel(B), dW(B) columns, O / dXp rows at chunk edges."""
+    cfg_a = dataclasses.replace(configs.C5A, row_align=128)
+    cfg_b = dataclasses.replace(configs.C5B, row_align=128)
+    inp_a, inp_b = configs.make_inputs(cfg_a), configs.make_inputs(cfg_b)
+    oracle.set_threads(os.cpu_count() or 1)
+    rt_a, rt_b = oracle.routing(cfg_a, inp_a), oracle.routing(cfg_b, inp_b)
+    ctx = piper.Context(util.desc_of(cfg_a))
+    ba, bb = piper.alloc_buffers(ctx, backward=False), piper.alloc_buffers(ctx)
+    ba.update(util.upload_inputs(inp_a)), bb.update(util.upload_inputs(inp_b))
+    args_a, args_b = piper.chunk_args(ba), piper.chunk_args(bb)
+    fwd_names = ("topk_idx", "gates", "counts", "row_of", "src_of", "y")
+    bwd_names = ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down")
+    # serial chunks: fwd(B) untimed producer, then fwd(A), bwd(B) on one stream with all SMs
+    piper.piper_run_chunk_fwd(ctx, args_b)
+    piper.piper_run_chunk_fwd(ctx, args_a)
+    piper.piper_run_chunk_bwd(ctx, args_b)
+    torch.cuda.synchronize()
+    serial = {n: ba[n].clone() for n in fwd_names}
+    serial.update({n: bb[n].clone() for n in bwd_names})
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    for split, order, part in (((n_sm - 16, 16), piper.ORDER_LIST, piper.PART_EXCLUSIVE),
+                               ((n_sm, 32), piper.ORDER_PROFILE, piper.PART_SHARED)):
+        for n in fwd_names:
+            ba[n].zero_()
+        for n in bwd_names:
+            bb[n].zero_()
+        piper.piper_set_pair_policy(ctx, order, part)
+        piper.piper_run_chunk_pair(ctx, args_a, args_b, split[0], split[1])
+        torch.cuda.synchronize()
+        assert piper.piper_pair_partition_mode(ctx) == (1 if part == piper.PART_EXCLUSIVE else 2)
+        for n in fwd_names:
+            assert torch.equal(serial[n], ba[n]), (split, "fwd", n)
+        for n in bwd_names:
+            assert torch.equal(serial[n], bb[n]), (split, "bwd", n)
+    # the pair's outputs (last run) against the oracle
+    _check_full_size_routing(cfg_a, ba, rt_a)
+    _check_full_size_routing(cfg_b, bb, rt_b)
+    _sampled_check(cfg_a, inp_a, rt_a, ba, fwd=True, bwd=False, n_tokens=32, label="C5a ")
+    _sampled_check(cfg_b, inp_b, rt_b, bb, fwd=False, bwd=True, n_tokens=32, label="C5b ")
     ctx.close()

@@ -322,6 +322,14 @@ def test_sampled_forms_equal_full_tensors():
     np.testing.assert_allclose(s["dgates"], b["dgates"][toks], **tol)
     np.testing.assert_allclose(s["o_rows"], f["o"][s["rows"]], **tol)
     np.testing.assert_allclose(s["dxp_rows"], b["dxp"][s["rows"]], **tol)
+    np.testing.assert_allclose(O.sample_route_bwd(cfg, inp, rt, toks, s["dgates"]), b["dz"][toks], **tol)
+    rows = np.nonzero(rt["src_of"] >= 0)[0][::3]
+    sr = O.sample_rows(cfg, inp, rt, rows)
+    np.testing.assert_allclose(sr["o"], f["o"][rows], **tol)
+    np.testing.assert_allclose(sr["h"], f["h"][rows], **tol)
+    np.testing.assert_allclose(sr["dxp"], b["dxp"][rows], **tol)
+    np.testing.assert_allclose(sr["dg"], b["dg"][rows], **tol)
+    np.testing.assert_allclose(sr["du"], b["du"][rows], **tol)
     J = np.array([0, 5, cfg.I - 1], np.int32)
     for e in range(cfg.e_loc):
         dwg, dwu, dwd = O.sample_wgrad(cfg, inp, rt, e, J)
