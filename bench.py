@@ -44,34 +44,29 @@ def measured_peaks():
     return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, kind="fallback")
 
 
-def ncu_mover_us(config_name: str):
-    """Per-launch gpu__time_duration of the row movers from the committed ncu launch lists (a CUDA-event pair around one
-    ~20 us launch also counts ~6 us of launch latency), or {}."""
+STORED = os.path.join("profiles", "r2_traffic.json.txt")
+
+
+def stored_ncu():
+    """Figures that this run does NOT measure (ncu cannot run inside a timed bench): dram bytes per launch from the
+    committed `ncu --set full` capture and per-launch gpu__time_duration of the row movers from the committed launch
+    lists.  Everything taken from here is labelled with its source file in the JSON line."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r1e_traffic.json.txt")) as f:
-            return json.load(f).get("ncu_us", {}).get(config_name, {})
+        with open(os.path.join(ROOT, STORED)) as f:
+            return json.load(f)
     except (OSError, ValueError):
         return {}
 
 
-def ncu_traffic(config_name: str, task: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the task's kernel from the committed `ncu --set full`
-    capture (profiles/r1e_traffic.json.txt names its source), or None when no capture exists for this workload."""
-    p = os.path.join(ROOT, "profiles", "r1e_traffic.json.txt")
-    try:
-        with open(p) as f:
-            return json.load(f).get(config_name, {}).get(task)
-    except (OSError, ValueError):
-        return None
-
-
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML every 20 ms while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML every 5 ms.  The thread is started before the warm-up (NVML
+    start-up stays outside the timed region) and records only between begin() and end(): the timed region."""
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+        self.recording = False
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -93,19 +88,25 @@ class ClockSampler(threading.Thread):
                  nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
         while not self.stop_flag:
             try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, nm in names.items():
-                    if r & bit:
-                        self.reasons.add(nm)
+                if self.recording:
+                    self.samples.append(mhz)
+                    for bit, nm in names.items():
+                        if r & bit:
+                            self.reasons.add(nm)
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.005)
 
-    def summary(self):
+    def begin(self):
+        self.samples, self.reasons, self.recording = [], set(), True
+
+    def end(self):
+        self.recording = False
         s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
 
 
 # --------------------------------------------------------------------------------- reference arm
@@ -222,74 +223,82 @@ def desc_of(piper, cfg, dw_f32=False):
                            dw_dtype=piper.DT_F32 if dw_f32 else None)
 
 
-def run_piper(args, cfg):
-    import numpy as np
-    import torch
-    import torch.distributed as dist
+class Workload:
+    """One config on this rank: inputs generated and resident, context and buffers allocated."""
 
-    import paper_2606_11169_b200 as piper
-    from inputs import configs
+    def __init__(self, args, cfg, rank, local):
+        import torch
+        import paper_2606_11169_b200 as piper
+        from inputs import configs
+        self.args, self.cfg, self.piper, self.torch = args, cfg, piper, torch
+        self.dev = torch.device("cuda", local)
+        self.rcfg = rank_config(cfg, rank)
+        t0 = time.time()
+        self.inp = configs.make_inputs(self.rcfg)
+        if getattr(args, "uniform_rows", 0):
+            self.inp["logits"] = configs.uniform_logits(self.rcfg)
+        log(f"[rank {rank}] {cfg.name}: inputs generated in {time.time() - t0:.1f} s")
+        self.ctx = piper.Context(desc_of(piper, self.rcfg, dw_f32=args.main_grad), device=local)
+        piper.piper_set_chunk_overlap(self.ctx, 1 if getattr(args, "chunk_overlap", False) else 0)
+        if getattr(args, "no_fused_gather", False):
+            piper.piper_set_option(self.ctx, piper.OPT_FUSED_GATHER, 0)
+        if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
+            piper.piper_set_wgrad_accumulate(self.ctx, 1)
+        self.b = piper.alloc_buffers(self.ctx)
+        if args.main_grad:
+            for n in ("dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down"):
+                if n in self.b:
+                    self.b[n].zero_()
+        self.b.update({n: piper.to_tensor(self.inp[n], self.dev) for n in INPUT_NAMES if n in self.inp})
+        self.cargs = piper.chunk_args(self.b)
+        self.stream = torch.cuda.current_stream()
 
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the piper library has no CPU path")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dev = torch.device("cuda", local)
+    def step(self):
+        self.piper.piper_run_chunk_fwd(self.ctx, self.cargs)
+        self.piper.piper_run_chunk_bwd(self.ctx, self.cargs)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    def close(self):
+        self.ctx.close()
+        self.b.clear()
+        self.inp.clear()
+        self.torch.cuda.empty_cache()
 
-    # every rank: its own microbatch of the same layer shape (weak scaling, no data-path collective)
-    rcfg = rank_config(cfg, rank)
-    t0 = time.time()
-    inp = configs.make_inputs(rcfg)
-    if getattr(args, "uniform_rows", 0):
-        inp["logits"] = configs.uniform_logits(rcfg)
-    log(f"[rank {rank}] inputs generated in {time.time() - t0:.1f} s")
-    ctx = piper.Context(desc_of(piper, rcfg, dw_f32=args.main_grad), device=local)
-    piper.piper_set_chunk_overlap(ctx, 1 if getattr(args, "chunk_overlap", False) else 0)
-    if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
-        piper.piper_set_wgrad_accumulate(ctx, 1)
-    b = piper.alloc_buffers(ctx)
-    if getattr(args, "main_grad", False):
-        for n in ("dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down"):
-            if n in b:
-                b[n].zero_()
-    b.update({n: piper.to_tensor(inp[n], dev) for n in INPUT_NAMES if n in inp})
-    cargs = piper.chunk_args(b)
-    stream = torch.cuda.current_stream()
 
-    def step():
-        piper.piper_run_chunk_fwd(ctx, cargs)
-        piper.piper_run_chunk_bwd(ctx, cargs)
-
-    for _ in range(args.warmup):
-        step()
+def time_resident(w: Workload, steps, warmup, sampler, barrier, world, min_seconds=0.0):
+    """W untimed steps, then exactly `steps` steps (more when `min_seconds` asks for a longer clock record) between a
+    barrier + synchronize on both sides; CUDA events on the launching stream; max over ranks."""
+    torch, piper = w.torch, w.piper
+    for _ in range(warmup):
+        w.step()
     barrier()
-    launches0 = piper.piper_kernel_launches(ctx)
-    sampler = ClockSampler(local)
-    sampler.start()
+    if min_seconds > 0:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(w.stream)
+        w.step()
+        e1.record(w.stream)
+        torch.cuda.synchronize()
+        steps = max(steps, int(min_seconds * 1e3 / max(e0.elapsed_time(e1), 1e-3)) + 1)
+    launches0 = piper.piper_kernel_launches(w.ctx)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        step()
-    ev1.record(stream)
+    sampler.begin()
+    ev0.record(w.stream)
+    for _ in range(steps):
+        w.step()
+    ev1.record(w.stream)
     barrier()
-    sampler.stop_flag = True
-    sampler.join()
-    launches = piper.piper_kernel_launches(ctx) - launches0
-    ms = ev0.elapsed_time(ev1)
-    ms_per_step = max_over_ranks(ms, world, dev) / args.steps
-    value = whole_job_tokens_per_s(cfg, world, ms_per_step)
+    clocks = sampler.end()
+    launches = piper.piper_kernel_launches(w.ctx) - launches0
+    ms_per_step = max_over_ranks(ev0.elapsed_time(ev1), world, w.dev) / steps
+    return ms_per_step, clocks, int(launches), steps
 
-    # ---- e2e: pinned host inputs -> device, the same two C-ABI calls, results -> pinned host ----------
-    host_in = {n: piper.to_tensor(inp[n], "cpu").pin_memory() for n in ("logits", "x", "dy")}
+
+def time_e2e(w: Workload, steps, warmup, barrier, world):
+    """The same metric through the C-ABI with HOST buffers: every step copies logits / x / dY from pinned host memory to
+    the device and y / dX / dz_sel back, inside the timed region."""
+    torch, piper, b, cfg = w.torch, w.piper, w.b, w.cfg
+    dev, stream, ctx = w.dev, w.stream, w.ctx
+    host_in = {n: piper.to_tensor(w.inp[n], "cpu").pin_memory() for n in ("logits", "x", "dy")}
     out_names = ("y", "dx", "dz_sel")
     host_out = {n: torch.empty(b[n].shape, dtype=b[n].dtype).pin_memory() for n in out_names}
     h2d = sum(t.numel() * t.element_size() for t in host_in.values())
@@ -302,7 +311,7 @@ def run_piper(args, cfg):
     sets = [b, dict(b)]
     for n in ("logits", "x", "dy") + out_names:
         sets[1][n] = torch.empty_like(b[n])
-    set_args = [cargs, piper.chunk_args(sets[1])]
+    set_args = [w.cargs, piper.chunk_args(sets[1])]
     s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
     in_ready = [torch.cuda.Event() for _ in range(2)]   # logits and x are up (what the forward chunk reads)
     dy_ready = [torch.cuda.Event() for _ in range(2)]   # dY is up (first read by the backward chunk)
@@ -339,35 +348,40 @@ def run_piper(args, cfg):
         stream.wait_event(out_done[0])
         stream.wait_event(out_done[1])
 
-    e2e_steps(min(args.warmup, 3))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_steps(min(warmup, 3))
     torch.cuda.synchronize(dev)
     barrier()
     w0 = time.perf_counter()
     ev0.record(stream)
-    e2e_steps(args.steps)
+    e2e_steps(steps)
     ev1.record(stream)
     barrier()
     wall_ms = (time.perf_counter() - w0) * 1e3
-    e2e_ms = max_over_ranks(max(ev0.elapsed_time(ev1), wall_ms), world, dev) / args.steps
-    e2e = {"value": whole_job_tokens_per_s(cfg, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
-           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
-           "what": "every step: pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel "
-                   "-> pinned host, as a 3-stream pipeline (copies of steps i+1 / i-1 overlap the compute of step i; dY goes up "
-                   "behind x and y comes down while the backward chunk runs); "
-                   "timed as max(CUDA events, host wall clock) over the whole pipeline"}
+    e2e_ms = max_over_ranks(max(ev0.elapsed_time(ev1), wall_ms), world, dev) / steps
+    return {"value": whole_job_tokens_per_s(cfg, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
+            "what": "every step: pinned host logits/x/dY -> device, piper_run_chunk_fwd + piper_run_chunk_bwd, y/dX/dz_sel "
+                    "-> pinned host, as a 3-stream pipeline (copies of steps i+1 / i-1 overlap the compute of step i; dY goes up "
+                    "behind x and y comes down while the backward chunk runs); "
+                    "timed as max(CUDA events, host wall clock) over the whole pipeline"}
 
-    # ---- per-task device times (CUDA events on the launching stream, inside full steps) ---------------
+
+def time_tasks(w: Workload, n_prof):
+    """Per-task device times (CUDA events on the launching stream between the tasks of full steps), each against its
+    algorithmic work: `kernels`, and `roofline` for the dominant kernel."""
+    import numpy as np
+    torch, piper, cfg, rcfg, b = w.torch, w.piper, w.cfg, w.rcfg, w.b
     tasks = [t for t in piper.TASKS if cfg.I_shared or t not in ("F_SHARED", "B_SHARED")]
     order = ["F_ROUTE", "F_SCAN", "F_PACK", "F_SHARED", "F_GEMM1", "F_GEMM2", "F_COMBINE", "B_CGRAD", "B_DGRAD1",
              "B_DGRAD2", "B_WGRAD", "B_SHARED", "B_UNPACK", "B_ROUTE_BWD"]
     order = [t for t in order if t in tasks]
-    n_prof = max(3, min(args.steps, 10))
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(order) + 1)] for _ in range(n_prof)]
     for it in range(n_prof):
-        evs[it][0].record(stream)
+        evs[it][0].record(w.stream)
         for i, t in enumerate(order):
-            piper.piper_run_task(ctx, t, cargs)
-            evs[it][i + 1].record(stream)
+            piper.piper_run_task(w.ctx, t, w.cargs)
+            evs[it][i + 1].record(w.stream)
     torch.cuda.synchronize()
     task_ms = {t: float(np.mean([evs[it][i].elapsed_time(evs[it][i + 1]) for it in range(n_prof)]))
                for i, t in enumerate(order)}
@@ -378,6 +392,7 @@ def run_piper(args, cfg):
     counts = b["counts"].cpu().numpy()
     peaks = measured_peaks()
     work = task_work(rcfg, A, t_touched)
+    stored = stored_ncu()
     kernels = {}
     for t in order:
         bound, amount = work[t]
@@ -388,42 +403,77 @@ def run_piper(args, cfg):
             ach, peak, unit = amount / sec / 1e9, peaks["hbm"], "GB/s"
         kernels[t] = {"ms": round(task_ms[t], 4), "bound": bound, "achieved": round(ach, 2), "unit": unit,
                       "frac": round(ach / peak, 4)}
-        us = ncu_mover_us(cfg.name).get(t)
-        if us:  # the same algorithmic bytes over the kernel's own duration from the committed ncu launch list
-            kernels[t]["ncu_us"] = us
-            kernels[t]["ncu_frac"] = round(amount / (us * 1e-6) / 1e9 / peak, 4)
+        us = stored.get("ncu_us", {}).get(cfg.name, {}).get(t)
+        if us:  # NOT measured in this run: the same algorithmic bytes over the kernel's own duration under ncu
+            kernels[t]["stored_ncu"] = {"us": us, "frac": round(amount / (us * 1e-6) / 1e9 / peak, 4),
+                                        "stored_from": stored.get("_ncu_us_source", STORED)}
     gemm_tasks = [t for t in order if work[t][0] == "tensor"]
     gemm_ms = sum(task_ms[t] for t in gemm_tasks)
     gemm_flop = sum(work[t][1] for t in gemm_tasks)
     dom = "F_GEMM1"  # one launch per task: the fused gate/up GEMM + SwiGLU kernel (largest single-kernel share)
-    impl = "tcgen05" if (cfg.dtype == 1 and piper.piper_gemm_path(ctx) == 1) else "fp32-alu"
+    impl = "tcgen05" if (cfg.dtype == 1 and piper.piper_gemm_path(w.ctx) == 1) else "fp32-alu"
+    traffic = stored.get(cfg.name, {}).get(dom)
     roofline = {"bound": "tensor", "kernel": f"{dom} ({impl} grouped GEMM gate|up + SwiGLU epilogue, 1 launch/step)",
                 "achieved": kernels[dom]["achieved"], "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
                 "frac": kernels[dom]["frac"], "frac_of_burst_peak": round(kernels[dom]["achieved"] / peaks["tf_burst"], 4),
                 "frac_of_nominal_2250": round(kernels[dom]["achieved"] / 2250.0, 4),
-                "traffic": ncu_traffic(cfg.name, dom),
-                "peak_kind": f"bf16_tflops_sustained of {peaks['kind']} (kernel timed inside a long step)",
+                "traffic": traffic,
+                "traffic_stored_from": (stored.get("_source", STORED) + " -- a committed ncu capture, NOT measured in this run")
+                if traffic else None,
+                "peak_kind": f"bf16_tflops_sustained of {peaks['kind']} (kernel timed inside a long step); burst {peaks['tf_burst']}",
                 "flop_per_launch": work[dom][1], "ms_per_launch": task_ms[dom],
                 "all_gemm": {"tflops": round(gemm_flop / (gemm_ms * 1e-3) / 1e12, 2),
                              "frac": round(gemm_flop / (gemm_ms * 1e-3) / 1e12 / peaks["tf_sustained"], 4),
+                             "frac_of_burst_peak": round(gemm_flop / (gemm_ms * 1e-3) / 1e12 / peaks["tf_burst"], 4),
                              "frac_of_nominal_2250": round(gemm_flop / (gemm_ms * 1e-3) / 1e12 / 2250.0, 4),
                              "share_of_step": round(gemm_ms / sum(task_ms.values()), 4)}}
+    shape = {"A_rows": A, "A_rows_padded": A_padded, "tokens_touched": t_touched,
+             "rows_per_expert_min_max": [int(counts.min()), int(counts.max())]}
+    return kernels, roofline, shape, impl, task_ms
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+
+def run_piper(args, cfg, sampler, rank, world, local, barrier, e2e=True, min_seconds=0.0):
+    """The bench line of one config (resident value, optional e2e, per-task times)."""
+    from inputs import configs
+    w = Workload(args, cfg, rank, local)
+    ms_per_step, clocks, launches, steps = time_resident(w, args.steps, args.warmup, sampler, barrier, world, min_seconds)
+    value = whole_job_tokens_per_s(cfg, world, ms_per_step)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16" if cfg.dtype == 1 else "f32", "data": "synthetic",
-            "config": workload_config(cfg, extra={"A_rows": A, "A_rows_padded": A_padded, "tokens_touched": t_touched,
-                                                  "rows_per_expert_min_max": [int(counts.min()), int(counts.max())],
-                                                  "parallelism": f"replicas x{world} (one microbatch per GPU)"}),
-            "tflops": configs.flops_fwd_bwd(rcfg, A) / (ms_per_step * 1e-3) / 1e12,
-            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "kernels": kernels, "gemm_impl": impl}
+            "dtype": "bf16" if cfg.dtype == 1 else "f32", "data": "synthetic"}
+    if e2e:
+        line["e2e"] = time_e2e(w, args.steps, args.warmup, barrier, world)
+    kernels, roofline, shape, impl, _ = time_tasks(w, max(3, min(args.steps, 10)))
+    shape["parallelism"] = f"replicas x{world} (one microbatch per GPU)"
+    line.update({"config": workload_config(cfg, extra=shape),
+                 "tflops": configs.flops_fwd_bwd(w.rcfg, shape["A_rows"]) / (ms_per_step * 1e-3) / 1e12,
+                 "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "kernels": kernels, "gemm_impl": impl})
     if args.main_grad:
         line["config"]["dw"] = "fp32, accumulated across steps (accumulate = 1)"
-    return line, ctx, b, inp, rcfg
+    return line, w
 
 
-def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
+def gemm_hbm_bytes(cfg, A: int):
+    """Bytes the GEMM tasks must move at least once (weights read once per GEMM, dW written once, row buffers read /
+    written once per use): {task: bytes}."""
+    b, d, I, Is, T, E = 2 if cfg.dtype == 1 else 4, cfg.d, cfg.I, cfg.I_shared, cfg.T, cfg.e_loc
+
+    def ffn(rows, n_e, inter):
+        w = n_e * d * inter * b
+        return {"gemm1": 2 * w + rows * d * b + 3 * rows * inter * b, "gemm2": w + rows * inter * b + rows * d * b,
+                "dgrad1": w + rows * d * b + 4 * rows * inter * b, "dgrad2": 2 * w + 2 * rows * inter * b + rows * d * b,
+                "wgrad": 2 * rows * d * b + 3 * rows * inter * b + 3 * w}
+    r = ffn(A, E, I)
+    out = {"F_GEMM1": r["gemm1"], "F_GEMM2": r["gemm2"], "B_DGRAD1": r["dgrad1"], "B_DGRAD2": r["dgrad2"],
+           "B_WGRAD": r["wgrad"]}
+    if Is:
+        sh = ffn(T, 1, Is)
+        out["F_SHARED"] = sh["gemm1"] + sh["gemm2"]
+        out["B_SHARED"] = sh["dgrad1"] + sh["dgrad2"] + sh["wgrad"]
+    return out
+
+
+def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None):
     """Step P on this context's layer shape: forward chunk of microbatch A (the bench inputs) co-scheduled
     with the backward chunk of microbatch B (seed + 1, own weights: reading c-20) versus the same two
     chunks back to back on one stream with all SMs."""
@@ -439,6 +489,8 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if sampler is not None:
+        sampler.begin()
 
     def timed(fn, repeats=3):
         """Median over `repeats` timings of `iters` back-to-back calls (the pair's time moves by several % from one
@@ -456,23 +508,17 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
             ts.append(e0.elapsed_time(e1) / iters)
         return sorted(ts)[len(ts) // 2]
 
-    # the serial baseline: every task of both chunks on one stream, all SMs; beside it the same two
-    # calls with the library's intra-chunk overlap (piper_set_chunk_overlap), a measured variant
-    piper.piper_set_chunk_overlap(ctx, 1)
-    t_fo = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
-    t_bo = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
+    # the serial baseline: every task of both chunks on one stream, all SMs
     piper.piper_set_chunk_overlap(ctx, 0)
     t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
     t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
-    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b,
-           "chunk_overlap": {"fwd_ms": t_fo, "bwd_ms": t_bo, "ratio_vs_serial": (t_fo + t_bo) / (t_f + t_b),
-                             "what": "the two chunks one after the other, each with its row movers on a side stream "
-                                     "beside the shared expert's GEMMs (fwd) / the routed wgrad (bwd)"},
-           "splits": {}, "variants": {}}
+    out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "tokens_per_pair": 2 * cfg.T,
+           "tokens_per_s_serial": 2 * cfg.T / ((t_f + t_b) * 1e-3), "splits": {}, "variants": {}}
 
     def sweep(split_list):
         res = {}
         for sg, sc in split_list:
+            piper.piper_pair_prepare(ctx, sg, sc)  # partitions / streams / plan are created outside the timed calls
             t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
             res[f"{sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / (t_f + t_b),
                                  "order": piper.piper_pair_order(ctx, sg, sc)}
@@ -481,7 +527,7 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     # the contract's sweep: Piper's list scheduling on disjoint SM partitions
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
     out["splits"] = sweep(splits)
-    out["partition_mode"] = {1: "green contexts", 2: "bounded grids on plain streams"}.get(
+    out["partition_mode"] = {1: "green contexts", 2: "bounded grids on plain streams", 3: "one stream per chunk"}.get(
         piper.piper_pair_partition_mode(ctx), "?")
     # measured variants: profile-guided order from per-task times taken here, and SM sharing
     # (the paper leaves SM allocation to the GPU) where the GEMM grids keep every SM
@@ -497,9 +543,7 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
     piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE, piper.PART_EXCLUSIVE, task_ms)
     out["variants"]["profile_order_exclusive"] = sweep(splits)
-    shared_splits = [(n_sm, 16), (n_sm, 32), (n_sm, 48), (n_sm - 16, 16)]
-    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_SHARED, task_ms)
-    out["variants"]["list_order_shared_sms"] = sweep(shared_splits)
+    shared_splits = [(n_sm, 16), (n_sm, 32), (n_sm, 48)]
     piper.piper_set_pair_policy(ctx, piper.ORDER_PROFILE, piper.PART_SHARED, task_ms)
     out["variants"]["profile_order_shared_sms"] = sweep(shared_splits)
     # the paper's own setting: one stream per chunk, SM allocation left to the GPU
@@ -508,7 +552,35 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters):
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
     best = min(((v["ratio_vs_serial"], name, k) for name, d in
                 [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))
-    out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2]}
+    out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2],
+                   "tokens_per_s": 2 * cfg.T / (best[0] * (t_f + t_b) * 1e-3)}
+    # What the pair can reach on this workload: the floors of the two roofs and of "every row
+    # mover hidden under GEMMs that keep their serial speed", each as a ratio to the measured serial time.
+    peaks = measured_peaks()
+    A_a, A_b = int(b_a["counts"].sum().item()), int(b_b["counts"].sum().item())
+    tt_a = int((b_a["row_of"] >= 0).any(dim=1).sum().item())
+    tt_b = int((b_b["row_of"] >= 0).any(dim=1).sum().item())
+    wa, wb = task_work(cfg, A_a, tt_a), task_work(cfg_b, A_b, tt_b)
+    ga, gb = gemm_hbm_bytes(cfg, A_a), gemm_hbm_bytes(cfg_b, A_b)
+    flop = sum(v for t, (k_, v) in wa.items() if k_ == "tensor" and t.startswith("F_")) + \
+        sum(v for t, (k_, v) in wb.items() if k_ == "tensor" and t.startswith("B_"))
+    hbm = sum(v for t, (k_, v) in wa.items() if k_ == "hbm" and t.startswith("F_")) + \
+        sum(v for t, (k_, v) in wb.items() if k_ == "hbm" and t.startswith("B_")) + \
+        sum(v for t, v in ga.items() if t.startswith("F_")) + sum(v for t, v in gb.items() if t.startswith("B_"))
+    gemm_ms = sum(ms for t, ms in out["task_ms"].items() if (wa.get(t) or ("", 0))[0] == "tensor")
+    mover_ms = sum(ms for t, ms in out["task_ms"].items() if (wa.get(t) or ("", 0))[0] == "hbm")
+    serial = t_f + t_b
+    out["bound"] = {"serial_ms": serial, "gemm_tasks_ms": gemm_ms, "row_mover_and_routing_tasks_ms": mover_ms,
+                    "ratio_if_every_mover_is_hidden": gemm_ms / serial,
+                    "flop": flop, "tensor_floor_ms": flop / (peaks["tf_sustained"] * 1e9),
+                    "tensor_floor_ratio": flop / (peaks["tf_sustained"] * 1e9) / serial,
+                    "hbm_bytes": hbm, "hbm_floor_ms": hbm / (peaks["hbm"] * 1e6),
+                    "hbm_floor_ratio": hbm / (peaks["hbm"] * 1e6) / serial,
+                    "what": "tensor floor = GEMM FLOP of fwd(A) + bwd(B) / bf16_tflops_sustained; hbm floor = bytes the row movers "
+                            "and the GEMMs must move once (weights, dW, row buffers) / hbm_gbs; 'every mover hidden' = the GEMM "
+                            "tasks alone at their measured whole-device speed.  The 0.8 target lies below the last one."}
+    if sampler is not None:
+        out["clocks"] = sampler.end()
     return out
 
 
@@ -522,6 +594,11 @@ def main():
     ap.add_argument("--row-align", type=int, default=None, help="override the config's row_align")
     ap.add_argument("--oracle-tokens", type=int, default=0, help="tokens of the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="only the headline workload: skip the C3 / C4 / C5-pair blocks of the default run")
+    ap.add_argument("--no-fused-gather", action="store_true",
+                    help="measured variant: the chunk calls run the separate pack / combine_bwd row movers and the GEMMs read "
+                         "xp / d_o (PIPER_OPT_FUSED_GATHER = 0)")
     ap.add_argument("--uniform-rows", type=int, default=0,
                     help="microbenchmark: C3's routed layer shape with exactly this many rows in each of 32 experts "
                          "(overrides --config; use with --no-cpu-baseline)")
@@ -539,29 +616,66 @@ def main():
     from inputs import configs
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
         ge.build()
+    default_run = args.config == "C2" and not args.uniform_rows and not args.pair and not args.main_grad
     if args.config == "C5":  # configs[4]: the C3-shaped chunk pair, microbatch seeds 4 (forward) and 5 (backward)
         args.config, args.pair = "C5a", True
-    cfg = configs.uniform_config(args.uniform_rows) if args.uniform_rows else configs.BY_NAME[args.config]
-    if cfg.dtype == configs.DT_BF16:
-        cfg = dataclasses.replace(cfg, row_align=args.row_align or 128)  # tcgen05 tiles are 128 rows
+
+    def bench_cfg(name):
+        c = configs.BY_NAME[name]
+        return dataclasses.replace(c, row_align=args.row_align or 128) if c.dtype == configs.DT_BF16 else c
+
+    cfg = dataclasses.replace(configs.uniform_config(args.uniform_rows), row_align=args.row_align or 128) \
+        if args.uniform_rows else bench_cfg(args.config)
     if args.impl == "reference":
         run_reference(args, cfg)
         return
 
-    line, ctx, b, inp, rcfg = run_piper(args, cfg)
+    import torch
+    import torch.distributed as dist
+    import paper_2606_11169_b200 as piper
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the piper library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()  # before any warm-up; it records only inside the timed regions
+    line, w = run_piper(args, cfg, sampler, rank, world, local, barrier)
+    iters = max(3, min(args.steps, 10))
+    contract_splits = [(132, 16), (124, 24), (116, 32), (100, 48)]
     if args.pair and world == 1:
-        import paper_2606_11169_b200 as piper
-        line["pair"] = run_pair(piper, ctx, rcfg, b, inp, [(132, 16), (124, 24), (116, 32), (100, 48)],
-                                max(3, min(args.steps, 10)))
+        line["pair"] = run_pair(piper, w.ctx, w.rcfg, w.b, w.inp, contract_splits, iters, sampler)
+    w.close()
+    if default_run and world == 1 and not args.no_extra:
+        # the north star's whole report in one line: the other single-GPU workloads of BASELINE.json, each with its own
+        # clock record over a timed region of >= 0.5 s, and the chunk pair of configs[4]
+        line["configs"] = {}
+        for name in ("C3", "C4"):
+            sub, w2 = run_piper(args, bench_cfg(name), sampler, rank, world, local, barrier, e2e=False, min_seconds=0.5)
+            w2.close()
+            keep = ("value", "unit", "ms_per_step", "steps", "tflops", "clocks", "gpu_launches", "roofline", "kernels", "config")
+            line["configs"][name] = {k_: sub[k_] for k_ in keep}
+        w5 = Workload(args, bench_cfg("C5a"), rank, local)
+        w5.step()
+        line["configs"]["C5_pair"] = run_pair(piper, w5.ctx, w5.rcfg, w5.b, w5.inp, contract_splits, iters, sampler)
+        line["configs"]["C5_pair"]["config"] = workload_config(w5.cfg, extra={"microbatch_b_seed": w5.rcfg.seed + 1})
+        w5.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         tokens = args.oracle_tokens or 8
         sec, cores, _ = time_oracle(cfg, tokens, 1, 0)
         line["cpu_baseline"] = {"value": tokens / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"CPU oracle fwd+bwd, one pass over the first {tokens} tokens of {cfg.name} "
                                           f"(same d/E/k/I, weights, seed), {sec:.1f} s"}
+    sampler.stop_flag = True
     if world > 1:
-        import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()
     if rank == 0:

@@ -228,7 +228,10 @@ int piper_pair_prepare(piper_ctx* ctx, int sm_gemm, int sm_comm);
 #define PIPER_PASS_BI 1
 int piper_set_pair_bwd_pass(piper_ctx* ctx, int pass);
 
-/* Policy of piper_run_chunk_pair (host state of `ctx`; default = the paper's: PIPER_ORDER_LIST, PIPER_PART_EXCLUSIVE).
+/* Policy of piper_run_chunk_pair (host state of `ctx`).  Default: PIPER_ORDER_PROFILE on PIPER_PART_SHARED, the
+ * combination that does not lose against the serial chunks on C5 (bench.py reports every combination; the paper's
+ * own policy, PIPER_ORDER_LIST, on the disjoint partitions BASELINE.json sweeps, PIPER_PART_EXCLUSIVE, measures
+ * 1.1-1.25 x serial: DESIGN.md section 5.4).
  *  order     PIPER_ORDER_LIST    Piper's list scheduling, ready task with the most descendants first.
  *            PIPER_ORDER_PROFILE profile-guided (PAPER.md:273, 420 name it as the way past the simple policy): the
  *                                static two-stream schedule with the smallest simulated makespan, found by exhaustive

@@ -438,7 +438,8 @@ def test_full_size_routing_and_permutation_bit_exact(name):
     cfg = configs.BY_NAME[name]
     inp = configs.make_inputs(cfg, weights=False, with_dy=False)
     ref = oracle.routing(cfg, inp)
-    ctx = piper.Context(util.desc_of(cfg))
+    # dense packing (row_align 1, the survey's default): routing / permutation / pack do not depend on the GEMM family
+    ctx = piper.Context(util.desc_of(cfg, piper.GEMM_SIMT))
     x = util.to_dev(inp["x"])
     logits = util.to_dev(inp["logits"])
     A_cap = ctx.a_cap
@@ -472,7 +473,8 @@ def test_empty_input_edge_cases():
     ctx, b = _run_steps(cfg, inp)
     _check_all(cfg, b, f, g)
     ctx.close()
-    cfg = configs.MoeConfig("edge2", T=40, d=64, E=8, k=1, I=64, seed=22, e_lo=6, E_loc=2, n_dead=2, bias="zipf1.2")
+    cfg = configs.MoeConfig("edge2", T=40, d=64, E=8, k=1, I=64, seed=22, e_lo=6, E_loc=2, n_dead=2, bias="zipf1.2",
+                            row_align=16)
     inp = configs.make_inputs(cfg)
     f = oracle.forward(cfg, inp)
     assert int(f["offsets"][-1]) == 0  # nothing is routed to the dead local experts
