@@ -178,9 +178,26 @@ int piper_dispatch_unpack(piper_ctx* ctx, const void* dxp, const int32_t* row_of
 int piper_route_bwd(piper_ctx* ctx, const float* logits, const int32_t* topk_idx, const float* gates,
                     const float* dgates, float* dz_sel, void* stream);
 
+/* N1 router GEMMs (Listing 1 `self.router(x)`): the step before F1 and after B6.
+ * piper_router_fwd: logits [T,E] fp32 = x [T,d] w_r [d,E] (+ bias [E] fp32, nullable; reading c-5: the bias is part of
+ * the logits).  bf16 layers: tcgen05 GEMM, products of bf16 values are exact and the sum is accumulated in fp32, so the
+ * logits differ from the exactly rounded sum by fp32 accumulation error only (~1e-6 relative): top-k selections on them
+ * agree with the oracle's except on rows whose k-th / (k+1)-th logit gap is below that error (reading c-18).
+ * piper_router_bwd: dz = dz_sel [T,k] scattered to the selected experts (gate modes 0, 1) or the dense [T,E] rows of
+ * mode 2; dw_r [d,E] fp32 = x^T dz (overwritten); dx_router [T,d] (activation dtype) = dz w_r^T, the router's part of
+ * dX (piper_dispatch_unpack_router adds it).  dz_scratch: T*E*4 bytes of caller-owned scratch.  On bf16 layers dz is
+ * split into two bf16 terms (relative error 2^-17) for the tensor cores. */
+int piper_router_fwd(piper_ctx* ctx, const void* x, const void* w_r, const float* bias, float* logits, void* stream);
+int piper_router_bwd(piper_ctx* ctx, const void* x, const void* w_r, const int32_t* topk_idx, const float* dz_sel,
+                     void* dz_scratch, float* dw_r, void* dx_router, void* stream);
+/* B5 with the router's term: dx[t] = sum_{j local} dxp[row_of[t,j]] (+ dx_shared[t]) (+ dx_router[t]), summed in fp32 in
+ * that order and rounded once. */
+int piper_dispatch_unpack_router(piper_ctx* ctx, const void* dxp, const int32_t* row_of, const void* dx_shared,
+                                 const void* dx_router, void* dx, void* stream);
+
 /* Every pointer of one microbatch (inputs, outputs and the scratch between forward and backward). */
 typedef struct {
-    const float* logits;                         /* [T,E]                                           */
+    const float* logits;                         /* [T,E]: input; an OUTPUT of the forward chunk when w_r != NULL */
     const void *x, *dy;                          /* [T,d]                                           */
     const void *w_gate, *w_up, *w_down;          /* routed experts                                  */
     const void *ws_gate, *ws_up, *ws_down;       /* shared expert (NULL when I_shared = 0)          */
@@ -191,6 +208,12 @@ typedef struct {
     void* y;                                     /* [T,d]                                           */
     void *d_o, *dg, *du, *dxp, *dgs, *dus, *dxs, *dx; /* backward activations                      */
     void *dw_gate, *dw_up, *dw_down, *dws_gate, *dws_up, *dws_down;
+    /* N1 (optional, all NULL = the boundary starts at the logits): with w_r != NULL the forward chunk first computes
+     * logits = x w_r + router_bias, and the backward chunk adds the router's dW_r and its term of dX */
+    const void* w_r;           /* [d,E]                                                             */
+    const float* router_bias;  /* [E] or NULL                                                       */
+    float* dw_r;               /* [d,E] fp32                                                        */
+    void *dx_router, *dz_scratch; /* [T,d]; T*E*4 bytes                                             */
 } piper_chunk_args;
 
 /* Whole forward chunk F1..F5 (+ shared expert) / backward chunk B1..B6 on one stream, all SMs:

@@ -54,6 +54,38 @@ void oracle_set_threads(int n) { g_threads = n < 1 ? 1 : n; }
 int oracle_get_threads() { return g_threads; }
 
 // ---------------------------------------------------------------------------------------------
+// 0. Router (Listing 1 `self.router(x)`; readings c-5, c-18): the step before F1.
+//    z[t,e] = sum_i x[t,i] W_r[i,e] + bias[e], in fp64 and unrounded (the generator's logits are this sum rounded to
+//    fp32 followed by one fp32 add of the bias).  Backward (Definition 5, last sentence): dW_r[i,e] = sum_t x[t,i]
+//    dz[t,e] and the router's part of dX, dX_r[t,i] = sum_e dz[t,e] W_r[i,e], for a dense dz [T,E].
+int oracle_router_fwd(const Desc* D, const void* x, const void* w_r, const float* bias, double* z) {
+    const int T = D->T, d = D->d, E = D->E;
+    for (int t = 0; t < T; ++t)
+        for (int e = 0; e < E; ++e) {
+            double acc = 0.0;
+            for (int i = 0; i < d; ++i) acc += ld(x, D->dtype, (size_t)t * d + i) * ld(w_r, D->dtype, (size_t)i * E + e);
+            z[(size_t)t * E + e] = acc + (bias ? (double)bias[e] : 0.0);
+        }
+    return 0;
+}
+int oracle_router_bwd(const Desc* D, const void* x, const void* w_r, const double* dz, double* dw_r, double* dx_r) {
+    const int T = D->T, d = D->d, E = D->E;
+    for (int i = 0; i < d; ++i)
+        for (int e = 0; e < E; ++e) {
+            double acc = 0.0;
+            for (int t = 0; t < T; ++t) acc += ld(x, D->dtype, (size_t)t * d + i) * dz[(size_t)t * E + e];
+            dw_r[(size_t)i * E + e] = acc;
+        }
+    for (int t = 0; t < T; ++t)
+        for (int i = 0; i < d; ++i) {
+            double acc = 0.0;
+            for (int e = 0; e < E; ++e) acc += dz[(size_t)t * E + e] * ld(w_r, D->dtype, (size_t)i * E + e);
+            dx_r[(size_t)t * d + i] = acc;
+        }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
 // 1. Routing (SURVEY.md §8c Definition 1; BASELINE.json:north_star part 1; tie rule c-6; c-7).
 //    topk_idx[t, 0..k) = the k experts with the largest logits, ties to the lowest index,
 //    listed by descending logit.  gates: mode 0 softmax over the selected k, mode 1 sigmoid

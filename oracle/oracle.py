@@ -28,7 +28,7 @@ def lib():
     global _lib
     if _lib is None:
         _lib = ctypes.CDLL(_build.build())
-        for name in ("oracle_route_topk", "oracle_permute", "oracle_pack", "oracle_ffn_fwd_rows", "oracle_combine",
+        for name in ("oracle_router_fwd", "oracle_router_bwd", "oracle_route_topk", "oracle_permute", "oracle_pack", "oracle_ffn_fwd_rows", "oracle_combine",
                      "oracle_combine_bwd", "oracle_ffn_bwd_rows", "oracle_wgrad", "oracle_ffn_cols", "oracle_unpack",
                      "oracle_route_bwd", "oracle_list_schedule"):
             getattr(_lib, name).restype = ctypes.c_int
@@ -66,6 +66,35 @@ def _f64(a: np.ndarray) -> np.ndarray:
 
 
 # ----------------------------------------------------------------------------------------- steps
+def router_fwd(cfg, x, w_r, bias=None):
+    """z = x W_r + bias in fp64, unrounded (plain loops in oracle.cpp)."""
+    z = np.empty((cfg.T, cfg.E), np.float64)
+    b32 = None if bias is None else np.ascontiguousarray(bias, np.float32)
+    D = _desc(cfg)
+    _chk(lib().oracle_router_fwd(ctypes.byref(D), _p(np.ascontiguousarray(x)), _p(np.ascontiguousarray(w_r)), _p(b32), _p(z)),
+         "router_fwd")
+    return z
+
+
+def dense_dz(cfg, topk_idx, dz):
+    """dz_sel [T,k] scattered to the selected experts' columns of a dense [T,E] array (mode 2: dz is dense already)."""
+    if cfg.gate_mode == 2:
+        return np.ascontiguousarray(dz, np.float64)
+    dense = np.zeros((cfg.T, cfg.E))
+    np.put_along_axis(dense, topk_idx.astype(np.int64), dz, axis=1)
+    return dense
+
+
+def router_bwd(cfg, x, w_r, dz_dense):
+    """dW_r = x^T dz and dX_r = dz W_r^T (plain loops in oracle.cpp)."""
+    dw = np.empty((cfg.d, cfg.E), np.float64)
+    dx = np.empty((cfg.T, cfg.d), np.float64)
+    D = _desc(cfg)
+    _chk(lib().oracle_router_bwd(ctypes.byref(D), _p(np.ascontiguousarray(x)), _p(np.ascontiguousarray(w_r)),
+                                 _p(np.ascontiguousarray(dz_dense, np.float64)), _p(dw), _p(dx)), "router_bwd")
+    return dw, dx
+
+
 def route_topk(cfg, logits):
     logits = np.ascontiguousarray(logits, dtype=np.float32)
     idx = np.empty((cfg.T, cfg.k), np.int32)

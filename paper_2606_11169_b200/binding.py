@@ -36,7 +36,8 @@ _CHUNK_FIELDS = ("logits", "x", "dy", "w_gate", "w_up", "w_down", "ws_gate", "ws
                  "xp", "g_save", "u_save", "h_save", "o",
                  "gs_save", "us_save", "hs_save", "s", "y",
                  "d_o", "dg", "du", "dxp", "dgs", "dus", "dxs", "dx",
-                 "dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down")
+                 "dw_gate", "dw_up", "dw_down", "dws_gate", "dws_up", "dws_down",
+                 "w_r", "router_bias", "dw_r", "dx_router", "dz_scratch")
 
 
 class ChunkArgs(ctypes.Structure):
@@ -197,6 +198,21 @@ def piper_dispatch_unpack(ctx, dxp, row_of, dx_shared, dx, stream=None):
               "piper_dispatch_unpack")
 
 
+def piper_router_fwd(ctx, x, w_r, bias, logits, stream=None):
+    ctx.check(lib().piper_router_fwd(ctx._h, _ptr(x), _ptr(w_r), _ptr(bias), _ptr(logits), _stream(stream)),
+              "piper_router_fwd")
+
+
+def piper_router_bwd(ctx, x, w_r, topk_idx, dz_sel, dz_scratch, dw_r, dx_router, stream=None):
+    ctx.check(lib().piper_router_bwd(ctx._h, _ptr(x), _ptr(w_r), _ptr(topk_idx), _ptr(dz_sel), _ptr(dz_scratch),
+                                     _ptr(dw_r), _ptr(dx_router), _stream(stream)), "piper_router_bwd")
+
+
+def piper_dispatch_unpack_router(ctx, dxp, row_of, dx_shared, dx_router, dx, stream=None):
+    ctx.check(lib().piper_dispatch_unpack_router(ctx._h, _ptr(dxp), _ptr(row_of), _ptr(dx_shared), _ptr(dx_router),
+                                                 _ptr(dx), _stream(stream)), "piper_dispatch_unpack_router")
+
+
 def piper_route_bwd(ctx, logits, topk_idx, gates, dgates, dz_sel, stream=None):
     ctx.check(lib().piper_route_bwd(ctx._h, _ptr(logits), _ptr(topk_idx), _ptr(gates), _ptr(dgates), _ptr(dz_sel),
                                     _stream(stream)), "piper_route_bwd")
@@ -333,6 +349,15 @@ def to_tensor(a, device="cuda"):
 def piper_gemm_path(ctx: Context) -> int:
     """1 = the routed-expert GEMMs of this context run on the tcgen05 kernels, 0 = on the FP32 ALUs."""
     return int(lib().piper_gemm_path(ctx._h))
+
+
+def alloc_router_buffers(ctx: Context) -> dict:
+    """Outputs / scratch of the router GEMMs (N1): logits (an output once w_r is given), dw_r, dx_router, dz_scratch."""
+    D, dev = ctx.desc, ctx.device
+    return dict(logits=torch.empty((D.T, D.E), dtype=torch.float32, device=dev),
+                dw_r=torch.empty((D.d, D.E), dtype=torch.float32, device=dev),
+                dx_router=torch.empty((D.T, D.d), dtype=ctx.torch_dtype, device=dev),
+                dz_scratch=torch.empty((D.T, D.E), dtype=torch.float32, device=dev))
 
 
 def alloc_buffers(ctx: Context, backward: bool = True) -> dict:

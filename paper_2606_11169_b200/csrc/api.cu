@@ -248,7 +248,7 @@ int piper_shared_ffn_fwd(piper_ctx* c, const void* x, const void* ws_gate, const
 int piper_combine(piper_ctx* c, const void* o, const int32_t* row_of, const float* gates, const void* s, void* y,
                   void* stream) {
     if (!c || !all_aligned(o, row_of, gates, y) || (s && !aligned16(s))) return PIPER_ERR_INVALID;
-    return launch_combine(c, full_lane(c, stream), o, row_of, gates, s, y, true);
+    return launch_combine(c, full_lane(c, stream), o, row_of, gates, s, nullptr, y, true);
 }
 
 int piper_combine_bwd(piper_ctx* c, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
@@ -304,7 +304,25 @@ int piper_shared_ffn_bwd(piper_ctx* c, const void* dy, const void* x, const void
 int piper_dispatch_unpack(piper_ctx* c, const void* dxp, const int32_t* row_of, const void* dx_shared, void* dx,
                           void* stream) {
     if (!c || !all_aligned(dxp, row_of, dx) || (dx_shared && !aligned16(dx_shared))) return PIPER_ERR_INVALID;
-    return launch_combine(c, full_lane(c, stream), dxp, row_of, nullptr, dx_shared, dx, false);
+    return launch_combine(c, full_lane(c, stream), dxp, row_of, nullptr, dx_shared, nullptr, dx, false);
+}
+
+int piper_dispatch_unpack_router(piper_ctx* c, const void* dxp, const int32_t* row_of, const void* dx_shared,
+                                 const void* dx_router, void* dx, void* stream) {
+    if (!c || !all_aligned(dxp, row_of, dx) || (dx_shared && !aligned16(dx_shared)) || (dx_router && !aligned16(dx_router)))
+        return PIPER_ERR_INVALID;
+    return launch_combine(c, full_lane(c, stream), dxp, row_of, nullptr, dx_shared, dx_router, dx, false);
+}
+
+int piper_router_fwd(piper_ctx* c, const void* x, const void* w_r, const float* bias, float* logits, void* stream) {
+    if (!c || !all_aligned(x, w_r, logits) || (bias && !aligned16(bias))) return PIPER_ERR_INVALID;
+    return launch_router_fwd(c, full_lane(c, stream), x, w_r, bias, logits);
+}
+
+int piper_router_bwd(piper_ctx* c, const void* x, const void* w_r, const int32_t* topk_idx, const float* dz_sel,
+                     void* dz_scratch, float* dw_r, void* dx_router, void* stream) {
+    if (!c || !all_aligned(x, w_r, topk_idx, dz_sel, dz_scratch, dw_r, dx_router)) return PIPER_ERR_INVALID;
+    return launch_router_bwd(c, full_lane(c, stream), x, w_r, topk_idx, dz_sel, dz_scratch, dw_r, dx_router);
 }
 
 int piper_route_bwd(piper_ctx* c, const float* logits, const int32_t* topk_idx, const float* gates, const float* dgates,

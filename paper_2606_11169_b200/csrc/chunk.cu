@@ -137,7 +137,13 @@ const int kEdges[][2] = {{F_ROUTE, F_SCAN},   {F_SCAN, F_PACK},    {F_PACK, F_GE
 constexpr int PART_BI = 1, PART_BW = 2, PART_ALL = 3;
 int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b, int parts = PART_ALL) {
     switch (task) {
-        case F_ROUTE: return launch_route_topk(c, ln, f->logits, f->topk_idx, f->gates, f->counts_global);
+        case F_ROUTE: {
+            if (f->w_r) {  // N1: the router GEMM writes the logits F1 reads
+                const int rc = launch_router_fwd(c, ln, f->x, f->w_r, f->router_bias, const_cast<float*>(f->logits));
+                if (rc != PIPER_OK) return rc;
+            }
+            return launch_route_topk(c, ln, f->logits, f->topk_idx, f->gates, f->counts_global);
+        }
         case F_SCAN: return launch_scan_rank(c, ln, f->topk_idx, f->counts, f->offsets, f->row_of, f->src_of);
         case F_PACK: return launch_pack(c, ln, f->x, f->gates, f->offsets, f->row_of, f->src_of, f->gate_rows, f->xp);
         case F_GEMM1: return ffn_gemm1(c, ln, routed_problem(c, f));
@@ -148,7 +154,7 @@ int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const p
             return rc != PIPER_OK ? rc : ffn_gemm2(c, ln, p);
         }
         case F_COMBINE:
-            return launch_combine(c, ln, f->o, f->row_of, f->gates, c->D.I_shared ? f->s : nullptr, f->y, true);
+            return launch_combine(c, ln, f->o, f->row_of, f->gates, c->D.I_shared ? f->s : nullptr, nullptr, f->y, true);
         case B_CGRAD:
             return launch_combine_bwd(c, ln, b->dy, b->o, b->src_of, b->row_of, b->gates, b->offsets, b->d_o, b->dgates);
         case B_DGRAD1: return ffn_dgrad1(c, ln, routed_problem(c, b));
@@ -165,8 +171,14 @@ int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const p
             return rc;
         }
         case B_UNPACK:
-            return launch_combine(c, ln, b->dxp, b->row_of, nullptr, c->D.I_shared ? b->dxs : nullptr, b->dx, false);
-        case B_ROUTE_BWD: return launch_route_bwd(c, ln, b->logits, b->topk_idx, b->gates, b->dgates, b->dz_sel);
+            return launch_combine(c, ln, b->dxp, b->row_of, nullptr, c->D.I_shared ? b->dxs : nullptr,
+                                  b->w_r ? b->dx_router : nullptr, b->dx, false);
+        case B_ROUTE_BWD: {
+            const int rc = launch_route_bwd(c, ln, b->logits, b->topk_idx, b->gates, b->dgates, b->dz_sel);
+            if (rc != PIPER_OK || !b->w_r) return rc;
+            // N1: dW_r = x^T dz and the router's term of dX (added by B_UNPACK, which therefore follows this task)
+            return launch_router_bwd(c, ln, b->x, b->w_r, b->topk_idx, b->dz_sel, b->dz_scratch, b->dw_r, b->dx_router);
+        }
     }
     return PIPER_ERR_INVALID;
 }
@@ -180,6 +192,7 @@ bool fwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
     if (ok && c->D.I_shared)
         ok = aligned16(a->ws_gate) && aligned16(a->ws_up) && aligned16(a->ws_down) && aligned16(a->gs_save) &&
              aligned16(a->us_save) && aligned16(a->hs_save) && aligned16(a->s);
+    if (ok && a->w_r) ok = aligned16(a->w_r) && (!a->router_bias || aligned16(a->router_bias));
     return ok;
 }
 bool bwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
@@ -189,12 +202,14 @@ bool bwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
     if (ok && c->D.I_shared)
         ok = aligned16(a->dgs) && aligned16(a->dus) && aligned16(a->dxs) && aligned16(a->dws_gate) &&
              aligned16(a->dws_up) && aligned16(a->dws_down);
+    if (ok && a->w_r) ok = aligned16(a->dw_r) && aligned16(a->dx_router) && aligned16(a->dz_scratch);
     return ok;
 }
 
 }  // namespace
 
 struct PairPlan {
+    bool router;  // the DAG has the N1 edge B.route_bwd -> B.unpack
     int32_t n, n_waits;
     int32_t task_of[N_TASKS], stream_of[N_TASKS], order[N_TASKS], waits[32][2], records[N_TASKS];
 };
@@ -277,7 +292,7 @@ int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
         PIPER_CUDA(c, cudaStreamWaitEvent(side.stream, fork, 0));
         int rc = run_task(c, B_WGRAD, ln, nullptr, a);
         if (rc != PIPER_OK) return rc;
-        for (int t : {B_UNPACK, B_ROUTE_BWD}) {
+        for (int t : {B_ROUTE_BWD, B_UNPACK}) {
             rc = run_task(c, t, side, nullptr, a);
             if (rc != PIPER_OK) return rc;
         }
@@ -285,7 +300,7 @@ int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
         PIPER_CUDA(c, cudaStreamWaitEvent(ln.stream, joined, 0));
         return PIPER_OK;
     }
-    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_ROUTE_BWD, B_UNPACK};
     for (int t : seq) {
         if (t == B_SHARED && !c->D.I_shared) continue;
         const int rc = run_task(c, t, ln, nullptr, a);
@@ -297,7 +312,7 @@ int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {
 int piper_run_chunk_bwd_input(piper_ctx* c, const piper_chunk_args* a, void* stream) {
     if (!c || !bwd_args_ok(c, a)) return PIPER_ERR_INVALID;
     const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
-    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+    const int seq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_SHARED, B_ROUTE_BWD, B_UNPACK};
     for (int t : seq) {
         if (t == B_SHARED && !c->D.I_shared) continue;
         const int rc = run_task(c, t, ln, nullptr, a, PART_BI);
@@ -342,24 +357,25 @@ void task_durations(const piper_ctx* c, float* ms) {
     ms[F_SHARED] = (float)(6 * dis * D.T / tf), ms[B_SHARED] = (float)(12 * dis * D.T / tf);
 }
 
-int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl);
+int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, bool router, PairPlan* pl);
 
 // The plan is a pure function of (descriptor, policy, split): computed once and kept (the profile-guided search
 // costs milliseconds of host time, which would otherwise sit between two launches).
-int make_plan(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+int make_plan(piper_ctx* c, int sm_gemm, int sm_comm, bool router, PairPlan* pl) {
     PairPlan* cached = static_cast<PairPlan*>(c->pair_plan);
-    if (cached && c->plan_sm_gemm == sm_gemm && c->plan_sm_comm == sm_comm) {
+    if (cached && c->plan_sm_gemm == sm_gemm && c->plan_sm_comm == sm_comm && cached->router == router) {
         *pl = *cached;
         return PIPER_OK;
     }
-    const int rc = make_plan_uncached(c, sm_gemm, sm_comm, pl);
+    const int rc = make_plan_uncached(c, sm_gemm, sm_comm, router, pl);
     if (rc != PIPER_OK) return rc;
     if (!cached) cached = new (std::nothrow) PairPlan(), c->pair_plan = cached;
     if (cached) *cached = *pl, c->plan_sm_gemm = sm_gemm, c->plan_sm_comm = sm_comm;
     return PIPER_OK;
 }
 
-int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, bool router, PairPlan* pl) {
+    pl->router = router;
     // task list of this layer (no shared expert -> its two tasks and their edges drop out)
     const bool shared = c->D.I_shared != 0;
     int32_t id_of[N_TASKS], n = 0;
@@ -373,6 +389,8 @@ int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
     int32_t edges[32][2], n_edges = 0, prio[N_TASKS];
     for (const auto& e : kEdges)
         if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
+    if (router)  // N1: B.route_bwd also produces the router's term of dX, which B.unpack adds
+        edges[n_edges][0] = id_of[B_ROUTE_BWD], edges[n_edges][1] = id_of[B_UNPACK], ++n_edges;
     for (int i = 0; i < n; ++i) pl->stream_of[i] = kStreamOf[pl->task_of[i]], prio[i] = pl->task_of[i] >= B_CGRAD ? 1 : 0;
     pl->n_waits = 0;
     if (c->pair_order == PIPER_ORDER_LIST)
@@ -398,7 +416,7 @@ bool split_ok(const piper_ctx* c, int sm_gemm, int sm_comm) {
 }
 
 // Partition + streams + schedule of a split (created once, kept until the split or the partition policy changes).
-int pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
+int pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm, bool router, PairPlan* pl) {
     if (!split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
     if (!c->green || c->green->sm_gemm != sm_gemm || c->green->sm_comm != sm_comm) {
         pair_release(c);
@@ -409,7 +427,7 @@ int pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm, PairPlan* pl) {
             return c->pair_part == PIPER_PART_EXCLUSIVE ? PIPER_ERR_UNSUPPORTED : PIPER_ERR_CUDA;
         }
     }
-    return make_plan(c, sm_gemm, sm_comm, pl);
+    return make_plan(c, sm_gemm, sm_comm, router, pl);
 }
 
 }  // namespace
@@ -432,7 +450,7 @@ int piper_set_pair_policy(piper_ctx* c, int order, int partition, const float* t
 int piper_pair_order(piper_ctx* c, int sm_gemm, int sm_comm, int32_t* order, int32_t* n) {
     if (!c || !order || !n || !split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
     PairPlan pl;
-    const int rc = make_plan(c, sm_gemm, sm_comm, &pl);
+    const int rc = make_plan(c, sm_gemm, sm_comm, false, &pl);
     if (rc != PIPER_OK) return rc;
     for (int i = 0; i < pl.n; ++i) order[i] = pl.task_of[pl.order[i]];
     *n = pl.n;
@@ -442,14 +460,14 @@ int piper_pair_order(piper_ctx* c, int sm_gemm, int sm_comm, int32_t* order, int
 int piper_pair_prepare(piper_ctx* c, int sm_gemm, int sm_comm) {
     if (!c) return PIPER_ERR_INVALID;
     PairPlan pl;
-    return pair_prepare(c, sm_gemm, sm_comm, &pl);
+    return pair_prepare(c, sm_gemm, sm_comm, false, &pl);
 }
 
 int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_chunk_args* b, int sm_gemm, int sm_comm,
                          void* stream) {
     if (!c || !fwd_args_ok(c, f) || !bwd_args_ok(c, b)) return PIPER_ERR_INVALID;
     PairPlan pl;
-    int rc = pair_prepare(c, sm_gemm, sm_comm, &pl);
+    int rc = pair_prepare(c, sm_gemm, sm_comm, b->w_r != nullptr, &pl);
     if (rc != PIPER_OK) return rc;
     GreenPartition* g = c->green;
     c->pair_mode = c->pair_part == PIPER_PART_CHUNK_STREAMS ? 3 : (g->green ? 1 : 2);
@@ -468,7 +486,7 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
         PIPER_CUDA(c, cudaStreamWaitEvent(lf.stream, fork, 0));
         PIPER_CUDA(c, cudaStreamWaitEvent(lb.stream, fork, 0));
         const int fseq[] = {F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE};
-        const int bseq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD};
+        const int bseq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_ROUTE_BWD, B_UNPACK};
         for (int i = 0; i < 7; ++i) {  // enqueued alternately, each chunk in its serial order
             if (fseq[i] != F_SHARED || c->D.I_shared) {
                 rc = run_task(c, fseq[i], lf, f, b);

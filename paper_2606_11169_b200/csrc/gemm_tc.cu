@@ -42,7 +42,7 @@ constexpr int kProfSlots = 16, kProfSlotWords = 160 * 8;  // debug counters: 16 
 constexpr int PANEL_M = 8;  // M tiles per panel of the tile order (L2 reuse of the weight tile)
 
 enum : int { K_MAJOR = 0, MN_MAJOR = 1 };
-enum : int { EPI_SWIGLU_FWD = 0, EPI_STORE = 1, EPI_SWIGLU_BWD = 2, EPI_WGRAD_SPLIT = 3, EPI_WGRAD = 4 };
+enum : int { EPI_SWIGLU_FWD = 0, EPI_STORE = 1, EPI_SWIGLU_BWD = 2, EPI_WGRAD_SPLIT = 3, EPI_WGRAD = 4, EPI_STORE_F32 = 5 };
 
 struct alignas(64) TcParams {
     CUtensorMap a[2], b[2];
@@ -72,6 +72,7 @@ struct alignas(64) TcParams {
     int out_f32;            // wgrad: dW is fp32 (o[] are fp32 maps, 32-column boxes); accum: add into dW (TMA reduce)
     int accum;
     int greedy;             // chunking: 1 = 256-row chunks and a short last one, 0 = equal chunks
+    const float* bias;      // EPI_STORE_F32: added per output column (router logits), or NULL
     int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
 };
 
@@ -218,7 +219,8 @@ __device__ __forceinline__ Tile decode_tile(const TcParams& P, const int* tp, co
         const int g = t / per_group, local = t - g * per_group;
         const int nt = local / P.m_tiles, mt = local - nt * P.m_tiles;
         const int lo = offsets[g], hi = offsets[g + 1];
-        r.g = g, r.m0 = mt * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + BK - 1) / BK;
+        // n_src = 2 (dense dW_r = x^T dz_hi + x^T dz_lo): the K range is walked once per (A, B) pair, kb_per_src blocks each
+        r.g = g, r.m0 = mt * BM, r.n0 = nt * P.tile_n, r.k0 = lo, r.nkb = (hi - lo + BK - 1) / BK * P.n_src;
     }
     return r;
 }
@@ -287,7 +289,22 @@ __device__ __forceinline__ void epilogue_tile(const TcParams& P, uint32_t taddr,
                         float v[16];
     #pragma unroll
                         for (int i = 0; i < 16; ++i) v[i] = zero ? 0.f : __uint_as_float(r0[i]);
-                        if (row_ok) {
+                        if (row_ok && EPI == EPI_STORE_F32) {
+                            // fp32 output (router logits / dW_r): acc (+ bias[column]), columns below n_limit (% 4 == 0)
+                            float* orow = reinterpret_cast<float*>(P.out0) + base;
+#pragma unroll
+                            for (int i = 0; i < 16; i += 4) {
+                                const int col = n0 + c + i;
+                                if (col < P.n_limit) {
+                                    float4 o = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+                                    if (P.bias) {
+                                        const float4 bb = *reinterpret_cast<const float4*>(P.bias + col);
+                                        o.x += bb.x, o.y += bb.y, o.z += bb.z, o.w += bb.w;
+                                    }
+                                    *reinterpret_cast<float4*>(orow + col) = o;
+                                }
+                            }
+                        } else if (row_ok) {
                             if (EPI == EPI_SWIGLU_BWD) {
                                 // v = dH; dG = dH * U * silu'(G), dU = dH * silu(G)
                                 float gv[16], uv[16], dg[16], du[16];
@@ -359,7 +376,7 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
                     uint64_t* bar = &full_bar[stage];
                     mbar_expect_tx(bar, STAGE_BYTES);
                     int src = 0, kk = kb;
-                    if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
+                    if (P.n_src == 2 && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
                     const int k = T.k0 + kk * BK;
                     // A: ragged_m -> rows m0.. of a row buffer (z = 0); wgrad -> columns m0.. of a row buffer
                     if (A_MAJOR == K_MAJOR) {
@@ -1756,6 +1773,12 @@ bool set_smem_attr() {
                                 Cfg2<EPI>::SMEM) == cudaSuccess;
 }
 
+template <int A_MAJOR, int B_MAJOR, int EPI>
+bool set_smem_attr1() {  // 1-CTA kernel only (the router's dense GEMMs)
+    return cudaFuncSetAttribute(tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                SMEM_BYTES) == cudaSuccess;
+}
+
 template <int A_MAJOR, int EPI>
 int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
     long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI>, CfgT<EPI>::SMEM);
@@ -1842,7 +1865,8 @@ int tc_init(piper_ctx* c) {
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
               set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>() &&
               set_smem_attr_t<MN_MAJOR, TEPI_SWIGLU_FWD>() && set_smem_attr_t<MN_MAJOR, TEPI_STORE>() &&
-              set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD>() && set_smem_attr_t<K_MAJOR, TEPI_STORE>();
+              set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD>() && set_smem_attr_t<K_MAJOR, TEPI_STORE>() &&
+              set_smem_attr1<K_MAJOR, MN_MAJOR, EPI_STORE_F32>() && set_smem_attr1<MN_MAJOR, MN_MAJOR, EPI_STORE_F32>();
     if (!ok) {
         cudaGetLastError();
         c->encode_tiled = nullptr;  // not an sm_100a device: the FP32-ALU kernels serve every request
@@ -2014,6 +2038,58 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     }
     const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
     return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * mt * P.n_tiles, two, "tc_ffn_wgrad_down");
+}
+
+// ---- dense GEMMs of the router (N1: z = x W_r, dW_r = x^T dz, dX_r = dz W_r^T) on the 1-CTA kernel ----------------------
+// One group over all T rows (offsets = {0, T}); 128 x 256 tiles; N <= 256 experts is a single N tile whose columns beyond
+// E the TMA fills with zeros.  bf16 x bf16 products are exact in fp32 and the accumulation is fp32 (TMEM).
+bool tc_router_supported(const piper_ctx* c) {
+    const piper_moe_desc& D = c->D;
+    return c->encode_tiled && D.dtype == PIPER_DTYPE_BF16 && D.E % 8 == 0 && D.d >= 64 && D.d % 8 == 0 && D.T >= 1;
+}
+
+// logits [T,E] fp32 = x [T,d] W_r [d,E] (+ bias[E])
+int tc_router_fwd(piper_ctx* c, Lane ln, const void* x, const void* w_r, const float* bias, float* logits) {
+    const piper_moe_desc& D = c->D;
+    TcParams P;
+    memset(&P, 0, sizeof(P));
+    P.offsets = c->shared_offsets, P.G = 1, P.ragged_m = 1, P.n_src = 1, P.tile_n = BN;
+    PIPER_MAP(&P.a[0], x, D.d, D.T, 1, BM);
+    PIPER_MAP(&P.b[0], w_r, D.E, D.d, 1, 64);
+    P.n_tiles = cdiv(D.E, BN), P.kb_per_src = cdiv(D.d, BK), P.n_limit = D.E, P.ld = D.E;
+    P.out0 = reinterpret_cast<__nv_bfloat16*>(logits), P.bias = bias;
+    return launch<K_MAJOR, MN_MAJOR, EPI_STORE_F32>(c, ln, P, (long long)cdiv(D.T, BM) * P.n_tiles, false, "tc_router_fwd");
+}
+
+// dW_r [d,E] fp32 = x^T dz with dz = hi + lo (two bf16 [T,E] tensors): one accumulator over both products
+int tc_router_wgrad(piper_ctx* c, Lane ln, const void* x, const void* dz_hi, const void* dz_lo, float* dw_r) {
+    const piper_moe_desc& D = c->D;
+    TcParams P;
+    memset(&P, 0, sizeof(P));
+    P.offsets = c->shared_offsets, P.G = 1, P.ragged_m = 0, P.n_src = 2, P.tile_n = BN;
+    PIPER_MAP(&P.a[0], x, D.d, D.T, 1, BK);
+    P.a[1] = P.a[0];
+    PIPER_MAP(&P.b[0], dz_hi, D.E, D.T, 1, BK);
+    PIPER_MAP(&P.b[1], dz_lo, D.E, D.T, 1, BK);
+    P.n_tiles = cdiv(D.E, BN), P.m_tiles = cdiv(D.d, BM), P.kb_per_src = cdiv(D.T, BK);
+    P.m_limit = D.d, P.n_limit = D.E, P.ld = D.E, P.group_stride = 0;
+    P.out0 = reinterpret_cast<__nv_bfloat16*>(dw_r);
+    return launch<MN_MAJOR, MN_MAJOR, EPI_STORE_F32>(c, ln, P, (long long)P.m_tiles * P.n_tiles, false, "tc_router_wgrad");
+}
+
+// dX_r [T,d] bf16 = dz W_r^T with dz = hi + lo
+int tc_router_dgrad(piper_ctx* c, Lane ln, const void* dz_hi, const void* dz_lo, const void* w_r, void* dx_r) {
+    const piper_moe_desc& D = c->D;
+    TcParams P;
+    memset(&P, 0, sizeof(P));
+    P.offsets = c->shared_offsets, P.G = 1, P.ragged_m = 1, P.n_src = 2, P.tile_n = BN;
+    PIPER_MAP(&P.a[0], dz_hi, D.E, D.T, 1, BM);
+    PIPER_MAP(&P.a[1], dz_lo, D.E, D.T, 1, BM);
+    PIPER_MAP(&P.b[0], w_r, D.E, D.d, 1, BN);
+    P.b[1] = P.b[0];
+    P.n_tiles = cdiv(D.d, BN), P.kb_per_src = cdiv(D.E, BK), P.n_limit = D.d, P.ld = D.d;
+    P.out0 = static_cast<__nv_bfloat16*>(dx_r);
+    return launch<K_MAJOR, K_MAJOR, EPI_STORE>(c, ln, P, (long long)cdiv(D.T, BM) * P.n_tiles, false, "tc_router_dgrad");
 }
 
 }  // namespace piper

@@ -248,12 +248,13 @@ pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const i
 template <bool BF16, bool WEIGHTED>
 __global__ void __launch_bounds__(kMoveWarps * 32)
 combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, const float* __restrict__ gates,
-               const int4* __restrict__ s, int T, int k, int row_packets, int S, int split_packets,
-               int4* __restrict__ y) {
+               const int4* __restrict__ s, const int4* __restrict__ s2, int T, int k, int row_packets, int S,
+               int split_packets, int4* __restrict__ y) {
     const int lane = threadIdx.x & 31;
     const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
     const int nwarps = gridDim.x * kMoveWarps;
-    const int n_src = k + (s != nullptr ? 1 : 0);
+    if (s == nullptr) s = s2, s2 = nullptr;  // token-row addends (shared expert, router path): s first, then s2
+    const int n_src = k + (s != nullptr ? 1 : 0) + (s2 != nullptr ? 1 : 0);
     for (int item = warp; item < T * S; item += nwarps) {
         const int t = item / S, sp = item - t * S;
         const int my_row = lane < k ? row_of[(size_t)t * k + lane] : -1;
@@ -277,7 +278,7 @@ combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, c
                     if (r < 0) continue;
                     src = o + (size_t)r * row_packets;
                 } else {
-                    src = s + (size_t)t * row_packets;
+                    src = (j == k ? s : s2) + (size_t)t * row_packets;
                 }
                 int4 nxt[U];
                 load_step(nxt, src, p0, lane, hi);  // in flight while the previous source is accumulated
@@ -416,16 +417,16 @@ int launch_pack(piper_ctx* c, Lane ln, const void* x, const float* gates, const 
 }
 
 int launch_combine(piper_ctx* c, Lane ln, const void* o, const int32_t* row_of, const float* gates, const void* s,
-                   void* y, bool weighted) {
+                   const void* s2, void* y, bool weighted) {
     const piper_moe_desc& D = c->D;
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
     int S, split_packets;
     choose_split(ln, D.T, row_packets, S, split_packets);
     const int items = D.T * S;
-    const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s);
+    const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s), *s24 = static_cast<const int4*>(s2);
     int4* y4 = static_cast<int4*>(y);
 #define PIPER_COMBINE(BF, W)                                                                              \
-    combine_kernel<BF, W><<<mover_blocks(ln, items, combine_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, D.T, D.k, row_packets, S, split_packets, y4)
+    combine_kernel<BF, W><<<mover_blocks(ln, items, combine_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, s24, D.T, D.k, row_packets, S, split_packets, y4)
     if (D.dtype == PIPER_DTYPE_BF16) {
         if (weighted) PIPER_COMBINE(true, true); else PIPER_COMBINE(true, false);
     } else {

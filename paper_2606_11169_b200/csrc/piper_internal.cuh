@@ -129,8 +129,8 @@ int launch_scan_rank(piper_ctx*, Lane, const int32_t* topk_idx, int32_t* counts,
                      int32_t* src_of);
 int launch_pack(piper_ctx*, Lane, const void* x, const float* gates, const int32_t* offsets, const int32_t* row_of,
                 const int32_t* src_of, float* gate_rows, void* xp);
-int launch_combine(piper_ctx*, Lane, const void* o, const int32_t* row_of, const float* gates, const void* s, void* y,
-                   bool weighted);
+int launch_combine(piper_ctx*, Lane, const void* o, const int32_t* row_of, const float* gates, const void* s,
+                   const void* s2, void* y, bool weighted);
 int launch_combine_bwd(piper_ctx*, Lane, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
                        const float* gates, const int32_t* offsets, void* d_o, float* dgates);
 
@@ -165,6 +165,16 @@ int tc_ffn_fwd2(piper_ctx*, Lane, const FfnProblem&);    // O = H W_down
 int tc_ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&);  // dG,dU from dO W_down^T and G,U
 int tc_ffn_dgrad2(piper_ctx*, Lane, const FfnProblem&);  // dXp = dG W_gate^T + dU W_up^T
 int tc_ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);   // dW_gate, dW_up, dW_down
+
+// dense GEMMs of the router (N1) on the 1-CTA tcgen05 kernel
+bool tc_router_supported(const piper_ctx*);
+int tc_router_fwd(piper_ctx*, Lane, const void* x, const void* w_r, const float* bias, float* logits);
+int tc_router_wgrad(piper_ctx*, Lane, const void* x, const void* dz_hi, const void* dz_lo, float* dw_r);
+int tc_router_dgrad(piper_ctx*, Lane, const void* dz_hi, const void* dz_lo, const void* w_r, void* dx_r);
+// router.cu
+int launch_router_fwd(piper_ctx*, Lane, const void* x, const void* w_r, const float* bias, float* logits);
+int launch_router_bwd(piper_ctx*, Lane, const void* x, const void* w_r, const int32_t* topk_idx, const float* dz_sel,
+                      void* dz_scratch, float* dw_r, void* dx_router);
 
 // ffn.cu: dispatch between the two GEMM families, task granularity used by the chunk scheduler
 int ffn_gemm1(piper_ctx*, Lane, const FfnProblem&);

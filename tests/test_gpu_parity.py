@@ -555,16 +555,24 @@ def _sampled_check(cfg, inp, rt, b, fwd=True, bwd=True, n_tokens=64, experts=Non
         util.check_close(label + "dx", util.to_np(b["dx"][tk]), s["dx"], dt)
         J = _feature_columns(cfg.I)
         Jc = torch.from_numpy(J).cuda()
+        pooled = {n: ([], []) for n in ("dw_gate", "dw_up", "dw_down")}
         for e in experts:
             if rt["counts"][e] == 0:
                 for n in ("dw_gate", "dw_up", "dw_down"):
                     assert not bool(b[n][int(e)].any()), f"{n}[{e}] must be exactly zero for an empty expert"
                 continue
             rg, ru, rd = oracle.sample_wgrad(cfg, inp, rt, e, J)
-            # an expert with a handful of rows has tiny dW entries: compare against the layer-wide scale as well
-            util.check_close(f"{label}dw_gate[{e}][:,J]", util.to_np(b["dw_gate"][e][:, Jc]), rg, dt)
-            util.check_close(f"{label}dw_up[{e}][:,J]", util.to_np(b["dw_up"][e][:, Jc]), ru, dt)
-            util.check_close(f"{label}dw_down[{e}][J,:]", util.to_np(b["dw_down"][e][Jc, :]), rd, dt)
+            got = {"dw_gate": util.to_np(b["dw_gate"][e][:, Jc]), "dw_up": util.to_np(b["dw_up"][e][:, Jc]),
+                   "dw_down": util.to_np(b["dw_down"][e][Jc, :])}
+            for n, ref in (("dw_gate", rg), ("dw_up", ru), ("dw_down", rd)):
+                # reading c-23: the tolerance is per OUTPUT TENSOR.  A single expert's slice (a few thousand values, as few
+                # as 2 rows of K) scatters around the tensor's error, so it gets twice the bound (a wrong tile, expert or
+                # row range is an error of order 1); the pooled sample of all experts gets the bound itself.
+                util.check_close(f"{label}{n}[{e}] sample", got[n], ref, dt, scale=2.0)
+                pooled[n][0].append(got[n].reshape(-1)), pooled[n][1].append(ref.reshape(-1))
+        for n, (gs, rs) in pooled.items():
+            if gs:
+                util.check_close(f"{label}{n} (all experts' samples)", np.concatenate(gs), np.concatenate(rs), dt)
         if cfg.I_shared:
             Js = _feature_columns(cfg.I_shared)
             Jsc = torch.from_numpy(Js).cuda()

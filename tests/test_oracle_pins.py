@@ -31,6 +31,57 @@ def spread_logits(cfg, rng, gap=0.05):
     return z
 
 
+# ------------------------------------------------------------------------------------- router
+def test_router_closed_forms_and_library_special_case():
+    """oracle_router_fwd / _bwd against what the mathematics fixes: one-hot tokens read a row of
+    W_r (+ bias), an all-ones token sums its columns, integer-valued inputs give exact integers; dW_r of a one-hot dz
+    is a token row of x and dX_r a column of W_r; on random data numpy's fp64 matmul; and the generator's logits
+    (inputs/configs.py, reading c-18) are this sum rounded to fp32 plus one fp32 add of the bias."""
+    cfg = small_cfg(T=6, d=12, E=6, k=3, dtype=C.DT_F32)
+    rng = np.random.default_rng(9)
+    w = rng.integers(-4, 5, size=(cfg.d, cfg.E)).astype(np.float32)
+    bias = rng.integers(-3, 4, size=cfg.E).astype(np.float32)
+    x = np.zeros((cfg.T, cfg.d), np.float32)
+    for t in range(5):
+        x[t, 2 * t] = 1.0
+    x[5] = 1.0
+    z = O.router_fwd(cfg, x, w, bias)
+    for t in range(5):
+        assert (z[t] == w[2 * t].astype(np.float64) + bias).all()
+    assert (z[5] == w.sum(0, dtype=np.float64) + bias).all()
+    assert (O.router_fwd(cfg, x, w) == z - bias).all()
+    xr = rng.normal(size=(cfg.T, cfg.d)).astype(np.float32)
+    dz = np.zeros((cfg.T, cfg.E))
+    dz[3, 4] = 2.0
+    dw, dx = O.router_bwd(cfg, xr, w, dz)
+    assert (dw[:, 4] == 2.0 * xr[3].astype(np.float64)).all() and not np.delete(dw, 4, axis=1).any()
+    assert (dx[3] == 2.0 * w[:, 4].astype(np.float64)).all() and not np.delete(dx, 3, axis=0).any()
+    dzr = rng.normal(size=(cfg.T, cfg.E))
+    dw, dx = O.router_bwd(cfg, xr, w, dzr)
+    np.testing.assert_allclose(dw, xr.astype(np.float64).T @ dzr, rtol=1e-13, atol=1e-14)
+    np.testing.assert_allclose(dx, dzr @ w.astype(np.float64).T, rtol=1e-13, atol=1e-14)
+    np.testing.assert_allclose(O.router_fwd(cfg, xr, w, bias), xr.astype(np.float64) @ w + bias, rtol=1e-13, atol=1e-14)
+    # central differences of <dz, z(x, W)>: the backward terms are the gradients of the forward
+    eps = 1e-6
+    xd, wd = xr.astype(np.float64), w.astype(np.float64)
+    for (t, i) in ((0, 0), (4, 7)):
+        xp_, xm_ = xd.copy(), xd.copy()
+        xp_[t, i] += eps
+        xm_[t, i] -= eps
+        num = ((xp_ @ wd - xm_ @ wd) * dzr).sum() / (2 * eps)
+        assert abs(num - dx[t, i]) < 1e-6 * max(1.0, abs(num))
+    # bf16 configs: the generator's logits = fl32(fl32(sum in fp64) + bias)
+    cfgb = dataclasses.replace(C.C3S, T=40)
+    inp = C.make_inputs(cfgb, weights=False, with_dy=False)
+    zb = O.router_fwd(cfgb, inp["x"], inp["w_r"])
+    assert (inp["logits"] == (zb.astype(np.float32) + inp["bias"][None, :]).astype(np.float32)).all()
+    # dense_dz scatters the k selected entries of each token to their experts' columns and leaves zeros elsewhere
+    idx = np.array([[2, 0, 5], [1, 4, 3]], np.int32)
+    dsel = np.array([[1.0, 2.0, 3.0], [4.0, 5.0, 6.0]])
+    dd = O.dense_dz(small_cfg(T=2, E=6, k=3), idx, dsel)
+    assert dd.tolist() == [[2.0, 0, 1.0, 0, 0, 3.0], [0, 4.0, 0, 6.0, 5.0, 0]]
+
+
 # ------------------------------------------------------------------------------------ routing
 @pytest.mark.parametrize("mode", [0, 1, 2])
 def test_route_invariants(mode):
