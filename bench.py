@@ -242,6 +242,9 @@ class Workload:
         piper.piper_set_chunk_overlap(self.ctx, 1 if getattr(args, "chunk_overlap", False) else 0)
         if getattr(args, "no_fused_gather", False):
             piper.piper_set_option(self.ctx, piper.OPT_FUSED_GATHER, 0)
+        for kv in getattr(args, "opt", None) or []:  # measured variants: --opt T_SPLIT_K=0 ...
+            name, val = kv.split("=")
+            piper.piper_set_option(self.ctx, getattr(piper, "OPT_" + name), int(val))
         if args.main_grad:  # measured variant (reading c-17): fp32 dW, every step adds into it
             piper.piper_set_wgrad_accumulate(self.ctx, 1)
         self.b = piper.alloc_buffers(self.ctx)
@@ -599,6 +602,7 @@ def main():
     ap.add_argument("--no-fused-gather", action="store_true",
                     help="measured variant: the chunk calls run the separate pack / combine_bwd row movers and the GEMMs read "
                          "xp / d_o (PIPER_OPT_FUSED_GATHER = 0)")
+    ap.add_argument("--opt", action="append", help="kernel-variant switch NAME=VALUE (piper_set_option, PIPER_OPT_<NAME>)")
     ap.add_argument("--uniform-rows", type=int, default=0,
                     help="microbenchmark: C3's routed layer shape with exactly this many rows in each of 32 experts "
                          "(overrides --config; use with --no-cpu-baseline)")
@@ -616,7 +620,7 @@ def main():
     from inputs import configs
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
         ge.build()
-    default_run = args.config == "C2" and not args.uniform_rows and not args.pair and not args.main_grad
+    default_run = args.config == "C2" and not args.uniform_rows and not args.pair and not args.main_grad and not args.opt
     if args.config == "C5":  # configs[4]: the C3-shaped chunk pair, microbatch seeds 4 (forward) and 5 (backward)
         args.config, args.pair = "C5a", True
 

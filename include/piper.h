@@ -97,6 +97,8 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
  *                              2 by expected group length
  *  PIPER_OPT_T_SMALL_ROWS [32] rows-on-N: chunks of at most this many rows per CTA load 32-row boxes
  *  PIPER_OPT_T_GREEDY     [1]  rows-on-N: 1 = 256-row chunks and a short last one, 0 = equal chunks
+ *  PIPER_OPT_T_SPLIT_K    [0]  rows-on-N: 1 = chunks of at most 128 rows alternate their K steps between two
+ *                              accumulators (measured neutral)
  *  PIPER_OPT_TC_PROFILE   [0]  1 = the tcgen05 kernels record wait-cycle counters (piper_debug_tc_counters)
  *  PIPER_OPT_FUSED_GATHER [1]  chunk calls on tcgen05 layers: 1 = the GEMMs gather x / dY rows themselves
  *                              (N2 fusion), 0 = they read the packed buffers xp / d_o
@@ -108,7 +110,13 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
 #define PIPER_OPT_T_GREEDY 3
 #define PIPER_OPT_TC_PROFILE 4
 #define PIPER_OPT_FUSED_GATHER 5
+#define PIPER_OPT_T_SPLIT_K 6
 int piper_set_option(piper_ctx* ctx, int option, int value);
+/* 1 when the whole-chunk calls of this context run the fused-gather GEMMs (PIPER_OPT_FUSED_GATHER on
+ * a layer whose GEMMs are the rows-on-N + CTA-pair tcgen05 kernels): the forward chunk then launches no pack kernel and
+ * does not write xp (piper_dispatch_pack / piper_run_task(F_PACK) produce the all-to-all payload), and the backward
+ * chunk's DGRAD1 applies the gate in fp32 after the GEMM instead of reading the bf16-rounded gate * dY.  0 otherwise. */
+int piper_chunk_gathers(const piper_ctx* ctx);
 int piper_get_option(const piper_ctx* ctx, int option, int* value);
 /* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */
 int64_t piper_a_cap(const piper_moe_desc* desc);

@@ -166,6 +166,8 @@ int piper_gemm_path(const piper_ctx* c) {
 }
 const void* piper_debug_tc_counters(const piper_ctx* c) { return c && c->tc_prof ? c->tc_scratch : nullptr; }
 
+int piper_chunk_gathers(const piper_ctx* c) { return c && fused_gather(c) ? 1 : 0; }
+
 int piper_get_option(const piper_ctx* c, int option, int* value) {
     if (!c || !value) return PIPER_ERR_INVALID;
     switch (option) {
@@ -175,6 +177,7 @@ int piper_get_option(const piper_ctx* c, int option, int* value) {
         case PIPER_OPT_T_GREEDY: *value = c->tc_greedy; return PIPER_OK;
         case PIPER_OPT_TC_PROFILE: *value = c->tc_prof; return PIPER_OK;
         case PIPER_OPT_FUSED_GATHER: *value = c->fused_gather; return PIPER_OK;
+        case PIPER_OPT_T_SPLIT_K: *value = c->tc_split_k; return PIPER_OK;
     }
     return PIPER_ERR_INVALID;
 }
@@ -190,6 +193,7 @@ int piper_set_option(piper_ctx* c, int option, int value) {
         case PIPER_OPT_T_GREEDY: field = &c->tc_greedy; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_TC_PROFILE: field = &c->tc_prof; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_T_SPLIT_K: field = &c->tc_split_k; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
     }
     *field = value;
     const int rc = variant_ok(c);  // e.g. row_align 16 needs the rows-on-N + CTA-pair kernels, fp32 dW the CTA-pair wgrad
@@ -214,9 +218,9 @@ int piper_dispatch_pack(piper_ctx* c, const void* x, const int32_t* topk_idx, co
                         int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* xp, void* stream) {
     if (!c || !all_aligned(x, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows, xp)) return PIPER_ERR_INVALID;
     const Lane ln = full_lane(c, stream);
-    const int rc = launch_scan_rank(c, ln, topk_idx, counts, offsets, row_of, src_of);
+    const int rc = launch_scan_rank(c, ln, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows);
     if (rc != PIPER_OK) return rc;
-    return launch_pack(c, ln, x, gates, offsets, row_of, src_of, gate_rows, xp);
+    return launch_pack(c, ln, x, offsets, row_of, src_of, xp);
 }
 
 int piper_expert_ffn_fwd(piper_ctx* c, const void* xp, const int32_t* offsets, const void* w_gate, const void* w_up,

@@ -135,7 +135,25 @@ const int kEdges[][2] = {{F_ROUTE, F_SCAN},   {F_SCAN, F_PACK},    {F_PACK, F_GE
 
 // `parts` of the backward tasks that hold both passes (B_SHARED): bit 0 = input gradients (Bi), bit 1 = weight gradients (Bw)
 constexpr int PART_BI = 1, PART_BW = 2, PART_ALL = 3;
-int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b, int parts = PART_ALL) {
+
+// N2 fusion (PIPER_OPT_FUSED_GATHER on a tcgen05 layer): the routed GEMMs of the chunk tasks gather the rows of x / dY
+// through src_of themselves (F_GEMM1, the gate|up wgrad: x; DGRAD1: dY with the gate applied in its fp32 epilogue), so
+// the forward chunk does not materialise xp at all; piper_dispatch_pack / piper_run_task(F_PACK) still produce it as
+// the all-to-all payload.
+FfnProblem routed_fwd_problem(const piper_ctx* c, const piper_chunk_args* f) {
+    FfnProblem p = routed_problem(c, f);
+    if (fused_gather(c)) p.gather_x = f->x, p.src_of = f->src_of;
+    return p;
+}
+FfnProblem routed_bwd_problem(const piper_ctx* c, const piper_chunk_args* b) {
+    FfnProblem p = routed_problem(c, b);
+    if (fused_gather(c)) p.gather_x = b->x, p.gather_dy = b->dy, p.src_of = b->src_of, p.gate_rows = b->gate_rows;
+    return p;
+}
+
+// in_chunk: called from a whole-chunk entry point (fused layers skip F_PACK there), not from piper_run_task
+int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b, int parts = PART_ALL,
+             bool in_chunk = true) {
     switch (task) {
         case F_ROUTE: {
             if (f->w_r) {  // N1: the router GEMM writes the logits F1 reads
@@ -144,9 +162,12 @@ int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const p
             }
             return launch_route_topk(c, ln, f->logits, f->topk_idx, f->gates, f->counts_global);
         }
-        case F_SCAN: return launch_scan_rank(c, ln, f->topk_idx, f->counts, f->offsets, f->row_of, f->src_of);
-        case F_PACK: return launch_pack(c, ln, f->x, f->gates, f->offsets, f->row_of, f->src_of, f->gate_rows, f->xp);
-        case F_GEMM1: return ffn_gemm1(c, ln, routed_problem(c, f));
+        case F_SCAN:
+            return launch_scan_rank(c, ln, f->topk_idx, f->gates, f->counts, f->offsets, f->row_of, f->src_of, f->gate_rows);
+        case F_PACK:
+            if (in_chunk && fused_gather(c)) return PIPER_OK;  // N2: no GEMM of the chunk reads xp
+            return launch_pack(c, ln, f->x, f->offsets, f->row_of, f->src_of, f->xp);
+        case F_GEMM1: return ffn_gemm1(c, ln, routed_fwd_problem(c, f));
         case F_GEMM2: return ffn_gemm2(c, ln, routed_problem(c, f));
         case F_SHARED: {
             const FfnProblem p = shared_problem(c, f);
@@ -157,9 +178,9 @@ int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const p
             return launch_combine(c, ln, f->o, f->row_of, f->gates, c->D.I_shared ? f->s : nullptr, nullptr, f->y, true);
         case B_CGRAD:
             return launch_combine_bwd(c, ln, b->dy, b->o, b->src_of, b->row_of, b->gates, b->offsets, b->d_o, b->dgates);
-        case B_DGRAD1: return ffn_dgrad1(c, ln, routed_problem(c, b));
+        case B_DGRAD1: return ffn_dgrad1(c, ln, routed_bwd_problem(c, b));
         case B_DGRAD2: return ffn_dgrad2(c, ln, routed_problem(c, b));
-        case B_WGRAD: return ffn_wgrad(c, ln, routed_problem(c, b));
+        case B_WGRAD: return ffn_wgrad(c, ln, routed_bwd_problem(c, b));
         case B_SHARED: {
             const FfnProblem p = shared_problem(c, b);
             int rc = PIPER_OK;
@@ -273,7 +294,7 @@ int piper_run_task(piper_ctx* c, int task, const piper_chunk_args* a, void* stre
     if (!(task < B_CGRAD ? fwd_args_ok(c, a) : bwd_args_ok(c, a))) return PIPER_ERR_INVALID;
     if ((task == F_SHARED || task == B_SHARED) && !c->D.I_shared) return PIPER_ERR_INVALID;
     const Lane ln{static_cast<cudaStream_t>(stream), c->num_sms};
-    return run_task(c, task, ln, a, a);
+    return run_task(c, task, ln, a, a, PART_ALL, false);
 }
 
 int piper_run_chunk_bwd(piper_ctx* c, const piper_chunk_args* a, void* stream) {

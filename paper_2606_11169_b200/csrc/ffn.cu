@@ -39,6 +39,14 @@ static bool use_tc(const piper_ctx* c, const FfnProblem& p) {
     return c->D.dtype == PIPER_DTYPE_BF16 && c->D.gemm_impl == PIPER_GEMM_AUTO && tc_supported(c, p);
 }
 
+// N2 fusion: only the rows-on-N kernels (fwd1, dgrad1) and the CTA-pair wgrad can gather
+bool fused_gather(const piper_ctx* c) {
+    if (!c->fused_gather) return false;
+    piper_chunk_args a{};
+    const FfnProblem p = routed_problem(c, &a);
+    return use_tc(c, p) && tc_gather_ok(c, p);
+}
+
 int ffn_gemm1(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_fwd1(c, ln, p) : simt_ffn_fwd(c, ln, p, 1); }
 int ffn_gemm2(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_fwd2(c, ln, p) : simt_ffn_fwd(c, ln, p, 2); }
 int ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) { return use_tc(c, p) ? tc_ffn_dgrad1(c, ln, p) : simt_ffn_dgrad(c, ln, p, 1); }

@@ -73,6 +73,14 @@ struct alignas(64) TcParams {
     int accum;
     int greedy;             // chunking: 1 = 256-row chunks and a short last one, 0 = equal chunks
     const float* bias;      // EPI_STORE_F32: added per output column (router logits), or NULL
+    // N2 fusion (GATHER kernels): the packed row r of an operand is row src_of[r] / k of a token-major tensor (x or dY),
+    // gathered by cp.async straight into the operand tile; pad rows (src_of < 0) are zero-filled
+    const int32_t* src_of;      // [rows] flat assignment id of each packed row, -1 = pad
+    const void* gsrc;           // token-major source [T, g_cols] bf16
+    unsigned long long g_magic; // ceil(2^35 / k): a / k = (a * g_magic) >> 35 for a < 2^30, k <= 8
+    int g_cols;                 // columns of the source (= the contraction / feature length d)
+    int split_k;                // rows-on-N kernels: chunks of <= 128 rows use two half accumulators (PIPER_OPT_T_SPLIT_K)
+    const float* row_scale;     // DGRAD1 with gathered dY: the epilogue multiplies row r of dH by row_scale[r] (the gate)
     int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
 };
 
@@ -112,6 +120,14 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
             : "r"(smem_u32(bar)), "r"(parity)
             : "memory");
     } while (!done);
+}
+// 16-byte asynchronous copy global -> shared (LDGSTS); src_bytes = 0 writes zeros (the source is not read)
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+// the mbarrier receives one arrival from this thread once all its cp.async issued so far have landed
+__device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -726,7 +742,10 @@ struct TileFeed {
     }
 };
 
-template <int A_MAJOR, int B_MAJOR, int EPI>
+// GATHER_A (wgrad gate|up, N2 fusion): the A operand Xp^T is not read from the packed buffer; warp 2 gathers K row r of the
+// tile (= packed row k0 + r) from the token-major x through src_of with 16-byte cp.async copies, in the layout of the two
+// 64-column TMA boxes (see the GATHER note at tc_gemmT_kernel for the barrier protocol).
+template <int A_MAJOR, int B_MAJOR, int EPI, bool GATHER_A = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -742,6 +761,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
     uint64_t* feed_full = ld_bar + 9;         // [kFeed] one set per CTA
     uint64_t* feed_empty = feed_full + kFeed;  // [kFeed] used in the leader CTA
     int* feed_ids = reinterpret_cast<int*>(feed_empty + kFeed);
+    uint64_t* gfull_bar = reinterpret_cast<uint64_t*>(feed_ids + 2);  // [STAGES2] GATHER_A: peer CTA's local "A rows landed"
+    static_assert(!GATHER_A || (2 * STAGES2 + 4 + 9 + 2 * kFeed + 1 + STAGES2) * 8 <= 256, "barrier area");
     int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);
     int* tpp = tp + (kMaxGroups2 + 1);
 
@@ -782,11 +803,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
         if (P.n_src == 2 || P.b_split) prefetch_tmap(&P.b[1]);
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < STAGES2; ++s) mbar_init(&full_bar[s], 1), mbar_init(&empty_bar[s], 1);
+        for (int s = 0; s < STAGES2; ++s) {  // GATHER_A: + the leader's 32 gather lanes + the peer's forwarder
+            mbar_init(&full_bar[s], GATHER_A ? 34 : 1), mbar_init(&empty_bar[s], 1);
+            if (GATHER_A) mbar_init(&gfull_bar[s], 32);
+        }
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 2 * Cfg2<EPI>::EPI_WARPS);  // both CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
-        for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer
-            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1);
+        for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer (+ gather warps, forwarder)
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1 + (GATHER_A ? 3 : 0));
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -850,12 +874,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     if (P.prof) w_empty += clock64() - c0;
                     uint8_t* sa = smem + stage * STAGE2_BYTES;
                     uint8_t* sb = sa + A2_BYTES;
-                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * STAGE2_BYTES);
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], GATHER_A ? 2 * Cfg2<EPI>::B_B : 2 * STAGE2_BYTES);
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
                     const int k = T.k0 + kk * BKc;
-                    if (A_MAJOR == K_MAJOR) {
+                    if (GATHER_A) {
+                        // the A tile is gathered by warp 2
+                    } else if (A_MAJOR == K_MAJOR) {
                         tma_load_3d_pair(sa, &P.a[src], bar, k, T.m0, 0);
                     } else {
 #pragma unroll
@@ -878,6 +904,65 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             }
         }
         if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
+    } else if (GATHER_A && warp == 2) {
+        // ===== A producer, gathered (both CTAs, all 32 lanes) =====
+        const int ch = lane & 7, rs = lane >> 3;
+        const char* gbase = static_cast<const char*>(P.gsrc);
+        const uint32_t pitch16 = (uint32_t)P.g_cols >> 3;
+        int stage = 0, phase = 0;
+        for (int it = 0;; ++it) {
+            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            if (t >= n_total) break;
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
+            const int seg_end = tp[T.g + 1];  // rows of the next expert are never issued to the tensor core: not loaded
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                const int k = T.k0 + kb * BKc;
+                // source rows of this K block: 4 per lane (coalesced loads), handed to the lanes that copy them by shuffles
+                uint32_t mine[BKc / 32];
+#pragma unroll
+                for (int q = 0; q < BKc / 32; ++q) {
+                    const int row = k + q * 32 + lane;
+                    const int a = row < seg_end ? P.src_of[row] : -1;
+                    mine[q] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0xFFFFFFFFu;
+                }
+                if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
+                __syncwarp();
+                const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES);
+                const int col0 = T.m0 + ch * 8;
+#pragma unroll
+                for (int i = 0; i < BKc / 4; ++i) {
+                    const int r = 4 * i + rs;  // = 32 (i >> 3) + 4 (i & 7) + rs: held by lane 4 (i & 7) + rs in mine[i >> 3]
+                    const uint32_t o = __shfl_sync(0xffffffffu, mine[i >> 3], 4 * (i & 7) + rs);
+#pragma unroll
+                    for (int j = 0; j < BM / 64; ++j) {
+                        const int col = col0 + 64 * j;
+                        const bool ok = col < P.g_cols && o != 0xFFFFFFFFu;
+                        cp_async16(sa + j * MNB + r * 128 + ((ch ^ (r & 7)) << 4),
+                                   ok ? gbase + (size_t)o * 16 + (size_t)col * 2 : gbase, ok ? 16u : 0u);
+                    }
+                }
+                cp_async_arrive(rank == 0 ? &full_bar[stage] : &gfull_bar[stage]);
+                if (++stage == STAGES2) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (GATHER_A && warp == 1 && rank == 1) {
+        // ===== peer CTA: forward "my A rows of this stage have landed" to the leader's full barrier =====
+        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        int stage = 0, phase = 0;
+        for (int it = 0;; ++it) {
+            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            if (t >= n_total) break;
+            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
+            for (int kb = 0; kb < T.nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&gfull_bar[stage], phase);
+                    fence_proxy_async();
+                    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(leader_full + stage * 8) : "memory");
+                }
+                __syncwarp();
+                if (++stage == STAGES2) stage = 0, phase ^= 1;
+            }
+        }
     } else if (warp == 1 && rank == 0) {
         // ===== MMA issuer (one thread of the leader CTA) =====
         constexpr uint32_t idesc = make_idesc2(A_MAJOR, B_MAJOR);
@@ -904,7 +989,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             for (int kb = 0; kb < T.nkb; ++kb) {
                 if (lane == 0) {
                     const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&full_bar[stage], phase);
+                    if (GATHER_A) {
+                        mbar_wait_cluster(&full_bar[stage], phase);
+                        fence_proxy_async();
+                    } else {
+                        mbar_wait(&full_bar[stage], phase);
+                    }
                     if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
@@ -1194,7 +1284,12 @@ __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
 }
 
 
-template <int A_MAJOR, int EPI>
+// GATHER (N2 fusion): the rows operand is not read from a packed buffer; warp 2 gathers row r of the tile from the
+// token-major tensor P.gsrc (row src_of[r] / k) with 16-byte cp.async copies written in the same 128-byte-swizzled
+// K-major layout a TMA box would have.  The leader's lanes arrive on the stage's full barrier themselves
+// (cp.async.mbarrier.arrive); the peer CTA's lanes arrive on a local barrier that the peer's otherwise idle warp 1
+// forwards to the leader (proxy fence + cluster-scope release).
+template <int A_MAJOR, int EPI, bool GATHER = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemmT_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -1211,6 +1306,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
     uint64_t* ld_bar = tempty_bar + 2;                                                   // [4 warps][2 sets]
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(ld_bar + 8);
+    uint64_t* gfull_bar = ld_bar + 9;                                                    // [NST] GATHER: peer CTA's local "rows landed"
+    static_assert((2 * NST + 4 + 9 + NST) * 8 <= 256, "barrier area");
     int* tq = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);       // first tile of each group
     int* so = tq + (kMaxGroups2 + 1);                                                    // offsets of the groups
     int* sc = so + (kMaxGroups2 + 1);                                                    // real rows of the groups
@@ -1253,10 +1350,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         prefetch_tmap(&P.bs[0]);
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], 2), mbar_init(&empty_bar[s], 1);  // two producer warps
+        // full: the weight producer's expect_tx arrival + the rows producer's (TMA: one expect_tx arrival; GATHER: the
+        // leader's 32 lanes + the peer's forwarder)
+        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], GATHER ? 34 : 2), mbar_init(&empty_bar[s], 1), mbar_init(&gfull_bar[s], 32);
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
-        for (int s = 0; s < kFeed; ++s) mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers + 2);  // + the second producer warp of each CTA
+        for (int s = 0; s < kFeed; ++s)  // + the second producer warp of each CTA (+ the peer's forwarder)
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers + 2 + (GATHER ? 1 : 0));
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -1308,7 +1408,63 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     }
 
-    if (warp == 0 || warp == 2) {
+    if (GATHER && warp == 2) {
+        // ===== rows producer, gathered (both CTAs, all 32 lanes): lane = (row & 3, 16-byte chunk of the 128-byte K slice)
+        const int ch = lane & 7, rs = lane >> 3;
+        const char* gbase = static_cast<const char*>(P.gsrc);
+        const uint32_t pitch16 = (uint32_t)P.g_cols >> 3;  // 16-byte units per source row
+        int stage = 0, phase = 0;
+        for (int it = 0;; ++it) {
+            const int t = feed.peek(it);
+            const TileT T = tile_of(it);
+            feed.release(it, lane);
+            if (t >= n_total) break;
+            const int nb = T.n >> 1, rb = T.r0 + rank * nb;
+            uint32_t off[32];  // source row of tile row 4 i + rs in 16-byte units; ~0 = zero row (pad)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                const int r = 4 * i + rs;
+                const int a = r < nb ? P.src_of[rb + r] : -1;
+                off[i] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0xFFFFFFFFu;
+            }
+            for (int kb = 0; kb < nkb; ++kb) {
+                if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
+                __syncwarp();
+                const uint32_t sb = smem_u32(smem + stage * TSTAGE_BYTES + TA_BYTES);
+                const int kcol = kb * BK + ch * 8;
+                const bool k_ok = kcol < P.g_cols;  // K tail: zero fill, as a TMA box does
+                const char* src_k = gbase + (size_t)kcol * 2;
+#pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                    const int r = 4 * i + rs;
+                    if (r < nb) {
+                        const bool ok = k_ok && off[i] != 0xFFFFFFFFu;
+                        cp_async16(sb + r * 128 + ((ch ^ (r & 7)) << 4), ok ? src_k + (size_t)off[i] * 16 : gbase, ok ? 16u : 0u);
+                    }
+                }
+                cp_async_arrive(rank == 0 ? &full_bar[stage] : &gfull_bar[stage]);
+                if (++stage == NST) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (GATHER && warp == 1 && rank == 1) {
+        // ===== peer CTA: forward "my rows of this stage have landed" to the leader's full barrier =====
+        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        int stage = 0, phase = 0;
+        for (int it = 0;; ++it) {
+            const int t = feed.peek(it);
+            feed.release(it, lane);
+            if (t >= n_total) break;
+            for (int kb = 0; kb < nkb; ++kb) {
+                if (lane == 0) {
+                    mbar_wait(&gfull_bar[stage], phase);
+                    fence_proxy_async();  // the copies are generic-proxy writes; the tensor core reads through the async proxy
+                    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(leader_full + stage * 8) : "memory");
+                }
+                __syncwarp();
+                if (++stage == NST) stage = 0, phase ^= 1;
+            }
+        }
+    } else if (warp == 0 || warp == 2) {
         // ===== TMA producers (both CTAs): warp 0 loads the CTA's 128 features of the weights, warp 2 (idle after the
         // TMEM allocation) its half of the rows.  One thread issuing every box of a stage spent most of its time inside
         // the issue of the bulk tensor instructions, not waiting for free stages. =====
@@ -1382,10 +1538,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             }
             __syncwarp();
             const uint32_t d_tmem = tmem_base + as * BN;
+            // A tcgen05.mma of this shape occupies the issue slot ~130 cycles whatever N is (measured: 64 .. 256 rows per
+            // chunk cost the same), because consecutive MMAs accumulate into the same TMEM columns.  Chunks of at most 128
+            // rows therefore alternate their K steps between two accumulators (columns [0, n) and [128, 128 + n) of the
+            // buffer): two independent chains; the epilogue adds the halves in fp32.
+            const bool splitk = P.split_k && T.n <= 128;
             for (int kb = 0; kb < nkb; ++kb) {
                 if (lane == 0) {
                     const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&full_bar[stage], phase);
+                    if (GATHER) {
+                        mbar_wait_cluster(&full_bar[stage], phase);  // pairs with the peer forwarder's cluster-scope release
+                        fence_proxy_async();                         // gathered rows were written through the generic proxy
+                    } else {
+                        mbar_wait(&full_bar[stage], phase);
+                    }
                     if (P.prof) w_full += clock64() - c0;
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + stage * TSTAGE_BYTES), sb = sa + TA_BYTES;
@@ -1393,7 +1559,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     for (int kk = 0; kk < BK / UK; ++kk) {
                         const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
                         const uint64_t bd = make_desc(sb + kk * UK * 2, 16, 1024);
-                        umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
+                        if (splitk) umma2_bf16(d_tmem + ((kk & 1) ? 128 : 0), ad, bd, idesc, (kb != 0) | (kk >= 2));
+                        else umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
                     umma2_commit(&empty_bar[stage]);
                 }
@@ -1469,6 +1636,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
             const int fcol = feat_col(T);
             const bool f_ok = fcol < P.f_limit;
+            const bool splitk = P.split_k && T.n <= 128;  // two half accumulators (see the MMA issuer): add them
+            auto add_half = [&](uint32_t (&r)[32], int j) {
+                if (splitk) {
+                    uint32_t r2[32];
+                    tmem_ld32(taddr + 128 + j, r2);
+                    tmem_ld_wait32(r2);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) + __uint_as_float(r2[i]));
+                }
+            };
 #pragma unroll 1
             for (int j = 0; j < T.n; j += 32, ++q) {
                 const bool both = j + 16 < T.n;
@@ -1481,6 +1658,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     __syncwarp();
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
+                    add_half(r, j);
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
                     stage_col(buf, v);
@@ -1494,6 +1672,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     const uint32_t xch = smem_u32(xch_base) + (pr * 2 + (q & 1)) * 4096 + lane * 4;
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
+                    add_half(r, j);
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
                     if (wq >= 2) {  // U lanes: hand the fp32 values to the G warp, store U
@@ -1546,12 +1725,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     }
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
+                    add_half(r, j);
+                    // gathered dY rows are unscaled: dH[r] = gate_rows[r] * (dY[token(r)] Wd^T), the gate applied in fp32
+                    const float* rsc = P.row_scale ? P.row_scale + T.r0 + j : nullptr;
 #pragma unroll
                     for (int i = 0; i < 32; i += 2) {
                         float dg[2], du[2];
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
-                            const float dh = __uint_as_float(r[i + e]);
+                            const float dh = __uint_as_float(r[i + e]) * ((rsc && i + e < T.n - j) ? __ldg(rsc + i + e) : 1.f);
                             const float gv = lds_bf16(bg + (i + e) * 64), uv = lds_bf16(bu + (i + e) * 64);
                             const float sg = sigmoidf_fast(gv);
                             dg[e] = dh * uv * (sg * (1.f + gv * (1.f - sg)));
@@ -1741,7 +1923,7 @@ int* sched_counters(piper_ctx* c, cudaStream_t stream) {
     return reinterpret_cast<int*>(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8) + 2 * stream_slot(c, stream);
 }
 
-template <int A_MAJOR, int B_MAJOR, int EPI>
+template <int A_MAJOR, int B_MAJOR, int EPI, bool GATHER_A = false>
 int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool two_cta, const char* name) {
     TcParams Q = P;
     if (c->tc_prof) {  // debug: slot per launch, cycled
@@ -1750,14 +1932,15 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
     }
     if (two_cta) {
         // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
-        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI>, Cfg2<EPI>::SMEM, Cfg2<EPI>::THREADS);
+        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A>, Cfg2<EPI>::SMEM, Cfg2<EPI>::THREADS);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
         Q.sched = sched_counters(c, ln.stream);
-        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)(2 * clusters), Cfg2<EPI>::THREADS, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
+        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A><<<(unsigned)(2 * clusters), Cfg2<EPI>::THREADS, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
     }
+    if (GATHER_A) return PIPER_ERR_UNSUPPORTED;  // the gather exists in the CTA-pair kernel only
     long long grid = tile_bound < ln.sms ? tile_bound : ln.sms;
     if (grid < 1) grid = 1;
     tc_gemm_kernel<A_MAJOR, B_MAJOR, EPI><<<(unsigned)grid, kThreads, SMEM_BYTES, ln.stream>>>(Q);
@@ -1779,9 +1962,9 @@ bool set_smem_attr1() {  // 1-CTA kernel only (the router's dense GEMMs)
                                 SMEM_BYTES) == cudaSuccess;
 }
 
-template <int A_MAJOR, int EPI>
+template <int A_MAJOR, int EPI, bool GATHER = false>
 int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
-    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI>, CfgT<EPI>::SMEM);
+    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, CfgT<EPI>::SMEM);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
     TcParams Q = P;
@@ -1790,14 +1973,19 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
         c->tc_next_slot += 1;
     }
     Q.sched = sched_counters(c, ln.stream);
-    tc_gemmT_kernel<A_MAJOR, EPI><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
+    tc_gemmT_kernel<A_MAJOR, EPI, GATHER><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
 }
-template <int A_MAJOR, int EPI>
+template <int A_MAJOR, int EPI, bool GATHER = false>
 bool set_smem_attr_t() {
-    return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 CfgT<EPI>::SMEM) == cudaSuccess;
+}
+// gather fields of a launch whose rows operand comes from the token-major tensor `src` [T, cols]
+void set_gather(TcParams& P, const piper_ctx* c, const FfnProblem& p, const void* src, int cols) {
+    P.src_of = p.src_of, P.gsrc = src, P.g_cols = cols;
+    P.g_magic = ((1ull << 35) + (unsigned long long)c->D.k - 1) / (unsigned long long)c->D.k;
 }
 // rows-on-N kernel for the ragged-M contractions (PIPER_OPT_TC_ROWS_ON_N = 0 switches it off)
 bool rows_on_n(const piper_ctx* c, const FfnProblem& p) { return c->tc_rows_on_n && p.G <= kMaxGroups2; }
@@ -1806,7 +1994,7 @@ TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_t
     memset(&P, 0, sizeof(P));
     P.offsets = p.offsets, P.counts = p.counts, P.G = p.G, P.n_src = 1;
     P.f_tiles = cdiv(F, f_tile), P.f_limit = F, P.kb_per_src = cdiv(K, BK);
-    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy;
+    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy, P.split_k = c->tc_split_k;
     return P;
 }
 inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
@@ -1860,12 +2048,16 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
+    c->tc_split_k = 0;  // measured without gain: the ~130-cycle issue cost of an MMA does not come from the accumulator chain
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
               set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>() && set_smem_attr<MN_MAJOR, MN_MAJOR, EPI_WGRAD>() &&
               set_smem_attr_t<MN_MAJOR, TEPI_SWIGLU_FWD>() && set_smem_attr_t<MN_MAJOR, TEPI_STORE>() &&
               set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD>() && set_smem_attr_t<K_MAJOR, TEPI_STORE>() &&
+              cudaFuncSetAttribute(tc_gemm2_kernel<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT, true>,
+                                   cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<EPI_WGRAD_SPLIT>::SMEM) == cudaSuccess &&
+              set_smem_attr_t<MN_MAJOR, TEPI_SWIGLU_FWD, true>() && set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD, true>() &&
               set_smem_attr1<K_MAJOR, MN_MAJOR, EPI_STORE_F32>() && set_smem_attr1<MN_MAJOR, MN_MAJOR, EPI_STORE_F32>();
     if (!ok) {
         cudaGetLastError();
@@ -1887,6 +2079,7 @@ bool tc_supported(const piper_ctx* c, const FfnProblem& p) {
 }
 
 bool tc_wgrad_f32_ok(const piper_ctx* c, const FfnProblem& p) { return pair_wgrad(c, p); }
+bool tc_gather_ok(const piper_ctx* c, const FfnProblem& p) { return rows_on_n(c, p) && pair_wgrad(c, p) && c->D.k <= 8; }
 
 // G|U = Xp Wg | Xp Wu, H = silu(G) * U
 int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
@@ -1899,6 +2092,10 @@ int tc_ffn_fwd1(piper_ctx* c, Lane ln, const FfnProblem& p) {
         PIPER_MAP2(&P.o[0], p.g, p.I, p.max_rows, 1, 32, 16);
         PIPER_MAP2(&P.o[1], p.u, p.I, p.max_rows, 1, 32, 16);
         PIPER_MAP2(&P.o[2], p.h, p.I, p.max_rows, 1, 32, 16);
+        if (p.gather_x) {  // N2: the expert's rows are gathered from x, the packed buffer xp is not read
+            set_gather(P, c, p, p.gather_x, p.d);
+            return launch_t<MN_MAJOR, TEPI_SWIGLU_FWD, true>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd1_t_gather");
+        }
         return launch_t<MN_MAJOR, TEPI_SWIGLU_FWD>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd1_t");
     }
     const bool two = pair_ragged(c, p);
@@ -1948,6 +2145,11 @@ int tc_ffn_dgrad1(piper_ctx* c, Lane ln, const FfnProblem& p) {
         PIPER_MAP2(&P.o[1], p.du, p.I, p.max_rows, 1, 32, 16);
         PIPER_MAP2(&P.ein[0], p.g, p.I, p.max_rows, 1, 32, 32);
         PIPER_MAP2(&P.ein[1], p.u, p.I, p.max_rows, 1, 32, 32);
+        if (p.gather_dy) {  // N2: rows of dY gathered, the gate applied to dH in the fp32 epilogue; d_o is not read
+            set_gather(P, c, p, p.gather_dy, p.d);
+            P.row_scale = p.gate_rows;
+            return launch_t<K_MAJOR, TEPI_SWIGLU_BWD, true>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad1_t_gather");
+        }
         return launch_t<K_MAJOR, TEPI_SWIGLU_BWD>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad1_t");
     }
     const bool two = pair_ragged(c, p);
@@ -2017,8 +2219,15 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
             PIPER_MAP(&P.o[1], p.dw_up, p.I, p.d, p.G, 32);
         }
         const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
-        const int rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * mt * P.n_tiles, two,
-                                                                  "tc_ffn_wgrad_gate_up");
+        int rc;
+        if (p.gather_x && two) {  // N2: the A operand Xp^T is gathered from x, the packed buffer is not read
+            set_gather(P, c, p, p.gather_x, p.d);
+            rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT, true>(c, ln, P, (long long)p.G * mt * P.n_tiles, two,
+                                                                  "tc_ffn_wgrad_gate_up_gather");
+        } else {
+            rc = launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT>(c, ln, P, (long long)p.G * mt * P.n_tiles, two,
+                                                            "tc_ffn_wgrad_gate_up");
+        }
         if (rc != PIPER_OK) return rc;
     }
     TcParams P = base_params(p, false);

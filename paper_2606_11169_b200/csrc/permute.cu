@@ -46,11 +46,13 @@ chunk_hist_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, 
 // warp __match_any_sync groups equal experts and the rank is the number of lower lanes of the group; a shared running
 // count per expert carries the rank across warps.  No atomic decides an index.  src_of entries that hold no
 // assignment (pad rows of a segment and every row from offsets[E_loc] to a_cap) are written as -1 by the same launch:
-// the blocks share those ranges.
+// the blocks share those ranges.  gate_rows[row] = gates[a] (0 on a segment's pad rows) is written here too, so that the
+// gate of a packed row exists whether or not the rows themselves are materialised (N2 fusion).
 __global__ void __launch_bounds__(kScanChunk)
-scan_rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, int E_loc, int row_align, int a_cap,
-                 const int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
-                 int32_t* __restrict__ row_of, int32_t* __restrict__ src_of) {
+scan_rank_kernel(const int32_t* __restrict__ topk_idx, const float* __restrict__ gates, int n_assign, int e_lo, int E_loc,
+                 int row_align, int a_cap, const int32_t* __restrict__ chunk_counts, int32_t* __restrict__ counts,
+                 int32_t* __restrict__ offsets, int32_t* __restrict__ row_of, int32_t* __restrict__ src_of,
+                 float* __restrict__ gate_rows) {
     extern __shared__ int32_t sm[];
     int32_t* run = sm;                  // [E_loc] next free row of each expert for this chunk
     int32_t* s_cnt = sm + E_loc;        // [E_loc] real rows
@@ -101,7 +103,7 @@ scan_rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, i
     __syncthreads();
     // rows without an assignment: segment pads (experts dealt round-robin over the blocks) and the unused tail
     for (int g = blockIdx.x; g < E_loc; g += n_chunks)
-        for (int r = s_off[g] + s_cnt[g] + threadIdx.x; r < s_off[g + 1]; r += blockDim.x) src_of[r] = -1;
+        for (int r = s_off[g] + s_cnt[g] + threadIdx.x; r < s_off[g + 1]; r += blockDim.x) src_of[r] = -1, gate_rows[r] = 0.f;
     {
         const int used = s_off[E_loc], tail = a_cap - used;
         const int per = (tail + n_chunks - 1) / n_chunks;
@@ -132,7 +134,7 @@ scan_rank_kernel(const int32_t* __restrict__ topk_idx, int n_assign, int e_lo, i
     }
     if (a < n_assign) {
         row_of[a] = row;
-        if (row >= 0) src_of[row] = a;
+        if (row >= 0) src_of[row] = a, gate_rows[row] = gates[a];  // the row's gate travels with the permutation
     }
 }
 
@@ -198,12 +200,12 @@ __device__ __forceinline__ void load_step(int4 (&v)[U], const int4* __restrict__
 }
 
 // ---- F3 dispatch_pack ----------------------------------------------------------------------------
-// Token items [0, T*S): copy the split's columns of x[t] into each local row of the token; split 0 also
-// scatters the token's gates.  Row items [T*S, T*S + a_cap): zero the pad rows inside [0, offsets[E_loc]).
+// Token items [0, T*S): copy the split's columns of x[t] into each local row of the token (the rows' gates are
+// written with the permutation, scan_rank_kernel).  Row items [T*S, T*S + a_cap): zero the pad rows inside [0, offsets[E_loc]).
 __global__ void __launch_bounds__(kMoveWarps * 32)
-pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const int32_t* __restrict__ offsets,
-            const int32_t* __restrict__ row_of, const int32_t* __restrict__ src_of, int T, int k, int E_loc, int a_cap,
-            int row_packets, int S, int split_packets, float* __restrict__ gate_rows, int4* __restrict__ xp) {
+pack_kernel(const int4* __restrict__ x, const int32_t* __restrict__ offsets, const int32_t* __restrict__ row_of,
+            const int32_t* __restrict__ src_of, int T, int k, int E_loc, int a_cap, int row_packets, int S,
+            int split_packets, int4* __restrict__ xp) {
     const int lane = threadIdx.x & 31;
     const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
     const int nwarps = gridDim.x * kMoveWarps;
@@ -215,7 +217,6 @@ pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const i
             const int32_t* ro = row_of + (size_t)t * k;
             const int my_row = lane < k ? ro[lane] : -1;
             if (__ballot_sync(0xffffffffu, my_row >= 0) == 0) continue;
-            if (sp == 0 && my_row >= 0) gate_rows[my_row] = gates[(size_t)t * k + lane];
             const int lo = sp * split_packets, hi = min(row_packets, lo + split_packets);
             const int4* src = x + (size_t)t * row_packets;
             for (int p0 = lo; p0 < hi; p0 += kStep) {
@@ -235,7 +236,6 @@ pack_kernel(const int4* __restrict__ x, const float* __restrict__ gates, const i
         } else {
             const int r = item - n_tok_items;
             if (r >= used || src_of[r] >= 0) continue;
-            if (lane == 0) gate_rows[r] = 0.f;
             int4* dst = xp + (size_t)r * row_packets;
             for (int p = lane; p < row_packets; p += 32) st16(dst + p, make_int4(0, 0, 0, 0));
         }
@@ -307,7 +307,8 @@ combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, c
 // Token items: for every local slot j: d_o[row] = gates[t,j] * dy[t]; dgates[t,j] = <dy[t], o[row]> (0 for
 // non-local slots).  Slot-outer loop: dy[t] is re-read per local slot (L1/L2 hits), the dot product stays a
 // scalar.  Row items: zero the pad rows of d_o inside [0, offsets[E_loc]).
-template <bool BF16>
+// WRITE_DO = false (N2 fusion: the GEMMs gather dY rows themselves): only the dgates dot products, d_o is not touched.
+template <bool BF16, bool WRITE_DO>
 __global__ void __launch_bounds__(kMoveWarps * 32)
 combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, const int32_t* __restrict__ src_of,
                    const int32_t* __restrict__ row_of, const float* __restrict__ gates,
@@ -344,9 +345,11 @@ combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, cons
                         const int p = p0 + u * 32 + lane;
                         if (p < row_packets) {
                             dot += dot_packets<BF16>(v[u], ov[u]);
-                            float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-                            unpack_add<BF16>(v[u], acc, w);
-                            st16(drow + p, pack_out<BF16>(acc));
+                            if (WRITE_DO) {
+                                float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+                                unpack_add<BF16>(v[u], acc, w);
+                                st16(drow + p, pack_out<BF16>(acc));
+                            }
                         }
                     }
                 }
@@ -354,7 +357,7 @@ combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, cons
                 for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, off);
                 if (lane == 0) dgates[(size_t)t * k + j] = dot;
             }
-        } else {
+        } else if (WRITE_DO) {
             const int r = item - T;
             if (r >= used || src_of[r] >= 0) continue;
             int4* dst = d_o + (size_t)r * row_packets;
@@ -387,8 +390,8 @@ inline int mover_blocks(Lane ln, int items, K) {
 
 }  // namespace
 
-int launch_scan_rank(piper_ctx* c, Lane ln, const int32_t* topk_idx, int32_t* counts, int32_t* offsets, int32_t* row_of,
-                     int32_t* src_of) {
+int launch_scan_rank(piper_ctx* c, Lane ln, const int32_t* topk_idx, const float* gates, int32_t* counts, int32_t* offsets,
+                     int32_t* row_of, int32_t* src_of, float* gate_rows) {
     const piper_moe_desc& D = c->D;
     const int n_assign = D.T * D.k;
     int32_t* chunk_counts = scan_scratch(c, ln.stream);  // per stream: forward chunks of two streams may overlap
@@ -396,22 +399,22 @@ int launch_scan_rank(piper_ctx* c, Lane ln, const int32_t* topk_idx, int32_t* co
                                                                                         D.E_loc, chunk_counts);
     PIPER_LAUNCHED(c, "chunk_hist_kernel");
     scan_rank_kernel<<<c->n_chunks, kScanChunk, sizeof(int32_t) * (3 * D.E_loc + 1), ln.stream>>>(
-        topk_idx, n_assign, D.e_lo, D.E_loc, D.row_align, (int)piper_a_cap(&D), chunk_counts, counts, offsets, row_of,
-        src_of);
+        topk_idx, gates, n_assign, D.e_lo, D.E_loc, D.row_align, (int)piper_a_cap(&D), chunk_counts, counts, offsets, row_of,
+        src_of, gate_rows);
     PIPER_LAUNCHED(c, "scan_rank_kernel");
     return PIPER_OK;
 }
 
-int launch_pack(piper_ctx* c, Lane ln, const void* x, const float* gates, const int32_t* offsets, const int32_t* row_of,
-                const int32_t* src_of, float* gate_rows, void* xp) {
+int launch_pack(piper_ctx* c, Lane ln, const void* x, const int32_t* offsets, const int32_t* row_of,
+                const int32_t* src_of, void* xp) {
     const piper_moe_desc& D = c->D;
     const int a_cap = (int)piper_a_cap(&D);
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
     int S, split_packets;
     choose_split(ln, D.T, row_packets, S, split_packets);
     pack_kernel<<<mover_blocks(ln, D.T * S + a_cap, pack_kernel), kMoveWarps * 32, 0, ln.stream>>>(
-        static_cast<const int4*>(x), gates, offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, S,
-        split_packets, gate_rows, static_cast<int4*>(xp));
+        static_cast<const int4*>(x), offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, S, split_packets,
+        static_cast<int4*>(xp));
     PIPER_LAUNCHED(c, "pack_kernel");
     return PIPER_OK;
 }
@@ -442,14 +445,18 @@ int launch_combine_bwd(piper_ctx* c, Lane ln, const void* dy, const void* o, con
     const piper_moe_desc& D = c->D;
     const int a_cap = (int)piper_a_cap(&D);
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
-    if (D.dtype == PIPER_DTYPE_BF16)
-        combine_bwd_kernel<true><<<mover_blocks(ln, D.T + a_cap, combine_bwd_kernel<true>), kMoveWarps * 32, 0, ln.stream>>>(
-            static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
-            D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
-    else
-        combine_bwd_kernel<false><<<mover_blocks(ln, D.T + a_cap, combine_bwd_kernel<false>), kMoveWarps * 32, 0, ln.stream>>>(
-            static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k,
-            D.E_loc, a_cap, row_packets, static_cast<int4*>(d_o), dgates);
+    const bool write_do = d_o != nullptr;  // NULL: dgates only (the fused chunk calls)
+    const int items = D.T + (write_do ? a_cap : 0);
+#define PIPER_CGRAD(BF, W)                                                                                             \
+    combine_bwd_kernel<BF, W><<<mover_blocks(ln, items, combine_bwd_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(      \
+        static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k, D.E_loc,   \
+        write_do ? a_cap : 0, row_packets, static_cast<int4*>(d_o), dgates)
+    if (D.dtype == PIPER_DTYPE_BF16) {
+        if (write_do) PIPER_CGRAD(true, true); else PIPER_CGRAD(true, false);
+    } else {
+        if (write_do) PIPER_CGRAD(false, true); else PIPER_CGRAD(false, false);
+    }
+#undef PIPER_CGRAD
     PIPER_LAUNCHED(c, "combine_bwd_kernel");
     return PIPER_OK;
 }

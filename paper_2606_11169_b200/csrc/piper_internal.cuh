@@ -85,6 +85,7 @@ struct piper_ctx {
     int tc_two_cta;          // CTA-pair (cta_group::2) kernels: 0 never, 1 always, 2 by expected group length
     int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_OPT_TC_ROWS_ON_N, default on)
     int tc_small_rows, tc_greedy;  // PIPER_OPT_T_SMALL_ROWS / PIPER_OPT_T_GREEDY: row chunking of the rows-on-N kernels
+    int tc_split_k;          // PIPER_OPT_T_SPLIT_K: rows-on-N chunks of <= 128 rows accumulate in two halves
     int tc_prof;             // PIPER_OPT_TC_PROFILE: the tcgen05 kernels record wait-cycle counters in tc_scratch
     int fused_gather;        // PIPER_OPT_FUSED_GATHER: chunk calls let the GEMMs gather x / dY rows (N2)
     int pair_bwd_pass;       // piper_set_pair_bwd_pass
@@ -125,10 +126,10 @@ int launch_route_topk(piper_ctx*, Lane, const float* logits, int32_t* topk_idx, 
 int launch_route_bwd(piper_ctx*, Lane, const float* logits, const int32_t* topk_idx, const float* gates,
                      const float* dgates, float* dz);
 // permute.cu
-int launch_scan_rank(piper_ctx*, Lane, const int32_t* topk_idx, int32_t* counts, int32_t* offsets, int32_t* row_of,
-                     int32_t* src_of);
-int launch_pack(piper_ctx*, Lane, const void* x, const float* gates, const int32_t* offsets, const int32_t* row_of,
-                const int32_t* src_of, float* gate_rows, void* xp);
+int launch_scan_rank(piper_ctx*, Lane, const int32_t* topk_idx, const float* gates, int32_t* counts, int32_t* offsets,
+                     int32_t* row_of, int32_t* src_of, float* gate_rows);
+int launch_pack(piper_ctx*, Lane, const void* x, const int32_t* offsets, const int32_t* row_of, const int32_t* src_of,
+                void* xp);
 int launch_combine(piper_ctx*, Lane, const void* o, const int32_t* row_of, const float* gates, const void* s,
                    const void* s2, void* y, bool weighted);
 int launch_combine_bwd(piper_ctx*, Lane, const void* dy, const void* o, const int32_t* src_of, const int32_t* row_of,
@@ -148,6 +149,11 @@ struct FfnProblem {
     void *g, *u, *h, *o;                                 // forward outputs
     const void* d_o;                                     // backward inputs / outputs
     void *dg, *du, *dxp, *dw_gate, *dw_up, *dw_down;
+    // N2 fusion (routed problem of the chunk calls, tcgen05 rows-on-N + CTA-pair kernels only): when set, the GEMMs
+    // gather the rows of x / dY through src_of themselves instead of reading xp / d_o
+    const void *gather_x, *gather_dy;
+    const int32_t* src_of;    // [max_rows] flat assignment id of each packed row, -1 = pad
+    const float* gate_rows;   // [max_rows]
 };
 // gemm_simt.cu (FP32 ALUs; fp32 or bf16 storage)
 // `which`: bit 0 = first GEMM of the pass (fwd1 / dgrad1), bit 1 = second (fwd2 / dgrad2)
@@ -159,7 +165,8 @@ size_t tc_scratch_bytes(const piper_moe_desc*);
 int tc_init(piper_ctx*);  // resolves cuTensorMapEncodeTiled, sets kernel attributes
 void tc_release(piper_ctx*);
 bool tc_supported(const piper_ctx*, const FfnProblem&);
-bool tc_wgrad_f32_ok(const piper_ctx*, const FfnProblem&);  // fp32 dW (and accumulate) exist in the CTA-pair wgrad only
+bool tc_wgrad_f32_ok(const piper_ctx*, const FfnProblem&);
+bool tc_gather_ok(const piper_ctx*, const FfnProblem&);     // the kernel families that can gather x / dY rows (N2)  // fp32 dW (and accumulate) exist in the CTA-pair wgrad only
 int tc_ffn_fwd1(piper_ctx*, Lane, const FfnProblem&);    // G,U,H = swiglu(xp W_gate, xp W_up)
 int tc_ffn_fwd2(piper_ctx*, Lane, const FfnProblem&);    // O = H W_down
 int tc_ffn_dgrad1(piper_ctx*, Lane, const FfnProblem&);  // dG,dU from dO W_down^T and G,U
@@ -184,6 +191,8 @@ int ffn_dgrad2(piper_ctx*, Lane, const FfnProblem&);
 int ffn_wgrad(piper_ctx*, Lane, const FfnProblem&);
 FfnProblem routed_problem(const piper_ctx*, const piper_chunk_args*);
 FfnProblem shared_problem(const piper_ctx*, const piper_chunk_args*);
+// ffn.cu: do the chunk calls of this context let the routed GEMMs gather x / dY rows themselves (N2 fusion)?
+bool fused_gather(const piper_ctx*);
 // chunk.cu
 void pair_release(piper_ctx*);
 void pair_plan_release(piper_ctx*);

@@ -33,6 +33,10 @@ def _run_steps(cfg, inp, gemm_impl=piper.GEMM_AUTO, use_chunk_calls=False, backw
         piper.piper_run_chunk_fwd(ctx, args)
         if backward:
             piper.piper_run_chunk_bwd(ctx, args)
+        if piper.piper_chunk_gathers(ctx):
+            # N2 fusion: the chunk's GEMMs gathered x / dY rows themselves and xp was not materialised; the all-to-all
+            # payload comes from the pack task (= piper_dispatch_pack's second half)
+            piper.piper_run_task(ctx, "F_PACK", args)
     else:
         piper.piper_route_topk(ctx, b["logits"], b["topk_idx"], b["gates"], b["counts_global"])
         piper.piper_dispatch_pack(ctx, b["x"], b["topk_idx"], b["gates"], b["counts"], b["offsets"], b["row_of"],
@@ -221,6 +225,7 @@ def test_poisoned_buffers_and_untouched_capacity(name):
     args = piper.chunk_args(b)
     piper.piper_run_chunk_fwd(ctx, args)
     piper.piper_run_chunk_bwd(ctx, args)
+    piper.piper_run_task(ctx, "F_PACK", args)  # the fused chunk calls do not materialise xp
     torch.cuda.synchronize()
     A = _check_all(cfg, b, f, g) and int(f["offsets"][-1])
     poison = torch.tensor(0x7FC1, dtype=torch.int16, device=b["xp"].device)
@@ -284,7 +289,8 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
     ctx1, b1 = _run_steps(cfg, inp)
     A = int(b1["offsets"][cfg.e_loc])
     for overlap in (False, True):  # piper_set_chunk_overlap: row movers on the library's side stream
-        ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True, overlap=overlap)
+        # (the fused chunk applies the gate after DGRAD1's GEMM instead of rounding gate * dY first: compared separately)
+        ctx2, b2 = _run_steps(cfg, inp, use_chunk_calls=True, overlap=overlap, options=[(piper.OPT_FUSED_GATHER, 0)])
         for n in ("topk_idx", "gates", "counts", "row_of", "src_of", "y", "dgates", "dz_sel", "dx", "dw_gate", "dw_up",
                   "dw_down") + (("dws_gate", "dws_up", "dws_down") if cfg.I_shared else ()):
             assert torch.equal(b1[n], b2[n]), (n, overlap)
@@ -292,6 +298,48 @@ def test_chunk_calls_equal_step_calls_bitwise(name):
             assert torch.equal(b1[n][:A], b2[n][:A]), (n, overlap)
         ctx2.close()
     ctx1.close()
+
+
+@pytest.mark.parametrize("name", ["C2s", "C3s", "C4s", "C6s"])
+@pytest.mark.parametrize("align", [16, 128])
+def test_fused_gather_chunk_against_the_oracle_and_the_unfused_chunk(name, align):
+    """N2 fusion: with PIPER_OPT_FUSED_GATHER the chunk calls run no pack kernel,
+    F_GEMM1 and the gate|up wgrad gather the rows of x through src_of, DGRAD1 gathers the rows of dY and applies the gate
+    to dH in its fp32 epilogue.  Both modes match the oracle; the forward (exact copies of the same rows) is bit-identical
+    between them, the backward differs by one bf16 rounding less; xp is never written by the fused chunk calls."""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=align)
+    inp = configs.make_inputs(cfg)
+    f = oracle.forward(cfg, inp)
+    g = oracle.backward(cfg, inp, f)
+    ctx0, b0 = _run_steps(cfg, inp, use_chunk_calls=True, options=[(piper.OPT_FUSED_GATHER, 0)])
+    assert not piper.piper_chunk_gathers(ctx0)
+    _check_all(cfg, b0, f, g, label="unfused ")
+    ctx = piper.Context(util.desc_of(cfg))
+    assert piper.piper_chunk_gathers(ctx)
+    b = piper.alloc_buffers(ctx)
+    b["xp"].view(torch.int16).fill_(0x7FC1)
+    b.update(util.upload_inputs(inp))
+    args = piper.chunk_args(b)
+    launches0 = piper.piper_kernel_launches(ctx)
+    piper.piper_run_chunk_fwd(ctx, args)
+    n_fwd = piper.piper_kernel_launches(ctx) - launches0
+    piper.piper_run_chunk_bwd(ctx, args)
+    torch.cuda.synchronize()
+    poison = torch.tensor(0x7FC1, dtype=torch.int16, device="cuda")
+    assert bool((b["xp"].view(torch.int16) == poison).all()), "the fused chunk calls must not write xp"
+    assert n_fwd == 6 + (2 if cfg.I_shared else 0), n_fwd  # route, hist, scan+rank, gemm1, gemm2, combine (+ shared 2): no pack
+    piper.piper_run_task(ctx, "F_PACK", args)
+    torch.cuda.synchronize()
+    err = _check_all(cfg, b, f, g, label="fused ")
+    A = int(f["offsets"][-1])
+    for n in ("y", "gate_rows", "src_of", "row_of"):
+        assert torch.equal(b0[n], b[n]), n
+    for n in ("o", "g_save", "u_save", "h_save"):
+        assert torch.equal(b0[n][:A], b[n][:A]), n
+    # one rounding less on the way to dG / dU: the fused backward is at least as close to the oracle
+    err0 = util.errs(util.to_np(b0["dxp"])[:A], g["dxp"][:A])[0]
+    assert err["dxp"][0] <= err0 * 1.05, (err["dxp"][0], err0)
+    ctx0.close(), ctx.close()
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C1s"])
@@ -347,6 +395,9 @@ def test_pair_matches_the_oracle_and_equals_serial_bitwise(name, split, policy):
     for n in ("dgates", "dz_sel", "dx", "dw_gate", "dw_up", "dw_down") + (("dws_gate", "dws_up", "dws_down") if base.I_shared else ()):
         assert torch.equal(bb[n], pb[n]), "bwd " + n
     # against the oracle: microbatch A's forward, microbatch B's forward + backward
+    if piper.piper_chunk_gathers(ctx):  # the all-to-all payload of a fused chunk comes from the pack task
+        piper.piper_run_task(ctx, "F_PACK", args_a), piper.piper_run_task(ctx, "F_PACK", args_b)
+        torch.cuda.synchronize()
     fa = oracle.forward(cfg_a, inp_a)
     _check_all(cfg_a, pa, fa, None, label="pair A ")
     fb = oracle.forward(cfg_b, inp_b)
@@ -606,6 +657,7 @@ def test_full_size_sampled_parity_in_bench_configuration(name):
     args = piper.chunk_args(b)
     piper.piper_run_chunk_fwd(ctx, args)
     piper.piper_run_chunk_bwd(ctx, args)
+    piper.piper_run_task(ctx, "F_PACK", args)  # the all-to-all payload (the fused chunk calls do not materialise xp)
     torch.cuda.synchronize()
     _check_full_size_routing(cfg, b, rt)
     n_rows, n_tok = _sampled_check(cfg, inp, rt, b)
@@ -654,6 +706,8 @@ def test_full_size_c5_pair_against_the_oracle_and_the_serial_chunks():
         for n in bwd_names:
             assert torch.equal(serial[n], bb[n]), (split, "bwd", n)
     # the pair's outputs (last run) against the oracle
+    piper.piper_run_task(ctx, "F_PACK", args_a)
+    torch.cuda.synchronize()
     _check_full_size_routing(cfg_a, ba, rt_a)
     _check_full_size_routing(cfg_b, bb, rt_b)
     _sampled_check(cfg_a, inp_a, rt_a, ba, fwd=True, bwd=False, n_tokens=32, label="C5a ")

@@ -20,7 +20,7 @@ pytestmark = pytest.mark.gpu
 
 # fp32 accumulation of K = d <= 7168 exact products of magnitude ~0.02: error ~ sqrt(d) * 2^-24 * |z| ~ 1e-5 at most
 EPS_GAP = 1e-4
-LOGIT_TOL = 2e-6  # relative Frobenius error of the logits (measured 2e-7 .. 6e-7)
+LOGIT_TOL = 1e-5  # north_star's fp32 bar; measured 4.5e-6 at d = 4096 (sequential fp32 accumulation: sqrt(d) * 2^-24)
 
 
 def _router_inputs(cfg):
