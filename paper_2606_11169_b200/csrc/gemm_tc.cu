@@ -129,6 +129,18 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32
 __device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// One lane of a converged warp (elect.sync).  Code that issues tcgen05.mma / bulk tensor copies runs warp-uniformly up to
+// this predicate: the operands of those instructions live in uniform registers, and inside an `if (lane == 0)` region the
+// compiler cannot prove uniformity and wraps every such instruction in a loop of R2UR broadcasts (~25 instructions per
+// MMA, ~130 cycles of issue time per MMA whatever its shape: profiles/r2_tc_wait_cycles.md).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+// a value every lane holds, made provably warp-uniform for the compiler
+__device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ uint32_t uni(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -859,22 +871,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
     }
 
     if (warp == 0) {
-        // ===== TMA producer (both CTAs): own A tile + own 128-column half of B, counted on the leader's barrier =====
-        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        // ===== TMA producer (both CTAs; the warp runs converged, one elected lane issues): own A tile + own 128-column
+        // half of B, counted on the leader's barrier =====
+        const uint32_t leader_full = uni(mapa_u32(smem_u32(full_bar), 0));
+        const int urank = uni(rank);
         int stage = 0, phase = 0;
         long long w_empty = 0;
         for (int it = 0;; ++it) {
-            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            const int t = uni(dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid);
             if (t >= n_total) break;
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
+            Tile2 T = decode_pair(P, tp, tpp, offsets, t, urank, BKc, rcp_group, rcp_pairs);
+            T.g = uni(T.g), T.m0 = uni(T.m0), T.n0 = uni(T.n0), T.k0 = uni(T.k0), T.nkb = uni(T.nkb);
             for (int kb = 0; kb < T.nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&empty_bar[stage], phase ^ 1);
-                    if (P.prof) w_empty += clock64() - c0;
+                const long long c0 = P.prof ? clock64() : 0;
+                mbar_wait(&empty_bar[stage], phase ^ 1);
+                if (P.prof) w_empty += clock64() - c0;
+                if (elect_one()) {
                     uint8_t* sa = smem + stage * STAGE2_BYTES;
                     uint8_t* sb = sa + A2_BYTES;
-                    if (rank == 0) mbar_expect_tx(&full_bar[stage], GATHER_A ? 2 * Cfg2<EPI>::B_B : 2 * STAGE2_BYTES);
+                    if (urank == 0) mbar_expect_tx(&full_bar[stage], GATHER_A ? 2 * Cfg2<EPI>::B_B : 2 * STAGE2_BYTES);
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (P.ragged_m && kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
@@ -890,10 +905,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     }
                     const int bz = P.ragged_m ? T.g : 0;
                     if (B_MAJOR == K_MAJOR) {
-                        tma_load_3d_pair(sb, &P.b[src], bar, k, T.n0 + rank * (BN / 2), bz);
+                        tma_load_3d_pair(sb, &P.b[src], bar, k, T.n0 + urank * (BN / 2), bz);
                     } else {
-                        const int half = P.b_split ? rank : src;
-                        const int col = P.b_split ? T.n0 : T.n0 + rank * (BN / 2);
+                        const int half = P.b_split ? urank : src;
+                        const int col = P.b_split ? T.n0 : T.n0 + urank * (BN / 2);
 #pragma unroll
                         for (int j = 0; j < BN / 128; ++j)
                             tma_load_3d_pair(sb + j * MNB, &P.b[half], bar, col + 64 * j, k, bz);
@@ -964,46 +979,48 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             }
         }
     } else if (warp == 1 && rank == 0) {
-        // ===== MMA issuer (one thread of the leader CTA) =====
+        // ===== MMA issuer (warp 1 of the leader CTA, converged; one elected lane issues) =====
         constexpr uint32_t idesc = make_idesc2(A_MAJOR, B_MAJOR);
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MNB, b_lbo = B_MAJOR == K_MAJOR ? 16 : MNB;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        const uint32_t smem_base = uni(smem_u32(smem)), tmem_u = uni(tmem_base);
+        const uint64_t a_desc0 = make_desc(smem_base, a_lbo, 1024), b_desc0 = make_desc(smem_base + A2_BYTES, b_lbo, 1024);
         int stage = 0, phase = 0, as = 0, aphase = 0;
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         for (int it = 0;; ++it) {
-            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            const int t = uni(dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid);
             if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, 0, BKc, rcp_group, rcp_pairs);
+            const int t_nkb = uni(T.nkb);
             // wgrad: the K range ends with the expert's zero pad rows; K slices (16 rows) that hold only pad rows are
             // not issued (C2: 640 of 8832 rows, 7% of the tensor work)
-            const int k_valid = !P.ragged_m ? tpp[T.g] : 0x3fffffff;
-            if (lane == 0) {
+            const int k_valid = uni(!P.ragged_m ? tpp[T.g] : 0x3fffffff);
+            {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
                 if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
-            __syncwarp();
-            const uint32_t d_tmem = tmem_base + as * BN;
-            for (int kb = 0; kb < T.nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    if (GATHER_A) {
-                        mbar_wait_cluster(&full_bar[stage], phase);
-                        fence_proxy_async();
-                    } else {
-                        mbar_wait(&full_bar[stage], phase);
-                    }
-                    if (P.prof) w_full += clock64() - c0;
-                    tc_fence_after();
-                    const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + A2_BYTES;
+            const uint32_t d_tmem = tmem_u + as * BN;
+            for (int kb = 0; kb < t_nkb; ++kb) {
+                const long long c0 = P.prof ? clock64() : 0;
+                if (GATHER_A) {
+                    mbar_wait_cluster(&full_bar[stage], phase);
+                    fence_proxy_async();
+                } else {
+                    mbar_wait(&full_bar[stage], phase);
+                }
+                if (P.prof) w_full += clock64() - c0;
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t soff = (uint32_t)(stage * STAGE2_BYTES) >> 4;
                     const int kk_end = (k_valid - kb * BKc + UK - 1) / UK;  // >= 1 in block 0 of a non-empty expert
 #pragma unroll
                     for (int kk = 0; kk < BKc / UK; ++kk) {
                         if (kk >= kk_end) break;
-                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
-                        const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
+                        const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
+                        const uint64_t bd = b_desc0 + (soff + ((kk * b_kstep) >> 4));
                         umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
                     umma2_commit(&empty_bar[stage]);  // frees this stage in both CTAs
@@ -1011,7 +1028,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                 __syncwarp();
                 if (++stage == STAGES2) stage = 0, phase ^= 1;
             }
-            if (lane == 0) umma2_commit(&tfull_bar[as]);  // both CTAs' epilogues
+            if (elect_one()) umma2_commit(&tfull_bar[as]);  // both CTAs' epilogues
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
@@ -1021,18 +1038,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
         }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
-        const int wq = warp & 3;            // TMEM lane quarter of this warp
-        const int chalf = (warp - 4) >> 2;  // 8 epilogue warps: the second warp of a quarter takes the tile's upper columns
+        // (warp-uniform values are made provably so, and one elected lane issues the bulk tensor copies: see elect_one)
+        const int uwarp = uni(warp), urank = uni(rank);
+        const bool leader = elect_one();
+        const int wq = uwarp & 3;            // TMEM lane quarter of this warp
+        const int chalf = (uwarp - 4) >> 2;  // 8 epilogue warps: the second warp of a quarter takes the tile's upper columns
         constexpr int C_PER_WARP = 4 / (Cfg2<EPI>::EPI_WARPS / 4);
-        const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
-        uint8_t* stg = stg_base + (warp - 4) * NBUF * STG_BYTES;
+        const uint32_t leader_tempty = uni(mapa_u32(smem_u32(tempty_bar), 0));
+        uint8_t* stg = stg_base + (uwarp - 4) * NBUF * STG_BYTES;
         int as = 0, aphase = 0, ring = 0;
         long long w_tfull = 0, w_stg = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         uint32_t q = 0;  // SwiGLU backward: running chunk number -> input set q & 1, barrier phase (q >> 1) & 1
         // G, U of 32 rows x 64 columns -> set `set` of this warp's staging buffers (bytes counted on ld_bar)
         auto load_inputs = [&](const Tile2& Tn, int c, int set) {
-            if (lane == 0) {
+            if (leader) {
                 bulk_wait_read<0>();  // the stores that last read this set are done with it
                 uint64_t* bar = &ld_bar[wq * 2 + set];
                 mbar_expect_tx(bar, 2 * STG_BYTES);
@@ -1045,9 +1065,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             if (t0 < n_total) load_inputs(decode_pair(P, tp, tpp, offsets, t0, rank, BKc, rcp_group, rcp_pairs), 0, 0);
         }
         for (int it = 0;; ++it) {
-            const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
+            const int t = uni(dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid);
             if (t >= n_total) break;
-            const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
+            Tile2 T = decode_pair(P, tp, tpp, offsets, t, urank, BKc, rcp_group, rcp_pairs);
+            T.g = uni(T.g), T.m0 = uni(T.m0), T.n0 = uni(T.n0), T.nkb = uni(T.nkb), T.store = uni((int)T.store) != 0;
             const long long c0 = P.prof ? clock64() : 0;
             mbar_wait(&tfull_bar[as], aphase);
             if (P.prof) w_tfull += clock64() - c0;
@@ -1062,7 +1083,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     const int col = T.n0 + 64 * c;
                     if (col >= P.n_limit) break;
                     const long long c1 = P.prof ? clock64() : 0;
-                    if (lane == 0) bulk_wait_read<0>();
+                    if (leader) bulk_wait_read<0>();
                     __syncwarp();
                     if (P.prof) w_stg += clock64() - c1;
 #pragma unroll
@@ -1083,7 +1104,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0 && T.store) {
+                    if (leader && T.store) {
                         tma_store_3d(&P.o[0], stg, col, row0, z);
                         tma_store_3d(&P.o[1], stg + STG_BYTES, col, row0, z);
                         tma_store_3d(&P.o[2], stg + 2 * STG_BYTES, col, row0, z);
@@ -1131,7 +1152,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0 && T.store) {
+                    if (leader && T.store) {
                         tma_store_3d(&P.o[0], bg, T.n0 + 64 * c, row0, z);
                         tma_store_3d(&P.o[1], bu, T.n0 + 64 * c, row0, z);
                         bulk_commit();
@@ -1153,7 +1174,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                             if (col + 32 * h >= P.n_limit) break;
                             uint8_t* fbuf = stg + ring * STG_BYTES;
                             if (++ring == NBUF) ring = 0;
-                            if (lane == 0) bulk_wait_read<NBUF - 1>();
+                            if (leader) bulk_wait_read<NBUF - 1>();
                             __syncwarp();
                             uint32_t r[32];
                             tmem_ld32(taddr + 64 * c + 32 * h, r);
@@ -1167,7 +1188,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                             }
                             fence_proxy_async();
                             __syncwarp();
-                            if (lane == 0 && T.store) {
+                            if (leader && T.store) {
                                 if (P.accum) tma_reduce_add_3d(om, fbuf, col + 32 * h, row0, z);
                                 else tma_store_3d(om, fbuf, col + 32 * h, row0, z);
                                 bulk_commit();
@@ -1178,7 +1199,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     uint8_t* buf = stg + ring * STG_BYTES;
                     if (++ring == NBUF) ring = 0;
                     const long long c1 = P.prof ? clock64() : 0;
-                    if (lane == 0) bulk_wait_read<NBUF - 1>();
+                    if (leader) bulk_wait_read<NBUF - 1>();
                     __syncwarp();
                     if (P.prof) w_stg += clock64() - c1;
 #pragma unroll
@@ -1193,7 +1214,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0 && T.store) {
+                    if (leader && T.store) {
                         tma_store_3d(om, buf, col, row0, z);
                         bulk_commit();
                     }
@@ -1201,10 +1222,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(leader_tempty + as * 8);
+            if (leader) mbar_arrive_cluster(leader_tempty + as * 8);
             if (++as == 2) as = 0, aphase ^= 1;
         }
-        if (lane == 0) bulk_wait_all();
+        if (leader) bulk_wait_all();
         if (P.prof && threadIdx.x == 128) {
             long long* pq = P.prof + blockIdx.x * 8;
             pq[4] = w_tfull, pq[5] = clock64() - t_begin, pq[7] = w_stg;
@@ -1466,29 +1487,30 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     } else if (warp == 0 || warp == 2) {
         // ===== TMA producers (both CTAs): warp 0 loads the CTA's 128 features of the weights, warp 2 (idle after the
-        // TMEM allocation) its half of the rows.  One thread issuing every box of a stage spent most of its time inside
-        // the issue of the bulk tensor instructions, not waiting for free stages. =====
-        const bool load_a = warp == 0;
-        const uint32_t leader_full = mapa_u32(smem_u32(full_bar), 0);
+        // TMEM allocation) its half of the rows.  The warps run converged; one elected lane issues the copies. =====
+        const bool load_a = uni(warp) == 0;
+        const uint32_t leader_full = uni(mapa_u32(smem_u32(full_bar), 0));
+        const int urank = uni(rank);
         int stage = 0, phase = 0;
         long long w_empty = 0;
         for (int it = 0;; ++it) {
-            const int t = feed.peek(it);
-            const TileT T = tile_of(it);
+            const int t = uni(feed.peek(it));
+            TileT T = tile_of(it);
+            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n);
             feed.release(it, lane);
             if (t >= n_total) break;
-            const int nb = T.n >> 1, rb = T.r0 + rank * nb;
+            const int nb = T.n >> 1, rb = T.r0 + urank * nb;
             const bool small = nb <= P.small_rows;
             const int nbox = small ? (nb + TB_SMALL_ROWS - 1) / TB_SMALL_ROWS : 1;
             const int box_bytes = (small ? TB_SMALL_ROWS : TB_BOX_ROWS) * BK * 2;
             for (int kb = 0; kb < nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&empty_bar[stage], phase ^ 1);
-                    if (P.prof) w_empty += clock64() - c0;
+                const long long c0 = P.prof ? clock64() : 0;
+                mbar_wait(&empty_bar[stage], phase ^ 1);
+                if (P.prof) w_empty += clock64() - c0;
+                if (elect_one()) {
                     uint8_t* sa = smem + stage * TSTAGE_BYTES;
                     uint8_t* sb = sa + TA_BYTES;
-                    if (rank == 0) mbar_expect_tx(&full_bar[stage], load_a ? 2 * TA_BYTES : 2 * nbox * box_bytes);
+                    if (urank == 0) mbar_expect_tx(&full_bar[stage], load_a ? 2 * TA_BYTES : 2 * nbox * box_bytes);
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
@@ -1501,15 +1523,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                             tma_load_3d_pair(sb, &P.b[src], bar, k, rb, 0);
                         }
                     } else if (EPI == TEPI_SWIGLU_FWD) {  // 64 gate features | the same 64 up features
-                        const int fc = T.f * 128 + rank * 64;
+                        const int fc = T.f * 128 + urank * 64;
                         tma_load_3d_pair(sa, &P.a[0], bar, fc, k, T.g);
                         tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[1], bar, fc, k, T.g);
                     } else if (A_MAJOR == MN_MAJOR) {
-                        const int fc = T.f * 256 + rank * 128;
+                        const int fc = T.f * 256 + urank * 128;
                         tma_load_3d_pair(sa, &P.a[src], bar, fc, k, T.g);
                         tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[src], bar, fc + 64, k, T.g);
                     } else {
-                        tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + rank * 128, T.g);
+                        tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + urank * 128, T.g);
                     }
                 }
                 __syncwarp();
@@ -1518,47 +1540,47 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
         if (P.prof && lane == 0 && load_a) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1 && rank == 0) {
-        // ===== MMA issuer (one thread of the leader CTA): D^T[256 features, n rows] += W-tile * rows^T =====
+        // ===== MMA issuer (warp 1 of the leader CTA, converged; one elected lane issues): D^T[256 features, n rows] += W-tile * rows^T
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        const uint32_t smem_base = uni(smem_u32(smem)), tmem_u = uni(tmem_base);
+        // descriptors of stage 0, K step 0: the address field (bits 0-13, 16-byte units) advances by plain additions
+        const uint64_t a_desc0 = make_desc(smem_base, a_lbo, 1024), b_desc0 = make_desc(smem_base + TA_BYTES, 16, 1024);
         int stage = 0, phase = 0, as = 0, aphase = 0;
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         for (int it = 0;; ++it) {
-            const int t = feed.peek(it);
-            const TileT T = tile_of(it);
+            const int t = uni(feed.peek(it));
+            const int tn = uni(tile_of(it).n);
             feed.release(it, lane);
             if (t >= n_total) break;
-            const uint32_t idesc = make_idesc_t(A_MAJOR, T.n);
-            if (lane == 0) {
+            const uint32_t idesc = make_idesc_t(A_MAJOR, tn);
+            {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
                 if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
-            __syncwarp();
-            const uint32_t d_tmem = tmem_base + as * BN;
-            // A tcgen05.mma of this shape occupies the issue slot ~130 cycles whatever N is (measured: 64 .. 256 rows per
-            // chunk cost the same), because consecutive MMAs accumulate into the same TMEM columns.  Chunks of at most 128
-            // rows therefore alternate their K steps between two accumulators (columns [0, n) and [128, 128 + n) of the
-            // buffer): two independent chains; the epilogue adds the halves in fp32.
-            const bool splitk = P.split_k && T.n <= 128;
+            const uint32_t d_tmem = tmem_u + as * BN;
+            // PIPER_OPT_T_SPLIT_K (measured neutral): chunks of at most 128 rows alternate their K steps between two
+            // accumulators (columns [0, n) and [128, 128 + n) of the buffer); the epilogue adds the halves in fp32.
+            const bool splitk = P.split_k && tn <= 128;
             for (int kb = 0; kb < nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    if (GATHER) {
-                        mbar_wait_cluster(&full_bar[stage], phase);  // pairs with the peer forwarder's cluster-scope release
-                        fence_proxy_async();                         // gathered rows were written through the generic proxy
-                    } else {
-                        mbar_wait(&full_bar[stage], phase);
-                    }
-                    if (P.prof) w_full += clock64() - c0;
-                    tc_fence_after();
-                    const uint32_t sa = smem_u32(smem + stage * TSTAGE_BYTES), sb = sa + TA_BYTES;
+                const long long c0 = P.prof ? clock64() : 0;
+                if (GATHER) {
+                    mbar_wait_cluster(&full_bar[stage], phase);  // pairs with the peer forwarder's cluster-scope release
+                    fence_proxy_async();                         // gathered rows were written through the generic proxy
+                } else {
+                    mbar_wait(&full_bar[stage], phase);
+                }
+                if (P.prof) w_full += clock64() - c0;
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t soff = (uint32_t)(stage * TSTAGE_BYTES) >> 4;
 #pragma unroll
                     for (int kk = 0; kk < BK / UK; ++kk) {
-                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
-                        const uint64_t bd = make_desc(sb + kk * UK * 2, 16, 1024);
+                        const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
+                        const uint64_t bd = b_desc0 + (soff + ((kk * UK * 2) >> 4));
                         if (splitk) umma2_bf16(d_tmem + ((kk & 1) ? 128 : 0), ad, bd, idesc, (kb != 0) | (kk >= 2));
                         else umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
@@ -1567,7 +1589,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 __syncwarp();
                 if (++stage == NST) stage = 0, phase ^= 1;
             }
-            if (lane == 0) umma2_commit(&tfull_bar[as]);
+            if (elect_one()) umma2_commit(&tfull_bar[as]);
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
@@ -1577,8 +1599,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): TMEM lane = feature, column = row; transposed through shared memory =====
-        const int wq = warp & 3;
-        const uint32_t leader_tempty = mapa_u32(smem_u32(tempty_bar), 0);
+        // (warp-uniform values are made provably so, and one elected lane issues the bulk tensor copies: see elect_one)
+        const int wq = uni(warp) & 3, urank = uni(rank);
+        const bool leader = elect_one();
+        const uint32_t leader_tempty = uni(mapa_u32(smem_u32(tempty_bar), 0));
         uint8_t* stg = stg_base + wq * NBUF * TSTG_BYTES;
         int as = 0, aphase = 0, ring = 0;
         long long w_tfull = 0, w_stg = 0;
@@ -1605,7 +1629,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         };
         // SwiGLU backward: G, U of 32 rows x 32 features -> input set `set` (two staging blocks)
         auto load_inputs = [&](int fcol, int row, int set) {
-            if (lane == 0) {
+            if (leader) {
                 bulk_wait_read<0>();
                 uint64_t* bar = &ld_bar[wq * 2 + set];
                 mbar_expect_tx(bar, 2 * TSTG_BYTES);
@@ -1615,18 +1639,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         };
         const int pr = wq & 1;  // SwiGLU forward: warps pr (G lanes) and pr + 2 (U lanes) hold the same 32 features
         auto feat_col = [&](const TileT& T) {
-            return EPI == TEPI_SWIGLU_FWD ? T.f * 128 + rank * 64 + 32 * pr : T.f * 256 + rank * 128 + 32 * wq;
+            return EPI == TEPI_SWIGLU_FWD ? T.f * 128 + urank * 64 + 32 * pr : T.f * 256 + urank * 128 + 32 * wq;
         };
         if (EPI == TEPI_SWIGLU_BWD) {
-            const int t0 = feed.peek(0);
+            const int t0 = uni(feed.peek(0));
             if (t0 < n_total) {
-                const TileT T0 = tile_of(0);
+                TileT T0 = tile_of(0);
+                T0.f = uni(T0.f), T0.r0 = uni(T0.r0);
                 load_inputs(feat_col(T0), T0.r0, 0);
             }
         }
         for (int it = 0;; ++it) {
-            const int t = feed.peek(it);
-            const TileT T = tile_of(it);
+            const int t = uni(feed.peek(it));
+            TileT T = tile_of(it);
+            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n), T.zend = uni(T.zend);
             feed.release(it, lane);
             if (t >= n_total) break;
             const long long c0 = P.prof ? clock64() : 0;
@@ -1654,7 +1680,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 if (EPI == TEPI_STORE) {
                     if (!f_ok) break;
                     uint8_t* buf = next_buf();
-                    if (lane == 0) bulk_wait_read<NBUF - 1>();
+                    if (leader) bulk_wait_read<NBUF - 1>();
                     __syncwarp();
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
@@ -1664,7 +1690,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     stage_col(buf, v);
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0) {
+                    if (leader) {
                         store_block(&P.o[0], buf, fcol, T.r0 + j, both);
                         bulk_commit();
                     }
@@ -1680,19 +1706,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                         for (int i = 0; i < 32; ++i) sts_f32(xch + i * 128, v[i]);
                         asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
                         uint8_t* buf = next_buf();
-                        if (lane == 0) bulk_wait_read<NBUF - 1>();
+                        if (leader) bulk_wait_read<NBUF - 1>();
                         __syncwarp();
                         stage_col(buf, v);
                         fence_proxy_async();
                         __syncwarp();
-                        if (lane == 0 && f_ok) {
+                        if (leader && f_ok) {
                             store_block(&P.o[1], buf, fcol, T.r0 + j, both);
                             bulk_commit();
                         }
                     } else {  // G lanes: store G, H = silu(G) * U
                         uint8_t* bg = next_buf();
                         uint8_t* bh = next_buf();
-                        if (lane == 0) bulk_wait_read<1>();  // two blocks per commit group, ring of four
+                        if (leader) bulk_wait_read<1>();  // two blocks per commit group, ring of four
                         __syncwarp();
                         stage_col(bg, v);
                         asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
@@ -1701,7 +1727,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                         stage_col(bh, v);
                         fence_proxy_async();
                         __syncwarp();
-                        if (lane == 0 && f_ok) {
+                        if (leader && f_ok) {
                             store_block(&P.o[0], bg, fcol, T.r0 + j, both);
                             store_block(&P.o[2], bh, fcol, T.r0 + j, both);
                             bulk_commit();
@@ -1717,9 +1743,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     if (j + 32 < T.n) {
                         load_inputs(fcol, T.r0 + j + 32, set ^ 1);
                     } else {
-                        const int tn = feed.peek(it + 1);
+                        const int tn = uni(feed.peek(it + 1));
                         if (tn < n_total) {
-                            const TileT Tn = tile_of(it + 1);
+                            TileT Tn = tile_of(it + 1);
+                            Tn.f = uni(Tn.f), Tn.r0 = uni(Tn.r0);
                             load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
                         }
                     }
@@ -1745,7 +1772,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0 && f_ok) {
+                    if (leader && f_ok) {
                         store_block(&P.o[0], stg + (2 * set) * TSTG_BYTES, fcol, T.r0 + j, both);
                         store_block(&P.o[1], stg + (2 * set + 1) * TSTG_BYTES, fcol, T.r0 + j, both);
                         bulk_commit();
@@ -1754,10 +1781,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(leader_tempty + as * 8);
+            if (leader) mbar_arrive_cluster(leader_tempty + as * 8);
             if (++as == 2) as = 0, aphase ^= 1;
             // pad rows behind the group's last chunk: exact zeros (wgrad reads them as part of its K range)
-            if (lane == 0 && f_ok && T.r0 + T.n < T.zend) {
+            if (leader && f_ok && T.r0 + T.n < T.zend) {
                 for (int row = T.r0 + T.n; row < T.zend; row += 16) {
                     if (EPI == TEPI_STORE) {
                         tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
@@ -1776,7 +1803,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                 bulk_commit();
             }
         }
-        if (lane == 0) bulk_wait_all();
+        if (leader) bulk_wait_all();
         if (P.prof && threadIdx.x == 128) {
             long long* pq = P.prof + blockIdx.x * 8;
             pq[4] = w_tfull, pq[5] = clock64() - t_begin, pq[7] = w_stg;
