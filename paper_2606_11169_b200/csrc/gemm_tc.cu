@@ -79,6 +79,7 @@ struct alignas(64) TcParams {
     const void* gsrc;           // token-major source [T, g_cols] bf16
     unsigned long long g_magic; // ceil(2^35 / k): a / k = (a * g_magic) >> 35 for a < 2^30, k <= 8
     int g_cols;                 // columns of the source (= the contraction / feature length d)
+    int prefetch_kb;            // rows-on-N kernels: the weight producer prefetches this many K blocks ahead into L2 (0 = off)
     int split_k;                // rows-on-N kernels: chunks of <= 128 rows use two half accumulators (PIPER_OPT_T_SPLIT_K)
     const float* row_scale;     // DGRAD1 with gathered dY: the epilogue multiplies row r of dH by row_scale[r] (the gate)
     int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
@@ -125,6 +126,10 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
+// the same with a predicate: ignore != 0 writes zeros and does not read the source
+__device__ __forceinline__ void cp_async16_z(uint32_t dst, const void* src, uint32_t ignore) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tcp.async.cg.shared.global [%0], [%1], 16, p;\n\t}" ::"r"(dst), "l"(src), "r"(ignore) : "memory");
+}
 // the mbarrier receives one arrival from this thread once all its cp.async issued so far have landed
 __device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -152,6 +157,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
             smem_u32(dst)),
         "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
+}
+// bring a box into L2 ahead of its load (no shared-memory destination, no barrier)
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
 }
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -942,19 +952,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                 }
                 if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
                 __syncwarp();
-                const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES);
+                // destination of row r = 4 i + rs, box j: sa + j MNB + r 128 + ((ch ^ (r & 7)) << 4), r & 7 = 4 (i & 1) + rs
+                const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES) + rs * 128;
+                const uint32_t d_even = sa + ((ch ^ rs) << 4), d_odd = sa + ((ch ^ (4 + rs)) << 4);
                 const int col0 = T.m0 + ch * 8;
+                const uint32_t c_bad0 = col0 < P.g_cols ? 0u : 1u, c_bad1 = col0 + 64 < P.g_cols ? 0u : 1u;
+                const char* src0 = gbase + (c_bad0 ? 0 : (size_t)col0 * 2);
+                const char* src1 = gbase + (c_bad1 ? 0 : (size_t)(col0 + 64) * 2);
 #pragma unroll
                 for (int i = 0; i < BKc / 4; ++i) {
-                    const int r = 4 * i + rs;  // = 32 (i >> 3) + 4 (i & 7) + rs: held by lane 4 (i & 7) + rs in mine[i >> 3]
+                    // row 4 i + rs = 32 (i >> 3) + 4 (i & 7) + rs: held by lane 4 (i & 7) + rs in mine[i >> 3]
                     const uint32_t o = __shfl_sync(0xffffffffu, mine[i >> 3], 4 * (i & 7) + rs);
-#pragma unroll
-                    for (int j = 0; j < BM / 64; ++j) {
-                        const int col = col0 + 64 * j;
-                        const bool ok = col < P.g_cols && o != 0xFFFFFFFFu;
-                        cp_async16(sa + j * MNB + r * 128 + ((ch ^ (r & 7)) << 4),
-                                   ok ? gbase + (size_t)o * 16 + (size_t)col * 2 : gbase, ok ? 16u : 0u);
-                    }
+                    const uint32_t z = o == 0xFFFFFFFFu ? 1u : 0u;
+                    const size_t ob = z ? 0 : (size_t)o * 16;
+                    const uint32_t d = ((i & 1) ? d_odd : d_even) + i * 512;
+                    cp_async16_z(d, src0 + ob, z | c_bad0);
+                    cp_async16_z(d + MNB, src1 + ob, z | c_bad1);
                 }
                 cp_async_arrive(rank == 0 ? &full_bar[stage] : &gfull_bar[stage]);
                 if (++stage == STAGES2) stage = 0, phase ^= 1;
@@ -1310,8 +1323,10 @@ __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
 // K-major layout a TMA box would have.  The leader's lanes arrive on the stage's full barrier themselves
 // (cp.async.mbarrier.arrive); the peer CTA's lanes arrive on a local barrier that the peer's otherwise idle warp 1
 // forwards to the leader (proxy fence + cluster-scope release).
+constexpr int kGatherWarps = 2;  // GATHER: warp 2 and one extra warp (8) share the rows of a tile
 template <int A_MAJOR, int EPI, bool GATHER = false>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemmT_kernel(const __grid_constant__ TcParams P) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATHER ? kThreads + 32 * (kGatherWarps - 1) : kThreads, 1)
+tc_gemmT_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     constexpr int NST = CfgT<EPI>::NST, NBUF = CfgT<EPI>::NBUF;
@@ -1373,11 +1388,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
     if (warp == 1 && lane == 0) {
         // full: the weight producer's expect_tx arrival + the rows producer's (TMA: one expect_tx arrival; GATHER: the
         // leader's 32 lanes + the peer's forwarder)
-        for (int s = 0; s < NST; ++s) mbar_init(&full_bar[s], GATHER ? 34 : 2), mbar_init(&empty_bar[s], 1), mbar_init(&gfull_bar[s], 32);
+        for (int s = 0; s < NST; ++s)
+            mbar_init(&full_bar[s], GATHER ? 2 + 32 * kGatherWarps : 2), mbar_init(&empty_bar[s], 1), mbar_init(&gfull_bar[s], 32 * kGatherWarps);
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 8);  // 4 warps x 2 CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
         for (int s = 0; s < kFeed; ++s)  // + the second producer warp of each CTA (+ the peer's forwarder)
-            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers + 2 + (GATHER ? 1 : 0));
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], kFeedConsumers + 2 + (GATHER ? 1 + 2 * (kGatherWarps - 1) : 0));
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -1429,11 +1445,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
         }
     }
 
-    if (GATHER && warp == 2) {
-        // ===== rows producer, gathered (both CTAs, all 32 lanes): lane = (row & 3, 16-byte chunk of the 128-byte K slice)
-        const int ch = lane & 7, rs = lane >> 3;
+    if (GATHER && (warp == 2 || warp >= 8)) {
+        // ===== rows producers, gathered (both CTAs; kGatherWarps warps, all 32 lanes): a lane owns one 16-byte chunk
+        // (ch) of the 128-byte K slice of the rows r = 8 q + 4 gw + rs; their swizzle term r & 7 = 4 gw + rs is a constant of
+        // the lane, so the destination of copy q is a fixed address + q * 1024 =====
+        const int gw = warp == 2 ? 0 : warp - 7;
+        const int ch = lane & 7, rs = lane >> 3, r_lane = 4 * gw + rs;
         const char* gbase = static_cast<const char*>(P.gsrc);
         const uint32_t pitch16 = (uint32_t)P.g_cols >> 3;  // 16-byte units per source row
+        const uint32_t dst_lane = smem_u32(smem) + TA_BYTES + r_lane * 128 + ((ch ^ r_lane) << 4);
+        constexpr int NQ = 128 / (4 * kGatherWarps);  // copies per lane and K block at most
         int stage = 0, phase = 0;
         for (int it = 0;; ++it) {
             const int t = feed.peek(it);
@@ -1441,28 +1462,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
             feed.release(it, lane);
             if (t >= n_total) break;
             const int nb = T.n >> 1, rb = T.r0 + rank * nb;
-            uint32_t off[32];  // source row of tile row 4 i + rs in 16-byte units; ~0 = zero row (pad)
+            uint32_t off[NQ];   // source row of tile row 8 q + r_lane in 16-byte units
+            uint32_t zmask = 0; // bit q: pad row (zero fill)
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-                const int r = 4 * i + rs;
+            for (int q = 0; q < NQ; ++q) {
+                const int r = 4 * kGatherWarps * q + r_lane;
                 const int a = r < nb ? P.src_of[rb + r] : -1;
-                off[i] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0xFFFFFFFFu;
+                off[q] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0u;
+                zmask |= a >= 0 ? 0u : 1u << q;
             }
+            const int nq = (nb - r_lane + 4 * kGatherWarps - 1) / (4 * kGatherWarps);  // rows r < nb
             for (int kb = 0; kb < nkb; ++kb) {
                 if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
                 __syncwarp();
-                const uint32_t sb = smem_u32(smem + stage * TSTAGE_BYTES + TA_BYTES);
+                const uint32_t dst = dst_lane + stage * TSTAGE_BYTES;
                 const int kcol = kb * BK + ch * 8;
-                const bool k_ok = kcol < P.g_cols;  // K tail: zero fill, as a TMA box does
-                const char* src_k = gbase + (size_t)kcol * 2;
+                const uint32_t k_bad = kcol < P.g_cols ? 0u : 0xFFFFFFFFu;  // K tail: zero fill, as a TMA box does
+                const char* src_k = gbase + (k_bad ? 0 : (size_t)kcol * 2);
 #pragma unroll
-                for (int i = 0; i < 32; ++i) {
-                    const int r = 4 * i + rs;
-                    if (r < nb) {
-                        const bool ok = k_ok && off[i] != 0xFFFFFFFFu;
-                        cp_async16(sb + r * 128 + ((ch ^ (r & 7)) << 4), ok ? src_k + (size_t)off[i] * 16 : gbase, ok ? 16u : 0u);
-                    }
-                }
+                for (int q = 0; q < NQ; ++q)
+                    if (q < nq) cp_async16_z(dst + q * (4 * kGatherWarps * 128), src_k + (size_t)off[q] * 16, (zmask & (1u << q)) | k_bad);
                 cp_async_arrive(rank == 0 ? &full_bar[stage] : &gfull_bar[stage]);
                 if (++stage == NST) stage = 0, phase ^= 1;
             }
@@ -1532,6 +1551,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) tc_gemm
                         tma_load_3d_pair(sa + MN_BLOCK_BYTES, &P.a[src], bar, fc + 64, k, T.g);
                     } else {
                         tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + urank * 128, T.g);
+                    }
+                    // The weights of a tile stream from HBM once; an SM holds NST stages (80 KB of weights) in flight, which
+                    // at the loaded HBM latency caps it near 40 GB/s.  Prefetching the box `prefetch_kb` K blocks ahead into
+                    // L2 makes the demand load an L2 hit (PIPER_OPT_T_PREFETCH).
+                    if (load_a && P.prefetch_kb > 0) {
+                        const int kbp = kb + P.prefetch_kb;
+                        if (kbp < nkb) {
+                            int srcp = 0, kkp = kbp;
+                            if (kbp >= P.kb_per_src) srcp = 1, kkp = kbp - P.kb_per_src;
+                            const int kp = kkp * BK;
+                            if (EPI == TEPI_SWIGLU_FWD) {
+                                const int fc = T.f * 128 + urank * 64;
+                                tma_prefetch_3d(&P.a[0], fc, kp, T.g), tma_prefetch_3d(&P.a[1], fc, kp, T.g);
+                            } else if (A_MAJOR == MN_MAJOR) {
+                                const int fc = T.f * 256 + urank * 128;
+                                tma_prefetch_3d(&P.a[srcp], fc, kp, T.g), tma_prefetch_3d(&P.a[srcp], fc + 64, kp, T.g);
+                            } else {
+                                tma_prefetch_3d(&P.a[srcp], kp, T.f * 256 + urank * 128, T.g);
+                            }
+                        }
                     }
                 }
                 __syncwarp();
@@ -1991,7 +2030,8 @@ bool set_smem_attr1() {  // 1-CTA kernel only (the router's dense GEMMs)
 
 template <int A_MAJOR, int EPI, bool GATHER = false>
 int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
-    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, CfgT<EPI>::SMEM);
+    constexpr int threads = GATHER ? kThreads + 32 * (kGatherWarps - 1) : kThreads;
+    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, CfgT<EPI>::SMEM, threads);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
     TcParams Q = P;
@@ -2000,7 +2040,7 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
         c->tc_next_slot += 1;
     }
     Q.sched = sched_counters(c, ln.stream);
-    tc_gemmT_kernel<A_MAJOR, EPI, GATHER><<<(unsigned)(2 * clusters), kThreads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
+    tc_gemmT_kernel<A_MAJOR, EPI, GATHER><<<(unsigned)(2 * clusters), threads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
 }
@@ -2021,7 +2061,7 @@ TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_t
     memset(&P, 0, sizeof(P));
     P.offsets = p.offsets, P.counts = p.counts, P.G = p.G, P.n_src = 1;
     P.f_tiles = cdiv(F, f_tile), P.f_limit = F, P.kb_per_src = cdiv(K, BK);
-    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy, P.split_k = c->tc_split_k;
+    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy, P.split_k = c->tc_split_k, P.prefetch_kb = c->tc_prefetch_kb;
     return P;
 }
 inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
@@ -2075,6 +2115,7 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
+    c->tc_prefetch_kb = 0;
     c->tc_split_k = 0;  // measured without gain: the ~130-cycle issue cost of an MMA does not come from the accumulator chain
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
