@@ -435,6 +435,50 @@ def time_tasks(w: Workload, n_prof):
     return kernels, roofline, shape, impl, task_ms
 
 
+def tc_counters(w: Workload):
+    """Debug wait-cycle counters of the tcgen05 kernels (PIPER_OPT_TC_PROFILE), one row per GEMM launch of each task:
+    cycles of the MMA-issuing warp's loop and the shares it spent waiting for operands / for a free accumulator, the
+    weight producer's share waiting for a free stage, the epilogue's shares waiting for an accumulator / a staging
+    buffer, tiles per cluster.  Mean over the leader CTAs."""
+    import ctypes
+    import numpy as np
+    torch, piper = w.torch, w.piper
+    piper.piper_set_option(w.ctx, piper.OPT_TC_PROFILE, 1)
+    ptr = piper.lib().piper_debug_tc_counters(w.ctx._h)
+    n_words = 16 * 160 * 8
+    rt = ctypes.CDLL("libcudart.so")
+
+    def read():
+        t = torch.empty(n_words, dtype=torch.int64, device=w.dev)
+        torch.cuda.synchronize()
+        rt.cudaMemcpy(ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(ptr), ctypes.c_size_t(n_words * 8), 3)
+        return t.cpu().numpy().reshape(16, 160, 8)
+
+    tasks = ["F_GEMM1", "F_GEMM2", "B_DGRAD1", "B_DGRAD2", "B_WGRAD"] + (["F_SHARED", "B_SHARED"] if w.cfg.I_shared else [])
+    rows = []
+    for t in tasks:
+        before = read()
+        piper.piper_run_task(w.ctx, t, w.cargs)
+        after = read()
+        for s in range(16):
+            if np.array_equal(before[s], after[s]):
+                continue
+            q = after[s]
+            lead, epi = q[:, 2] > 0, q[:, 5] > 0
+            if not lead.any():
+                continue
+            loop = q[lead, 2].astype(float)
+            rows.append({"task": t, "launch_slot": s, "clusters": int(lead.sum()), "mma_loop_cycles": float(loop.mean()),
+                         "mma_wait_operands": float((q[lead, 0] / loop).mean()),
+                         "mma_wait_accumulator": float((q[lead, 1] / loop).mean()),
+                         "producer_wait_stage": float((q[lead, 3] / loop).mean()),
+                         "epilogue_wait_accumulator": float((q[epi, 4] / np.maximum(q[epi, 5], 1)).mean()),
+                         "epilogue_wait_staging": float((q[epi, 7] / np.maximum(q[epi, 5], 1)).mean()),
+                         "tiles_per_cluster": float(q[lead, 6].mean()), "loop_max_over_min": float(loop.max() / loop.min())})
+    piper.piper_set_option(w.ctx, piper.OPT_TC_PROFILE, 0)
+    return rows
+
+
 def run_piper(args, cfg, sampler, rank, world, local, barrier, e2e=True, min_seconds=0.0):
     """The bench line of one config (resident value, optional e2e, per-task times)."""
     from inputs import configs
@@ -453,6 +497,8 @@ def run_piper(args, cfg, sampler, rank, world, local, barrier, e2e=True, min_sec
                  "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "kernels": kernels, "gemm_impl": impl})
     if args.main_grad:
         line["config"]["dw"] = "fp32, accumulated across steps (accumulate = 1)"
+    if getattr(args, "tc_counters", False) and impl == "tcgen05":
+        line["tc_counters"] = tc_counters(w)
     return line, w
 
 
@@ -602,6 +648,8 @@ def main():
     ap.add_argument("--no-fused-gather", action="store_true",
                     help="measured variant: the chunk calls run the separate pack / combine_bwd row movers and the GEMMs read "
                          "xp / d_o (PIPER_OPT_FUSED_GATHER = 0)")
+    ap.add_argument("--tc-counters", action="store_true",
+                    help="add the tcgen05 kernels' debug wait-cycle counters per GEMM task (PIPER_OPT_TC_PROFILE) to the line")
     ap.add_argument("--opt", action="append", help="kernel-variant switch NAME=VALUE (piper_set_option, PIPER_OPT_<NAME>)")
     ap.add_argument("--uniform-rows", type=int, default=0,
                     help="microbenchmark: C3's routed layer shape with exactly this many rows in each of 32 experts "

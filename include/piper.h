@@ -101,8 +101,9 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
  *                              accumulators (measured neutral)
  *  PIPER_OPT_T_PREFETCH   [0]  rows-on-N: the weight producer prefetches the box this many K blocks ahead into L2
  *  PIPER_OPT_TC_PROFILE   [0]  1 = the tcgen05 kernels record wait-cycle counters (piper_debug_tc_counters)
- *  PIPER_OPT_FUSED_GATHER [1]  chunk calls on tcgen05 layers: 1 = the GEMMs gather x / dY rows themselves
- *                              (N2 fusion), 0 = they read the packed buffers xp / d_o
+ *  PIPER_OPT_FUSED_GATHER [1]  chunk calls on tcgen05 layers (N2 fusion): 0 = the GEMMs read the packed buffers xp / d_o;
+ *                              1 = F_GEMM1 and the gate|up wgrad gather the rows of x themselves, no pack kernel runs;
+ *                              2 = also DGRAD1 gathers the rows of dY and applies the gate in its fp32 epilogue
  * Returns PIPER_ERR_INVALID for unknown options / values, PIPER_ERR_UNSUPPORTED when the layer cannot run the
  * variant (e.g. fp32 dW without the CTA-pair wgrad). */
 #define PIPER_OPT_TC_ROWS_ON_N 0
@@ -116,8 +117,9 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
 int piper_set_option(piper_ctx* ctx, int option, int value);
 /* 1 when the whole-chunk calls of this context run the fused-gather GEMMs (PIPER_OPT_FUSED_GATHER on
  * a layer whose GEMMs are the rows-on-N + CTA-pair tcgen05 kernels): the forward chunk then launches no pack kernel and
- * does not write xp (piper_dispatch_pack / piper_run_task(F_PACK) produce the all-to-all payload), and the backward
- * chunk's DGRAD1 applies the gate in fp32 after the GEMM instead of reading the bf16-rounded gate * dY.  0 otherwise. */
+ * does not write xp (piper_dispatch_pack / piper_run_task(F_PACK) produce the all-to-all payload); with the option at 2
+ * the backward chunk's DGRAD1 applies the gate in fp32 after the GEMM instead of reading the bf16-rounded gate * dY.
+ * 0 otherwise. */
 int piper_chunk_gathers(const piper_ctx* ctx);
 int piper_get_option(const piper_ctx* ctx, int option, int* value);
 /* Rows the row buffers must hold: T*min(k,E_loc) + E_loc*(row_align-1). */

@@ -193,7 +193,7 @@ int piper_set_option(piper_ctx* c, int option, int value) {
         case PIPER_OPT_T_SMALL_ROWS: field = &c->tc_small_rows; if (value < 0 || value > 128) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_T_GREEDY: field = &c->tc_greedy; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_TC_PROFILE: field = &c->tc_prof; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
-        case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_T_SPLIT_K: field = &c->tc_split_k; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_T_PREFETCH: field = &c->tc_prefetch_kb; if (value < 0 || value > 64) return PIPER_ERR_INVALID; break;
     }

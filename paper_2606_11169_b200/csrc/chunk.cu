@@ -147,7 +147,10 @@ FfnProblem routed_fwd_problem(const piper_ctx* c, const piper_chunk_args* f) {
 }
 FfnProblem routed_bwd_problem(const piper_ctx* c, const piper_chunk_args* b) {
     FfnProblem p = routed_problem(c, b);
-    if (fused_gather(c)) p.gather_x = b->x, p.gather_dy = b->dy, p.src_of = b->src_of, p.gate_rows = b->gate_rows;
+    if (fused_gather(c)) {
+        p.gather_x = b->x, p.src_of = b->src_of;
+        if (c->fused_gather >= 2) p.gather_dy = b->dy, p.gate_rows = b->gate_rows;  // DGRAD1 from dY, gate in its epilogue
+    }
     return p;
 }
 

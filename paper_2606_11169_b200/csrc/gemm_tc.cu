@@ -767,8 +767,10 @@ struct TileFeed {
 // GATHER_A (wgrad gate|up, N2 fusion): the A operand Xp^T is not read from the packed buffer; warp 2 gathers K row r of the
 // tile (= packed row k0 + r) from the token-major x through src_of with 16-byte cp.async copies, in the layout of the two
 // 64-column TMA boxes (see the GATHER note at tc_gemmT_kernel for the barrier protocol).
+constexpr int kGatherWarpsA = 4;  // GATHER_A: warp 2 and three extra warps (behind the epilogue warps) share the K rows of a block
 template <int A_MAJOR, int B_MAJOR, int EPI, bool GATHER_A = false>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 1) tc_gemm2_kernel(const __grid_constant__ TcParams P) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS + (GATHER_A ? 32 * (kGatherWarpsA - 1) : 0), 1)
+tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     constexpr int STAGES2 = Cfg2<EPI>::NST, NBUF = Cfg2<EPI>::NBUF, BKc = Cfg2<EPI>::BKc, MNB = Cfg2<EPI>::MNB;
@@ -826,13 +828,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES2; ++s) {  // GATHER_A: + the leader's 32 gather lanes + the peer's forwarder
-            mbar_init(&full_bar[s], GATHER_A ? 34 : 1), mbar_init(&empty_bar[s], 1);
-            if (GATHER_A) mbar_init(&gfull_bar[s], 32);
+            mbar_init(&full_bar[s], GATHER_A ? 2 + 32 * kGatherWarpsA : 1), mbar_init(&empty_bar[s], 1);
+            if (GATHER_A) mbar_init(&gfull_bar[s], 32 * kGatherWarpsA);
         }
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 2 * Cfg2<EPI>::EPI_WARPS);  // both CTAs
         for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
         for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer (+ gather warps, forwarder)
-            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1 + (GATHER_A ? 3 : 0));
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1 + (GATHER_A ? 2 * kGatherWarpsA + 1 : 0));
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -929,45 +931,45 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             }
         }
         if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
-    } else if (GATHER_A && warp == 2) {
-        // ===== A producer, gathered (both CTAs, all 32 lanes) =====
-        const int ch = lane & 7, rs = lane >> 3;
+    } else if (GATHER_A && (warp == 2 || warp >= 4 + Cfg2<EPI>::EPI_WARPS)) {
+        // ===== A producers, gathered (both CTAs; kGatherWarpsA warps, all 32 lanes): a lane owns one 16-byte chunk (ch) of
+        // the two 64-column boxes of the K rows r = 16 q + 4 gw + rs; their swizzle term r & 7 = 4 (gw & 1) + rs is a constant
+        // of the lane, so the destination of copy (q, box j) is a fixed address + q * 2048 + j * MNB =====
+        const int gw = warp == 2 ? 0 : warp - (3 + Cfg2<EPI>::EPI_WARPS);
+        const int ch = lane & 7, rs = lane >> 3, r_lane = 4 * gw + rs;
         const char* gbase = static_cast<const char*>(P.gsrc);
         const uint32_t pitch16 = (uint32_t)P.g_cols >> 3;
+        const uint32_t dst_lane = smem_u32(smem) + r_lane * 128 + ((ch ^ (r_lane & 7)) << 4);
+        constexpr int NQ = BKc / (4 * kGatherWarpsA);
         int stage = 0, phase = 0;
         for (int it = 0;; ++it) {
             const int t = dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid;
             if (t >= n_total) break;
             const Tile2 T = decode_pair(P, tp, tpp, offsets, t, rank, BKc, rcp_group, rcp_pairs);
             const int seg_end = tp[T.g + 1];  // rows of the next expert are never issued to the tensor core: not loaded
+            const int col0 = T.m0 + ch * 8;
+            const uint32_t c_bad0 = col0 < P.g_cols ? 0u : 1u, c_bad1 = col0 + 64 < P.g_cols ? 0u : 1u;
+            const char* src0 = gbase + (c_bad0 ? 0 : (size_t)col0 * 2);
+            const char* src1 = gbase + (c_bad1 ? 0 : (size_t)(col0 + 64) * 2);
             for (int kb = 0; kb < T.nkb; ++kb) {
                 const int k = T.k0 + kb * BKc;
-                // source rows of this K block: 4 per lane (coalesced loads), handed to the lanes that copy them by shuffles
-                uint32_t mine[BKc / 32];
+                uint32_t off[NQ], zmask = 0;
 #pragma unroll
-                for (int q = 0; q < BKc / 32; ++q) {
-                    const int row = k + q * 32 + lane;
+                for (int q = 0; q < NQ; ++q) {
+                    const int row = k + 4 * kGatherWarpsA * q + r_lane;
                     const int a = row < seg_end ? P.src_of[row] : -1;
-                    mine[q] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0xFFFFFFFFu;
+                    off[q] = a >= 0 ? (uint32_t)(((unsigned long long)a * P.g_magic) >> 35) * pitch16 : 0u;
+                    zmask |= a >= 0 ? 0u : 1u << q;
                 }
                 if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
                 __syncwarp();
-                // destination of row r = 4 i + rs, box j: sa + j MNB + r 128 + ((ch ^ (r & 7)) << 4), r & 7 = 4 (i & 1) + rs
-                const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES) + rs * 128;
-                const uint32_t d_even = sa + ((ch ^ rs) << 4), d_odd = sa + ((ch ^ (4 + rs)) << 4);
-                const int col0 = T.m0 + ch * 8;
-                const uint32_t c_bad0 = col0 < P.g_cols ? 0u : 1u, c_bad1 = col0 + 64 < P.g_cols ? 0u : 1u;
-                const char* src0 = gbase + (c_bad0 ? 0 : (size_t)col0 * 2);
-                const char* src1 = gbase + (c_bad1 ? 0 : (size_t)(col0 + 64) * 2);
+                const uint32_t dst = dst_lane + stage * STAGE2_BYTES;
 #pragma unroll
-                for (int i = 0; i < BKc / 4; ++i) {
-                    // row 4 i + rs = 32 (i >> 3) + 4 (i & 7) + rs: held by lane 4 (i & 7) + rs in mine[i >> 3]
-                    const uint32_t o = __shfl_sync(0xffffffffu, mine[i >> 3], 4 * (i & 7) + rs);
-                    const uint32_t z = o == 0xFFFFFFFFu ? 1u : 0u;
-                    const size_t ob = z ? 0 : (size_t)o * 16;
-                    const uint32_t d = ((i & 1) ? d_odd : d_even) + i * 512;
-                    cp_async16_z(d, src0 + ob, z | c_bad0);
-                    cp_async16_z(d + MNB, src1 + ob, z | c_bad1);
+                for (int q = 0; q < NQ; ++q) {
+                    const uint32_t z = zmask & (1u << q);
+                    const size_t ob = (size_t)off[q] * 16;
+                    cp_async16_z(dst + q * (4 * kGatherWarpsA * 128), src0 + ob, z | c_bad0);
+                    cp_async16_z(dst + q * (4 * kGatherWarpsA * 128) + MNB, src1 + ob, z | c_bad1);
                 }
                 cp_async_arrive(rank == 0 ? &full_bar[stage] : &gfull_bar[stage]);
                 if (++stage == STAGES2) stage = 0, phase ^= 1;
@@ -985,7 +987,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
                 if (lane == 0) {
                     mbar_wait(&gfull_bar[stage], phase);
                     fence_proxy_async();
-                    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(leader_full + stage * 8) : "memory");
+                    // plain remote arrive: the cluster-scope release form is a GPU-scope membar per K block (1-2 us in this
+                    // thread: the whole kernel ran at its pace).  The rows are read by this CTA's own tensor core, after the
+                    // proxy fence above; the arrival only tells the leader that it may issue.
+                    mbar_arrive_cluster(leader_full + stage * 8);
                 }
                 __syncwarp();
                 if (++stage == STAGES2) stage = 0, phase ^= 1;
@@ -1018,12 +1023,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Cfg2<EPI>::THREADS, 
             const uint32_t d_tmem = tmem_u + as * BN;
             for (int kb = 0; kb < t_nkb; ++kb) {
                 const long long c0 = P.prof ? clock64() : 0;
-                if (GATHER_A) {
-                    mbar_wait_cluster(&full_bar[stage], phase);
-                    fence_proxy_async();
-                } else {
-                    mbar_wait(&full_bar[stage], phase);
-                }
+                mbar_wait(&full_bar[stage], phase);
+                if (GATHER_A) fence_proxy_async();  // gathered rows were written through the generic proxy
                 if (P.prof) w_full += clock64() - c0;
                 tc_fence_after();
                 if (elect_one()) {
@@ -1498,7 +1499,10 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                 if (lane == 0) {
                     mbar_wait(&gfull_bar[stage], phase);
                     fence_proxy_async();  // the copies are generic-proxy writes; the tensor core reads through the async proxy
-                    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(leader_full + stage * 8) : "memory");
+                    // plain remote arrive: the cluster-scope release form is a GPU-scope membar per K block (1-2 us in this
+                    // thread: the whole kernel ran at its pace).  The rows are read by this CTA's own tensor core, after the
+                    // proxy fence above; the arrival only tells the leader that it may issue.
+                    mbar_arrive_cluster(leader_full + stage * 8);
                 }
                 __syncwarp();
                 if (++stage == NST) stage = 0, phase ^= 1;
@@ -1607,8 +1611,8 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
             for (int kb = 0; kb < nkb; ++kb) {
                 const long long c0 = P.prof ? clock64() : 0;
                 if (GATHER) {
-                    mbar_wait_cluster(&full_bar[stage], phase);  // pairs with the peer forwarder's cluster-scope release
-                    fence_proxy_async();                         // gathered rows were written through the generic proxy
+                    mbar_wait(&full_bar[stage], phase);
+                    fence_proxy_async();  // gathered rows were written through the generic proxy
                 } else {
                     mbar_wait(&full_bar[stage], phase);
                 }
@@ -1998,11 +2002,12 @@ int launch(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, bool 
     }
     if (two_cta) {
         // tile_bound counts tile pairs; one cluster of two CTAs per pair, one CTA per SM
-        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A>, Cfg2<EPI>::SMEM, Cfg2<EPI>::THREADS);
+        constexpr int threads = Cfg2<EPI>::THREADS + (GATHER_A ? 32 * (kGatherWarpsA - 1) : 0);
+        long long clusters = resident_clusters(c, ln, tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A>, Cfg2<EPI>::SMEM, threads);
         if (tile_bound < clusters) clusters = tile_bound;
         if (clusters < 1) clusters = 1;
         Q.sched = sched_counters(c, ln.stream);
-        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A><<<(unsigned)(2 * clusters), Cfg2<EPI>::THREADS, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
+        tc_gemm2_kernel<A_MAJOR, B_MAJOR, EPI, GATHER_A><<<(unsigned)(2 * clusters), threads, Cfg2<EPI>::SMEM, ln.stream>>>(Q);
         PIPER_LAUNCHED(c, name);
         return PIPER_OK;
     }
