@@ -240,8 +240,6 @@ class Workload:
         log(f"[rank {rank}] {cfg.name}: inputs generated in {time.time() - t0:.1f} s")
         self.ctx = piper.Context(desc_of(piper, self.rcfg, dw_f32=args.main_grad), device=local)
         piper.piper_set_chunk_overlap(self.ctx, 1 if getattr(args, "chunk_overlap", False) else 0)
-        if getattr(args, "no_fused_gather", False):
-            piper.piper_set_option(self.ctx, piper.OPT_FUSED_GATHER, 0)
         for kv in getattr(args, "opt", None) or []:  # measured variants: --opt T_SPLIT_K=0 ...
             name, val = kv.split("=")
             piper.piper_set_option(self.ctx, getattr(piper, "OPT_" + name), int(val))
@@ -645,9 +643,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true",
                     help="only the headline workload: skip the C3 / C4 / C5-pair blocks of the default run")
-    ap.add_argument("--no-fused-gather", action="store_true",
-                    help="measured variant: the chunk calls run the separate pack / combine_bwd row movers and the GEMMs read "
-                         "xp / d_o (PIPER_OPT_FUSED_GATHER = 0)")
     ap.add_argument("--tc-counters", action="store_true",
                     help="add the tcgen05 kernels' debug wait-cycle counters per GEMM task (PIPER_OPT_TC_PROFILE) to the line")
     ap.add_argument("--opt", action="append", help="kernel-variant switch NAME=VALUE (piper_set_option, PIPER_OPT_<NAME>)")

@@ -101,7 +101,7 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
  *                              accumulators (measured neutral)
  *  PIPER_OPT_T_PREFETCH   [0]  rows-on-N: the weight producer prefetches the box this many K blocks ahead into L2
  *  PIPER_OPT_TC_PROFILE   [0]  1 = the tcgen05 kernels record wait-cycle counters (piper_debug_tc_counters)
- *  PIPER_OPT_FUSED_GATHER [1]  chunk calls on tcgen05 layers (N2 fusion): 0 = the GEMMs read the packed buffers xp / d_o;
+ *  PIPER_OPT_FUSED_GATHER [0]  chunk calls on tcgen05 layers (N2 fusion): 0 = the GEMMs read the packed buffers xp / d_o;
  *                              1 = F_GEMM1 and the gate|up wgrad gather the rows of x themselves, no pack kernel runs;
  *                              2 = also DGRAD1 gathers the rows of dY and applies the gate in its fp32 epilogue
  * Returns PIPER_ERR_INVALID for unknown options / values, PIPER_ERR_UNSUPPORTED when the layer cannot run the

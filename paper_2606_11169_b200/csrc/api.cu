@@ -135,7 +135,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
         piper_destroy(c);
         return PIPER_ERR_CUDA;
     }
-    c->fused_gather = 1;
+    c->fused_gather = 0;  // N2 fusion is built and parity-tested but measured slower than pack + TMA (DESIGN.md finding 19)
     c->pair_order = PIPER_ORDER_PROFILE, c->pair_part = PIPER_PART_SHARED;  // the policy that does not lose to serial
     const int rc = variant_ok(c);
     if (rc != PIPER_OK) {
