@@ -79,8 +79,6 @@ struct alignas(64) TcParams {
     const void* gsrc;           // token-major source [T, g_cols] bf16
     unsigned long long g_magic; // ceil(2^35 / k): a / k = (a * g_magic) >> 35 for a < 2^30, k <= 8
     int g_cols;                 // columns of the source (= the contraction / feature length d)
-    int prefetch_kb;            // rows-on-N kernels: the weight producer prefetches this many K blocks ahead into L2 (0 = off)
-    int split_k;                // rows-on-N kernels: chunks of <= 128 rows use two half accumulators (PIPER_OPT_T_SPLIT_K)
     const float* row_scale;     // DGRAD1 with gathered dY: the epilogue multiplies row r of dH by row_scale[r] (the gate)
     int small_rows;         // chunks of at most this many rows per CTA load 32-row activation boxes
 };
@@ -157,11 +155,6 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
             smem_u32(dst)),
         "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
-}
-// bring a box into L2 ahead of its load (no shared-memory destination, no barrier)
-__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2) {
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2)
-                 : "memory");
 }
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -399,16 +392,17 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
     const int n_total = total_tiles(P, tp);
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer (the warp runs converged, one elected lane issues: see elect_one) =====
         int stage = 0, phase = 0;
         long long w_empty = 0;
         for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
-            const Tile T = decode_tile(P, tp, offsets, t);
+            Tile T = decode_tile(P, tp, offsets, t);
+            T.g = uni(T.g), T.m0 = uni(T.m0), T.n0 = uni(T.n0), T.k0 = uni(T.k0), T.nkb = uni(T.nkb);
             for (int kb = 0; kb < T.nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&empty_bar[stage], phase ^ 1);
-                    if (P.prof) w_empty += clock64() - c0;
+                const long long c0 = P.prof ? clock64() : 0;
+                mbar_wait(&empty_bar[stage], phase ^ 1);
+                if (P.prof) w_empty += clock64() - c0;
+                if (elect_one()) {
                     uint8_t* sa = smem + stage * STAGE_BYTES;
                     uint8_t* sb = sa + A_BYTES;
                     uint64_t* bar = &full_bar[stage];
@@ -443,34 +437,35 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
         }
         if (P.prof && lane == 0) P.prof[blockIdx.x * 8 + 3] = w_empty;
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread) =====
+        // ===== MMA issuer (warp 1, converged; one elected lane issues) =====
         constexpr uint32_t idesc = make_idesc(A_MAJOR, B_MAJOR);
         constexpr uint32_t a_lbo = A_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES, b_lbo = B_MAJOR == K_MAJOR ? 16 : MN_BLOCK_BYTES;
         constexpr uint32_t a_kstep = A_MAJOR == K_MAJOR ? UK * 2 : UK * 128, b_kstep = B_MAJOR == K_MAJOR ? UK * 2 : UK * 128;
+        const uint32_t smem_base = uni(smem_u32(smem)), tmem_u = uni(tmem_base);
+        const uint64_t a_desc0 = make_desc(smem_base, a_lbo, 1024), b_desc0 = make_desc(smem_base + A_BYTES, b_lbo, 1024);
         int stage = 0, phase = 0, as = 0, aphase = 0;
         long long w_full = 0, w_tempty = 0, n_tiles_done = 0;
         const long long t_begin = P.prof ? clock64() : 0;
         for (int t = blockIdx.x; t < n_total; t += gridDim.x) {
-            const Tile T = decode_tile(P, tp, offsets, t);
-            if (lane == 0) {
+            const int t_nkb = uni(decode_tile(P, tp, offsets, t).nkb);
+            {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&tempty_bar[as], aphase ^ 1);
                 if (P.prof) w_tempty += clock64() - c0, ++n_tiles_done;
                 tc_fence_after();
             }
-            __syncwarp();
-            const uint32_t d_tmem = tmem_base + as * BN;
-            for (int kb = 0; kb < T.nkb; ++kb) {
-                if (lane == 0) {
-                    const long long c0 = P.prof ? clock64() : 0;
-                    mbar_wait(&full_bar[stage], phase);
-                    if (P.prof) w_full += clock64() - c0;
-                    tc_fence_after();
-                    const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+            const uint32_t d_tmem = tmem_u + as * BN;
+            for (int kb = 0; kb < t_nkb; ++kb) {
+                const long long c0 = P.prof ? clock64() : 0;
+                mbar_wait(&full_bar[stage], phase);
+                if (P.prof) w_full += clock64() - c0;
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t soff = (uint32_t)(stage * STAGE_BYTES) >> 4;
 #pragma unroll
                     for (int kk = 0; kk < BK / UK; ++kk) {
-                        const uint64_t ad = make_desc(sa + kk * a_kstep, a_lbo, 1024);
-                        const uint64_t bd = make_desc(sb + kk * b_kstep, b_lbo, 1024);
+                        const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
+                        const uint64_t bd = b_desc0 + (soff + ((kk * b_kstep) >> 4));
                         umma_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
                     umma_commit(&empty_bar[stage]);  // frees the smem slot when these MMAs have read it
@@ -478,7 +473,7 @@ __global__ void __launch_bounds__(kThreads, 1) tc_gemm_kernel(const __grid_const
                 __syncwarp();
                 if (++stage == STAGES) stage = 0, phase ^= 1;
             }
-            if (lane == 0) umma_commit(&tfull_bar[as]);  // accumulator complete (immediately if nkb == 0)
+            if (elect_one()) umma_commit(&tfull_bar[as]);  // accumulator complete (immediately if nkb == 0)
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
         }
@@ -1556,26 +1551,6 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                     } else {
                         tma_load_3d_pair(sa, &P.a[src], bar, k, T.f * 256 + urank * 128, T.g);
                     }
-                    // The weights of a tile stream from HBM once; an SM holds NST stages (80 KB of weights) in flight, which
-                    // at the loaded HBM latency caps it near 40 GB/s.  Prefetching the box `prefetch_kb` K blocks ahead into
-                    // L2 makes the demand load an L2 hit (PIPER_OPT_T_PREFETCH).
-                    if (load_a && P.prefetch_kb > 0) {
-                        const int kbp = kb + P.prefetch_kb;
-                        if (kbp < nkb) {
-                            int srcp = 0, kkp = kbp;
-                            if (kbp >= P.kb_per_src) srcp = 1, kkp = kbp - P.kb_per_src;
-                            const int kp = kkp * BK;
-                            if (EPI == TEPI_SWIGLU_FWD) {
-                                const int fc = T.f * 128 + urank * 64;
-                                tma_prefetch_3d(&P.a[0], fc, kp, T.g), tma_prefetch_3d(&P.a[1], fc, kp, T.g);
-                            } else if (A_MAJOR == MN_MAJOR) {
-                                const int fc = T.f * 256 + urank * 128;
-                                tma_prefetch_3d(&P.a[srcp], fc, kp, T.g), tma_prefetch_3d(&P.a[srcp], fc + 64, kp, T.g);
-                            } else {
-                                tma_prefetch_3d(&P.a[srcp], kp, T.f * 256 + urank * 128, T.g);
-                            }
-                        }
-                    }
                 }
                 __syncwarp();
                 if (++stage == NST) stage = 0, phase ^= 1;
@@ -1605,17 +1580,10 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                 tc_fence_after();
             }
             const uint32_t d_tmem = tmem_u + as * BN;
-            // PIPER_OPT_T_SPLIT_K (measured neutral): chunks of at most 128 rows alternate their K steps between two
-            // accumulators (columns [0, n) and [128, 128 + n) of the buffer); the epilogue adds the halves in fp32.
-            const bool splitk = P.split_k && tn <= 128;
             for (int kb = 0; kb < nkb; ++kb) {
                 const long long c0 = P.prof ? clock64() : 0;
-                if (GATHER) {
-                    mbar_wait(&full_bar[stage], phase);
-                    fence_proxy_async();  // gathered rows were written through the generic proxy
-                } else {
-                    mbar_wait(&full_bar[stage], phase);
-                }
+                mbar_wait(&full_bar[stage], phase);
+                if (GATHER) fence_proxy_async();  // gathered rows were written through the generic proxy
                 if (P.prof) w_full += clock64() - c0;
                 tc_fence_after();
                 if (elect_one()) {
@@ -1624,8 +1592,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                     for (int kk = 0; kk < BK / UK; ++kk) {
                         const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
                         const uint64_t bd = b_desc0 + (soff + ((kk * UK * 2) >> 4));
-                        if (splitk) umma2_bf16(d_tmem + ((kk & 1) ? 128 : 0), ad, bd, idesc, (kb != 0) | (kk >= 2));
-                        else umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
+                        umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
                     umma2_commit(&empty_bar[stage]);
                 }
@@ -1705,16 +1672,6 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
             const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
             const int fcol = feat_col(T);
             const bool f_ok = fcol < P.f_limit;
-            const bool splitk = P.split_k && T.n <= 128;  // two half accumulators (see the MMA issuer): add them
-            auto add_half = [&](uint32_t (&r)[32], int j) {
-                if (splitk) {
-                    uint32_t r2[32];
-                    tmem_ld32(taddr + 128 + j, r2);
-                    tmem_ld_wait32(r2);
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) + __uint_as_float(r2[i]));
-                }
-            };
 #pragma unroll 1
             for (int j = 0; j < T.n; j += 32, ++q) {
                 const bool both = j + 16 < T.n;
@@ -1727,7 +1684,6 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                     __syncwarp();
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
-                    add_half(r, j);
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
                     stage_col(buf, v);
@@ -1741,7 +1697,6 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                     const uint32_t xch = smem_u32(xch_base) + (pr * 2 + (q & 1)) * 4096 + lane * 4;
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
-                    add_half(r, j);
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
                     if (wq >= 2) {  // U lanes: hand the fp32 values to the G warp, store U
@@ -1795,7 +1750,6 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                     }
                     tmem_ld32(taddr + j, r);
                     tmem_ld_wait32(r);
-                    add_half(r, j);
                     // gathered dY rows are unscaled: dH[r] = gate_rows[r] * (dY[token(r)] Wd^T), the gate applied in fp32
                     const float* rsc = P.row_scale ? P.row_scale + T.r0 + j : nullptr;
 #pragma unroll
@@ -2066,7 +2020,7 @@ TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_t
     memset(&P, 0, sizeof(P));
     P.offsets = p.offsets, P.counts = p.counts, P.G = p.G, P.n_src = 1;
     P.f_tiles = cdiv(F, f_tile), P.f_limit = F, P.kb_per_src = cdiv(K, BK);
-    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy, P.split_k = c->tc_split_k, P.prefetch_kb = c->tc_prefetch_kb;
+    P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy;
     return P;
 }
 inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
@@ -2120,8 +2074,6 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
-    c->tc_prefetch_kb = 0;
-    c->tc_split_k = 0;  // measured without gain: the ~130-cycle issue cost of an MMA does not come from the accumulator chain
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
