@@ -245,7 +245,8 @@ pack_kernel(const int4* __restrict__ x, const int32_t* __restrict__ offsets, con
 // ---- F5 combine / B5 unpack ------------------------------------------------------------------------
 // y[t] = sum_{j local} w_j * o[row_of[t,j]] (+ s[t]);  WEIGHTED: w_j = gates[t,j], else 1 (unpack).
 // fp32 accumulation in slot order j = 0..k-1 then s, one rounding on store.
-template <bool BF16, bool WEIGHTED>
+// TWO: a second token-row addend s2 after s (the router's term of dX, N1); the common kernels are compiled without it.
+template <bool BF16, bool WEIGHTED, bool TWO>
 __global__ void __launch_bounds__(kMoveWarps * 32)
 combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, const float* __restrict__ gates,
                const int4* __restrict__ s, const int4* __restrict__ s2, int T, int k, int row_packets, int S,
@@ -253,8 +254,7 @@ combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, c
     const int lane = threadIdx.x & 31;
     const int warp = blockIdx.x * kMoveWarps + (threadIdx.x >> 5);
     const int nwarps = gridDim.x * kMoveWarps;
-    if (s == nullptr) s = s2, s2 = nullptr;  // token-row addends (shared expert, router path): s first, then s2
-    const int n_src = k + (s != nullptr ? 1 : 0) + (s2 != nullptr ? 1 : 0);
+    const int n_src = k + (s != nullptr ? 1 : 0) + (TWO ? 1 : 0);
     for (int item = warp; item < T * S; item += nwarps) {
         const int t = item / S, sp = item - t * S;
         const int my_row = lane < k ? row_of[(size_t)t * k + lane] : -1;
@@ -278,7 +278,7 @@ combine_kernel(const int4* __restrict__ o, const int32_t* __restrict__ row_of, c
                     if (r < 0) continue;
                     src = o + (size_t)r * row_packets;
                 } else {
-                    src = (j == k ? s : s2) + (size_t)t * row_packets;
+                    src = ((TWO && (j > k || s == nullptr)) ? s2 : s) + (size_t)t * row_packets;
                 }
                 int4 nxt[U];
                 load_step(nxt, src, p0, lane, hi);  // in flight while the previous source is accumulated
@@ -428,12 +428,15 @@ int launch_combine(piper_ctx* c, Lane ln, const void* o, const int32_t* row_of, 
     const int items = D.T * S;
     const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s), *s24 = static_cast<const int4*>(s2);
     int4* y4 = static_cast<int4*>(y);
-#define PIPER_COMBINE(BF, W)                                                                              \
-    combine_kernel<BF, W><<<mover_blocks(ln, items, combine_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, s24, D.T, D.k, row_packets, S, split_packets, y4)
-    if (D.dtype == PIPER_DTYPE_BF16) {
-        if (weighted) PIPER_COMBINE(true, true); else PIPER_COMBINE(true, false);
+#define PIPER_COMBINE(BF, W, TW)                                                                          \
+    combine_kernel<BF, W, TW><<<mover_blocks(ln, items, combine_kernel<BF, W, TW>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, s24, D.T, D.k, row_packets, S, split_packets, y4)
+    if (s2 != nullptr) {  // only B5 with the router's term carries a second addend
+        if (weighted) return PIPER_ERR_INVALID;
+        if (D.dtype == PIPER_DTYPE_BF16) PIPER_COMBINE(true, false, true); else PIPER_COMBINE(false, false, true);
+    } else if (D.dtype == PIPER_DTYPE_BF16) {
+        if (weighted) PIPER_COMBINE(true, true, false); else PIPER_COMBINE(true, false, false);
     } else {
-        if (weighted) PIPER_COMBINE(false, true); else PIPER_COMBINE(false, false);
+        if (weighted) PIPER_COMBINE(false, true, false); else PIPER_COMBINE(false, false, false);
     }
 #undef PIPER_COMBINE
     PIPER_LAUNCHED(c, "combine_kernel");
