@@ -1265,13 +1265,15 @@ constexpr int T_PANEL = 8;  // chunks per panel of the tile order (the panel's r
 //                           // rows per activation TMA box
 constexpr int TA_BYTES = 128 * BK * 2;                     // 128 features x 64 K
 constexpr int TB_BYTES = 128 * BK * 2;                     // up to 128 rows x 64 K per CTA
-constexpr int TSTAGE_BYTES = TA_BYTES + TB_BYTES;
 constexpr int TSTG_BYTES = 32 * 32 * 2;                    // staging block: 32 rows x 32 features bf16
-template <int EPI>
+// DUAL: a tile may carry two row chunks of one expert (up to 2 x 256 rows) through one pass over the weights: a stage holds
+// the weight slice once and both chunks' row slices, and both TMEM accumulators belong to the tile (see tc_gemmT_kernel).
+template <int EPI, bool DUAL = false>
 struct CfgT {
-    static constexpr int NST = 5;
-    static constexpr int NBUF = 4;                         // staging blocks per epilogue warp
-    static constexpr int RING_BYTES = NST * TSTAGE_BYTES, STG_TOTAL = 4 * NBUF * TSTG_BYTES;
+    static constexpr int NST = DUAL ? 4 : 5;
+    static constexpr int NBUF = DUAL ? 3 : 4;              // staging blocks per epilogue warp
+    static constexpr int STAGE_BYTES = TA_BYTES + (DUAL ? 2 : 1) * TB_BYTES;
+    static constexpr int RING_BYTES = NST * STAGE_BYTES, STG_TOTAL = 4 * NBUF * TSTG_BYTES;
     static constexpr int XCH_BYTES = EPI == TEPI_SWIGLU_FWD ? 2 * 2 * 32 * 32 * 4 : 0;  // fp32 U exchange, 2 pairs x 2
     static constexpr int ZERO_BYTES = 16 * 32 * 2;         // a zero block for the pad rows
     static constexpr int SCHED_BYTES = 256;                // tile feed: 8 ids + 2 x 8 mbarriers
@@ -1281,7 +1283,8 @@ struct CfgT {
 
 struct TileT {
     int g, f, r0, n;  // group, feature tile, first packed row, rows (multiple of 16, <= 256)
-    int zend;         // last chunk of a group: end of the group's padded segment (rows [r0 + n, zend) are zeroed)
+    int zend;         // last chunk of a group: end of the group's padded segment (rows [r0 + n + n1, zend) are zeroed)
+    int n1;           // DUAL: rows of the tile's second chunk (it starts at r0 + n), 0 = none
 };
 // An expert's rows are cut into nch chunks of cs rows: about equal, cs a multiple of 16 and <= 256.
 __device__ __forceinline__ void t_plan(int rows, int& nch, int& cs, int greedy) {
@@ -1289,23 +1292,28 @@ __device__ __forceinline__ void t_plan(int rows, int& nch, int& cs, int greedy) 
     cs = greedy ? 256 : (n0 ? ((rows + n0 - 1) / n0 + 15) & ~15 : 16);
     nch = (rows + cs - 1) / cs;
 }
-// tq / so / sc: first tile, first packed row and real row count of each group, in shared memory
-__device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, const int* so, const int* sc, int t) {
+// tq / so / sc: first tile, first packed row and real row count of each group, in shared memory.  dual: a tile takes two
+// consecutive chunks (the last tile of a group with an odd chunk count takes one).
+__device__ __forceinline__ TileT decode_t(const TcParams& P, const int* tq, const int* so, const int* sc, int t, bool dual) {
     int g = 0;
     while (g + 1 < P.G && tq[g + 1] <= t) ++g;
     const int local = t - tq[g], rows = sc[g];
     const int* offsets = so;
     int nch, cs;
     t_plan(rows, nch, cs, P.greedy);
-    // panels of T_PANEL chunks; inside a panel feature-major with the chunk fastest
+    const int nun = dual ? (nch + 1) >> 1 : nch;  // tiles along the rows
+    // panels of T_PANEL row tiles; inside a panel feature-major with the row tile fastest
     const int per_panel = T_PANEL * P.f_tiles;
     const int panel = local / per_panel, rem = local - panel * per_panel;
-    const int pc = min(T_PANEL, nch - panel * T_PANEL);
-    const int f = rem / pc, c = panel * T_PANEL + (rem - f * pc);
+    const int pc = min(T_PANEL, nun - panel * T_PANEL);
+    const int f = rem / pc, u = panel * T_PANEL + (rem - f * pc);
+    const int c = dual ? 2 * u : u;
     const int left = rows - c * cs;
     TileT r;
     r.g = g, r.f = f, r.r0 = offsets[g] + c * cs, r.n = min(cs, (left + 15) & ~15);
-    r.zend = c == nch - 1 ? offsets[g + 1] : r.r0 + r.n;
+    r.n1 = (dual && c + 1 < nch) ? min(cs, (left - cs + 15) & ~15) : 0;
+    const bool last = (r.n1 ? c + 1 : c) == nch - 1;
+    r.zend = last ? offsets[g + 1] : r.r0 + r.n + r.n1;
     return r;
 }
 __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
@@ -1320,19 +1328,21 @@ __host__ __device__ constexpr uint32_t make_idesc_t(int a_major, int n) {
 // (cp.async.mbarrier.arrive); the peer CTA's lanes arrive on a local barrier that the peer's otherwise idle warp 1
 // forwards to the leader (proxy fence + cluster-scope release).
 constexpr int kGatherWarps = 2;  // GATHER: warp 2 and one extra warp (8) share the rows of a tile
-template <int A_MAJOR, int EPI, bool GATHER = false>
+template <int A_MAJOR, int EPI, bool GATHER = false, bool DUAL = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GATHER ? kThreads + 32 * (kGatherWarps - 1) : kThreads, 1)
 tc_gemmT_kernel(const __grid_constant__ TcParams P) {
+    static_assert(!DUAL || (EPI == TEPI_STORE && !GATHER), "two-chunk tiles: plain-store kernels only");
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    constexpr int NST = CfgT<EPI>::NST, NBUF = CfgT<EPI>::NBUF;
-    uint8_t* stg_base = smem + CfgT<EPI>::RING_BYTES;
-    uint8_t* xch_base = stg_base + CfgT<EPI>::STG_TOTAL;
-    uint8_t* zero_blk = xch_base + CfgT<EPI>::XCH_BYTES;
-    uint64_t* feed_full = reinterpret_cast<uint64_t*>(zero_blk + CfgT<EPI>::ZERO_BYTES);  // [kFeed] one set per CTA
+    using Cfg = CfgT<EPI, DUAL>;
+    constexpr int NST = Cfg::NST, NBUF = Cfg::NBUF, TSTAGE = Cfg::STAGE_BYTES;
+    uint8_t* stg_base = smem + Cfg::RING_BYTES;
+    uint8_t* xch_base = stg_base + Cfg::STG_TOTAL;
+    uint8_t* zero_blk = xch_base + Cfg::XCH_BYTES;
+    uint64_t* feed_full = reinterpret_cast<uint64_t*>(zero_blk + Cfg::ZERO_BYTES);  // [kFeed] one set per CTA
     uint64_t* feed_empty = feed_full + kFeed;                                              // [kFeed] used in the leader CTA
     int* feed_ids = reinterpret_cast<int*>(feed_empty + kFeed);                            // [kFeed] one set per CTA
-    uint64_t* full_bar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(feed_full) + CfgT<EPI>::SCHED_BYTES);
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(feed_full) + Cfg::SCHED_BYTES);
     uint64_t* empty_bar = full_bar + NST;                                                // one set per CTA
     uint64_t* tfull_bar = empty_bar + NST;                                               // [2] one set per CTA
     uint64_t* tempty_bar = tfull_bar + 2;                                                // [2] used in the leader CTA
@@ -1351,7 +1361,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
     const int32_t* __restrict__ counts = P.counts;
 
     if (warp == 3) {  // zero block; exclusive scan of the tiles per group
-        for (int i = lane; i < CfgT<EPI>::ZERO_BYTES / 16; i += 32) st_shared16(zero_blk + 16 * i, make_uint4(0, 0, 0, 0));
+        for (int i = lane; i < Cfg::ZERO_BYTES / 16; i += 32) st_shared16(zero_blk + 16 * i, make_uint4(0, 0, 0, 0));
         fence_proxy_async();
         int carry = 0;
         if (lane == 0) so[P.G] = offsets[P.G];
@@ -1363,7 +1373,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                 so[g] = lo, sc[g] = rows;
                 t_plan(rows, nch, cs, P.greedy);
             }
-            const int v = nch * P.f_tiles;
+            const int v = (DUAL ? (nch + 1) >> 1 : nch) * P.f_tiles;
             int x = v;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -1406,7 +1416,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
     auto tile_of = [&](int it) {
         const volatile int* w = feed.slot(it);
         TileT T;
-        T.g = w[1], T.f = w[2], T.r0 = w[3], T.n = w[4], T.zend = w[5];
+        T.g = w[1], T.f = w[2], T.r0 = w[3], T.n = w[4], T.zend = w[5], T.n1 = DUAL ? w[6] : 0;
         return T;
     };
 
@@ -1418,13 +1428,13 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
             const int slot = it & (kFeed - 1);
             mbar_wait(&feed_empty[slot], ((it / kFeed) & 1) ^ 1);
             const int t = it == 0 ? pair_id : n_pairs_grid + atomicAdd(P.sched, 1);
-            int w[6] = {t, 0, 0, 0, 0, 0};
+            int w[7] = {t, 0, 0, 0, 0, 0, 0};
             if (t < n_total) {
-                const TileT T = decode_t(P, tq, so, sc, t);
-                w[1] = T.g, w[2] = T.f, w[3] = T.r0, w[4] = T.n, w[5] = T.zend;
+                const TileT T = decode_t(P, tq, so, sc, t, DUAL);
+                w[1] = T.g, w[2] = T.f, w[3] = T.r0, w[4] = T.n, w[5] = T.zend, w[6] = T.n1;
             }
 #pragma unroll
-            for (int i = 0; i < 6; ++i) {
+            for (int i = 0; i < 7; ++i) {
                 *reinterpret_cast<volatile int*>(&feed_ids[slot * kFeedWords + i]) = w[i];
                 asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(peer_ids + (slot * kFeedWords + i) * 4), "r"(w[i]) : "memory");
             }
@@ -1471,7 +1481,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
             for (int kb = 0; kb < nkb; ++kb) {
                 if (lane == 0) mbar_wait(&empty_bar[stage], phase ^ 1);
                 __syncwarp();
-                const uint32_t dst = dst_lane + stage * TSTAGE_BYTES;
+                const uint32_t dst = dst_lane + stage * TSTAGE;
                 const int kcol = kb * BK + ch * 8;
                 const uint32_t k_bad = kcol < P.g_cols ? 0u : 0xFFFFFFFFu;  // K tail: zero fill, as a TMA box does
                 const char* src_k = gbase + (k_bad ? 0 : (size_t)kcol * 2);
@@ -1514,21 +1524,27 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
         for (int it = 0;; ++it) {
             const int t = uni(feed.peek(it));
             TileT T = tile_of(it);
-            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n);
+            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n), T.n1 = uni(T.n1);
             feed.release(it, lane);
             if (t >= n_total) break;
             const int nb = T.n >> 1, rb = T.r0 + urank * nb;
             const bool small = nb <= P.small_rows;
             const int nbox = small ? (nb + TB_SMALL_ROWS - 1) / TB_SMALL_ROWS : 1;
             const int box_bytes = (small ? TB_SMALL_ROWS : TB_BOX_ROWS) * BK * 2;
+            // DUAL: the second chunk's half of this CTA, behind the first one's slot
+            const int nb1 = T.n1 >> 1, rb1 = T.r0 + T.n + urank * nb1;
+            const bool small1 = nb1 <= P.small_rows;
+            const int nbox1 = nb1 == 0 ? 0 : (small1 ? (nb1 + TB_SMALL_ROWS - 1) / TB_SMALL_ROWS : 1);
+            const int box_bytes1 = (small1 ? TB_SMALL_ROWS : TB_BOX_ROWS) * BK * 2;
             for (int kb = 0; kb < nkb; ++kb) {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&empty_bar[stage], phase ^ 1);
                 if (P.prof) w_empty += clock64() - c0;
                 if (elect_one()) {
-                    uint8_t* sa = smem + stage * TSTAGE_BYTES;
+                    uint8_t* sa = smem + stage * TSTAGE;
                     uint8_t* sb = sa + TA_BYTES;
-                    if (urank == 0) mbar_expect_tx(&full_bar[stage], load_a ? 2 * TA_BYTES : 2 * nbox * box_bytes);
+                    if (urank == 0)
+                        mbar_expect_tx(&full_bar[stage], load_a ? 2 * TA_BYTES : 2 * (nbox * box_bytes + (DUAL ? nbox1 * box_bytes1 : 0)));
                     const uint32_t bar = leader_full + stage * 8;
                     int src = 0, kk = kb;
                     if (kb >= P.kb_per_src) src = 1, kk = kb - P.kb_per_src;
@@ -1539,6 +1555,15 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                                 tma_load_3d_pair(sb + i * box_bytes, &P.bs[src], bar, k, rb + i * TB_SMALL_ROWS, 0);
                         } else {
                             tma_load_3d_pair(sb, &P.b[src], bar, k, rb, 0);
+                        }
+                        if (DUAL && nb1) {
+                            uint8_t* sb1 = sb + TB_BYTES;
+                            if (small1) {
+                                for (int i = 0; i < nbox1; ++i)
+                                    tma_load_3d_pair(sb1 + i * box_bytes1, &P.bs[src], bar, k, rb1 + i * TB_SMALL_ROWS, 0);
+                            } else {
+                                tma_load_3d_pair(sb1, &P.b[src], bar, k, rb1, 0);
+                            }
                         }
                     } else if (EPI == TEPI_SWIGLU_FWD) {  // 64 gate features | the same 64 up features
                         const int fc = T.f * 128 + urank * 64;
@@ -1569,7 +1594,7 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
         const long long t_begin = P.prof ? clock64() : 0;
         for (int it = 0;; ++it) {
             const int t = uni(feed.peek(it));
-            const int tn = uni(tile_of(it).n);
+            const int tn = uni(tile_of(it).n), tn1 = DUAL ? uni(tile_of(it).n1) : 0;
             feed.release(it, lane);
             if (t >= n_total) break;
             const uint32_t idesc = make_idesc_t(A_MAJOR, tn);
@@ -1580,6 +1605,14 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                 tc_fence_after();
             }
             const uint32_t d_tmem = tmem_u + as * BN;
+            // DUAL: the tile's second chunk accumulates in the other buffer (the next one in the epilogue's order), from
+            // the same weight slice of every stage
+            const int as1 = as ^ 1, aphase1 = as == 1 ? aphase ^ 1 : aphase;
+            const uint32_t idesc1 = make_idesc_t(A_MAJOR, tn1 ? tn1 : 16), d_tmem1 = tmem_u + as1 * BN;
+            if (DUAL && tn1) {
+                mbar_wait(&tempty_bar[as1], aphase1 ^ 1);
+                tc_fence_after();
+            }
             for (int kb = 0; kb < nkb; ++kb) {
                 const long long c0 = P.prof ? clock64() : 0;
                 mbar_wait(&full_bar[stage], phase);
@@ -1587,21 +1620,33 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
                 if (P.prof) w_full += clock64() - c0;
                 tc_fence_after();
                 if (elect_one()) {
-                    const uint32_t soff = (uint32_t)(stage * TSTAGE_BYTES) >> 4;
+                    const uint32_t soff = (uint32_t)(stage * TSTAGE) >> 4;
 #pragma unroll
                     for (int kk = 0; kk < BK / UK; ++kk) {
                         const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
                         const uint64_t bd = b_desc0 + (soff + ((kk * UK * 2) >> 4));
                         umma2_bf16(d_tmem, ad, bd, idesc, (kb | kk) != 0);
                     }
+                    if (DUAL && tn1) {
+#pragma unroll
+                        for (int kk = 0; kk < BK / UK; ++kk) {
+                            const uint64_t ad = a_desc0 + (soff + ((kk * a_kstep) >> 4));
+                            const uint64_t bd = b_desc0 + (soff + ((TB_BYTES + kk * UK * 2) >> 4));
+                            umma2_bf16(d_tmem1, ad, bd, idesc1, (kb | kk) != 0);
+                        }
+                    }
                     umma2_commit(&empty_bar[stage]);
                 }
                 __syncwarp();
                 if (++stage == NST) stage = 0, phase ^= 1;
             }
-            if (elect_one()) umma2_commit(&tfull_bar[as]);
+            if (elect_one()) {
+                umma2_commit(&tfull_bar[as]);
+                if (DUAL && tn1) umma2_commit(&tfull_bar[as1]);
+            }
             __syncwarp();
             if (++as == 2) as = 0, aphase ^= 1;
+            if (DUAL && tn1 && ++as == 2) as = 0, aphase ^= 1;
         }
         if (P.prof && lane == 0) {
             long long* pq = P.prof + blockIdx.x * 8;
@@ -1662,142 +1707,151 @@ tc_gemmT_kernel(const __grid_constant__ TcParams P) {
         for (int it = 0;; ++it) {
             const int t = uni(feed.peek(it));
             TileT T = tile_of(it);
-            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n), T.zend = uni(T.zend);
+            T.g = uni(T.g), T.f = uni(T.f), T.r0 = uni(T.r0), T.n = uni(T.n), T.zend = uni(T.zend), T.n1 = uni(T.n1);
             feed.release(it, lane);
             if (t >= n_total) break;
-            const long long c0 = P.prof ? clock64() : 0;
-            mbar_wait(&tfull_bar[as], aphase);
-            if (P.prof) w_tfull += clock64() - c0;
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
-            const int fcol = feat_col(T);
-            const bool f_ok = fcol < P.f_limit;
+            // DUAL: a tile's two chunks are drained one after the other, the second from the other accumulator
+            const int n_half = (DUAL && T.n1) ? 2 : 1;
 #pragma unroll 1
-            for (int j = 0; j < T.n; j += 32, ++q) {
-                const bool both = j + 16 < T.n;
-                uint32_t r[32];
-                float v[32];
-                if (EPI == TEPI_STORE) {
-                    if (!f_ok) break;
-                    uint8_t* buf = next_buf();
-                    if (leader) bulk_wait_read<NBUF - 1>();
-                    __syncwarp();
-                    tmem_ld32(taddr + j, r);
-                    tmem_ld_wait32(r);
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-                    stage_col(buf, v);
-                    fence_proxy_async();
-                    __syncwarp();
-                    if (leader) {
-                        store_block(&P.o[0], buf, fcol, T.r0 + j, both);
-                        bulk_commit();
-                    }
-                } else if (EPI == TEPI_SWIGLU_FWD) {
-                    const uint32_t xch = smem_u32(xch_base) + (pr * 2 + (q & 1)) * 4096 + lane * 4;
-                    tmem_ld32(taddr + j, r);
-                    tmem_ld_wait32(r);
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-                    if (wq >= 2) {  // U lanes: hand the fp32 values to the G warp, store U
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) sts_f32(xch + i * 128, v[i]);
-                        asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
+            for (int half = 0; half < n_half; ++half) {
+                TileT H = T;
+                if (half) H.r0 = T.r0 + T.n, H.n = T.n1;
+                if (half + 1 < n_half) H.zend = T.r0 + T.n;
+                const long long c0 = P.prof ? clock64() : 0;
+                mbar_wait(&tfull_bar[as], aphase);
+                if (P.prof) w_tfull += clock64() - c0;
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + as * BN;
+                const int fcol = feat_col(H);
+                const bool f_ok = fcol < P.f_limit;
+    #pragma unroll 1
+                for (int j = 0; j < H.n; j += 32, ++q) {
+                    const bool both = j + 16 < H.n;
+                    uint32_t r[32];
+                    float v[32];
+                    if (EPI == TEPI_STORE) {
+                        if (!f_ok) break;
                         uint8_t* buf = next_buf();
                         if (leader) bulk_wait_read<NBUF - 1>();
                         __syncwarp();
+                        tmem_ld32(taddr + j, r);
+                        tmem_ld_wait32(r);
+    #pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
                         stage_col(buf, v);
                         fence_proxy_async();
                         __syncwarp();
-                        if (leader && f_ok) {
-                            store_block(&P.o[1], buf, fcol, T.r0 + j, both);
+                        if (leader) {
+                            store_block(&P.o[0], buf, fcol, H.r0 + j, both);
                             bulk_commit();
                         }
-                    } else {  // G lanes: store G, H = silu(G) * U
-                        uint8_t* bg = next_buf();
-                        uint8_t* bh = next_buf();
-                        if (leader) bulk_wait_read<1>();  // two blocks per commit group, ring of four
-                        __syncwarp();
-                        stage_col(bg, v);
-                        asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) v[i] = v[i] * sigmoidf_fast(v[i]) * lds_f32(xch + i * 128);
-                        stage_col(bh, v);
+                    } else if (EPI == TEPI_SWIGLU_FWD) {
+                        const uint32_t xch = smem_u32(xch_base) + (pr * 2 + (q & 1)) * 4096 + lane * 4;
+                        tmem_ld32(taddr + j, r);
+                        tmem_ld_wait32(r);
+    #pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+                        if (wq >= 2) {  // U lanes: hand the fp32 values to the G warp, store U
+    #pragma unroll
+                            for (int i = 0; i < 32; ++i) sts_f32(xch + i * 128, v[i]);
+                            asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
+                            uint8_t* buf = next_buf();
+                            if (leader) bulk_wait_read<NBUF - 1>();
+                            __syncwarp();
+                            stage_col(buf, v);
+                            fence_proxy_async();
+                            __syncwarp();
+                            if (leader && f_ok) {
+                                store_block(&P.o[1], buf, fcol, H.r0 + j, both);
+                                bulk_commit();
+                            }
+                        } else {  // G lanes: store G, H = silu(G) * U
+                            uint8_t* bg = next_buf();
+                            uint8_t* bh = next_buf();
+                            if (leader) bulk_wait_read<1>();  // two blocks per commit group, ring of four
+                            __syncwarp();
+                            stage_col(bg, v);
+                            asm volatile("bar.sync %0, 64;" ::"r"(1 + pr) : "memory");
+    #pragma unroll
+                            for (int i = 0; i < 32; ++i) v[i] = v[i] * sigmoidf_fast(v[i]) * lds_f32(xch + i * 128);
+                            stage_col(bh, v);
+                            fence_proxy_async();
+                            __syncwarp();
+                            if (leader && f_ok) {
+                                store_block(&P.o[0], bg, fcol, H.r0 + j, both);
+                                store_block(&P.o[2], bh, fcol, H.r0 + j, both);
+                                bulk_commit();
+                            }
+                        }
+                    } else {
+                        // accumulator = dH; dG = dH * U * silu'(G), dU = dH * silu(G), in place over the staged G, U
+                        const int set = q & 1;
+                        const uint32_t bg = smem_u32(stg + (2 * set) * TSTG_BYTES) + lane * 2, bu = bg + TSTG_BYTES;
+                        const long long c1 = P.prof ? clock64() : 0;
+                        mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
+                        if (P.prof) w_stg += clock64() - c1;
+                        if (j + 32 < H.n) {
+                            load_inputs(fcol, H.r0 + j + 32, set ^ 1);
+                        } else {
+                            const int tn = uni(feed.peek(it + 1));
+                            if (tn < n_total) {
+                                TileT Tn = tile_of(it + 1);
+                                Tn.f = uni(Tn.f), Tn.r0 = uni(Tn.r0);
+                                load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
+                            }
+                        }
+                        tmem_ld32(taddr + j, r);
+                        tmem_ld_wait32(r);
+                        // gathered dY rows are unscaled: dH[r] = gate_rows[r] * (dY[token(r)] Wd^T), the gate applied in fp32
+                        const float* rsc = P.row_scale ? P.row_scale + H.r0 + j : nullptr;
+    #pragma unroll
+                        for (int i = 0; i < 32; i += 2) {
+                            float dg[2], du[2];
+    #pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const float dh = __uint_as_float(r[i + e]) * ((rsc && i + e < H.n - j) ? __ldg(rsc + i + e) : 1.f);
+                                const float gv = lds_bf16(bg + (i + e) * 64), uv = lds_bf16(bu + (i + e) * 64);
+                                const float sg = sigmoidf_fast(gv);
+                                dg[e] = dh * uv * (sg * (1.f + gv * (1.f - sg)));
+                                du[e] = dh * (gv * sg);
+                            }
+                            const uint32_t pg = f2_to_bf2(dg[0], dg[1]), pu = f2_to_bf2(du[0], du[1]);
+                            sts_u16(bg + i * 64, pg & 0xffffu), sts_u16(bg + (i + 1) * 64, pg >> 16);
+                            sts_u16(bu + i * 64, pu & 0xffffu), sts_u16(bu + (i + 1) * 64, pu >> 16);
+                        }
                         fence_proxy_async();
                         __syncwarp();
                         if (leader && f_ok) {
-                            store_block(&P.o[0], bg, fcol, T.r0 + j, both);
-                            store_block(&P.o[2], bh, fcol, T.r0 + j, both);
+                            store_block(&P.o[0], stg + (2 * set) * TSTG_BYTES, fcol, H.r0 + j, both);
+                            store_block(&P.o[1], stg + (2 * set + 1) * TSTG_BYTES, fcol, H.r0 + j, both);
                             bulk_commit();
                         }
                     }
-                } else {
-                    // accumulator = dH; dG = dH * U * silu'(G), dU = dH * silu(G), in place over the staged G, U
-                    const int set = q & 1;
-                    const uint32_t bg = smem_u32(stg + (2 * set) * TSTG_BYTES) + lane * 2, bu = bg + TSTG_BYTES;
-                    const long long c1 = P.prof ? clock64() : 0;
-                    mbar_wait(&ld_bar[wq * 2 + set], (q >> 1) & 1);
-                    if (P.prof) w_stg += clock64() - c1;
-                    if (j + 32 < T.n) {
-                        load_inputs(fcol, T.r0 + j + 32, set ^ 1);
-                    } else {
-                        const int tn = uni(feed.peek(it + 1));
-                        if (tn < n_total) {
-                            TileT Tn = tile_of(it + 1);
-                            Tn.f = uni(Tn.f), Tn.r0 = uni(Tn.r0);
-                            load_inputs(feat_col(Tn), Tn.r0, set ^ 1);
-                        }
-                    }
-                    tmem_ld32(taddr + j, r);
-                    tmem_ld_wait32(r);
-                    // gathered dY rows are unscaled: dH[r] = gate_rows[r] * (dY[token(r)] Wd^T), the gate applied in fp32
-                    const float* rsc = P.row_scale ? P.row_scale + T.r0 + j : nullptr;
-#pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        float dg[2], du[2];
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            const float dh = __uint_as_float(r[i + e]) * ((rsc && i + e < T.n - j) ? __ldg(rsc + i + e) : 1.f);
-                            const float gv = lds_bf16(bg + (i + e) * 64), uv = lds_bf16(bu + (i + e) * 64);
-                            const float sg = sigmoidf_fast(gv);
-                            dg[e] = dh * uv * (sg * (1.f + gv * (1.f - sg)));
-                            du[e] = dh * (gv * sg);
-                        }
-                        const uint32_t pg = f2_to_bf2(dg[0], dg[1]), pu = f2_to_bf2(du[0], du[1]);
-                        sts_u16(bg + i * 64, pg & 0xffffu), sts_u16(bg + (i + 1) * 64, pg >> 16);
-                        sts_u16(bu + i * 64, pu & 0xffffu), sts_u16(bu + (i + 1) * 64, pu >> 16);
-                    }
-                    fence_proxy_async();
-                    __syncwarp();
-                    if (leader && f_ok) {
-                        store_block(&P.o[0], stg + (2 * set) * TSTG_BYTES, fcol, T.r0 + j, both);
-                        store_block(&P.o[1], stg + (2 * set + 1) * TSTG_BYTES, fcol, T.r0 + j, both);
-                        bulk_commit();
-                    }
                 }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (leader) mbar_arrive_cluster(leader_tempty + as * 8);
-            if (++as == 2) as = 0, aphase ^= 1;
-            // pad rows behind the group's last chunk: exact zeros (wgrad reads them as part of its K range)
-            if (leader && f_ok && T.r0 + T.n < T.zend) {
-                for (int row = T.r0 + T.n; row < T.zend; row += 16) {
-                    if (EPI == TEPI_STORE) {
-                        tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
-                    } else if (EPI == TEPI_SWIGLU_FWD) {
-                        if (wq >= 2) {
-                            tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
+                tc_fence_before();
+                __syncwarp();
+                if (leader) mbar_arrive_cluster(leader_tempty + as * 8);
+                if (++as == 2) as = 0, aphase ^= 1;
+                // pad rows behind the group's last chunk: exact zeros (wgrad reads them as part of its K range)
+                if (leader && f_ok && H.r0 + H.n < H.zend) {
+                    for (int row = H.r0 + H.n; row < H.zend; row += 16) {
+                        if (EPI == TEPI_STORE) {
+                            tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
+                        } else if (EPI == TEPI_SWIGLU_FWD) {
+                            if (wq >= 2) {
+                                tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
+                            } else {
+                                tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
+                                tma_store_3d(&P.o[2], zero_blk, fcol, row, 0);
+                            }
                         } else {
                             tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
-                            tma_store_3d(&P.o[2], zero_blk, fcol, row, 0);
+                            tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
                         }
-                    } else {
-                        tma_store_3d(&P.o[0], zero_blk, fcol, row, 0);
-                        tma_store_3d(&P.o[1], zero_blk, fcol, row, 0);
                     }
+                    bulk_commit();
                 }
-                bulk_commit();
+        
             }
         }
         if (leader) bulk_wait_all();
@@ -1987,10 +2041,10 @@ bool set_smem_attr1() {  // 1-CTA kernel only (the router's dense GEMMs)
                                 SMEM_BYTES) == cudaSuccess;
 }
 
-template <int A_MAJOR, int EPI, bool GATHER = false>
+template <int A_MAJOR, int EPI, bool GATHER = false, bool DUAL = false>
 int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, const char* name) {
     constexpr int threads = GATHER ? kThreads + 32 * (kGatherWarps - 1) : kThreads;
-    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, CfgT<EPI>::SMEM, threads);
+    long long clusters = resident_clusters(c, ln, tc_gemmT_kernel<A_MAJOR, EPI, GATHER, DUAL>, CfgT<EPI, DUAL>::SMEM, threads);
     if (tile_bound < clusters) clusters = tile_bound;
     if (clusters < 1) clusters = 1;
     TcParams Q = P;
@@ -1999,14 +2053,14 @@ int launch_t(piper_ctx* c, Lane ln, const TcParams& P, long long tile_bound, con
         c->tc_next_slot += 1;
     }
     Q.sched = sched_counters(c, ln.stream);
-    tc_gemmT_kernel<A_MAJOR, EPI, GATHER><<<(unsigned)(2 * clusters), threads, CfgT<EPI>::SMEM, ln.stream>>>(Q);
+    tc_gemmT_kernel<A_MAJOR, EPI, GATHER, DUAL><<<(unsigned)(2 * clusters), threads, CfgT<EPI, DUAL>::SMEM, ln.stream>>>(Q);
     PIPER_LAUNCHED(c, name);
     return PIPER_OK;
 }
-template <int A_MAJOR, int EPI, bool GATHER = false>
+template <int A_MAJOR, int EPI, bool GATHER = false, bool DUAL = false>
 bool set_smem_attr_t() {
-    return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                CfgT<EPI>::SMEM) == cudaSuccess;
+    return cudaFuncSetAttribute(tc_gemmT_kernel<A_MAJOR, EPI, GATHER, DUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                CfgT<EPI, DUAL>::SMEM) == cudaSuccess;
 }
 // gather fields of a launch whose rows operand comes from the token-major tensor `src` [T, cols]
 void set_gather(TcParams& P, const piper_ctx* c, const FfnProblem& p, const void* src, int cols) {
@@ -2023,6 +2077,8 @@ TcParams t_params(const piper_ctx* c, const FfnProblem& p, int F, int K, int f_t
     P.small_rows = c->tc_small_rows, P.greedy = c->tc_greedy;
     return P;
 }
+// two-chunk tiles (DUAL) for the plain-store rows-on-N kernels: when a group can hold more than one chunk
+bool dual_tiles(const piper_ctx* c, const FfnProblem& p) { return c->tc_dual && p.max_group_rows > 256; }
 inline long long t_tile_bound(const FfnProblem& p, int f_tiles) { return (long long)(cdiv(p.max_rows, 256) + p.G) * f_tiles; }
 
 // Pairing M tiles of one expert costs a duplicate tile per odd group: use the CTA-pair kernel when the groups are
@@ -2074,6 +2130,7 @@ int tc_init(piper_ctx* c) {
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
+    c->tc_dual = 0;  // measured slower (DESIGN.md finding 22)
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
@@ -2082,6 +2139,7 @@ int tc_init(piper_ctx* c) {
               set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD>() && set_smem_attr_t<K_MAJOR, TEPI_STORE>() &&
               cudaFuncSetAttribute(tc_gemm2_kernel<MN_MAJOR, MN_MAJOR, EPI_WGRAD_SPLIT, true>,
                                    cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<EPI_WGRAD_SPLIT>::SMEM) == cudaSuccess &&
+              set_smem_attr_t<MN_MAJOR, TEPI_STORE, false, true>() && set_smem_attr_t<K_MAJOR, TEPI_STORE, false, true>() &&
               set_smem_attr_t<MN_MAJOR, TEPI_SWIGLU_FWD, true>() && set_smem_attr_t<K_MAJOR, TEPI_SWIGLU_BWD, true>() &&
               set_smem_attr1<K_MAJOR, MN_MAJOR, EPI_STORE_F32>() && set_smem_attr1<MN_MAJOR, MN_MAJOR, EPI_STORE_F32>();
     if (!ok) {
@@ -2147,6 +2205,7 @@ int tc_ffn_fwd2(piper_ctx* c, Lane ln, const FfnProblem& p) {
         PIPER_MAP(&P.b[0], p.h, p.I, p.max_rows, 1, TB_BOX_ROWS);
         PIPER_MAP(&P.bs[0], p.h, p.I, p.max_rows, 1, TB_SMALL_ROWS);
         PIPER_MAP2(&P.o[0], p.o, p.d, p.max_rows, 1, 32, 16);
+        if (dual_tiles(c, p)) return launch_t<MN_MAJOR, TEPI_STORE, false, true>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd2_t2");
         return launch_t<MN_MAJOR, TEPI_STORE>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_fwd2_t");
     }
     const bool two = pair_ragged(c, p);
@@ -2205,6 +2264,7 @@ int tc_ffn_dgrad2(piper_ctx* c, Lane ln, const FfnProblem& p) {
         PIPER_MAP(&P.bs[1], p.du, p.I, p.max_rows, 1, TB_SMALL_ROWS);
         P.n_src = 2;
         PIPER_MAP2(&P.o[0], p.dxp, p.d, p.max_rows, 1, 32, 16);
+        if (dual_tiles(c, p)) return launch_t<K_MAJOR, TEPI_STORE, false, true>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad2_t2");
         return launch_t<K_MAJOR, TEPI_STORE>(c, ln, P, t_tile_bound(p, P.f_tiles), "tc_ffn_dgrad2_t");
     }
     const bool two = pair_ragged(c, p);

@@ -186,10 +186,19 @@ def test_more_local_experts_than_the_cta_pair_kernels_index():
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
-@pytest.mark.parametrize("family", ["rows_on_m", "one_cta"])
+@pytest.mark.parametrize("family", ["rows_on_m", "one_cta", "dual_tiles"])
 def test_fallback_kernel_families(name, family):
     """The rows-on-M CTA-pair kernels and the 1-CTA kernels (DESIGN.md section 5.1 b, c) stay correct: they serve
-    layers with more than 192 local experts.  piper_set_option selects them (host state of the context)."""
+    layers with more than 192 local experts; so do the two-chunk tiles of the plain-store rows-on-N kernels (a measured
+    variant).  piper_set_option selects them (host state of the context)."""
+    if family == "dual_tiles":
+        cfg = dataclasses.replace(configs.BY_NAME[name], row_align=16)
+        inp = configs.make_inputs(cfg)
+        f = oracle.forward(cfg, inp)
+        ctx, b = _run_steps(cfg, inp, use_chunk_calls=True, options=[(piper.OPT_T_DUAL, 1)])
+        _check_all(cfg, b, f, oracle.backward(cfg, inp, f))
+        ctx.close()
+        return
     opts = [(piper.OPT_TC_ROWS_ON_N, 0)] + ([(piper.OPT_TC_2CTA, 0)] if family == "one_cta" else [])
     cfg = dataclasses.replace(configs.BY_NAME[name], row_align=128)
     inp = configs.make_inputs(cfg)
