@@ -205,6 +205,47 @@ int piper_router_bwd(piper_ctx* ctx, const void* x, const void* w_r, const int32
 int piper_dispatch_unpack_router(piper_ctx* ctx, const void* dxp, const int32_t* row_of, const void* dx_shared,
                                  const void* dx_router, void* dx, void* stream);
 
+/* N4 expert parallelism over peer memory (`Shard` inserts an all-to-all before and after
+ * the expert Chunk).  n_ranks GPUs, T tokens each; rank r owns the experts [r * E / n_ranks, (r + 1) * E / n_ranks) = the
+ * context's [e_lo, e_lo + E_loc).  The pack / combine row movers address the owners' buffers directly through peer pointers
+ * (NVLink / NVSwitch peer memory) instead of filling a send buffer for an all-to-all-v.  Protocol per microbatch:
+ *   piper_route_topk on every rank; the ranks all-gather counts_global -> all_counts [n_ranks, E] (the caller's collective);
+ *   piper_ep_plan      every rank derives, without further communication, its own experts' counts [E_loc] (totals over the
+ *                      ranks) and offsets [E_loc + 1] (aligned exclusive scan) and send_base [E] = the row, in the owner's
+ *                      buffer, where its own rows of expert e start (rows of an expert are ordered by source rank, then token:
+ *                      by global token id rank * T + t, exactly the buffer piper_dispatch_pack builds over the concatenated
+ *                      tokens);
+ *   piper_ep_dispatch  stable ranks of this rank's assignments, then peer stores of the token rows, of the global assignment
+ *                      ids ((rank * T + t) * k + j) and of the gates into the owners' xp / src_of / gate_rows; dest_row [T,k]
+ *                      keeps the row of each assignment in its owner's buffer;
+ *   piper_ep_finish_recv (owner) zero pad rows of a received row buffer, src_of = -1 on pads and beyond offsets[E_loc];
+ *   the owner runs piper_expert_ffn_fwd / _bwd on what it received, through a context created with T * n_ranks tokens;
+ *   piper_ep_combine   y[t] = sum_j gates[t,j] * peer_o[owner(j)][dest_row[t,j]] (+ s[t]);
+ *   piper_ep_dispatch_bwd  peer_d_o[owner][row] = gates[t,j] * dy[t], dgates[t,j] = <dy[t], peer_o[owner][row]>;
+ *   piper_ep_unpack    dx[t] = sum_j peer_dxp[owner(j)][dest_row[t,j]] (+ dx_shared[t]).
+ * peer_* are DEVICE arrays of n_ranks device pointers (entry r = rank r's buffer, mapped into this GPU's address space: CUDA
+ * IPC, cudaDeviceEnablePeerAccess or symmetric memory; with n_ranks = 1, or all ranks on one GPU, plain pointers).  Row buffers
+ * of an owner hold piper_ep_a_cap() rows.  No kernel waits on another rank's kernel: the steps are ordered by the caller's
+ * streams and collectives (a barrier between dispatch and the owners' FFN, and before combine).  Needs E % n_ranks == 0 and
+ * e_lo = rank * E_loc; one dispatch of a context at a time. */
+int64_t piper_ep_a_cap(const piper_moe_desc* desc, int n_ranks);
+int piper_ep_plan(piper_ctx* ctx, const int32_t* all_counts, int rank, int n_ranks, int32_t* counts, int32_t* offsets,
+                  int32_t* send_base, void* stream);
+/* The same plan on the host, from HOST arrays (no GPU): for callers that size messages on the host, and for CPU tests. */
+int piper_ep_plan_host(const int32_t* all_counts, int32_t E, int32_t n_ranks, int32_t rank, int32_t row_align, int32_t* counts,
+                       int32_t* offsets, int32_t* send_base);
+int piper_ep_dispatch(piper_ctx* ctx, const void* x, const int32_t* topk_idx, const float* gates, const int32_t* send_base,
+                      int rank, int n_ranks, void* const* peer_xp, int32_t* const* peer_src_of, float* const* peer_gate_rows,
+                      int32_t* dest_row, void* stream);
+int piper_ep_finish_recv(piper_ctx* ctx, const int32_t* counts, const int32_t* offsets, int n_ranks, int32_t* src_of,
+                         float* gate_rows, void* rows, void* stream);
+int piper_ep_combine(piper_ctx* ctx, void* const* peer_o, const int32_t* topk_idx, const int32_t* dest_row, const float* gates,
+                     const void* s, void* y, void* stream);
+int piper_ep_dispatch_bwd(piper_ctx* ctx, const void* dy, const int32_t* topk_idx, const int32_t* dest_row, const float* gates,
+                          void* const* peer_o, void* const* peer_d_o, float* dgates, void* stream);
+int piper_ep_unpack(piper_ctx* ctx, void* const* peer_dxp, const int32_t* topk_idx, const int32_t* dest_row,
+                    const void* dx_shared, void* dx, void* stream);
+
 /* Every pointer of one microbatch (inputs, outputs and the scratch between forward and backward). */
 typedef struct {
     const float* logits;                         /* [T,E]: input; an OUTPUT of the forward chunk when w_r != NULL */

@@ -57,6 +57,7 @@ def lib() -> ctypes.CDLL:
             raise PiperError(f"CUDA library missing: {path}")
         L = ctypes.CDLL(path)
         L.piper_a_cap.restype = ctypes.c_int64
+        L.piper_ep_a_cap.restype = ctypes.c_int64
         L.piper_kernel_launches.restype = ctypes.c_int64
         L.piper_last_cuda_error.restype = ctypes.c_char_p
         L.piper_debug_tc_counters.restype = ctypes.c_void_p
@@ -211,6 +212,62 @@ def piper_router_bwd(ctx, x, w_r, topk_idx, dz_sel, dz_scratch, dw_r, dx_router,
 def piper_dispatch_unpack_router(ctx, dxp, row_of, dx_shared, dx_router, dx, stream=None):
     ctx.check(lib().piper_dispatch_unpack_router(ctx._h, _ptr(dxp), _ptr(row_of), _ptr(dx_shared), _ptr(dx_router),
                                                  _ptr(dx), _stream(stream)), "piper_dispatch_unpack_router")
+
+
+# ---- N4: expert parallelism over peer memory (include/piper.h) ------------------------------------------------------
+def ptr_table(tensors, device=None):
+    """Device array of the tensors' data pointers (the peer_* arguments)."""
+    dev = tensors[0].device if device is None else device
+    return torch.tensor([t.data_ptr() for t in tensors], dtype=torch.int64, device=dev)
+
+
+def piper_ep_a_cap(desc: MoeDesc, n_ranks: int) -> int:
+    return int(lib().piper_ep_a_cap(ctypes.byref(desc), int(n_ranks)))
+
+
+def piper_ep_plan_host(all_counts, rank: int, row_align: int = 1):
+    """Host-only: all_counts [n_ranks, E] int32 numpy -> (counts [E_loc], offsets [E_loc + 1], send_base [E])."""
+    import numpy as np
+    ac = np.ascontiguousarray(all_counts, np.int32)
+    R, E = ac.shape
+    counts, offsets, send_base = np.empty(E // R, np.int32), np.empty(E // R + 1, np.int32), np.empty(E, np.int32)
+    rc = lib().piper_ep_plan_host(_vp(ac.ctypes.data), _i32(E), _i32(R), _i32(rank), _i32(row_align), _vp(counts.ctypes.data),
+                                  _vp(offsets.ctypes.data), _vp(send_base.ctypes.data))
+    if rc != PIPER_OK:
+        raise PiperError(f"piper_ep_plan_host: status {rc}")
+    return counts, offsets, send_base
+
+
+def piper_ep_plan(ctx, all_counts, rank, n_ranks, counts, offsets, send_base, stream=None):
+    ctx.check(lib().piper_ep_plan(ctx._h, _ptr(all_counts), int(rank), int(n_ranks), _ptr(counts), _ptr(offsets),
+                                  _ptr(send_base), _stream(stream)), "piper_ep_plan")
+
+
+def piper_ep_dispatch(ctx, x, topk_idx, gates, send_base, rank, n_ranks, peer_xp, peer_src_of, peer_gate_rows, dest_row,
+                      stream=None):
+    ctx.check(lib().piper_ep_dispatch(ctx._h, _ptr(x), _ptr(topk_idx), _ptr(gates), _ptr(send_base), int(rank), int(n_ranks),
+                                      _ptr(peer_xp), _ptr(peer_src_of), _ptr(peer_gate_rows), _ptr(dest_row), _stream(stream)),
+              "piper_ep_dispatch")
+
+
+def piper_ep_finish_recv(ctx, counts, offsets, n_ranks, src_of, gate_rows, rows, stream=None):
+    ctx.check(lib().piper_ep_finish_recv(ctx._h, _ptr(counts), _ptr(offsets), int(n_ranks), _ptr(src_of), _ptr(gate_rows),
+                                         _ptr(rows), _stream(stream)), "piper_ep_finish_recv")
+
+
+def piper_ep_combine(ctx, peer_o, topk_idx, dest_row, gates, s, y, stream=None):
+    ctx.check(lib().piper_ep_combine(ctx._h, _ptr(peer_o), _ptr(topk_idx), _ptr(dest_row), _ptr(gates), _ptr(s), _ptr(y),
+                                     _stream(stream)), "piper_ep_combine")
+
+
+def piper_ep_dispatch_bwd(ctx, dy, topk_idx, dest_row, gates, peer_o, peer_d_o, dgates, stream=None):
+    ctx.check(lib().piper_ep_dispatch_bwd(ctx._h, _ptr(dy), _ptr(topk_idx), _ptr(dest_row), _ptr(gates), _ptr(peer_o),
+                                          _ptr(peer_d_o), _ptr(dgates), _stream(stream)), "piper_ep_dispatch_bwd")
+
+
+def piper_ep_unpack(ctx, peer_dxp, topk_idx, dest_row, dx_shared, dx, stream=None):
+    ctx.check(lib().piper_ep_unpack(ctx._h, _ptr(peer_dxp), _ptr(topk_idx), _ptr(dest_row), _ptr(dx_shared), _ptr(dx),
+                                    _stream(stream)), "piper_ep_unpack")
 
 
 def piper_route_bwd(ctx, logits, topk_idx, gates, dgates, dz_sel, stream=None):

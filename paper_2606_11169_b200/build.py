@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpiper.so")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "chunk.cu", "ffn.cu", "gemm_simt.cu", "gemm_tc.cu", "permute.cu", "route.cu", "router.cu", "sched.cpp"]
+SOURCES = ["api.cu", "chunk.cu", "ep.cu", "ffn.cu", "gemm_simt.cu", "gemm_tc.cu", "permute.cu", "route.cu", "router.cu", "sched.cpp"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = os.environ.get("PIPER_EXTRA_NVCC", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-Wno-deprecated-gpu-targets", "-std=c++17", "-Xcompiler", "-fPIC",
          "-I", INC, "-I", CSRC]

@@ -25,13 +25,14 @@ inline int n_chunks_of(const piper_moe_desc* D) { return cdiv(D->T * D->k, kScan
 inline size_t round256(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t chunk_counts, chunk_counts_per, shared_offsets, tc_scratch, total;
+    size_t chunk_counts, chunk_counts_per, ep_scratch, shared_offsets, tc_scratch, total;
 };
 WsLayout ws_layout(const piper_moe_desc* D) {
     WsLayout L{};
     const size_t per = round256(sizeof(int32_t) * (size_t)n_chunks_of(D) * D->E_loc);
     size_t at = 0;
     L.chunk_counts = at, L.chunk_counts_per = per, at += per * kSchedSlots;
+    L.ep_scratch = at, at += round256(sizeof(int32_t) * (size_t)n_chunks_of(D) * D->E);
     L.shared_offsets = at, at += 256;
     L.tc_scratch = at, at += tc_scratch_bytes(D);
     L.total = at;
@@ -121,6 +122,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
     c->n_chunks = n_chunks_of(D);
     c->chunk_counts = reinterpret_cast<int32_t*>(c->ws + L.chunk_counts);
     c->chunk_counts_stride = L.chunk_counts_per / sizeof(int32_t);
+    c->ep_scratch = reinterpret_cast<int32_t*>(c->ws + L.ep_scratch);
     c->shared_offsets = reinterpret_cast<int32_t*>(c->ws + L.shared_offsets);
     c->tc_scratch = c->ws + L.tc_scratch;
     bool ok = cudaSetDevice(device) == cudaSuccess &&

@@ -66,6 +66,7 @@ struct piper_ctx {
     int n_chunks;            // ceil(T*k / kScanChunk)
     int32_t* chunk_counts;   // [kSchedSlots][n_chunks][E_loc]  per-chunk local-expert histograms, one set per stream slot
     size_t chunk_counts_stride;  // int32 elements between two slots' histograms
+    int32_t* ep_scratch;     // [n_chunks][E] chunk histograms over all experts (N4 dispatch)
     int32_t* shared_offsets; // [2] = {0, T}: the shared expert as one group
     int64_t launches;
     int pair_mode;
