@@ -180,6 +180,7 @@ int piper_get_option(const piper_ctx* c, int option, int* value) {
         case PIPER_OPT_TC_PROFILE: *value = c->tc_prof; return PIPER_OK;
         case PIPER_OPT_FUSED_GATHER: *value = c->fused_gather; return PIPER_OK;
         case PIPER_OPT_T_DUAL: *value = c->tc_dual; return PIPER_OK;
+        case PIPER_OPT_WGRAD_STORE_WARP: *value = c->tc_store_warp; return PIPER_OK;
     }
     return PIPER_ERR_INVALID;
 }
@@ -196,6 +197,7 @@ int piper_set_option(piper_ctx* c, int option, int value) {
         case PIPER_OPT_TC_PROFILE: field = &c->tc_prof; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_T_DUAL: field = &c->tc_dual; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_WGRAD_STORE_WARP: field = &c->tc_store_warp; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
     }
     *field = value;
     const int rc = variant_ok(c);  // e.g. row_align 16 needs the rows-on-N + CTA-pair kernels, fp32 dW the CTA-pair wgrad

@@ -48,6 +48,7 @@ struct alignas(64) TcParams {
     CUtensorMap a[2], b[2];
     CUtensorMap bs[2];         // rows-on-N kernel: the activation operand again with 32-row boxes (short chunks)
     CUtensorMap o[3], ein[2];  // CTA-pair kernel: outputs / epilogue inputs as 64-column x 32-row store / load boxes
+    CUtensorMap ow[2];         // CTA-pair wgrad with the store warp: the dW outputs as 64-column x 128-row boxes
     const int32_t* offsets;  // [G+1] device
     int G;
     int ragged_m;    // 1: tiles run over the packed rows (fwd / dgrad); 0: over groups (wgrad)
@@ -63,6 +64,7 @@ struct alignas(64) TcParams {
     long long group_stride;  // wgrad: elements between two experts' dW
     __nv_bfloat16 *out0, *out1, *out2;
     const __nv_bfloat16 *in0, *in1;
+    int store_warp;   // CTA-pair wgrad, bf16 dW: one 128-row bulk store per chunk from warp 2 (long K ranges), see Cfg2::STORE_WARP
     long long* prof;  // debug (PIPER_OPT_TC_PROFILE): [gridDim.x][8] wait-cycle counters, else NULL
     // rows-on-N kernel (tc_gemmT_kernel)
     const int32_t* counts;  // [G] device: real rows per group
@@ -608,7 +610,11 @@ struct Cfg2 {
     static constexpr int NBUF = EPI == EPI_SWIGLU_BWD ? 4 : (BKc == 128 ? (EPI_WARPS == 8 ? 1 : 2) : 3);
     static constexpr int A_B = BM * BKc * 2, B_B = (BN / 2) * BKc * 2, STAGE_B = A_B + B_B, MNB = 64 * BKc * 2;
     static constexpr int RING_BYTES = NST * STAGE_B, STG_TOTAL = EPI_WARPS * NBUF * STG_BYTES;
-    static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + 256 + 2 * (kMaxGroups2 + 1) * 4;
+    // wgrad (bf16 output, no gathered operand): warp 2, idle after the TMEM allocation, issues the bulk
+    // stores of the blocks the epilogue warps stage, so that the drain of an accumulator does not wait for the store issue
+    static constexpr bool STORE_WARP = WG && EPI_WARPS == 4;  // NBUF = 2
+    static constexpr int BAR_BYTES = 320;  // barriers (256) + the store warp's "staging buffer free" barriers (8 x 8)
+    static constexpr int SMEM = RING_BYTES + STG_TOTAL + 1024 + BAR_BYTES + 2 * (kMaxGroups2 + 1) * 4;
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 constexpr int PANEL_PAIRS = 8;
@@ -782,12 +788,17 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     int* feed_ids = reinterpret_cast<int*>(feed_empty + kFeed);
     uint64_t* gfull_bar = reinterpret_cast<uint64_t*>(feed_ids + 2);  // [STAGES2] GATHER_A: peer CTA's local "A rows landed"
     static_assert(!GATHER_A || (2 * STAGES2 + 4 + 9 + 2 * kFeed + 1 + STAGES2) * 8 <= 256, "barrier area");
-    int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + 256);
+    uint64_t* sfull_bar = ld_bar;  // store warp: [2] block staged by the four epilogue warps (the SwiGLU input barriers are unused then)
+    uint64_t* sempty_bar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(full_bar) + 256);  // [2] block read by its store
+    int* tp = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(full_bar) + Cfg2<EPI>::BAR_BYTES);
     int* tpp = tp + (kMaxGroups2 + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = (int)cluster_ctarank();
     const int pair_id = blockIdx.x >> 1, n_pairs_grid = gridDim.x >> 1;
+    // the store warp serves bf16 outputs of long K ranges (the host decides); fp32 dW blocks and short tiles keep one
+    // 32-row store per epilogue warp
+    bool store_warp = Cfg2<EPI>::STORE_WARP && !GATHER_A && P.store_warp != 0;
     const int32_t* __restrict__ offsets = P.offsets;
 
     if (!P.ragged_m) {  // wgrad: offsets and real row counts of the groups (read by decode_pair / the MMA issuer)
@@ -816,6 +827,19 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
             if (lane == 0) tpp[P.G] = carry;
         }
     }
+    // wgrad: draw tiles from the counter only when the experts' K ranges are long and uneven (C4: one expert holds 16% of
+    // the rows, so a static stride leaves some clusters two of its tiles); equal or short tiles keep the static stride
+    // (the draw costs an atomic and a cluster-scope release per tile: -2% on C2, -7% on C3's 2-3 K-block tiles).
+    bool dynamic = true;  // computed by every warp (same data, same answer): static tiles bypass the feed altogether
+    if (!P.ragged_m) {
+        int mx = 0;
+        for (int g = lane; g < P.G; g += 32) mx = max(mx, offsets[g + 1] - offsets[g]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        const int total = offsets[P.G];
+        dynamic = total >= 512 * P.G && (long long)mx * P.G > 2ll * total;
+        if (P.store_warp == 2 && (dynamic || total < 512 * P.G)) store_warp = false;  // by the real group lengths
+    }
     if (warp == 0 && lane == 0) {
         prefetch_tmap(&P.a[0]), prefetch_tmap(&P.b[0]);
         if (P.n_src == 2) prefetch_tmap(&P.a[1]);
@@ -827,9 +851,9 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
             if (GATHER_A) mbar_init(&gfull_bar[s], 32 * kGatherWarpsA);
         }
         for (int s = 0; s < 2; ++s) mbar_init(&tfull_bar[s], 1), mbar_init(&tempty_bar[s], 2 * Cfg2<EPI>::EPI_WARPS);  // both CTAs
-        for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], 1);
-        for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer (+ gather warps, forwarder)
-            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1 + (GATHER_A ? 2 * kGatherWarpsA + 1 : 0));
+        for (int s = 0; s < 8; ++s) mbar_init(&ld_bar[s], store_warp && s < 2 ? 4 : 1), mbar_init(&sempty_bar[s], 1);
+        for (int s = 0; s < kFeed; ++s)  // consumers: (producer + epilogue warps) x 2 CTAs + the MMA issuer (+ gather warps, forwarder / store warps)
+            mbar_init(&feed_full[s], 1), mbar_init(&feed_empty[s], 2 * (1 + Cfg2<EPI>::EPI_WARPS) + 1 + (GATHER_A ? 2 * kGatherWarpsA + 1 : 0) + (store_warp ? 2 : 0));
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc2(tmem_ptr, 512);
@@ -845,18 +869,6 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
     TileFeed feed;
     feed.ids = feed_ids, feed.full = feed_full, feed.empty_addr = mapa_u32(smem_u32(feed_empty), 0);
 
-    // wgrad: draw tiles from the counter only when the experts' K ranges are long and uneven (C4: one expert holds 16% of
-    // the rows, so a static stride leaves some clusters two of its tiles); equal or short tiles keep the static stride
-    // (the draw costs an atomic and a cluster-scope release per tile: -2% on C2, -7% on C3's 2-3 K-block tiles).
-    bool dynamic = true;  // computed by every warp (same data, same answer): static tiles bypass the feed altogether
-    if (!P.ragged_m) {
-        int mx = 0;
-        for (int g = lane; g < P.G; g += 32) mx = max(mx, offsets[g + 1] - offsets[g]);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        const int total = offsets[P.G];
-        dynamic = total >= 512 * P.G && (long long)mx * P.G > 2ll * total;
-    }
     if (dynamic && warp == 3 && rank == 0 && lane == 0) {
         // ===== tile feeder (one thread of the leader CTA), see TileFeed =====
         const uint32_t peer_ids = mapa_u32(smem_u32(feed_ids), 1), peer_full = mapa_u32(smem_u32(feed_full), 1);
@@ -1045,6 +1057,43 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
             long long* pq = P.prof + blockIdx.x * 8;
             pq[0] = w_full, pq[1] = w_tempty, pq[2] = clock64() - t_begin, pq[6] = n_tiles_done;
         }
+    } else if (Cfg2<EPI>::STORE_WARP && !GATHER_A && warp == 2) {
+        // ===== store warp (both CTAs, wgrad with bf16 output): one bulk store of 128 rows x 64 columns per chunk instead
+        // of one per epilogue warp (a bulk tensor store costs its issuing warp ~130 cycles whatever its size: 16 of them per
+        // tile were 12 % of the epilogue warps' time on the short K ranges of C3).  The four epilogue warps stage their 32
+        // rows side by side in block n & 1; this warp stores the block and hands it back once the copy has read it.
+        if (store_warp) {
+            const int urank = uni(rank);
+            const bool leader = elect_one();  // one lane issues every store: the bulk groups are per thread
+            uint32_t n = 0;                   // chunks so far: block n & 1, barrier phase (n >> 1) & 1
+            for (int it = 0;; ++it) {
+                const int t = uni(dynamic ? feed.take(it, lane) : pair_id + it * n_pairs_grid);
+                if (t >= n_total) break;
+                Tile2 T = decode_pair(P, tp, tpp, offsets, t, urank, BKc, rcp_group, rcp_pairs);
+                T.g = uni(T.g), T.m0 = uni(T.m0), T.n0 = uni(T.n0), T.store = uni((int)T.store) != 0;
+                const int z = P.ragged_m ? 0 : T.g;
+#pragma unroll 1
+                for (int c = 0; c < 4; ++c) {
+                    const bool split = EPI == EPI_WGRAD_SPLIT;
+                    const CUtensorMap* om = split ? &P.ow[c >> 1] : &P.ow[0];
+                    const int col = split ? T.n0 + 64 * (c & 1) : T.n0 + 64 * c;
+                    if (col >= P.n_limit) continue;
+                    const int b = n & 1, ph = (n >> 1) & 1;
+                    ++n;
+                    mbar_wait(&sfull_bar[b], ph);
+                    if (leader) {
+                        if (T.store) {
+                            tma_store_3d(om, stg_base + b * (4 * STG_BYTES), col, T.m0, z);
+                            bulk_commit();
+                            bulk_wait_read<0>();
+                        }
+                        mbar_arrive(&sempty_bar[b]);
+                    }
+                    __syncwarp();
+                }
+            }
+            if (leader) bulk_wait_all();
+        }
     } else if (warp >= 4) {
         // ===== epilogue (both CTAs): this CTA's 128 rows of the 256-row accumulator =====
         // (warp-uniform values are made provably so, and one elected lane issues the bulk tensor copies: see elect_one)
@@ -1205,11 +1254,17 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
                         }
                         continue;
                     }
-                    uint8_t* buf = stg + ring * STG_BYTES;
+                    // store warp: the four warps' blocks of chunk q lie side by side in block q & 1 (one 128-row store)
+                    uint8_t* buf = store_warp ? stg_base + (ring * 4 + (uwarp - 4)) * STG_BYTES : stg + ring * STG_BYTES;
+                    const int sb = ring;
                     if (++ring == NBUF) ring = 0;
                     const long long c1 = P.prof ? clock64() : 0;
-                    if (leader) bulk_wait_read<NBUF - 1>();
-                    __syncwarp();
+                    if (store_warp) {
+                        mbar_wait(&sempty_bar[sb], ((q >> 1) & 1) ^ 1);
+                    } else {
+                        if (leader) bulk_wait_read<NBUF - 1>();
+                        __syncwarp();
+                    }
                     if (P.prof) w_stg += clock64() - c1;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -1223,7 +1278,10 @@ tc_gemm2_kernel(const __grid_constant__ TcParams P) {
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (leader && T.store) {
+                    if (store_warp) {
+                        if (leader) mbar_arrive(&sfull_bar[sb]);
+                        ++q;
+                    } else if (leader && T.store) {
                         tma_store_3d(om, buf, col, row0, z);
                         bulk_commit();
                     }
@@ -2131,6 +2189,7 @@ int tc_init(piper_ctx* c) {
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
     c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
     c->tc_dual = 0;  // measured slower (DESIGN.md finding 22)
+    c->tc_store_warp = 2;
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();
     bool ok = set_smem_attr<K_MAJOR, MN_MAJOR, EPI_SWIGLU_FWD>() && set_smem_attr<K_MAJOR, MN_MAJOR, EPI_STORE>() &&
               set_smem_attr<K_MAJOR, K_MAJOR, EPI_SWIGLU_BWD>() && set_smem_attr<K_MAJOR, K_MAJOR, EPI_STORE>() &&
@@ -2284,6 +2343,12 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
     const bool two = pair_wgrad(c, p);
     const bool f32 = c->D.dw_dtype == PIPER_DTYPE_F32;  // fp32 dW from bf16 operands: the CTA-pair kernel only
     if ((f32 || p.accumulate) && !(two && f32)) return PIPER_ERR_UNSUPPORTED;
+    // One 128-row store per chunk from the store warp when the K ranges are long and even (>= 512 rows per expert expected
+    // under uniform routing, and the kernel finds no expert with more than twice the mean: C2 wgrad 2.31 -> 2.21 ms).  On
+    // short ranges the epilogue warps are the critical path and the hand-over costs more than the store issue it saves
+    // (C3, 252 rows per expert: 0.83 -> 0.96 ms; C4, skewed: 1.46 -> 1.55 ms), so they keep their own 32-row stores.
+    const bool sw = two && !f32 && Cfg2<EPI_WGRAD>::STORE_WARP &&
+                    (c->tc_store_warp == 2 ? (long long)p.exp_rows >= 512ll * p.G : c->tc_store_warp == 1);
     {
         TcParams P = base_params(p, false);
         P.counts = p.counts;
@@ -2300,8 +2365,13 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
             if (rc != PIPER_OK) return rc;
             P.out_f32 = 1, P.accum = p.accumulate;
         } else if (two) {
+            P.store_warp = (sw && !p.gather_x) ? c->tc_store_warp : 0;
             PIPER_MAP(&P.o[0], p.dw_gate, p.I, p.d, p.G, 32);
             PIPER_MAP(&P.o[1], p.dw_up, p.I, p.d, p.G, 32);
+            if (P.store_warp) {
+                PIPER_MAP(&P.ow[0], p.dw_gate, p.I, p.d, p.G, 128);
+                PIPER_MAP(&P.ow[1], p.dw_up, p.I, p.d, p.G, 128);
+            }
         }
         const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
         int rc;
@@ -2328,7 +2398,9 @@ int tc_ffn_wgrad(piper_ctx* c, Lane ln, const FfnProblem& p) {
         if (rc != PIPER_OK) return rc;
         P.out_f32 = 1, P.accum = p.accumulate;
     } else if (two) {
+        P.store_warp = sw ? c->tc_store_warp : 0;
         PIPER_MAP(&P.o[0], p.dw_down, p.d, p.I, p.G, 32);
+        if (sw) PIPER_MAP(&P.ow[0], p.dw_down, p.d, p.I, p.G, 128);
     }
     const long long mt = two ? (P.m_tiles + 1) / 2 : P.m_tiles;
     return launch<MN_MAJOR, MN_MAJOR, EPI_WGRAD>(c, ln, P, (long long)p.G * mt * P.n_tiles, two, "tc_ffn_wgrad_down");

@@ -87,6 +87,7 @@ struct piper_ctx {
     int tc_rows_on_n;        // rows-on-N kernels for fwd / dgrad (PIPER_OPT_TC_ROWS_ON_N, default on)
     int tc_small_rows, tc_greedy;  // PIPER_OPT_T_SMALL_ROWS / PIPER_OPT_T_GREEDY: row chunking of the rows-on-N kernels
     int tc_dual;             // PIPER_OPT_T_DUAL: two-chunk tiles in the plain-store rows-on-N kernels
+    int tc_store_warp;       // PIPER_OPT_WGRAD_STORE_WARP: 0 / 1 / 2 = by expected group length
     int tc_prof;             // PIPER_OPT_TC_PROFILE: the tcgen05 kernels record wait-cycle counters in tc_scratch
     int fused_gather;        // PIPER_OPT_FUSED_GATHER: chunk calls let the GEMMs gather x / dY rows (N2)
     int pair_bwd_pass;       // piper_set_pair_bwd_pass

@@ -186,16 +186,19 @@ def test_more_local_experts_than_the_cta_pair_kernels_index():
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
-@pytest.mark.parametrize("family", ["rows_on_m", "one_cta", "dual_tiles"])
+@pytest.mark.parametrize("family", ["rows_on_m", "one_cta", "dual_tiles", "wgrad_store_warp", "wgrad_warp_stores"])
 def test_fallback_kernel_families(name, family):
     """The rows-on-M CTA-pair kernels and the 1-CTA kernels (DESIGN.md section 5.1 b, c) stay correct: they serve
     layers with more than 192 local experts; so do the two-chunk tiles of the plain-store rows-on-N kernels (a measured
     variant).  piper_set_option selects them (host state of the context)."""
-    if family == "dual_tiles":
+    if family in ("dual_tiles", "wgrad_store_warp", "wgrad_warp_stores"):
+        # wgrad: both ways of storing dW (the default picks one by the expected group length)
+        opt = {"dual_tiles": (piper.OPT_T_DUAL, 1), "wgrad_store_warp": (piper.OPT_WGRAD_STORE_WARP, 1),
+               "wgrad_warp_stores": (piper.OPT_WGRAD_STORE_WARP, 0)}[family]
         cfg = dataclasses.replace(configs.BY_NAME[name], row_align=16)
         inp = configs.make_inputs(cfg)
         f = oracle.forward(cfg, inp)
-        ctx, b = _run_steps(cfg, inp, use_chunk_calls=True, options=[(piper.OPT_T_DUAL, 1)])
+        ctx, b = _run_steps(cfg, inp, use_chunk_calls=True, options=[opt])
         _check_all(cfg, b, f, oracle.backward(cfg, inp, f))
         ctx.close()
         return
