@@ -337,8 +337,31 @@ int piper_set_pair_bwd_pass(piper_ctx* ctx, int pass);
 #define PIPER_PART_EXCLUSIVE 0
 #define PIPER_PART_SHARED 1
 int piper_set_pair_policy(piper_ctx* ctx, int order, int partition, const float* task_ms);
-/* The pick sequence (PIPER_TASK_* ids, n <= 14 written to order[14]) the current policy yields for a split. */
+/* The pick sequence (PIPER_TASK_* ids, caller tasks included; n <= 18 written to order[18]) the current policy yields
+ * for a split. */
 int piper_pair_order(piper_ctx* ctx, int sm_gemm, int sm_comm, int32_t* order, int32_t* n);
+
+/* N3 (Fig. 3b, Listing 1, "Chunk.exec"): the rest of the overlapped
+ * block - attention forward before the MoE chunk of microbatch A, attention backward after the MoE chunk of microbatch
+ * B - as CALLER TASKS of the pair.  A caller task is an opaque function that enqueues its work on the stream it is given
+ * (it must not synchronise; sm_count is its side's SM budget, for kernels that bound their own grids); the pair puts it into
+ * the task DAG of piper_run_chunk_pair and schedules it with the library's tasks (list order or profile order, the
+ * event rule of PAPER.md:279-286):
+ *   PIPER_SLOT_F_PRE   produces x / logits of the forward microbatch:  before F.route, F.pack, F.shared
+ *   PIPER_SLOT_F_POST  consumes y:                                     after F.combine
+ *   PIPER_SLOT_B_PRE   produces dY of the backward microbatch:         before B.cgrad, B.shared
+ *   PIPER_SLOT_B_POST  consumes dX / dz_sel (and the router's dW_r):   after B.unpack, B.route_bwd
+ * side: 0 = the pack/combine ("communication-side") stream, 1 = the GEMM stream.  est_ms: duration on the whole device
+ * for PIPER_ORDER_PROFILE.  fn = NULL clears the slot.  piper_run_chunk_fwd / _bwd do not run caller tasks (the caller
+ * simply enqueues them around those calls).  A non-zero return of fn aborts the pair call with PIPER_ERR_INVALID.
+ * Host state of `ctx`; `user` must stay valid while the slot is set. */
+typedef int (*piper_caller_task_fn)(void* user, void* cuda_stream, int sm_count);
+#define PIPER_SLOT_F_PRE 0
+#define PIPER_SLOT_F_POST 1
+#define PIPER_SLOT_B_PRE 2
+#define PIPER_SLOT_B_POST 3
+#define PIPER_TASK_CALLER_F_PRE 14 /* ids of the caller tasks in piper_pair_order: 14 + slot */
+int piper_pair_set_caller_task(piper_ctx* ctx, int slot, piper_caller_task_fn fn, void* user, float est_ms, int side);
 /* One task of the pair DAG (SURVEY.md §8c c-sched numbering) on `stream` with all SMs: the unit that
  * piper_run_chunk_fwd / _bwd / _pair enqueue, exposed so that each step can be timed on its own
  * (bench.py's roofline block).  F_* tasks read `a` as the forward microbatch, B_* as the backward one. */
@@ -382,7 +405,7 @@ int piper_pair_partition_mode(const piper_ctx* ctx);
  * event).  Returns PIPER_ERR_INVALID on a cycle or a bad edge. */
 int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const int32_t* prio,
                         int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records);
-/* Profile-guided counterpart (PIPER_ORDER_PROFILE): exhaustive search of the static two-stream schedule (n <= 16,
+/* Profile-guided counterpart (PIPER_ORDER_PROFILE): exhaustive search of the static two-stream schedule (n <= 18,
  * stream_of in {0,1}) with the smallest makespan under durations dur[n], simulated with the event rule of
  * PAPER.md:279-286; ties go to the lexicographically smallest pick sequence.  Outputs as piper_list_schedule plus
  * *makespan (nullable), in the unit of dur. */

@@ -354,12 +354,43 @@ def piper_set_pair_policy(ctx, order: int, partition: int, task_ms=None):
     ctx.check(lib().piper_set_pair_policy(ctx._h, int(order), int(partition), arr), "piper_set_pair_policy")
 
 
+CALLER_SLOTS = ("F_PRE", "F_POST", "B_PRE", "B_POST")
+SLOT_F_PRE, SLOT_F_POST, SLOT_B_PRE, SLOT_B_POST = range(4)
+CALLER_TASK_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int)
+
+
 def piper_pair_order(ctx, sm_gemm: int, sm_comm: int):
-    """Task names in the pick sequence the current policy yields for this split."""
-    order = (ctypes.c_int32 * 14)()
+    """Task names in the pick sequence the current policy yields for this split (caller tasks: "X_F_PRE" ...)."""
+    order = (ctypes.c_int32 * 18)()
     n = _i32(0)
     ctx.check(lib().piper_pair_order(ctx._h, int(sm_gemm), int(sm_comm), order, ctypes.byref(n)), "piper_pair_order")
-    return [TASKS[order[i]] for i in range(n.value)]
+    names = TASKS + tuple("X_" + s for s in CALLER_SLOTS)
+    return [names[order[i]] for i in range(n.value)]
+
+
+def piper_pair_set_caller_task(ctx, slot: int, fn, est_ms: float = 0.0, side: int = 1):
+    """N3: `fn(stream_ptr: int, sm_count: int)` becomes a task of piper_run_chunk_pair (include/piper.h); it must only
+    enqueue work on that stream.  fn = None clears the slot.  The ctypes thunk is kept alive on the context."""
+    keep = ctx.__dict__.setdefault("_caller_thunks", {})
+    if fn is None:
+        ctx.check(lib().piper_pair_set_caller_task(ctx._h, int(slot), CALLER_TASK_FN(0), None, ctypes.c_float(0.0), int(side)),
+                  "piper_pair_set_caller_task")
+        keep.pop(slot, None)
+        return
+
+    def thunk(_user, stream, sms):
+        try:
+            fn(int(stream or 0), int(sms))
+            return 0
+        except Exception:  # an exception must not cross the C boundary: the pair call reports the failure
+            import traceback
+            traceback.print_exc()
+            return 1
+
+    cfn = CALLER_TASK_FN(thunk)
+    ctx.check(lib().piper_pair_set_caller_task(ctx._h, int(slot), cfn, None, ctypes.c_float(float(est_ms)), int(side)),
+              "piper_pair_set_caller_task")
+    keep[slot] = cfn
 
 
 def piper_schedule_search(n, edges, stream_of, dur):

@@ -124,7 +124,9 @@ GreenPartition* make_partition(piper_ctx* c, int sm_gemm, int sm_comm, bool want
 // ---- the tasks ------------------------------------------------------------------------------------
 enum Task {
     F_ROUTE, F_SCAN, F_PACK, F_GEMM1, F_GEMM2, F_SHARED, F_COMBINE,
-    B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD, N_TASKS
+    B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_UNPACK, B_ROUTE_BWD, N_TASKS,
+    // N3: caller tasks of the pair (piper_pair_set_caller_task), id = N_TASKS + slot
+    X_F_PRE = N_TASKS, X_F_POST, X_B_PRE, X_B_POST, N_ALL
 };
 constexpr int COMM = 0, GEMM = 1;
 const int kStreamOf[N_TASKS] = {COMM, COMM, COMM, GEMM, GEMM, GEMM, COMM, COMM, GEMM, GEMM, GEMM, GEMM, COMM, COMM};
@@ -132,6 +134,10 @@ const int kEdges[][2] = {{F_ROUTE, F_SCAN},   {F_SCAN, F_PACK},    {F_PACK, F_GE
                          {F_GEMM2, F_COMBINE}, {F_SCAN, F_GEMM1},   {F_SCAN, F_COMBINE},   {F_SHARED, F_COMBINE},
                          {B_CGRAD, B_DGRAD1},  {B_DGRAD1, B_DGRAD2}, {B_DGRAD2, B_UNPACK},  {B_CGRAD, B_WGRAD},
                          {B_DGRAD1, B_WGRAD},  {B_SHARED, B_UNPACK}, {B_CGRAD, B_ROUTE_BWD}};
+// caller tasks: x / logits of the forward microbatch come from F_PRE, y goes to F_POST; dY of the backward microbatch
+// comes from B_PRE, dX / dz_sel go to B_POST (include/piper.h, piper_pair_set_caller_task)
+const int kCallerEdges[][2] = {{X_F_PRE, F_ROUTE},  {X_F_PRE, F_PACK},  {X_F_PRE, F_SHARED},    {F_COMBINE, X_F_POST},
+                               {X_B_PRE, B_CGRAD},  {X_B_PRE, B_SHARED}, {B_UNPACK, X_B_POST}, {B_ROUTE_BWD, X_B_POST}};
 
 // `parts` of the backward tasks that hold both passes (B_SHARED): bit 0 = input gradients (Bi), bit 1 = weight gradients (Bw)
 constexpr int PART_BI = 1, PART_BW = 2, PART_ALL = 3;
@@ -157,6 +163,15 @@ FfnProblem routed_bwd_problem(const piper_ctx* c, const piper_chunk_args* b) {
 // in_chunk: called from a whole-chunk entry point (fused layers skip F_PACK there), not from piper_run_task
 int run_task(piper_ctx* c, int task, Lane ln, const piper_chunk_args* f, const piper_chunk_args* b, int parts = PART_ALL,
              bool in_chunk = true) {
+    if (task >= X_F_PRE && task < N_ALL) {  // the caller's function enqueues its own work on the lane's stream
+        const int slot = task - X_F_PRE;
+        if (!c->caller_fn[slot]) return PIPER_ERR_INVALID;
+        if (c->caller_fn[slot](c->caller_user[slot], ln.stream, ln.sms) != 0) {
+            snprintf(c->err, sizeof(c->err), "caller task of slot %d failed", slot);
+            return PIPER_ERR_INVALID;
+        }
+        return PIPER_OK;
+    }
     switch (task) {
         case F_ROUTE: {
             if (f->w_r) {  // N1: the router GEMM writes the logits F1 reads
@@ -235,7 +250,7 @@ bool bwd_args_ok(const piper_ctx* c, const piper_chunk_args* a) {
 struct PairPlan {
     bool router;  // the DAG has the N1 edge B.route_bwd -> B.unpack
     int32_t n, n_waits;
-    int32_t task_of[N_TASKS], stream_of[N_TASKS], order[N_TASKS], waits[32][2], records[N_TASKS];
+    int32_t task_of[N_ALL], stream_of[N_ALL], order[N_ALL], waits[32][2], records[N_ALL];
 };
 
 void pair_plan_release(piper_ctx* c) {
@@ -402,28 +417,36 @@ int make_plan_uncached(piper_ctx* c, int sm_gemm, int sm_comm, bool router, Pair
     pl->router = router;
     // task list of this layer (no shared expert -> its two tasks and their edges drop out)
     const bool shared = c->D.I_shared != 0;
-    int32_t id_of[N_TASKS], n = 0;
-    for (int t = 0; t < N_TASKS; ++t) {
+    int32_t id_of[N_ALL], n = 0;
+    for (int t = 0; t < N_ALL; ++t) {
         id_of[t] = -1;
         if (!shared && (t == F_SHARED || t == B_SHARED)) continue;
         if (t == B_WGRAD && c->pair_bwd_pass == PIPER_PASS_BI) continue;  // F || Bi: the weight gradients run later
+        if (t >= X_F_PRE && !c->caller_fn[t - X_F_PRE]) continue;          // N3: caller tasks that are set
         id_of[t] = n, pl->task_of[n] = t, ++n;
     }
     pl->n = n;
-    int32_t edges[32][2], n_edges = 0, prio[N_TASKS];
+    int32_t edges[32][2], n_edges = 0, prio[N_ALL];
     for (const auto& e : kEdges)
+        if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
+    for (const auto& e : kCallerEdges)
         if (id_of[e[0]] >= 0 && id_of[e[1]] >= 0) edges[n_edges][0] = id_of[e[0]], edges[n_edges][1] = id_of[e[1]], ++n_edges;
     if (router)  // N1: B.route_bwd also produces the router's term of dX, which B.unpack adds
         edges[n_edges][0] = id_of[B_ROUTE_BWD], edges[n_edges][1] = id_of[B_UNPACK], ++n_edges;
-    for (int i = 0; i < n; ++i) pl->stream_of[i] = kStreamOf[pl->task_of[i]], prio[i] = pl->task_of[i] >= B_CGRAD ? 1 : 0;
+    for (int i = 0; i < n; ++i) {
+        const int t = pl->task_of[i];
+        pl->stream_of[i] = t >= X_F_PRE ? c->caller_side[t - X_F_PRE] : kStreamOf[t];
+        prio[i] = (t >= B_CGRAD && t < N_TASKS) || t == X_B_PRE || t == X_B_POST ? 1 : 0;
+    }
     pl->n_waits = 0;
     if (c->pair_order == PIPER_ORDER_LIST)
         return piper_list_schedule(n, n_edges, &edges[0][0], pl->stream_of, prio, pl->order, &pl->waits[0][0], &pl->n_waits,
                                    pl->records);
     // durations on the partitions: GEMM tasks scale with the SM count; the row movers saturate HBM with about a
     // third of the SMs, below that they scale with the SM count
-    float full[N_TASKS], dur[N_TASKS];
+    float full[N_ALL], dur[N_ALL];
     task_durations(c, full);
+    for (int sl = 0; sl < 4; ++sl) full[X_F_PRE + sl] = c->caller_ms[sl];
     const float fg = (float)c->num_sms / (float)(sm_gemm < c->num_sms ? sm_gemm : c->num_sms);
     const float fc = sm_comm * 3 >= c->num_sms ? 1.f : (float)c->num_sms / (3.f * (float)sm_comm);
     for (int i = 0; i < n; ++i) dur[i] = full[pl->task_of[i]] * (pl->stream_of[i] == GEMM ? fg : fc);
@@ -471,6 +494,14 @@ int piper_set_pair_policy(piper_ctx* c, int order, int partition, const float* t
     return PIPER_OK;
 }
 
+int piper_pair_set_caller_task(piper_ctx* c, int slot, piper_caller_task_fn fn, void* user, float est_ms, int side) {
+    if (!c || slot < 0 || slot > 3 || (side != COMM && side != GEMM) || !(est_ms >= 0.f)) return PIPER_ERR_INVALID;
+    c->caller_fn[slot] = fn, c->caller_user[slot] = fn ? user : nullptr;
+    c->caller_ms[slot] = fn ? est_ms : 0.f, c->caller_side[slot] = side;
+    pair_plan_release(c);  // the DAG changes
+    return PIPER_OK;
+}
+
 int piper_pair_order(piper_ctx* c, int sm_gemm, int sm_comm, int32_t* order, int32_t* n) {
     if (!c || !order || !n || !split_ok(c, sm_gemm, sm_comm)) return PIPER_ERR_INVALID;
     PairPlan pl;
@@ -509,14 +540,19 @@ int piper_run_chunk_pair(piper_ctx* c, const piper_chunk_args* f, const piper_ch
         PIPER_CUDA(c, cudaEventRecord(fork, user));
         PIPER_CUDA(c, cudaStreamWaitEvent(lf.stream, fork, 0));
         PIPER_CUDA(c, cudaStreamWaitEvent(lb.stream, fork, 0));
-        const int fseq[] = {F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE};
-        const int bseq[] = {B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_ROUTE_BWD, B_UNPACK};
-        for (int i = 0; i < 7; ++i) {  // enqueued alternately, each chunk in its serial order
-            if (fseq[i] != F_SHARED || c->D.I_shared) {
+        const int fseq[] = {X_F_PRE, F_ROUTE, F_SCAN, F_PACK, F_SHARED, F_GEMM1, F_GEMM2, F_COMBINE, X_F_POST};
+        const int bseq[] = {X_B_PRE, B_CGRAD, B_DGRAD1, B_DGRAD2, B_WGRAD, B_SHARED, B_ROUTE_BWD, B_UNPACK, X_B_POST};
+        auto in_plan = [&](int t) {
+            if (t >= X_F_PRE) return c->caller_fn[t - X_F_PRE] != nullptr;
+            if ((t == F_SHARED || t == B_SHARED) && !c->D.I_shared) return false;
+            return !(t == B_WGRAD && parts == PART_BI);
+        };
+        for (int i = 0; i < 9; ++i) {  // enqueued alternately, each chunk in its serial order
+            if (in_plan(fseq[i])) {
                 rc = run_task(c, fseq[i], lf, f, b);
                 if (rc != PIPER_OK) return rc;
             }
-            if ((bseq[i] != B_SHARED || c->D.I_shared) && !(bseq[i] == B_WGRAD && parts == PART_BI)) {
+            if (in_plan(bseq[i])) {
                 rc = run_task(c, bseq[i], lb, f, b, parts);
                 if (rc != PIPER_OK) return rc;
             }

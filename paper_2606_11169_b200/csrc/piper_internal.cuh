@@ -18,7 +18,7 @@ namespace piper {
 constexpr int kMaxK = 8;          // top-k bound (register arrays in route / combine kernels)
 constexpr int kMaxE = 512;        // expert bound of the router kernel (16 values per lane)
 constexpr int kScanChunk = 1024;  // assignments per block of the histogram / rank kernels
-constexpr int kMaxEvents = 20;    // one per pair task + fork/join
+constexpr int kMaxEvents = 24;    // one per pair task (14 + 4 caller tasks) + fork/join
 
 // Where a task's kernels run: stream + the number of SMs its persistent grids may occupy.
 struct Lane {
@@ -78,6 +78,10 @@ struct piper_ctx {
     void* pair_plan;             // cached schedule of the pair for (plan_sm_gemm, plan_sm_comm)
     int plan_sm_gemm, plan_sm_comm;
     float pair_task_ms[14];      // caller's task durations on the whole device (PIPER_ORDER_PROFILE)
+    piper_caller_task_fn caller_fn[4];  // N3: caller tasks of the pair (piper_pair_set_caller_task), by slot
+    void* caller_user[4];
+    float caller_ms[4];
+    int caller_side[4];
     char err[256];
     void* encode_tiled;      // cuTensorMapEncodeTiled, resolved at create time
     piper::GreenPartition* green;

@@ -77,65 +77,61 @@ extern "C" int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* ed
 
 // ---- profile-guided variant ---------------------------------------------------------------------------
 // PAPER.md:273 and 420 name profile-guided scheduling as the way past the simple policy above.  With a
-// duration per task the static two-stream schedule can be searched exhaustively for a DAG of this size:
-// every pair of per-stream sequences (linear extensions of the DAG restricted to a stream) is simulated
-// under the event rule (a task starts when its stream is free and all its producers have finished) and
-// the pair with the smallest makespan wins; ties go to the lexicographically smallest pick sequence, so
-// the result is a pure function of the inputs.
+// duration per task the static two-stream schedule of a DAG of this size can be searched exactly.  A schedule is a
+// pair of per-stream sequences, run under the event rule (a task starts when its stream is free and all its
+// producers have finished); the search appends tasks in the order of their start times (every schedule has exactly
+// one such order, up to ties), depth first with the task ids ascending, and cuts a branch whose lower bound - the
+// remaining work of either stream, or the earliest start of a ready task plus the longest chain behind it - cannot
+// beat the best schedule found so far.  The first schedule with the smallest makespan in that order wins, i.e. ties
+// go to the lexicographically smallest pick sequence: the result is a pure function of the inputs.
 namespace {
 
 struct Search {
-    int n;
+    int n = 0;
     std::vector<std::vector<int32_t>> preds;
-    const int32_t* stream_of;
-    const float* dur;
-    std::vector<std::vector<int32_t>> seqs[2];
+    const int32_t* stream_of = nullptr;
+    const float* dur = nullptr;
+    std::vector<double> tail;  // dur[v] + the longest chain of successors behind v (streams ignored)
+    std::vector<double> fin;
+    std::vector<char> used;
+    std::vector<int32_t> cur, best_order;
+    double free_at[2] = {0, 0}, rem[2] = {0, 0}, best = -1.0;
 
-    void extensions(int s, std::vector<int32_t>& cur, std::vector<char>& used) {
-        bool any = false;
-        for (int32_t v = 0; v < n; ++v) {
-            if (stream_of[v] != s || used[v]) continue;
-            bool ok = true;
-            for (int32_t p : preds[v]) ok = ok && (stream_of[p] != s || used[p]);
-            if (!ok) continue;
-            any = true;
-            used[v] = 1, cur.push_back(v);
-            extensions(s, cur, used);
-            cur.pop_back(), used[v] = 0;
-        }
-        if (!any) {
-            size_t want = 0;
-            for (int32_t v = 0; v < n; ++v) want += stream_of[v] == s;
-            if (cur.size() == want) seqs[s].push_back(cur);
-        }
+    double start_of(int32_t v) const {
+        double start = free_at[stream_of[v]];
+        for (int32_t p : preds[v])
+            if (fin[p] > start) start = fin[p];
+        return start;
     }
-    // simulate; returns makespan or a negative value on deadlock; `order` = tasks by start time
-    double simulate(const std::vector<int32_t>& a, const std::vector<int32_t>& b, std::vector<int32_t>& order) const {
-        const std::vector<int32_t>* q[2] = {&a, &b};
-        size_t head[2] = {0, 0};
-        double free_at[2] = {0, 0};
-        std::vector<double> fin(n, -1.0);
-        order.clear();
-        while (head[0] < a.size() || head[1] < b.size()) {
-            int pick = -1;
-            double best = 0;
-            for (int s = 0; s < 2; ++s) {
-                if (head[s] >= q[s]->size()) continue;
-                const int32_t v = (*q[s])[head[s]];
-                double start = free_at[s];
-                bool ready = true;
-                for (int32_t p : preds[v]) {
-                    if (fin[p] < 0) ready = false;
-                    else if (fin[p] > start) start = fin[p];
-                }
-                if (ready && (pick < 0 || start < best)) pick = s, best = start;
-            }
-            if (pick < 0) return -1.0;
-            const int32_t v = (*q[pick])[head[pick]++];
-            fin[v] = best + dur[v], free_at[pick] = fin[v];
-            order.push_back(v);
+    bool ready(int32_t v) const {
+        if (used[v]) return false;
+        for (int32_t p : preds[v])
+            if (!used[p]) return false;
+        return true;
+    }
+    void dfs(double last_start) {
+        if ((int)cur.size() == n) {
+            const double m = free_at[0] > free_at[1] ? free_at[0] : free_at[1];
+            if (best < 0 || m < best - 1e-9) best = m, best_order = cur;
+            return;
         }
-        return free_at[0] > free_at[1] ? free_at[0] : free_at[1];
+        double lb = free_at[0] + rem[0] > free_at[1] + rem[1] ? free_at[0] + rem[0] : free_at[1] + rem[1];
+        for (int32_t v = 0; v < n; ++v)
+            if (ready(v)) {
+                const double e = start_of(v) + tail[v];
+                if (e > lb) lb = e;
+            }
+        if (best >= 0 && lb >= best - 1e-9) return;
+        for (int32_t v = 0; v < n; ++v) {
+            if (!ready(v)) continue;
+            const double start = start_of(v);
+            if (start < last_start - 1e-12) continue;  // not the start-time order of this schedule: found on another branch
+            const int s = stream_of[v];
+            const double keep_free = free_at[s];
+            used[v] = 1, fin[v] = start + dur[v], free_at[s] = fin[v], rem[s] -= dur[v], cur.push_back(v);
+            dfs(start);
+            cur.pop_back(), rem[s] += dur[v], free_at[s] = keep_free, fin[v] = -1.0, used[v] = 0;
+        }
     }
 };
 
@@ -144,32 +140,46 @@ struct Search {
 extern "C" int piper_schedule_search(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of,
                                      const float* dur, int32_t* order, int32_t* waits, int32_t* n_waits,
                                      int32_t* records, float* makespan) {
-    if (n < 0 || n > 16 || n_edges < 0 || (n_edges > 0 && !edges) || (n > 0 && (!stream_of || !dur || !order || !records)) ||
+    if (n < 0 || n > 18 || n_edges < 0 || (n_edges > 0 && !edges) || (n > 0 && (!stream_of || !dur || !order || !records)) ||
         !n_waits)
         return PIPER_ERR_INVALID;
     Search S;
     S.n = n, S.stream_of = stream_of, S.dur = dur;
     S.preds.assign(n, {});
+    std::vector<std::vector<int32_t>> succs(n);
     for (int32_t i = 0; i < n_edges; ++i) {
         const int32_t s = edges[2 * i], t = edges[2 * i + 1];
         if (s < 0 || s >= n || t < 0 || t >= n || s == t) return PIPER_ERR_INVALID;
-        S.preds[t].push_back(s);
+        S.preds[t].push_back(s), succs[s].push_back(t);
     }
     for (int32_t v = 0; v < n; ++v)
         if ((stream_of[v] != 0 && stream_of[v] != 1) || !(dur[v] >= 0.f)) return PIPER_ERR_INVALID;
-    for (int s = 0; s < 2; ++s) {
-        std::vector<int32_t> cur;
-        std::vector<char> used(n, 0);
-        S.extensions(s, cur, used);
-    }
-    double best = -1.0;
-    std::vector<int32_t> best_order, cand;
-    for (const auto& a : S.seqs[0])
-        for (const auto& b : S.seqs[1]) {
-            const double m = S.simulate(a, b, cand);
-            if (m < 0) continue;
-            if (best < 0 || m < best - 1e-9 || (m < best + 1e-9 && cand < best_order)) best = m, best_order = cand;
+    // longest chain behind every task, in reverse topological order (Kahn on the successor counts); a cycle leaves tasks out
+    S.tail.assign(n, 0.0);
+    {
+        std::vector<int32_t> left(n), stack;
+        for (int32_t v = 0; v < n; ++v) {
+            left[v] = (int32_t)succs[v].size();
+            if (!left[v]) stack.push_back(v);
         }
+        int32_t done = 0;
+        while (!stack.empty()) {
+            const int32_t v = stack.back();
+            stack.pop_back(), ++done;
+            double longest = 0;
+            for (int32_t t : succs[v])
+                if (S.tail[t] > longest) longest = S.tail[t];
+            S.tail[v] = dur[v] + longest;
+            for (int32_t p : S.preds[v])
+                if (--left[p] == 0) stack.push_back(p);
+        }
+        if (done != n) return PIPER_ERR_INVALID;  // cycle
+    }
+    S.fin.assign(n, -1.0), S.used.assign(n, 0);
+    for (int32_t v = 0; v < n; ++v) S.rem[stream_of[v]] += dur[v];
+    S.dfs(0.0);
+    const double best = S.best;
+    const std::vector<int32_t>& best_order = S.best_order;
     if (best < 0) return PIPER_ERR_INVALID;  // cycle
     for (int32_t i = 0; i < n; ++i) order[i] = best_order[i];
     int32_t nw = 0;

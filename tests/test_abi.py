@@ -155,3 +155,30 @@ def test_schedule_search_on_the_pair_dag_beats_the_list_order():
     assert again[0].tolist() == order.tolist()  # deterministic
     with pytest.raises(piper.PiperError):
         piper.piper_schedule_search(3, [[0, 1], [1, 2], [2, 0]], [0, 1, 0], [1, 1, 1])
+
+
+def test_schedule_search_with_the_four_caller_tasks_of_the_overlapped_block():
+    """N3 (Fig. 3b): the pair DAG with attention forward / backward as caller tasks on the GEMM stream and the
+    two residual slots on the pack/combine stream (piper_pair_set_caller_task): 18 tasks must still be searched in a time
+    a first call can afford, every edge respected, and the makespan no worse than the list order's."""
+    import time
+    g = json.load(open(os.path.join(ROOT, "tests", "golden", "pair_dag.json")))
+    n0, edges, stream_of = len(g["nodes"]), [list(e) for e in g["edges"]], list(g["stream_of"])
+    idx = {name: i for i, name in enumerate(g["nodes"])}
+    pre_f, post_f, pre_b, post_b = n0, n0 + 1, n0 + 2, n0 + 3
+    edges += [[pre_f, idx["F.route"]], [pre_f, idx["F.pack"]], [pre_f, idx["F.shared"]], [idx["F.combine"], post_f],
+              [pre_b, idx["B.cgrad"]], [pre_b, idx["B.shared_bwd"]], [idx["B.unpack"], post_b], [idx["B.route_bwd"], post_b]]
+    stream_of += [1, 0, 0, 1]
+    dur = np.array([.03, .03, .15, .58, .32, .56, .3, .3, .37, .58, 1.0, 1.2, .3, .02, .9, .05, .05, 1.8], np.float32)
+    t0 = time.time()
+    order, waits, records, mk = piper.piper_schedule_search(n0 + 4, edges, stream_of, dur)
+    assert time.time() - t0 < 1.0  # branch and bound: about a millisecond (the product of all per-stream sequences took seconds)
+    pos = {v: i for i, v in enumerate(order.tolist())}
+    wait_set = set(map(tuple, waits.tolist()))
+    for s, t in edges:
+        assert pos[s] < pos[t]
+        assert (stream_of[s] == stream_of[t]) != ((s, t) in wait_set)
+    prio = list(g["prio"]) + [0, 0, 1, 1]
+    lo, _, _ = piper.piper_list_schedule(n0 + 4, edges, stream_of, prio)
+    seq_list = [[v for v in lo.tolist() if stream_of[v] == s] for s in (0, 1)]
+    assert mk <= _simulate(n0 + 4, edges, stream_of, dur.tolist(), seq_list) + 1e-6
