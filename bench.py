@@ -500,6 +500,67 @@ def run_piper(args, cfg, sampler, rank, world, local, barrier, e2e=True, min_sec
     return line, w
 
 
+def time_torch_eager(w: Workload, steps=5, warmup=2):
+    """Context, not the product: the same fwd+bwd chunk written with stock PyTorch ops (top-k, gather, a loop of torch.mm
+    over the experts, index_add, autograd), which is what the paper's Chunks execute ("stock PyTorch
+    ops"), on the same device, inputs and dtype.  No kernel or entry point of this library is on that path."""
+    import torch
+    import torch.nn.functional as F
+    from inputs import configs
+    cfg, b = w.rcfg, w.b
+    T, k, lo, El = cfg.T, cfg.k, cfg.e_lo, cfg.e_loc
+    names = ["w_gate", "w_up", "w_down"] + (["ws_gate", "ws_up", "ws_down"] if cfg.I_shared else [])
+    params = {n: b[n].detach().clone().requires_grad_(True) for n in names}
+    x = b["x"].detach().clone().requires_grad_(True)
+    logits = b["logits"].detach().clone().requires_grad_(True)
+    dy = b["dy"]
+
+    def step():
+        for t in [x, logits] + list(params.values()):
+            t.grad = None
+        topv, topi = logits.topk(k, dim=1)
+        if cfg.gate_mode == configs.GATE_SOFTMAX_RENORM:
+            gates = torch.softmax(topv, dim=1)
+        elif cfg.gate_mode == configs.GATE_SIGMOID_RENORM:
+            sg = torch.sigmoid(topv)
+            gates = sg / sg.sum(dim=1, keepdim=True)
+        else:
+            gates = torch.softmax(logits, dim=1).gather(1, topi)
+        flat_e, flat_g = topi.reshape(-1), gates.reshape(-1)
+        flat_t = torch.arange(T, device=x.device).repeat_interleave(k)
+        local = (flat_e >= lo) & (flat_e < lo + El)
+        e_l, t_l, g_l = flat_e[local] - lo, flat_t[local], flat_g[local]
+        order = torch.argsort(e_l, stable=True)
+        tok, gate = t_l[order], g_l[order]
+        counts = torch.bincount(e_l, minlength=El).tolist()  # the host needs the split sizes: a sync, as in eager MoE code
+        xp = x[tok]
+        outs, start = [], 0
+        for e, n in enumerate(counts):
+            seg = xp[start:start + n]
+            h = F.silu(seg @ params["w_gate"][e]) * (seg @ params["w_up"][e])
+            outs.append(h @ params["w_down"][e])
+            start += n
+        o = torch.cat(outs) * gate.to(x.dtype)[:, None]
+        y = torch.zeros_like(x).index_add_(0, tok, o)
+        if cfg.I_shared:
+            y = y + (F.silu(x @ params["ws_gate"][0]) * (x @ params["ws_up"][0])) @ params["ws_down"][0]
+        y.backward(dy)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    return {"value": T / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps,
+            "what": "the same chunk (route, permute, expert FFNs, combine, backward through autograd) in stock PyTorch eager ops "
+                    "on this GPU: cuBLAS GEMMs per expert in a Python loop, bf16, fp32 routing; context only (PAPER.md:137, 326)"}
+
+
 def gemm_hbm_bytes(cfg, A: int):
     """Bytes the GEMM tasks must move at least once (weights read once per GEMM, dW written once, row buffers read /
     written once per use): {task: bytes}."""
@@ -700,6 +761,12 @@ def main():
     contract_splits = [(132, 16), (124, 24), (116, 32), (100, 48)]
     if args.pair and world == 1:
         line["pair"] = run_pair(piper, w.ctx, w.rcfg, w.b, w.inp, contract_splits, iters, sampler)
+    if rank == 0 and world == 1 and not args.no_extra and cfg.dtype == configs.DT_BF16:
+        try:
+            line["torch_eager"] = time_torch_eager(w)
+        except RuntimeError as e:  # e.g. out of memory beside the library's buffers: the context line is optional
+            line["torch_eager"] = {"unavailable": str(e).splitlines()[0][:200]}
+        torch.cuda.empty_cache()
     w.close()
     if default_run and world == 1 and not args.no_extra:
         # the north star's whole report in one line: the other single-GPU workloads of BASELINE.json, each with its own
