@@ -581,7 +581,52 @@ def gemm_hbm_bytes(cfg, A: int):
     return out
 
 
-def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None):
+def overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm):
+    """N3 (Fig. 3b): the whole overlapped block - attention forward of microbatch A in front of its MoE
+    chunk, attention backward of microbatch B behind its MoE chunk - with the attention as CALLER tasks of the pair
+    (piper_pair_set_caller_task).  The attention here is torch's fused SDPA (library code, causal, heads of 128, sequences
+    of up to 4096 tokens; its output is not wired into x: a timing stand-in for the caller's own kernels)."""
+    import torch
+    H, S = max(1, cfg.d // 128), min(cfg.T, 4096)
+    B = max(1, cfg.T // S)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    q, k, v, dout = (torch.randn(B, H, S, 128, device=dev, dtype=torch.bfloat16) for _ in range(4))
+    ops = torch.ops.aten
+    fwd = ops._scaled_dot_product_flash_attention(q, k, v, 0.0, True, False)
+    o, lse, cq, ck, mq, mk, seed, off = fwd[:8]
+
+    def attn_fwd(stream_ptr=None, sms=0):
+        with torch.cuda.stream(torch.cuda.ExternalStream(stream_ptr) if stream_ptr else torch.cuda.current_stream()):
+            ops._scaled_dot_product_flash_attention(q, k, v, 0.0, True, False)
+
+    def attn_bwd(stream_ptr=None, sms=0):
+        with torch.cuda.stream(torch.cuda.ExternalStream(stream_ptr) if stream_ptr else torch.cuda.current_stream()):
+            ops._scaled_dot_product_flash_attention_backward(dout, q, k, v, o, lse, cq, ck, mq, mk, 0.0, True, seed, off)
+
+    t_af, t_ab = timed(attn_fwd), timed(attn_bwd)
+    t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
+    t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
+    serial = timed(lambda: (attn_fwd(), piper.piper_run_chunk_fwd(ctx, args_a), piper.piper_run_chunk_bwd(ctx, args_b), attn_bwd()))
+    res = {"attention": f"torch SDPA (flash), causal, batch {B} x {H} heads x {S} tokens x 128, bf16", "attn_fwd_ms": t_af,
+           "attn_bwd_ms": t_ab, "chunk_fwd_ms": t_f, "chunk_bwd_ms": t_b, "serial_ms": serial, "variants": {}}
+    piper.piper_pair_set_caller_task(ctx, piper.SLOT_F_PRE, attn_fwd, est_ms=t_af, side=1)
+    piper.piper_pair_set_caller_task(ctx, piper.SLOT_B_POST, attn_bwd, est_ms=t_ab, side=1)
+    for name, order, part, splits in (("list_order_exclusive", piper.ORDER_LIST, piper.PART_EXCLUSIVE, [(132, 16), (116, 32)]),
+                                      ("profile_order_shared_sms", piper.ORDER_PROFILE, piper.PART_SHARED, [(n_sm, 32)]),
+                                      ("chunk_streams", piper.ORDER_LIST, piper.PART_CHUNK_STREAMS, [(n_sm, 16)])):
+        piper.piper_set_pair_policy(ctx, order, part, task_ms)
+        for sg, sc in splits:
+            piper.piper_pair_prepare(ctx, sg, sc)
+            t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
+            res["variants"][f"{name} {sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / serial,
+                                                    "order": piper.piper_pair_order(ctx, sg, sc)}
+    piper.piper_pair_set_caller_task(ctx, piper.SLOT_F_PRE, None)
+    piper.piper_pair_set_caller_task(ctx, piper.SLOT_B_POST, None)
+    piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
+    return res
+
+
+def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=False):
     """Step P on this context's layer shape: forward chunk of microbatch A (the bench inputs) co-scheduled
     with the backward chunk of microbatch B (seed + 1, own weights: reading c-20) versus the same two
     chunks back to back on one stream with all SMs."""
@@ -658,6 +703,8 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None):
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_CHUNK_STREAMS, task_ms)
     out["variants"]["chunk_streams_gpu_allocates_sms"] = sweep([(n_sm, 16)])
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
+    if attn:
+        out["overlapped_block"] = overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm)
     best = min(((v["ratio_vs_serial"], name, k) for name, d in
                 [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))
     out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2],
@@ -715,6 +762,9 @@ def main():
                          "stream beside the shared expert's GEMMs / the routed wgrad (default: one stream; measured "
                          "neutral, C2 6.67 -> 6.82 ms, C3 4.22 -> 4.23 ms: the GEMM beside them slows by what they hide)")
     ap.add_argument("--pair", action="store_true", help="also time step P (chunk pair vs serial) on this shape")
+    ap.add_argument("--attn", action="store_true",
+                    help="with --pair: also time the whole overlapped block (N3), attention forward / backward (torch SDPA) as "
+                         "caller tasks of the pair")
     ap.add_argument("--main-grad", action="store_true",
                     help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")
     args = ap.parse_args()
@@ -760,7 +810,7 @@ def main():
     iters = max(3, min(args.steps, 10))
     contract_splits = [(132, 16), (124, 24), (116, 32), (100, 48)]
     if args.pair and world == 1:
-        line["pair"] = run_pair(piper, w.ctx, w.rcfg, w.b, w.inp, contract_splits, iters, sampler)
+        line["pair"] = run_pair(piper, w.ctx, w.rcfg, w.b, w.inp, contract_splits, iters, sampler, attn=args.attn)
     if rank == 0 and world == 1 and not args.no_extra and cfg.dtype == configs.DT_BF16:
         try:
             line["torch_eager"] = time_torch_eager(w)
