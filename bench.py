@@ -394,6 +394,7 @@ def time_tasks(w: Workload, n_prof):
     peaks = measured_peaks()
     work = task_work(rcfg, A, t_touched)
     stored = stored_ncu()
+    gemm_bytes = gemm_hbm_bytes(rcfg, A)
     kernels = {}
     for t in order:
         bound, amount = work[t]
@@ -404,6 +405,10 @@ def time_tasks(w: Workload, n_prof):
             ach, peak, unit = amount / sec / 1e9, peaks["hbm"], "GB/s"
         kernels[t] = {"ms": round(task_ms[t], 4), "bound": bound, "achieved": round(ach, 2), "unit": unit,
                       "frac": round(ach / peak, 4)}
+        if bound == "tensor" and t in gemm_bytes:  # the other roof of a GEMM task: weights, dW and row buffers moved once
+            gbs = gemm_bytes[t] / sec / 1e9
+            kernels[t]["hbm_gbs_at_least"] = round(gbs, 1)
+            kernels[t]["hbm_frac"] = round(gbs / peaks["hbm"], 4)
         us = stored.get("ncu_us", {}).get(cfg.name, {}).get(t)
         if us:  # NOT measured in this run: the same algorithmic bytes over the kernel's own duration under ncu
             kernels[t]["stored_ncu"] = {"us": us, "frac": round(amount / (us * 1e-6) / 1e9 / peak, 4),
