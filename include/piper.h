@@ -405,10 +405,12 @@ int piper_pair_partition_mode(const piper_ctx* ctx);
  * event).  Returns PIPER_ERR_INVALID on a cycle or a bad edge. */
 int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const int32_t* prio,
                         int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records);
-/* Profile-guided counterpart (PIPER_ORDER_PROFILE): exhaustive search of the static two-stream schedule (n <= 18,
- * stream_of in {0,1}) with the smallest makespan under durations dur[n], simulated with the event rule of
- * PAPER.md:279-286; ties go to the lexicographically smallest pick sequence.  Outputs as piper_list_schedule plus
- * *makespan (nullable), in the unit of dur. */
+/* Profile-guided counterpart (PIPER_ORDER_PROFILE): exact search (branch and bound with a dominance rule) of the static
+ * two-stream schedule (n <= 18, stream_of in {0,1}) with the smallest makespan under durations dur[n], simulated with
+ * the event rule of PAPER.md:279-286; ties go to the first schedule in the search order (ready tasks by ascending id),
+ * so the result is a pure function of the inputs.  The search visits at most 2^21 states (the pair DAG with its caller
+ * tasks needs ~10^3); on a DAG that needs more, the best schedule found within the budget is returned (always valid,
+ * then not proven optimal).  Outputs as piper_list_schedule plus *makespan (nullable), in the unit of dur. */
 int piper_schedule_search(int32_t n, int32_t n_edges, const int32_t* edges, const int32_t* stream_of, const float* dur,
                           int32_t* order, int32_t* waits, int32_t* n_waits, int32_t* records, float* makespan);
 

@@ -7,6 +7,7 @@
 // dependency that ran on another stream, and records one only if a consumer runs on another stream.
 #include <cstdint>
 #include <utility>
+#include <unordered_map>
 #include <vector>
 
 #include "piper.h"
@@ -79,22 +80,36 @@ extern "C" int piper_list_schedule(int32_t n, int32_t n_edges, const int32_t* ed
 // PAPER.md:273 and 420 name profile-guided scheduling as the way past the simple policy above.  With a
 // duration per task the static two-stream schedule of a DAG of this size can be searched exactly.  A schedule is a
 // pair of per-stream sequences, run under the event rule (a task starts when its stream is free and all its
-// producers have finished); the search appends tasks in the order of their start times (every schedule has exactly
-// one such order, up to ties), depth first with the task ids ascending, and cuts a branch whose lower bound - the
-// remaining work of either stream, or the earliest start of a ready task plus the longest chain behind it - cannot
-// beat the best schedule found so far.  The first schedule with the smallest makespan in that order wins, i.e. ties
-// go to the lexicographically smallest pick sequence: the result is a pure function of the inputs.
+// producers have finished).  The search appends ready tasks depth first, task ids ascending, and cuts a branch
+//  (a) whose lower bound - the remaining work of either stream, or the earliest start of a ready task plus the longest
+//      chain behind it - cannot beat the best schedule found so far, or
+//  (b) whose state is dominated by a state seen before with the same set of scheduled tasks: both streams free no
+//      later and every producer that still has consumers finished no later (whatever completes the one completes the
+//      other no later; this is what folds the orders of independent tasks into one).
+// The first schedule with the smallest makespan in that order wins, so the result is a pure function of the inputs
+// (PAPER.md:290).  A budget of kSearchNodes visited states bounds the host time on adversarial DAGs (the pair DAG with
+// its four caller tasks takes ~10^3): past it the best schedule found so far is returned.
 namespace {
+
+constexpr long long kSearchNodes = 1 << 21;
+
+struct Seen {
+    double free_at[2];
+    double fin[18];  // finish time of scheduled tasks that still have unscheduled consumers, else 0
+};
 
 struct Search {
     int n = 0;
-    std::vector<std::vector<int32_t>> preds;
+    std::vector<std::vector<int32_t>> preds, succs;
     const int32_t* stream_of = nullptr;
     const float* dur = nullptr;
     std::vector<double> tail;  // dur[v] + the longest chain of successors behind v (streams ignored)
     std::vector<double> fin;
     std::vector<char> used;
     std::vector<int32_t> cur, best_order;
+    std::unordered_map<uint32_t, Seen> seen;
+    uint32_t mask = 0;
+    long long nodes = 0;
     double free_at[2] = {0, 0}, rem[2] = {0, 0}, best = -1.0;
 
     double start_of(int32_t v) const {
@@ -109,12 +124,39 @@ struct Search {
             if (!used[p]) return false;
         return true;
     }
-    void dfs(double last_start) {
+    // true when a state seen before with this set of scheduled tasks is no later in every respect; records this one otherwise
+    bool dominated() {
+        Seen now;
+        now.free_at[0] = free_at[0], now.free_at[1] = free_at[1];
+        for (int32_t v = 0; v < 18; ++v) now.fin[v] = 0;
+        for (int32_t v = 0; v < n; ++v) {
+            if (!used[v]) continue;
+            for (int32_t t : succs[v])
+                if (!used[t]) now.fin[v] = fin[v];
+        }
+        auto it = seen.find(mask);
+        if (it == seen.end()) {
+            seen.emplace(mask, now);
+            return false;
+        }
+        const Seen& old = it->second;
+        bool old_le = old.free_at[0] <= now.free_at[0] + 1e-12 && old.free_at[1] <= now.free_at[1] + 1e-12;
+        bool now_le = now.free_at[0] <= old.free_at[0] + 1e-12 && now.free_at[1] <= old.free_at[1] + 1e-12;
+        for (int32_t v = 0; v < n; ++v) {
+            old_le = old_le && old.fin[v] <= now.fin[v] + 1e-12;
+            now_le = now_le && now.fin[v] <= old.fin[v] + 1e-12;
+        }
+        if (old_le) return true;
+        if (now_le) it->second = now;  // the better of two comparable states is kept; incomparable: the first
+        return false;
+    }
+    void dfs() {
         if ((int)cur.size() == n) {
             const double m = free_at[0] > free_at[1] ? free_at[0] : free_at[1];
             if (best < 0 || m < best - 1e-9) best = m, best_order = cur;
             return;
         }
+        if (best >= 0 && ++nodes > kSearchNodes) return;  // budget spent: keep the best schedule found
         double lb = free_at[0] + rem[0] > free_at[1] + rem[1] ? free_at[0] + rem[0] : free_at[1] + rem[1];
         for (int32_t v = 0; v < n; ++v)
             if (ready(v)) {
@@ -122,15 +164,15 @@ struct Search {
                 if (e > lb) lb = e;
             }
         if (best >= 0 && lb >= best - 1e-9) return;
+        if (!cur.empty() && dominated()) return;
         for (int32_t v = 0; v < n; ++v) {
             if (!ready(v)) continue;
             const double start = start_of(v);
-            if (start < last_start - 1e-12) continue;  // not the start-time order of this schedule: found on another branch
             const int s = stream_of[v];
             const double keep_free = free_at[s];
-            used[v] = 1, fin[v] = start + dur[v], free_at[s] = fin[v], rem[s] -= dur[v], cur.push_back(v);
-            dfs(start);
-            cur.pop_back(), rem[s] += dur[v], free_at[s] = keep_free, fin[v] = -1.0, used[v] = 0;
+            used[v] = 1, mask |= 1u << v, fin[v] = start + dur[v], free_at[s] = fin[v], rem[s] -= dur[v], cur.push_back(v);
+            dfs();
+            cur.pop_back(), rem[s] += dur[v], free_at[s] = keep_free, fin[v] = -1.0, mask &= ~(1u << v), used[v] = 0;
         }
     }
 };
@@ -146,7 +188,8 @@ extern "C" int piper_schedule_search(int32_t n, int32_t n_edges, const int32_t* 
     Search S;
     S.n = n, S.stream_of = stream_of, S.dur = dur;
     S.preds.assign(n, {});
-    std::vector<std::vector<int32_t>> succs(n);
+    std::vector<std::vector<int32_t>>& succs = S.succs;
+    succs.assign(n, {});
     for (int32_t i = 0; i < n_edges; ++i) {
         const int32_t s = edges[2 * i], t = edges[2 * i + 1];
         if (s < 0 || s >= n || t < 0 || t >= n || s == t) return PIPER_ERR_INVALID;
@@ -177,7 +220,7 @@ extern "C" int piper_schedule_search(int32_t n, int32_t n_edges, const int32_t* 
     }
     S.fin.assign(n, -1.0), S.used.assign(n, 0);
     for (int32_t v = 0; v < n; ++v) S.rem[stream_of[v]] += dur[v];
-    S.dfs(0.0);
+    S.dfs();
     const double best = S.best;
     const std::vector<int32_t>& best_order = S.best_order;
     if (best < 0) return PIPER_ERR_INVALID;  // cycle

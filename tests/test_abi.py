@@ -182,3 +182,28 @@ def test_schedule_search_with_the_four_caller_tasks_of_the_overlapped_block():
     lo, _, _ = piper.piper_list_schedule(n0 + 4, edges, stream_of, prio)
     seq_list = [[v for v in lo.tolist() if stream_of[v] == s] for s in (0, 1)]
     assert mk <= _simulate(n0 + 4, edges, stream_of, dur.tolist(), seq_list) + 1e-6
+
+
+def test_schedule_search_stays_bounded_on_sparse_18_task_dags():
+    """Almost independent tasks are the hard case for an exact search (every order of a stream's tasks is a schedule):
+    the dominance rule folds them and a node budget caps the rest.  The result must be a valid schedule, no worse than
+    the list order, found within a second."""
+    import time
+    rng = np.random.default_rng(3)
+    for _ in range(40):
+        n = 18
+        p = float(rng.choice([0.03, 0.05, 0.1, 0.2]))
+        edges = [[a, b] for a in range(n) for b in range(a + 1, n) if rng.random() < p]
+        stream_of = rng.integers(0, 2, n).tolist()
+        dur = (rng.random(n) * float(rng.choice([1, 10])) + 0.01).astype(np.float32)
+        t0 = time.time()
+        order, waits, records, mk = piper.piper_schedule_search(n, edges, stream_of, dur)
+        assert time.time() - t0 < 3.0
+        pos = {v: i for i, v in enumerate(order.tolist())}
+        assert sorted(pos) == list(range(n))
+        assert all(pos[s] < pos[t] for s, t in edges)
+        seqs = [[v for v in order.tolist() if stream_of[v] == s] for s in (0, 1)]
+        assert _simulate(n, edges, stream_of, dur.tolist(), seqs) == pytest.approx(mk, rel=1e-5)
+        lo, _, _ = piper.piper_list_schedule(n, edges, stream_of, [0] * n)
+        seq_list = [[v for v in lo.tolist() if stream_of[v] == s] for s in (0, 1)]
+        assert mk <= _simulate(n, edges, stream_of, dur.tolist(), seq_list) + 1e-4
