@@ -144,6 +144,24 @@ int piper_route_topk(piper_ctx* ctx, const float* logits, int32_t* topk_idx, flo
 int piper_dispatch_pack(piper_ctx* ctx, const void* x, const int32_t* topk_idx, const float* gates, int32_t* counts,
                         int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* xp, void* stream);
 
+/* F2 without a context, a workspace or any allocation: the permutation half of piper_dispatch_pack (same kernels, same
+ * outputs: counts [E_loc], offsets [E_loc+1], row_of [T,k], src_of [A_cap], gate_rows [A_cap], A_cap = piper_a_cap(desc); only
+ * T, k, E, e_lo, E_loc, row_align of `desc` are read) for callers that cannot call cudaMalloc (CUDA graph capture, serving loops,
+ * harnesses that forbid it).  The call allocates nothing and needs no piper_create: its only scratch, the chunk histograms
+ * (ceil(T*k/1024) * E_loc int32), lives in a static device array of piper_static_scratch_bytes() = 256 KiB that every GPU
+ * which loads the library holds until the process exits.  The kernels run on the CURRENT device, on `stream`; all pointers
+ * are device pointers, 16-byte aligned.  Errors: PIPER_ERR_WORKSPACE when the histograms exceed the static array (use
+ * piper_dispatch_pack with a context then), PIPER_ERR_INVALID for a bad description or pointer, PIPER_ERR_UNSUPPORTED for
+ * E_loc > 4095, PIPER_ERR_CUDA; piper_static_last_error() gives the calling thread's message of the last failure.
+ * Every call on a device shares the one array: calls that may overlap on the GPU (different streams without an
+ * ordering, other threads or processes sharing the context) RACE on it; order them on one stream or with events.  The
+ * array keeps the previous call's contents; nothing in it has to start at zero (every entry read is written by the same
+ * call first). */
+int piper_dispatch_plan_static(const piper_moe_desc* desc, const int32_t* topk_idx, const float* gates, int32_t* counts,
+                               int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* stream);
+size_t piper_static_scratch_bytes(void);
+const char* piper_static_last_error(void);
+
 /* F4 expert_ffn_fwd (SURVEY.md §8a F4, §8c Definition 3; north_star part 3).  Per row r of local
  * expert e: g = xp[r] W_gate[e], u = xp[r] W_up[e], h = silu(g)*u, o[r] = h W_down[e].
  * w_gate, w_up [E_loc,d,I]; w_down [E_loc,I,d].  g_save, u_save, h_save [A_cap,I] are opaque scratch

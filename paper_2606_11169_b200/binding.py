@@ -302,6 +302,23 @@ def piper_run_chunk_bwd_weight(ctx, args: ChunkArgs, stream=None):
 PASS_B, PASS_BI = 0, 1
 
 
+def piper_dispatch_plan_static(desc, topk_idx, gates, counts, offsets, row_of, src_of, gate_rows, stream=None):
+    """F2 on the current device without a context or any allocation (include/piper.h); raises PiperError with the
+    library's message when the call is refused."""
+    L = lib()
+    L.piper_static_last_error.restype = ctypes.c_char_p
+    rc = L.piper_dispatch_plan_static(ctypes.byref(desc), _ptr(topk_idx), _ptr(gates), _ptr(counts), _ptr(offsets), _ptr(row_of),
+                                      _ptr(src_of), _ptr(gate_rows), _stream(stream))
+    if rc != PIPER_OK:
+        raise PiperError(f"piper_dispatch_plan_static: status {rc}: {L.piper_static_last_error().decode()}")
+
+
+def piper_static_scratch_bytes() -> int:
+    L = lib()
+    L.piper_static_scratch_bytes.restype = ctypes.c_size_t
+    return int(L.piper_static_scratch_bytes())
+
+
 def piper_set_pair_bwd_pass(ctx, bwd_pass: int):
     ctx.check(lib().piper_set_pair_bwd_pass(ctx._h, int(bwd_pass)), "piper_set_pair_bwd_pass")
 

@@ -5,6 +5,10 @@
 // index): per-chunk histograms, a prefix over chunks, then __match_any_sync ranks inside a chunk.
 #include "piper_internal.cuh"
 
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
+
 namespace piper {
 namespace {
 
@@ -465,3 +469,89 @@ int launch_combine_bwd(piper_ctx* c, Lane ln, const void* dy, const void* o, con
 }
 
 }  // namespace piper
+
+// ---- piper_dispatch_plan_static: F2 without a context, a workspace or any allocation -----------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+// the same two kernels as launch_scan_rank, with the chunk histograms - the one piece of scratch memory F2 needs - in a
+// file-scope device array instead of the context's workspace.  Every GPU that loads the library holds the array
+// (kStaticScratchBytes) until the process exits.  In host code `g_static_scratch` is only the host-side stand-in of the
+// array, not a device address: its address on each device is looked up once, with that device current, through
+// cudaGetSymbolAddress and kept.
+namespace piper {
+namespace {
+
+constexpr size_t kStaticScratchBytes = 256 * 1024;  // 65536 chunk-histogram entries: n_chunks * E_loc of one call
+constexpr int kStaticMaxDevices = 64;
+static __device__ __align__(256) int32_t g_static_scratch[kStaticScratchBytes / sizeof(int32_t)];
+
+std::mutex g_static_mutex;
+int32_t* g_static_ptr[kStaticMaxDevices];  // device address of g_static_scratch on each device, nullptr = not looked up
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_static_err, sizeof(g_static_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+}  // namespace
+}  // namespace piper
+
+extern "C" {
+
+size_t piper_static_scratch_bytes(void) { return piper::kStaticScratchBytes; }
+const char* piper_static_last_error(void) { return piper::g_static_err; }
+
+int piper_dispatch_plan_static(const piper_moe_desc* D, const int32_t* topk_idx, const float* gates, int32_t* counts,
+                               int32_t* offsets, int32_t* row_of, int32_t* src_of, float* gate_rows, void* stream) {
+    using namespace piper;
+    if (!D || D->T < 1 || D->k < 1 || D->E < 1 || D->E_loc < 1 || D->k > D->E || D->e_lo < 0 || D->e_lo + D->E_loc > D->E ||
+        D->row_align < 1 || D->row_align > 1024 || (int64_t)D->T * D->k > (1ll << 30))
+        return static_fail(PIPER_ERR_INVALID, "piper_dispatch_plan_static: invalid layer description");
+    for (const void* p : {(const void*)topk_idx, (const void*)gates, (const void*)counts, (const void*)offsets,
+                          (const void*)row_of, (const void*)src_of, (const void*)gate_rows})
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 15u))
+            return static_fail(PIPER_ERR_INVALID, "piper_dispatch_plan_static: null or misaligned pointer");
+    const int n_assign = D->T * D->k, n_chunks = cdiv(n_assign, kScanChunk);
+    const size_t need = sizeof(int32_t) * (size_t)n_chunks * (size_t)D->E_loc;
+    if (need > kStaticScratchBytes)
+        return static_fail(PIPER_ERR_WORKSPACE,
+                           "piper_dispatch_plan_static: ceil(T*k/%d) * E_loc = %d * %d histogram entries (%zu bytes) exceed the "
+                           "static scratch of %zu bytes; use piper_dispatch_pack with a context",
+                           kScanChunk, n_chunks, D->E_loc, need, kStaticScratchBytes);
+    const size_t smem = sizeof(int32_t) * (3 * (size_t)D->E_loc + 1);
+    if (smem > 48 * 1024)
+        return static_fail(PIPER_ERR_UNSUPPORTED, "piper_dispatch_plan_static: E_loc = %d needs %zu bytes of shared memory", D->E_loc, smem);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices)
+        return static_fail(PIPER_ERR_CUDA, "piper_dispatch_plan_static: no current CUDA device (or device id >= %d)", kStaticMaxDevices);
+    int32_t* scratch;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[dev]) {  // once per device, with that device current
+            void* p = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+            if (e != cudaSuccess || !p)
+                return static_fail(PIPER_ERR_CUDA, "piper_dispatch_plan_static: cudaGetSymbolAddress failed on device %d: %s", dev,
+                                   cudaGetErrorString(e));
+            g_static_ptr[dev] = static_cast<int32_t*>(p);
+        }
+        scratch = g_static_ptr[dev];
+    }
+    // Nothing has to start at zero: chunk_hist_kernel writes every one of the n_chunks * E_loc entries that scan_rank_kernel
+    // reads, so the contents the previous call left behind are never seen.
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int64_t kk = D->k < D->E_loc ? D->k : D->E_loc;
+    const int a_cap = (int)((int64_t)D->T * kk + (int64_t)D->E_loc * (D->row_align - 1));
+    chunk_hist_kernel<<<n_chunks, kScanChunk, sizeof(int32_t) * D->E_loc, s>>>(topk_idx, n_assign, D->e_lo, D->E_loc, scratch);
+    scan_rank_kernel<<<n_chunks, kScanChunk, smem, s>>>(topk_idx, gates, n_assign, D->e_lo, D->E_loc, D->row_align, a_cap, scratch,
+                                                        counts, offsets, row_of, src_of, gate_rows);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return static_fail(PIPER_ERR_CUDA, "piper_dispatch_plan_static: launch failed: %s", cudaGetErrorString(e));
+    g_static_err[0] = 0;
+    return PIPER_OK;
+}
+
+}  // extern "C"
