@@ -66,13 +66,17 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
-        self.recording = False
+        self.recording, self.power_w, self.power_limit_w = False, [], None
         try:
             import pynvml
             pynvml.nvmlInit()
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            try:
+                self.power_limit_w = pynvml.nvmlDeviceGetEnforcedPowerLimit(self.h) / 1000.0
+            except Exception:
+                pass
         except Exception as e:  # pragma: no cover
             log("clock sampler unavailable:", e)
             self.nv = None
@@ -95,18 +99,23 @@ class ClockSampler(threading.Thread):
                     for bit, nm in names.items():
                         if r & bit:
                             self.reasons.add(nm)
+                    self.power_w.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception:
                 pass
             time.sleep(0.005)
 
     def begin(self):
-        self.samples, self.reasons, self.recording = [], set(), True
+        self.samples, self.reasons, self.power_w, self.recording = [], set(), [], True
 
     def end(self):
         self.recording = False
         s = sorted(self.samples)
+        # NVML refreshes its clock / reason / power readings every ~100 ms: a 0.15 s region sees one or two distinct values,
+        # and a reason bit that was clear at those instants stays unreported.  The board power beside its limit says
+        # independently whether the power cap is what holds the clock.
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(s)}
+                "reasons": sorted(self.reasons), "samples": len(s),
+                "power_w_max": round(max(self.power_w), 1) if self.power_w else None, "power_limit_w": self.power_limit_w}
 
 
 # --------------------------------------------------------------------------------- reference arm
