@@ -300,6 +300,16 @@ def time_resident(w: Workload, steps, warmup, sampler, barrier, world, min_secon
     clocks = sampler.end()
     launches = piper.piper_kernel_launches(w.ctx) - launches0
     ms_per_step = max_over_ranks(ev0.elapsed_time(ev1), world, w.dev) / steps
+    if clocks.get("samples") and ev0.elapsed_time(ev1) < 400.0:
+        # NVML refreshes clock, throttle reasons and power every ~100 ms (power is an average over longer still): a timed
+        # region of K = 20 steps (0.14 s) shows one or two stale readings.  The same loop therefore keeps running, untimed,
+        # for 0.6 s more under the sampler, and that record is reported beside the timed region's own.
+        n_more = int(600.0 / max(ms_per_step, 1e-3)) + 1
+        sampler.begin()
+        for _ in range(n_more):
+            w.step()
+        torch.cuda.synchronize()
+        clocks["same_loop_continued_untimed"] = dict(sampler.end(), steps=n_more)
     return ms_per_step, clocks, int(launches), steps
 
 
@@ -682,12 +692,44 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
     out = {"fwd_ms": t_f, "bwd_ms": t_b, "serial_ms": t_f + t_b, "tokens_per_pair": 2 * cfg.T,
            "tokens_per_s_serial": 2 * cfg.T / ((t_f + t_b) * 1e-3), "splits": {}, "variants": {}}
 
+    def serial_fn():
+        piper.piper_run_chunk_fwd(ctx, args_a)
+        piper.piper_run_chunk_bwd(ctx, args_b)
+
+    serial_beside = []
+
+    def timed_beside_serial(fn, repeats=8):
+        """The pair and the serial chunks (fwd(A) then bwd(B) on one stream, all SMs) timed alternately, a few calls
+        each, the order swapped every repeat: under the power cap the same kernels slow down by several % while a run
+        warms the board, so a baseline taken once at the start would flatter itself.  Medians of the pair's time, of the
+        serial time beside it and of their ratio."""
+        for _ in range(2):
+            fn()
+        serial_fn()
+        tp, ts, ratio = [], [], []
+        n_in = max(3, iters // 2)
+        for r in range(repeats):
+            pair_first = r % 2 == 1
+            t = {}
+            for which in ((0, 1) if pair_first else (1, 0)):
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(n_in):
+                    (fn if which == 0 else serial_fn)()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                t[which] = e0.elapsed_time(e1) / n_in
+            tp.append(t[0]), ts.append(t[1]), ratio.append(t[0] / t[1])
+        serial_beside.extend(ts)
+        med = lambda v: sorted(v)[len(v) // 2]
+        return med(tp), med(ts), med(ratio)
+
     def sweep(split_list):
         res = {}
         for sg, sc in split_list:
             piper.piper_pair_prepare(ctx, sg, sc)  # partitions / streams / plan are created outside the timed calls
-            t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
-            res[f"{sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / (t_f + t_b),
+            t_p, t_s, ratio = timed_beside_serial(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
+            res[f"{sg}:{sc}"] = {"pair_ms": t_p, "serial_ms_beside": t_s, "ratio_vs_serial": ratio,
                                  "order": piper.piper_pair_order(ctx, sg, sc)}
         return res
 
@@ -721,8 +763,12 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
         out["overlapped_block"] = overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm)
     best = min(((v["ratio_vs_serial"], name, k) for name, d in
                 [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))
-    out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2],
-                   "tokens_per_s": 2 * cfg.T / (best[0] * (t_f + t_b) * 1e-3)}
+    best_ms = dict([("list_order_exclusive", out["splits"])] + list(out["variants"].items()))[best[1]][best[2]]["pair_ms"]
+    out["best"] = {"ratio_vs_serial": best[0], "variant": best[1], "split": best[2], "pair_ms": best_ms,
+                   "tokens_per_s": 2 * cfg.T / (best_ms * 1e-3)}
+    out["serial_back_to_back_ms"] = sorted(serial_beside)[len(serial_beside) // 2]
+    out["ratio_is"] = ("pair_ms / serial_ms_beside: the serial chunks (fwd(A) then bwd(B) on one stream, all SMs) re-timed "
+                       "beside every pair timing, alternating; serial_ms = fwd and bwd timed separately at the start")
     # What the pair can reach on this workload: the floors of the two roofs and of "every row
     # mover hidden under GEMMs that keep their serial speed", each as a ratio to the measured serial time.
     peaks = measured_peaks()
@@ -753,6 +799,37 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
     return out
 
 
+def run_ab(w: Workload, spec: str, blocks: int, per: int):
+    """Paired A/B of one kernel-variant switch inside one process (`--ab NAME=v0,v1,...`): blocks of `per` timed steps
+    alternate between the values (order reversed every block, one untimed step after each switch), so the drift of the
+    power-capped clocks while the board warms hits every value alike.  Separate bench runs of the same library differ by
+    several % on one box and cannot resolve a 1-2 % change (DESIGN.md findings 30, 31)."""
+    import statistics
+    torch, piper = w.torch, w.piper
+    name, vals = spec.split("=")
+    vals = [int(v) for v in vals.split(",")]
+    opt = getattr(piper, "OPT_" + name)
+    for _ in range(10):
+        w.step()
+    torch.cuda.synchronize()
+    times = {v: [] for v in vals}
+    for b in range(blocks):
+        for v in (vals if b % 2 == 0 else vals[::-1]):
+            piper.piper_set_option(w.ctx, opt, v)
+            w.step()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(w.stream)
+            for _ in range(per):
+                w.step()
+            e1.record(w.stream)
+            torch.cuda.synchronize()
+            times[v].append(e0.elapsed_time(e1) / per)
+    base = statistics.mean(times[vals[0]])
+    return {"option": "PIPER_OPT_" + name, "blocks": blocks, "steps_per_block": per, "workload": w.cfg.name,
+            "values": {str(v): {"mean_ms": statistics.mean(t), "median_ms": statistics.median(t), "min_ms": min(t),
+                                "vs_first_pct": 100 * (statistics.mean(t) / base - 1)} for v, t in times.items()}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -779,6 +856,11 @@ def main():
     ap.add_argument("--attn", action="store_true",
                     help="with --pair: also time the whole overlapped block (N3), attention forward / backward (torch SDPA) as "
                          "caller tasks of the pair")
+    ap.add_argument("--ab", default=None,
+                    help="paired A/B of a kernel-variant switch, NAME=v0,v1,...: alternates the values inside one process "
+                         "(--ab-blocks blocks of --ab-steps timed steps per value) and prints only that comparison")
+    ap.add_argument("--ab-blocks", type=int, default=30)
+    ap.add_argument("--ab-steps", type=int, default=5)
     ap.add_argument("--main-grad", action="store_true",
                     help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")
     args = ap.parse_args()
@@ -818,6 +900,11 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.ab:
+        w = Workload(args, cfg, rank, local)
+        print(json.dumps({"ab": run_ab(w, args.ab, args.ab_blocks, args.ab_steps)}), flush=True)
+        w.close()
+        return
     sampler = ClockSampler(local)
     sampler.start()  # before any warm-up; it records only inside the timed regions
     line, w = run_piper(args, cfg, sampler, rank, world, local, barrier)

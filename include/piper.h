@@ -96,7 +96,9 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
  *  PIPER_OPT_TC_2CTA      [2]  CTA-pair kernels: 0 never (1-CTA kernels; bf16 dW, row_align % 128 only), 1 always,
  *                              2 by expected group length
  *  PIPER_OPT_T_SMALL_ROWS [32] rows-on-N: chunks of at most this many rows per CTA load 32-row boxes
- *  PIPER_OPT_T_GREEDY     [1]  rows-on-N: 1 = 256-row chunks and a short last one, 0 = equal chunks
+ *  PIPER_OPT_T_GREEDY     [0]  rows-on-N: how an expert's rows are cut into chunks of at most 256: 0 = equal chunks
+ *                              (a multiple of 16 rows each), 1 = 256-row chunks and a short last one (measured slower: the
+ *                              short chunk streams a whole weight slice for a few rows)
  *  PIPER_OPT_T_DUAL       [0]  rows-on-N plain-store kernels (F_GEMM2, DGRAD2): 1 = a tile takes two row chunks of an
  *                              expert through one pass over the weights (both accumulators); measured slower
  *  PIPER_OPT_WGRAD_STORE_WARP [2] CTA-pair wgrad with bf16 dW: 1 = one 128-row bulk store per 64-column chunk, issued by a

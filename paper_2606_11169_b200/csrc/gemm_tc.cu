@@ -2187,7 +2187,8 @@ int tc_init(piper_ctx* c) {
     cudaGetLastError();
     c->encode_tiled = fn;
     if (cudaMemset(c->tc_scratch + (size_t)kProfSlots * kProfSlotWords * 8, 0, kSchedSlots * 8) != cudaSuccess) return PIPER_ERR_CUDA;
-    c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_greedy = 1, c->tc_two_cta = 2;
+    c->tc_prof = 0, c->tc_rows_on_n = 1, c->tc_small_rows = TB_SMALL_ROWS, c->tc_two_cta = 2;
+    c->tc_greedy = 0;  // equal chunks: C2 -6 %, C3 -0.9 %, C4 -0.2 % per step against 256-row chunks + a short tail (finding 31)
     c->tc_dual = 0;  // measured slower (DESIGN.md finding 22)
     c->tc_store_warp = 2;
     c->map_cache = new (std::nothrow) MapCacheEntry[kMapCache]();

@@ -186,15 +186,18 @@ def test_more_local_experts_than_the_cta_pair_kernels_index():
 
 
 @pytest.mark.parametrize("name", ["C3s", "C4s", "C6s"])
-@pytest.mark.parametrize("family", ["rows_on_m", "one_cta", "dual_tiles", "wgrad_store_warp", "wgrad_warp_stores"])
+@pytest.mark.parametrize("family", ["rows_on_m", "one_cta", "dual_tiles", "wgrad_store_warp", "wgrad_warp_stores",
+                                    "greedy_chunks", "equal_chunks"])
 def test_fallback_kernel_families(name, family):
     """The rows-on-M CTA-pair kernels and the 1-CTA kernels (DESIGN.md section 5.1 b, c) stay correct: they serve
     layers with more than 192 local experts; so do the two-chunk tiles of the plain-store rows-on-N kernels (a measured
     variant).  piper_set_option selects them (host state of the context)."""
-    if family in ("dual_tiles", "wgrad_store_warp", "wgrad_warp_stores"):
-        # wgrad: both ways of storing dW (the default picks one by the expected group length)
+    if family in ("dual_tiles", "wgrad_store_warp", "wgrad_warp_stores", "greedy_chunks", "equal_chunks"):
+        # wgrad: both ways of storing dW (the default picks one by the expected group length); rows-on-N kernels: both
+        # ways of cutting an expert's rows into chunks (256-row chunks and a short last one / equal chunks)
         opt = {"dual_tiles": (piper.OPT_T_DUAL, 1), "wgrad_store_warp": (piper.OPT_WGRAD_STORE_WARP, 1),
-               "wgrad_warp_stores": (piper.OPT_WGRAD_STORE_WARP, 0)}[family]
+               "wgrad_warp_stores": (piper.OPT_WGRAD_STORE_WARP, 0), "greedy_chunks": (piper.OPT_T_GREEDY, 1),
+               "equal_chunks": (piper.OPT_T_GREEDY, 0)}[family]
         cfg = dataclasses.replace(configs.BY_NAME[name], row_align=16)
         inp = configs.make_inputs(cfg)
         f = oracle.forward(cfg, inp)
