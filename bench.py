@@ -808,14 +808,19 @@ def run_ab(w: Workload, spec: str, blocks: int, per: int):
     torch, piper = w.torch, w.piper
     name, vals = spec.split("=")
     vals = [int(v) for v in vals.split(",")]
-    opt = getattr(piper, "OPT_" + name)
+    if name == "CHUNK_OVERLAP":  # not a piper_set_option switch: piper_set_chunk_overlap (row movers on the side stream)
+        def set_value(v):
+            piper.piper_set_chunk_overlap(w.ctx, v)
+    else:
+        def set_value(v):
+            piper.piper_set_option(w.ctx, getattr(piper, "OPT_" + name), v)
     for _ in range(10):
         w.step()
     torch.cuda.synchronize()
     times = {v: [] for v in vals}
     for b in range(blocks):
         for v in (vals if b % 2 == 0 else vals[::-1]):
-            piper.piper_set_option(w.ctx, opt, v)
+            set_value(v)
             w.step()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(w.stream)
@@ -825,7 +830,7 @@ def run_ab(w: Workload, spec: str, blocks: int, per: int):
             torch.cuda.synchronize()
             times[v].append(e0.elapsed_time(e1) / per)
     base = statistics.mean(times[vals[0]])
-    return {"option": "PIPER_OPT_" + name, "blocks": blocks, "steps_per_block": per, "workload": w.cfg.name,
+    return {"option": name, "blocks": blocks, "steps_per_block": per, "workload": w.cfg.name,
             "values": {str(v): {"mean_ms": statistics.mean(t), "median_ms": statistics.median(t), "min_ms": min(t),
                                 "vs_first_pct": 100 * (statistics.mean(t) / base - 1)} for v, t in times.items()}}
 
