@@ -605,7 +605,7 @@ def gemm_hbm_bytes(cfg, A: int):
     return out
 
 
-def overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm):
+def overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, timed_beside, n_sm):
     """N3 (Fig. 3b): the whole overlapped block - attention forward of microbatch A in front of its MoE
     chunk, attention backward of microbatch B behind its MoE chunk - with the attention as CALLER tasks of the pair
     (piper_pair_set_caller_task).  The attention here is torch's fused SDPA (library code, causal, heads of 128, sequences
@@ -630,7 +630,10 @@ def overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm):
     t_af, t_ab = timed(attn_fwd), timed(attn_bwd)
     t_f = timed(lambda: piper.piper_run_chunk_fwd(ctx, args_a))
     t_b = timed(lambda: piper.piper_run_chunk_bwd(ctx, args_b))
-    serial = timed(lambda: (attn_fwd(), piper.piper_run_chunk_fwd(ctx, args_a), piper.piper_run_chunk_bwd(ctx, args_b), attn_bwd()))
+    def serial_block():
+        attn_fwd(), piper.piper_run_chunk_fwd(ctx, args_a), piper.piper_run_chunk_bwd(ctx, args_b), attn_bwd()
+
+    serial = timed(serial_block)
     res = {"attention": f"torch SDPA (flash), causal, batch {B} x {H} heads x {S} tokens x 128, bf16", "attn_fwd_ms": t_af,
            "attn_bwd_ms": t_ab, "chunk_fwd_ms": t_f, "chunk_bwd_ms": t_b, "serial_ms": serial, "variants": {}}
     piper.piper_pair_set_caller_task(ctx, piper.SLOT_F_PRE, attn_fwd, est_ms=t_af, side=1)
@@ -641,8 +644,8 @@ def overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm):
         piper.piper_set_pair_policy(ctx, order, part, task_ms)
         for sg, sc in splits:
             piper.piper_pair_prepare(ctx, sg, sc)
-            t_p = timed(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc))
-            res["variants"][f"{name} {sg}:{sc}"] = {"pair_ms": t_p, "ratio_vs_serial": t_p / serial,
+            t_p, t_s, ratio = timed_beside(lambda: piper.piper_run_chunk_pair(ctx, args_a, args_b, sg, sc), base=serial_block)
+            res["variants"][f"{name} {sg}:{sc}"] = {"pair_ms": t_p, "serial_ms_beside": t_s, "ratio_vs_serial": ratio,
                                                     "order": piper.piper_pair_order(ctx, sg, sc)}
     piper.piper_pair_set_caller_task(ctx, piper.SLOT_F_PRE, None)
     piper.piper_pair_set_caller_task(ctx, piper.SLOT_B_POST, None)
@@ -698,14 +701,15 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
 
     serial_beside = []
 
-    def timed_beside_serial(fn, repeats=8):
+    def timed_beside_serial(fn, repeats=8, base=None):
         """The pair and the serial chunks (fwd(A) then bwd(B) on one stream, all SMs) timed alternately, a few calls
         each, the order swapped every repeat: under the power cap the same kernels slow down by several % while a run
         warms the board, so a baseline taken once at the start would flatter itself.  Medians of the pair's time, of the
         serial time beside it and of their ratio."""
+        base_fn = base or serial_fn
         for _ in range(2):
             fn()
-        serial_fn()
+        base_fn()
         tp, ts, ratio = [], [], []
         n_in = max(3, iters // 2)
         for r in range(repeats):
@@ -715,12 +719,13 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
                 torch.cuda.synchronize()
                 e0.record(stream)
                 for _ in range(n_in):
-                    (fn if which == 0 else serial_fn)()
+                    (fn if which == 0 else base_fn)()
                 e1.record(stream)
                 torch.cuda.synchronize()
                 t[which] = e0.elapsed_time(e1) / n_in
             tp.append(t[0]), ts.append(t[1]), ratio.append(t[0] / t[1])
-        serial_beside.extend(ts)
+        if base is None:
+            serial_beside.extend(ts)
         med = lambda v: sorted(v)[len(v) // 2]
         return med(tp), med(ts), med(ratio)
 
@@ -760,7 +765,7 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
     out["variants"]["chunk_streams_gpu_allocates_sms"] = sweep([(n_sm, 16)])
     piper.piper_set_pair_policy(ctx, piper.ORDER_LIST, piper.PART_EXCLUSIVE)
     if attn:
-        out["overlapped_block"] = overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, n_sm)
+        out["overlapped_block"] = overlapped_block(piper, ctx, cfg, args_a, args_b, task_ms, timed, timed_beside_serial, n_sm)
     best = min(((v["ratio_vs_serial"], name, k) for name, d in
                 [("list_order_exclusive", out["splits"])] + list(out["variants"].items()) for k, v in d.items()))
     best_ms = dict([("list_order_exclusive", out["splits"])] + list(out["variants"].items()))[best[1]][best[2]]["pair_ms"]
