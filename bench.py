@@ -804,11 +804,12 @@ def run_pair(piper, ctx, cfg, b_a, inp_a, splits, iters, sampler=None, attn=Fals
     return out
 
 
-def run_ab(w: Workload, spec: str, blocks: int, per: int):
+def run_ab(w: Workload, spec: str, blocks: int, per: int, tasks=None):
     """Paired A/B of one kernel-variant switch inside one process (`--ab NAME=v0,v1,...`): blocks of `per` timed steps
     alternate between the values (order reversed every block, one untimed step after each switch), so the drift of the
     power-capped clocks while the board warms hits every value alike.  Separate bench runs of the same library differ by
-    several % on one box and cannot resolve a 1-2 % change (DESIGN.md findings 30, 31)."""
+    several % on one box and cannot resolve a 1-2 % change (DESIGN.md findings 30, 31).  With `tasks` (--ab-tasks, names of
+    the pair DAG's tasks) a timed unit is those tasks run once each through piper_run_task instead of a whole step."""
     import statistics
     torch, piper = w.torch, w.piper
     name, vals = spec.split("=")
@@ -819,6 +820,13 @@ def run_ab(w: Workload, spec: str, blocks: int, per: int):
     else:
         def set_value(v):
             piper.piper_set_option(w.ctx, getattr(piper, "OPT_" + name), v)
+    def unit():
+        if tasks:
+            for t in tasks:
+                piper.piper_run_task(w.ctx, t, w.cargs)
+        else:
+            w.step()
+
     for _ in range(10):
         w.step()
     torch.cuda.synchronize()
@@ -826,16 +834,16 @@ def run_ab(w: Workload, spec: str, blocks: int, per: int):
     for b in range(blocks):
         for v in (vals if b % 2 == 0 else vals[::-1]):
             set_value(v)
-            w.step()
+            unit()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(w.stream)
             for _ in range(per):
-                w.step()
+                unit()
             e1.record(w.stream)
             torch.cuda.synchronize()
             times[v].append(e0.elapsed_time(e1) / per)
     base = statistics.mean(times[vals[0]])
-    return {"option": name, "blocks": blocks, "steps_per_block": per, "workload": w.cfg.name,
+    return {"option": name, "blocks": blocks, "steps_per_block": per, "workload": w.cfg.name, "unit": tasks or "step",
             "values": {str(v): {"mean_ms": statistics.mean(t), "median_ms": statistics.median(t), "min_ms": min(t),
                                 "vs_first_pct": 100 * (statistics.mean(t) / base - 1)} for v, t in times.items()}}
 
@@ -871,6 +879,7 @@ def main():
                          "(--ab-blocks blocks of --ab-steps timed steps per value) and prints only that comparison")
     ap.add_argument("--ab-blocks", type=int, default=30)
     ap.add_argument("--ab-steps", type=int, default=5)
+    ap.add_argument("--ab-tasks", default=None, help="with --ab: time these tasks (comma-separated, e.g. F_COMBINE,B_UNPACK) instead of whole steps")
     ap.add_argument("--main-grad", action="store_true",
                     help="measured variant: fp32 dW accumulated across steps (dw_dtype F32, accumulate = 1)")
     args = ap.parse_args()
@@ -912,7 +921,8 @@ def main():
 
     if args.ab:
         w = Workload(args, cfg, rank, local)
-        print(json.dumps({"ab": run_ab(w, args.ab, args.ab_blocks, args.ab_steps)}), flush=True)
+        print(json.dumps({"ab": run_ab(w, args.ab, args.ab_blocks, args.ab_steps,
+                                       args.ab_tasks.split(",") if args.ab_tasks else None)}), flush=True)
         w.close()
         return
     sampler = ClockSampler(local)

@@ -105,6 +105,9 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
  *                              store warp from blocks the four epilogue warps stage side by side; 0 = one 32-row store
  *                              per epilogue warp; 2 = store warp for long, even groups (>= 512 rows per expert expected
  *                              and real, no expert above twice the mean: the kernel looks at offsets)
+ *  PIPER_OPT_MOVE_ITEMS   [8]  row movers: a token's row is split by columns so that about this many work items exist per
+ *                              resident warp (1..64)
+ *  PIPER_OPT_MOVE_CAP     [16] row movers: at most this many blocks per SM of the lane (1..64)
  *  PIPER_OPT_TC_PROFILE   [0]  1 = the tcgen05 kernels record wait-cycle counters (piper_debug_tc_counters)
  *  PIPER_OPT_FUSED_GATHER [0]  chunk calls on tcgen05 layers (N2 fusion): 0 = the GEMMs read the packed buffers xp / d_o;
  *                              1 = F_GEMM1 and the gate|up wgrad gather the rows of x themselves, no pack kernel runs;
@@ -119,6 +122,8 @@ const void* piper_debug_tc_counters(const piper_ctx* ctx);
 #define PIPER_OPT_FUSED_GATHER 5
 #define PIPER_OPT_T_DUAL 6
 #define PIPER_OPT_WGRAD_STORE_WARP 7
+#define PIPER_OPT_MOVE_ITEMS 8
+#define PIPER_OPT_MOVE_CAP 9
 int piper_set_option(piper_ctx* ctx, int option, int value);
 /* 1 when the whole-chunk calls of this context run the fused-gather GEMMs (PIPER_OPT_FUSED_GATHER on
  * a layer whose GEMMs are the rows-on-N + CTA-pair tcgen05 kernels): the forward chunk then launches no pack kernel and

@@ -327,7 +327,7 @@ def piper_pair_prepare(ctx, sm_gemm: int, sm_comm: int):
     ctx.check(lib().piper_pair_prepare(ctx._h, int(sm_gemm), int(sm_comm)), "piper_pair_prepare")
 
 
-OPT_TC_ROWS_ON_N, OPT_TC_2CTA, OPT_T_SMALL_ROWS, OPT_T_GREEDY, OPT_TC_PROFILE, OPT_FUSED_GATHER, OPT_T_DUAL, OPT_WGRAD_STORE_WARP = range(8)
+OPT_TC_ROWS_ON_N, OPT_TC_2CTA, OPT_T_SMALL_ROWS, OPT_T_GREEDY, OPT_TC_PROFILE, OPT_FUSED_GATHER, OPT_T_DUAL, OPT_WGRAD_STORE_WARP, OPT_MOVE_ITEMS, OPT_MOVE_CAP = range(10)
 
 
 def piper_set_option(ctx, option: int, value: int):

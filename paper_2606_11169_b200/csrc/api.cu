@@ -137,6 +137,7 @@ int piper_create(const piper_moe_desc* D, int device, void* workspace, size_t wo
         piper_destroy(c);
         return PIPER_ERR_CUDA;
     }
+    c->move_items = 8, c->move_cap = 16;  // measured on C3
     c->fused_gather = 0;  // N2 fusion is built and parity-tested but measured slower than pack + TMA (DESIGN.md finding 19)
     c->pair_order = PIPER_ORDER_PROFILE, c->pair_part = PIPER_PART_SHARED;  // the policy that does not lose to serial
     const int rc = variant_ok(c);
@@ -181,6 +182,8 @@ int piper_get_option(const piper_ctx* c, int option, int* value) {
         case PIPER_OPT_FUSED_GATHER: *value = c->fused_gather; return PIPER_OK;
         case PIPER_OPT_T_DUAL: *value = c->tc_dual; return PIPER_OK;
         case PIPER_OPT_WGRAD_STORE_WARP: *value = c->tc_store_warp; return PIPER_OK;
+        case PIPER_OPT_MOVE_ITEMS: *value = c->move_items; return PIPER_OK;
+        case PIPER_OPT_MOVE_CAP: *value = c->move_cap; return PIPER_OK;
     }
     return PIPER_ERR_INVALID;
 }
@@ -198,6 +201,8 @@ int piper_set_option(piper_ctx* c, int option, int value) {
         case PIPER_OPT_FUSED_GATHER: field = &c->fused_gather; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_T_DUAL: field = &c->tc_dual; if (value != 0 && value != 1) return PIPER_ERR_INVALID; break;
         case PIPER_OPT_WGRAD_STORE_WARP: field = &c->tc_store_warp; if (value < 0 || value > 2) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_MOVE_ITEMS: field = &c->move_items; if (value < 1 || value > 64) return PIPER_ERR_INVALID; break;
+        case PIPER_OPT_MOVE_CAP: field = &c->move_cap; if (value < 1 || value > 64) return PIPER_ERR_INVALID; break;
     }
     *field = value;
     const int rc = variant_ok(c);  // e.g. row_align 16 needs the rows-on-N + CTA-pair kernels, fp32 dW the CTA-pair wgrad

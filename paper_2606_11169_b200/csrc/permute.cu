@@ -18,12 +18,6 @@ namespace {
 #ifndef PIPER_MOVE_U
 #define PIPER_MOVE_U 4
 #endif
-#ifndef PIPER_MOVE_ITEMS
-#define PIPER_MOVE_ITEMS 8
-#endif
-#ifndef PIPER_MOVE_CAP
-#define PIPER_MOVE_CAP 16
-#endif
 constexpr int kMoveWarps = PIPER_MOVE_WARPS;  // warps per block of the row movers
 
 // ---- F2 phase 1: per-chunk histogram of local experts ------------------------------------------
@@ -370,12 +364,12 @@ combine_bwd_kernel(const int4* __restrict__ dy, const int4* __restrict__ o, cons
     }
 }
 
-// Column splits per token so that about PIPER_MOVE_ITEMS items exist per resident warp of the lane: with sparse local
+// Column splits per token so that about move_items (PIPER_OPT_MOVE_ITEMS) items exist per resident warp of the lane: with sparse local
 // slots (C3: a third of the tokens has none, the others 1-4) the work per item varies, and finer items even it out
 // (C3 combine 82.8 -> 75.8 us, unpack 81.9 -> 73.7 us against 2 items per warp; C2 unchanged).
-inline void choose_split(Lane ln, int T, int row_packets, int& S, int& split_packets) {
+inline void choose_split(const piper_ctx* c, Lane ln, int T, int row_packets, int& S, int& split_packets) {
     const int warps = ln.sms * 48;
-    int want = (PIPER_MOVE_ITEMS * warps + T - 1) / T;
+    int want = (c->move_items * warps + T - 1) / T;
     const int max_s = (row_packets + kStep - 1) / kStep;
     if (want > max_s) want = max_s;
     if (want < 1) want = 1;
@@ -386,9 +380,9 @@ inline void choose_split(Lane ln, int T, int row_packets, int& S, int& split_pac
 // Grid: one warp per item up to a few waves of resident blocks (more, shorter-lived blocks than fit at once
 // measured faster than an exactly-resident persistent grid: finishing blocks are replaced at once).
 template <typename K>
-inline int mover_blocks(Lane ln, int items, K) {
+inline int mover_blocks(const piper_ctx* c, Lane ln, int items, K) {
     int blocks = cdiv(items, kMoveWarps);
-    const int cap = ln.sms * PIPER_MOVE_CAP;
+    const int cap = ln.sms * c->move_cap;
     return blocks < cap ? (blocks < 1 ? 1 : blocks) : cap;
 }
 
@@ -415,8 +409,8 @@ int launch_pack(piper_ctx* c, Lane ln, const void* x, const int32_t* offsets, co
     const int a_cap = (int)piper_a_cap(&D);
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
     int S, split_packets;
-    choose_split(ln, D.T, row_packets, S, split_packets);
-    pack_kernel<<<mover_blocks(ln, D.T * S + a_cap, pack_kernel), kMoveWarps * 32, 0, ln.stream>>>(
+    choose_split(c, ln, D.T, row_packets, S, split_packets);
+    pack_kernel<<<mover_blocks(c, ln, D.T * S + a_cap, pack_kernel), kMoveWarps * 32, 0, ln.stream>>>(
         static_cast<const int4*>(x), offsets, row_of, src_of, D.T, D.k, D.E_loc, a_cap, row_packets, S, split_packets,
         static_cast<int4*>(xp));
     PIPER_LAUNCHED(c, "pack_kernel");
@@ -428,12 +422,12 @@ int launch_combine(piper_ctx* c, Lane ln, const void* o, const int32_t* row_of, 
     const piper_moe_desc& D = c->D;
     const int row_packets = (int)((size_t)D.d * esize(D.dtype) / 16);
     int S, split_packets;
-    choose_split(ln, D.T, row_packets, S, split_packets);
+    choose_split(c, ln, D.T, row_packets, S, split_packets);
     const int items = D.T * S;
     const int4 *o4 = static_cast<const int4*>(o), *s4 = static_cast<const int4*>(s), *s24 = static_cast<const int4*>(s2);
     int4* y4 = static_cast<int4*>(y);
 #define PIPER_COMBINE(BF, W, TW)                                                                          \
-    combine_kernel<BF, W, TW><<<mover_blocks(ln, items, combine_kernel<BF, W, TW>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, s24, D.T, D.k, row_packets, S, split_packets, y4)
+    combine_kernel<BF, W, TW><<<mover_blocks(c, ln, items, combine_kernel<BF, W, TW>), kMoveWarps * 32, 0, ln.stream>>>(o4, row_of, gates, s4, s24, D.T, D.k, row_packets, S, split_packets, y4)
     if (s2 != nullptr) {  // only B5 with the router's term carries a second addend
         if (weighted) return PIPER_ERR_INVALID;
         if (D.dtype == PIPER_DTYPE_BF16) PIPER_COMBINE(true, false, true); else PIPER_COMBINE(false, false, true);
@@ -455,7 +449,7 @@ int launch_combine_bwd(piper_ctx* c, Lane ln, const void* dy, const void* o, con
     const bool write_do = d_o != nullptr;  // NULL: dgates only (the fused chunk calls)
     const int items = D.T + (write_do ? a_cap : 0);
 #define PIPER_CGRAD(BF, W)                                                                                             \
-    combine_bwd_kernel<BF, W><<<mover_blocks(ln, items, combine_bwd_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(      \
+    combine_bwd_kernel<BF, W><<<mover_blocks(c, ln, items, combine_bwd_kernel<BF, W>), kMoveWarps * 32, 0, ln.stream>>>(      \
         static_cast<const int4*>(dy), static_cast<const int4*>(o), src_of, row_of, gates, offsets, D.T, D.k, D.E_loc,   \
         write_do ? a_cap : 0, row_packets, static_cast<int4*>(d_o), dgates)
     if (D.dtype == PIPER_DTYPE_BF16) {

@@ -95,6 +95,7 @@ struct piper_ctx {
     int tc_prof;             // PIPER_OPT_TC_PROFILE: the tcgen05 kernels record wait-cycle counters in tc_scratch
     int fused_gather;        // PIPER_OPT_FUSED_GATHER: chunk calls let the GEMMs gather x / dY rows (N2)
     int pair_bwd_pass;       // piper_set_pair_bwd_pass
+    int move_items, move_cap;  // PIPER_OPT_MOVE_ITEMS / PIPER_OPT_MOVE_CAP: work items per resident warp / blocks per SM of the row movers
     unsigned long long sched_clock;
     piper::SchedSlot sched_slots[piper::kSchedSlots];
     piper::ClusterCacheEntry cluster_cache[piper::kClusterCache];

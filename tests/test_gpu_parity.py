@@ -222,6 +222,23 @@ def test_fallback_kernel_families(name, family):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["C3s", "C4s"])
+@pytest.mark.parametrize("items,cap", [(1, 1), (3, 5), (64, 64)])
+def test_row_mover_grid_options(name, items, cap):
+    """PIPER_OPT_MOVE_ITEMS / PIPER_OPT_MOVE_CAP only size the row movers' grids and column splits: any value gives the
+    same bits as the defaults (and therefore the oracle's results)."""
+    cfg = dataclasses.replace(configs.BY_NAME[name], row_align=16)
+    inp = configs.make_inputs(cfg)
+    ctx0, ref = _run_steps(cfg, inp, use_chunk_calls=True)
+    ctx0.close()
+    ctx, b = _run_steps(cfg, inp, use_chunk_calls=True, options=[(piper.OPT_MOVE_ITEMS, items), (piper.OPT_MOVE_CAP, cap)])
+    A = int(ref["offsets"][cfg.e_loc].item())
+    for n in ("xp", "y", "d_o", "dgates", "dx"):
+        x, y = (ref[n][:A], b[n][:A]) if n in ("xp", "d_o") else (ref[n], b[n])
+        assert torch.equal(x.view(torch.uint8), y.view(torch.uint8)), n
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["C2s", "C3s", "C4s", "C6s"])
 def test_poisoned_buffers_and_untouched_capacity(name):
     """No result may depend on what a buffer held before (pad rows are written, never assumed), and no kernel may
